@@ -1,0 +1,364 @@
+"""Pins for the whole oracle step (CPU only): conservation, div B, fixed points, exact reduction to
+1D, direction permutation, EMF-rule special cases, Orszag-Tang point symmetry, second-order
+convergence on the exact circularly polarised Alfven wave and first-order
+convergence to the textbook exact Euler Riemann solution."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2511_20337_b200 import workloads as wl
+
+G = 5.0 / 3.0
+
+
+def divb(Bf, nx, ny, nz, box):
+    f = wl.split_faces(Bf, nx, ny, nz)
+    d = np.zeros((nz, ny, nx))
+    if "bx" in f:
+        d += (f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) / (box[0] / nx)
+    if "by" in f:
+        d += (f["by"][:, 1:, :] - f["by"][:, :-1, :]) / (box[1] / ny)
+    if "bz" in f:
+        d += (f["bz"][1:, :, :] - f["bz"][:-1, :, :]) / (box[2] / nz)
+    return d
+
+
+def ksum(a):
+    return math.fsum(np.asarray(a, dtype=np.float64).ravel().tolist())
+
+
+# ------------------------------------------------------------------ invariants (north_star)
+
+def test_conservation_and_divb_orszag_tang_100_steps(oracle):
+    w = wl.orszag_tang_2d(64, nsteps=100)
+    oracle.load(w)
+    tot0 = [ksum(w.U[v]) for v in (0, 1, 2, 3, 7)]
+    absm = ksum(np.abs(w.U[1])) + ksum(np.abs(w.U[2]))
+    assert oracle.step(100) == 0
+    U, Bf = oracle.get_state()
+    tot1 = [ksum(U[v]) for v in (0, 1, 2, 3, 7)]
+    assert abs(tot1[0] - tot0[0]) <= 1e-12 * abs(tot0[0])
+    assert abs(tot1[4] - tot0[4]) <= 1e-12 * abs(tot0[4])
+    for a in (1, 2, 3):
+        assert abs(tot1[a] - tot0[a]) <= 1e-12 * absm          # R16: momentum scaled by sum |m|
+    d = divb(Bf, w.nx, w.ny, w.nz, w.box)
+    bmax = np.abs(Bf).max()
+    assert np.abs(d).max() * (w.box[0] / w.nx) <= 1e-12 * bmax
+    # cell-centred B is the face mean (R7) and the periodic duplicate face equals face 0
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    assert np.array_equal(U[4], 0.5 * (f["bx"][:, :, :-1] + f["bx"][:, :, 1:]))
+    assert np.array_equal(U[5], 0.5 * (f["by"][:, :-1, :] + f["by"][:, 1:, :]))
+    assert np.array_equal(f["bx"][:, :, 0], f["bx"][:, :, -1])
+    assert np.array_equal(f["by"][:, 0, :], f["by"][:, -1, :])
+
+
+def test_conservation_and_divb_3d(oracle):
+    w = wl.random_smooth(12, 10, 9, seed=3, box=(1.0, 0.8, 1.1))
+    oracle.load(w)
+    tot0 = [ksum(w.U[v]) for v in (0, 1, 2, 3, 7)]
+    absm = sum(ksum(np.abs(w.U[a])) for a in (1, 2, 3))
+    assert oracle.step(20) == 0
+    U, Bf = oracle.get_state()
+    for n, v in enumerate((0, 1, 2, 3, 7)):
+        scale = absm if v in (1, 2, 3) else abs(tot0[n])
+        assert abs(ksum(U[v]) - tot0[n]) <= 1e-12 * scale
+    d = divb(Bf, w.nx, w.ny, w.nz, w.box)
+    assert np.abs(d).max() * min(w.box[a] / n for a, n in enumerate((w.nx, w.ny, w.nz))) <= 1e-12 * np.abs(Bf).max()
+
+
+def test_ct_keeps_divergence_for_any_dt(oracle):
+    """telescoping: the discrete divergence is unchanged whatever the EMFs and dt are"""
+    w = wl.random_smooth(8, 6, 5, seed=11)
+    oracle.load(w)
+    d0 = divb(w.Bface, w.nx, w.ny, w.nz, w.box)
+    out = oracle.debug_euler(0.37, want=("Bf1",))          # absurdly large dt on purpose
+    d1 = divb(out["Bf1"], w.nx, w.ny, w.nz, w.box)
+    assert np.abs(d1 - d0).max() <= 1e-11 * np.abs(out["Bf1"]).max() * w.nx
+
+
+# ------------------------------------------------------------------ fixed points, dt closed form
+
+@pytest.mark.parametrize("shape", [(16, 1, 1), (8, 12, 1), (6, 5, 7)])
+def test_uniform_state_is_a_bitwise_fixed_point(oracle, shape):
+    nx, ny, nz = shape
+    rho, p = 1.3, 0.7
+    v = np.array([0.4, -0.3, 0.2])
+    B = np.array([0.5, 0.8, -0.6])
+    shp = (nz, ny, nx)
+    U = wl.conserved_from_fields(np.full(shp, rho), [np.full(shp, x) for x in v], [np.full(shp, x) for x in B],
+                                 np.full(shp, p), G)
+    faces = {nm: np.full(s, B["xyz".index(nm[1])]) for nm, s in wl.face_shapes(nx, ny, nz)}
+    Bf = wl.join_faces(faces, nx, ny, nz)
+    box = (1.0, 0.7, 1.9)
+    assert oracle.init(nx, ny, nz, 2, G, 0.3, 0) == 0
+    oracle.set_box(*box)
+    oracle.set_state(U, Bf)
+    # closed form: cfl * min_d dx_d / (|v_d| + c_f,d), c_f from the magnetosonic quartic
+    dts = []
+    for d, n in enumerate(shape):
+        if n == 1:
+            continue
+        a2, b2, bn2 = G * p / rho, B @ B / rho, B[d] ** 2 / rho
+        cf = math.sqrt(0.5 * (a2 + b2 + math.sqrt((a2 + b2) ** 2 - 4 * a2 * bn2)))
+        dts.append(0.3 * (box[d] / n) / (abs(v[d]) + cf))
+    assert abs(oracle.get_dt() - min(dts)) <= 4e-16 * min(dts)
+    assert oracle.step(3) == 0
+    U1, Bf1 = oracle.get_state()
+    assert np.array_equal(U1, U) and np.array_equal(Bf1, Bf)
+
+
+# ------------------------------------------------------------------ EMF rule (R6)
+
+def test_emf_uniform_state_equals_cell_emf(oracle):
+    nx, ny, nz = 5, 4, 6
+    shp = (nz, ny, nx)
+    v = np.array([0.4, -0.3, 0.2])
+    B = np.array([0.5, 0.8, -0.6])
+    U = wl.conserved_from_fields(np.full(shp, 1.1), [np.full(shp, x) for x in v], [np.full(shp, x) for x in B],
+                                 np.full(shp, 0.9), G)
+    Bf = wl.join_faces({nm: np.full(s, B["xyz".index(nm[1])]) for nm, s in wl.face_shapes(nx, ny, nz)}, nx, ny, nz)
+    oracle.init(nx, ny, nz, 2, G, 0.3, 0)
+    oracle.set_state(U, Bf)
+    E = oracle.debug_euler(0.01, want=("E",))["E"]
+    Ec = -np.cross(v, B)
+    for e in range(3):
+        assert np.allclose(E[e], Ec[e], rtol=1e-13, atol=1e-14)
+
+
+def test_emf_reduces_to_1d_flux_for_invariant_data(oracle):
+    """y-invariant data => Ez(i-1/2, j-1/2) = -F_x[B_y](i-1/2) for any weights (R6 iii)"""
+    w1 = wl.random_smooth(16, 1, 1, seed=5)
+    nx, ny = 16, 6
+    U = np.repeat(w1.U, ny, axis=2)
+    f1 = wl.split_faces(w1.Bface, 16, 1, 1)
+    By0 = w1.U[5, 0, 0, :]
+    faces = {"bx": np.repeat(f1["bx"], ny, axis=1), "by": np.repeat(By0[None, None, :], ny + 1, axis=1)}
+    oracle.init(nx, ny, 1, 2, G, 0.3, 0)
+    oracle.set_box(1.0, 1.0, 1.0)
+    oracle.set_state(U, wl.join_faces(faces, nx, ny, 1))
+    out = oracle.debug_euler(0.003, want=("E", "F"))
+    Ez, Fx_By = out["E"][2], out["F"][0, 5]
+    assert np.abs(Ez + Fx_By).max() <= 1e-14 * (1 + np.abs(Fx_By).max())
+    assert np.abs(Fx_By).max() > 1e-3
+
+
+# ------------------------------------------------------------------ dimensional consistency (R8 consequence)
+
+def _embed(w1, axis, ncopy):
+    """pose the 1D x-problem w1 along `axis` (0 x, 1 y, 2 z) on a grid with `ncopy` invariant cells
+    in the other active directions; vector components are permuted cyclically with the axes"""
+    n = w1.nx
+    q = {v: w1.U[v, 0, 0, :] for v in range(8)}
+    bn = wl.split_faces(w1.Bface, n, 1, 1)["bx"][0, 0, :]          # n+1 faces
+    perm = [(axis + m) % 3 for m in range(3)]                       # 1D (x,y,z) -> lab components
+    if axis == 0:
+        shape, box = (n, ncopy, 1), (1.0, ncopy / n, 1.0)
+    elif axis == 1:
+        shape, box = (ncopy, n, 1), (ncopy / n, 1.0, 1.0)
+    else:
+        shape, box = (ncopy, ncopy, n), (ncopy / n, ncopy / n, 1.0)
+    nx, ny, nz = shape
+    shp = (nz, ny, nx)
+
+    def along(a):                                                   # broadcast a 1D profile along `axis`
+        idx = [None, None, None]
+        idx[2 - axis] = slice(None)
+        return np.broadcast_to(np.asarray(a)[tuple(idx)], shp).copy()
+    U = np.zeros((8,) + shp)
+    U[0] = along(q[0])
+    U[7] = along(q[7])
+    for m in range(3):
+        U[1 + perm[m]] = along(q[1 + m])
+        U[4 + perm[m]] = along(q[4 + m])
+    faces = {}
+    for nm, s in wl.face_shapes(nx, ny, nz):
+        d = "xyz".index(nm[1])
+        if d == axis:
+            idx = [None, None, None]
+            idx[2 - axis] = slice(None)
+            faces[nm] = np.broadcast_to(bn[tuple(idx)], s).copy()
+        else:
+            # transverse face field = the (uniform along its own normal) cell value of that component
+            m = perm.index(d)
+            prof = q[4 + m]
+            idx = [None, None, None]
+            idx[2 - axis] = slice(None)
+            faces[nm] = np.broadcast_to(prof[tuple(idx)], s).copy()
+    return shape, box, U, wl.join_faces(faces, nx, ny, nz), perm, along
+
+
+@pytest.mark.parametrize("limiter", [0, 1])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_grid_aligned_run_reproduces_the_1d_solution(oracle, axis, limiter):
+    """north_star invariant: a 2D/3D run with data invariant in the other directions, stepped with
+    the dt sequence of the 1D run, equals the 1D run; posed along y or z it equals the x result with
+    permuted components (tests the direction rotation and all three EMF components)"""
+    n = 32
+    # a discontinuous 1D problem (Brio-Wu-like, Bx = 0.75) plus smooth transverse structure
+    w1 = wl.random_smooth(n, 1, 1, seed=7, amp=0.3)
+    x = wl.cell_centres(n, 1.0)
+    left = (x > 0.25) & (x < 0.75)
+    V = {0: np.where(left, 1.0, 0.125), 7: np.where(left, 1.0, 0.1)}
+    rho, p = V[0], V[7]
+    vel = [0.2 * np.sin(2 * np.pi * x), 0.1 * np.cos(2 * np.pi * x), 0.05 * np.sin(4 * np.pi * x)]
+    Bc = [np.full(n, 0.75), np.where(left, 1.0, -1.0), 0.3 * np.cos(2 * np.pi * x)]
+    shp = (1, 1, n)
+    U1 = wl.conserved_from_fields(rho.reshape(shp), [a.reshape(shp) for a in vel], [a.reshape(shp) for a in Bc],
+                                  p.reshape(shp), 2.0)
+    w1 = wl.Workload("bw", n, 1, 1, (1.0, 1.0, 1.0), 2.0, 0.3, limiter, 12, U1,
+                     wl.join_faces({"bx": np.full((1, 1, n + 1), 0.75)}, n, 1, 1))
+    oracle.load(w1)
+    dts = []
+    for _ in range(12):
+        assert oracle.step(1) == 0
+        dts.append(oracle.get_dt())
+    Uref, _ = oracle.get_state()
+    shape, box, U, Bf, perm, along = _embed(w1, axis, 4)
+    assert oracle.init(*shape, 2, 2.0, 0.3, limiter) == 0
+    oracle.set_box(*box)
+    oracle.set_state(U, Bf)
+    for dt in dts:
+        assert oracle.step_fixed_dt(1, dt) == 0
+    Um, Bfm = oracle.get_state()
+    comp = {0: 0, 7: 7}
+    for m in range(3):
+        comp[1 + m] = 1 + perm[m]
+        comp[4 + m] = 4 + perm[m]
+    for v in range(8):
+        ref = along(Uref[v, 0, 0, :])
+        scale = np.abs(ref).max() + 1e-300
+        assert np.abs(Um[comp[v]] - ref).max() <= 1e-12 * max(scale, 1.0), (v, axis)
+    # something actually happened
+    assert np.abs(Uref - w1.U).max() > 1e-2
+
+
+# ------------------------------------------------------------------ symmetry
+
+def test_orszag_tang_point_symmetry(oracle):
+    """noise-free OT is invariant under (x,y) -> (1-x,1-y) with v, B odd"""
+    w = wl.orszag_tang_2d(48, noise=0.0)
+    oracle.load(w)
+    assert oracle.step(40) == 0
+    U, Bf = oracle.get_state()
+    flip = lambda a: a[:, ::-1, ::-1]
+    for v, s in ((0, 1), (7, 1), (1, -1), (2, -1), (4, -1), (5, -1)):
+        assert np.abs(U[v] - s * flip(U[v])).max() <= 1e-12 * (np.abs(U[v]).max()), v
+    assert np.abs(U[3]).max() == 0.0 and np.abs(U[6]).max() == 0.0
+
+
+# ------------------------------------------------------------------ exact solutions
+
+def _cpa_error(oracle, w):
+    """run one period with CFL steps, last step clipped; L1 error of cell B against the initial state"""
+    oracle.load(w)
+    t, n = 0.0, 0
+    while True:
+        U, Bf = oracle.get_state()
+        oracle.set_state(U, Bf)            # so that get_dt returns the CFL dt of this state
+        dt = oracle.get_dt()
+        if t + dt < w.t_end:
+            assert oracle.step_fixed_dt(1, dt) == 0
+            t += dt
+            n += 1
+        else:
+            assert oracle.step_fixed_dt(1, w.t_end - t) == 0
+            n += 1
+            break
+    U, _ = oracle.get_state()
+    err = math.sqrt(sum(np.abs(U[4 + s] - w.U[4 + s]).mean() ** 2 for s in range(3)))
+    return err, n
+
+
+def test_cp_alfven_1d_second_order(oracle):
+    e128, _ = _cpa_error(oracle, wl.cp_alfven_1d(128))
+    e256, _ = _cpa_error(oracle, wl.cp_alfven_1d(256))
+    order = math.log2(e128 / e256)
+    assert order >= 1.9, (e128, e256, order)
+    assert e256 < 1e-4
+
+
+def test_cp_alfven_3d_second_order(oracle):
+    """config 1 (64x32x32, MC, CFL 0.4) against the exact solution after one period"""
+    e32, n32 = _cpa_error(oracle, wl.cp_alfven_3d(32, noise=0.0))
+    e64, n64 = _cpa_error(oracle, wl.cp_alfven_3d(64, noise=0.0))
+    order = math.log2(e32 / e64)
+    assert order >= 1.8, (e32, e64, order)
+    assert e64 < 4e-3
+    assert 55 <= n64 <= 70
+
+
+def _exact_euler_riemann(rL, uL, pL, rR, uR, pR, g, xi):
+    """textbook exact Riemann solver for the Euler equations (Toro ch. 4), sampled at xi = x/t"""
+    cL, cR = math.sqrt(g * pL / rL), math.sqrt(g * pR / rR)
+
+    def f(p, r, pk, c):
+        if p > pk:
+            A, B = 2 / ((g + 1) * r), (g - 1) / (g + 1) * pk
+            return (p - pk) * math.sqrt(A / (p + B))
+        return 2 * c / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1)
+    lo, hi = 1e-12, 10 * max(pL, pR)
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if f(mid, rL, pL, cL) + f(mid, rR, pR, cR) + uR - uL > 0:
+            hi = mid
+        else:
+            lo = mid
+    ps = 0.5 * (lo + hi)
+    us = 0.5 * (uL + uR) + 0.5 * (f(ps, rR, pR, cR) - f(ps, rL, pL, cL))
+    out = np.empty((3, xi.size))
+    for n, s in enumerate(xi):
+        if s <= us:
+            r, u, p, c, sg = rL, uL, pL, cL, 1.0
+        else:
+            r, u, p, c, sg = rR, uR, pR, cR, -1.0
+        if ps > p:                                                  # shock
+            S = u - sg * c * math.sqrt((g + 1) / (2 * g) * ps / p + (g - 1) / (2 * g))
+            if sg * (s - S) < 0:
+                out[:, n] = (r, u, p)
+            else:
+                out[:, n] = (r * ((ps / p + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * ps / p + 1)), us, ps)
+        else:                                                       # rarefaction
+            cs = c * (ps / p) ** ((g - 1) / (2 * g))
+            head, tail = u - sg * c, us - sg * cs
+            if sg * (s - head) < 0:
+                out[:, n] = (r, u, p)
+            elif sg * (s - tail) > 0:
+                out[:, n] = (r * (ps / p) ** (1 / g), us, ps)
+            else:
+                cc = 2 / (g + 1) * (c + sg * (g - 1) / 2 * (u - s))
+                out[:, n] = (r * (cc / c) ** (2 / (g - 1)), 2 / (g + 1) * (sg * c + (g - 1) / 2 * u + s),
+                             p * (cc / c) ** (2 * g / (g - 1)))
+    return out, ps, us
+
+
+def _sod_error(oracle, n):
+    g = 1.4
+    x = wl.cell_centres(n, 1.0)
+    left = (x > 0.25) & (x < 0.75)                                 # periodic box: two mirrored tubes
+    shp = (1, 1, n)
+    z = np.zeros(shp)
+    rho = np.where(left, 1.0, 0.125).reshape(shp)
+    p = np.where(left, 1.0, 0.1).reshape(shp)
+    U = wl.conserved_from_fields(rho, [z, z, z], [z, z, z], p, g)
+    w = wl.Workload("sod", n, 1, 1, (1.0, 1.0, 1.0), g, 0.4, 0, 0, U, np.zeros(n + 1), t_end=0.1)
+    oracle.load(w)
+    t = 0.0
+    while t < w.t_end - 1e-15:
+        Uc, Bf = oracle.get_state()
+        oracle.set_state(Uc, Bf)
+        dt = min(oracle.get_dt(), w.t_end - t)
+        assert oracle.step_fixed_dt(1, dt) == 0
+        t += dt
+    Uc, _ = oracle.get_state()
+    sel = x > 0.5                                                   # the tube centred at x = 0.75
+    ex, ps, us = _exact_euler_riemann(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, g, (x[sel] - 0.75) / w.t_end)
+    return np.abs(Uc[0, 0, 0, sel] - ex[0]).mean(), ps, us
+
+
+def test_hydro_shock_tube_converges_to_exact_riemann_solution(oracle):
+    e1, ps, us = _sod_error(oracle, 200)
+    e2, _, _ = _sod_error(oracle, 400)
+    # Toro's tabulated star values for Sod's problem (Riemann Solvers..., Table 4.2): p* = 0.30313, u* = 0.92745
+    assert abs(ps - 0.30313) < 1e-5 and abs(us - 0.92745) < 1e-5
+    assert e2 < 0.65 * e1 and e2 < 5e-3, (e1, e2)      # ~first order in L1 at discontinuities
