@@ -1,0 +1,110 @@
+/*
+ * pluto.h -- C-ABI boundary of libpluto_b200.so: the fp64 finite-volume ideal-MHD time step of
+ * gPLUTO (arxiv 2511.20337) as hand-written CUDA kernels for sm_100a.
+ *
+ * The step (one call of pluto_step advances full RK2 steps) is, per RK stage:
+ *   periodic ghost fill        (periodic boxes PAPER.md:254,360; pack/unpack Fig. 4)
+ *   conservative -> primitive  (Eq. 7)
+ *   PLM reconstruction of the primitives with a minmod / MC limiter (Eq. 6; reading R4)
+ *   HLLD Riemann flux per sweep direction (Eq. 8; HLLD [56] PAPER.md:260; reading R5)
+ *   flux-difference update     (Eq. 4; Fig. 2)
+ *   constrained transport: upwind edge EMFs + face-B curl update (reading R6)
+ * and once per step the RK2 combine (Eq. 5's increment form; reading R3) and the
+ * CFL max-signal-speed reduction for dt (reading R8).  Readings R1..R16 are listed in DESIGN.md.
+ *
+ * Everything is fp64.  One global context (the five north-star calls carry no handle).
+ * All entry points return 0 (PLUTO_OK) or a negative error code; no exceptions, aborts or stdout.
+ * There is NO CPU fallback: without a CUDA device every compute entry point returns PLUTO_ECUDA.
+ *
+ * Pointer arguments named U / Bface may be HOST or DEVICE pointers (the library asks the CUDA
+ * runtime which); the caller owns them, the library copies in/out and never keeps them.
+ *
+ * Array layouts (doubles, SoA, i contiguous -- PAPER.md:154):
+ *   U     : 8*nz*ny*nx, interior zones only, U[v][k][j][i]; v = 0 rho, 1-3 rho*v_{x,y,z},
+ *           4-6 B_{x,y,z} (cell centred), 7 E   (component order of Eq. 2)
+ *   Bface : [bx: nz*ny*(nx+1)] [by: nz*(ny+1)*nx] [bz: (nz+1)*ny*nx, only if nz > 1];
+ *           face index 0 lies on the lower domain boundary; the last face of a family duplicates
+ *           face 0 (periodic): ignored on input, written equal to face 0 on output.
+ */
+#ifndef PLUTO_B200_H
+#define PLUTO_B200_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    PLUTO_OK     =  0,
+    PLUTO_EINVAL = -1,   /* bad argument */
+    PLUTO_ESTATE = -2,   /* call order: not initialised / no state set */
+    PLUTO_ECUDA  = -3,   /* CUDA runtime error or no device (see pluto_last_error) */
+    PLUTO_EPHYS  = -4,   /* non-finite or non-positive density / pressure met during a step */
+    PLUTO_ENOMEM = -5    /* device allocation failed or registered workspace too small */
+};
+
+enum { PLUTO_MINMOD = 0, PLUTO_MC = 1 };
+
+/* Create (or re-create) the context for an nx x ny x nz periodic box of cubic cells with Lx = 1
+ * (override with pluto_set_box).  ny >= 2 and nx >= 2 are required (2D when nz == 1, 3D when
+ * nz >= 2); every active extent must be >= ghost.  ghost >= 2 layers are kept around the padded
+ * device arrays (PLM needs 2).  gamma > 1 (Gamma of Eq. 3), cfl > 0, limiter PLUTO_MINMOD|PLUTO_MC.
+ * Allocates device memory unless a large enough workspace was registered before. */
+int    pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter);
+
+/* Copy a state in.  Cell-centred B of every active dimension is OVERWRITTEN by the mean of its two
+ * faces (reading R7); E is taken as given.  Resets the time to 0. */
+int    pluto_set_state(const double *U, const double *Bface);
+
+/* Advance nsteps full SSP-RK2 steps, each with its own CFL dt computed on the device from the
+ * state at the start of the step.  Returns after the work has completed on the stream.
+ * PLUTO_EPHYS if an unphysical zone was met (state then undefined). */
+int    pluto_step(int nsteps);
+
+/* dt used by the most recent step; before any step since set_state: the dt the next step will
+ * use.  NaN if not initialised. */
+double pluto_get_dt(void);
+
+/* Copy the state out (either pointer may be NULL). */
+int    pluto_get_state(double *U, double *Bface);
+
+/* ---- extensions the five calls cannot express ---- */
+
+int    pluto_set_box(double Lx, double Ly, double Lz);      /* cell sizes dx_d = L_d / n_d (R11) */
+int    pluto_step_fixed_dt(int nsteps, double dt);          /* same step with dt imposed (R8: 1D pin, clipping) */
+double pluto_get_time(void);                                /* sum of dt since set_state */
+int    pluto_set_stream(void *cuda_stream);                 /* cudaStream_t to launch on (NULL: default) */
+size_t pluto_workspace_bytes(int nx, int ny, int nz, int ghost);
+int    pluto_set_workspace(void *dev, size_t bytes);        /* caller-owned device memory, used by the next pluto_init */
+int    pluto_finalize(void);
+const char *pluto_last_error(void);
+int    pluto_device_count(void);                            /* 0 without a usable CUDA device */
+
+/* Enqueue nsteps steps without waiting (no error check, no host synchronisation); used for timing
+ * with CUDA events on the stream given to pluto_set_stream.  pluto_sync waits and returns
+ * PLUTO_EPHYS / PLUTO_ECUDA like pluto_step. */
+int    pluto_step_async(int nsteps);
+int    pluto_sync(void);
+
+/* Number of kernel launches enqueued by this library since pluto_init (for bench.py's gpu_launches). */
+long long pluto_launch_count(void);
+
+/* Tuning switches: opt = PLUTO_OPT_*, returns the previous value or PLUTO_EINVAL. */
+enum {
+    PLUTO_OPT_GRAPH = 1    /* 1 (default): replay one captured CUDA graph per step; 0: plain launches */
+};
+int    pluto_set_option(int opt, int value);
+
+/* One Euler stage S -> S + L(S) from the CURRENT state with the given dt, for per-kernel parity
+ * tests; the state is not advanced.  Any pointer may be NULL (host or device pointers).
+ *   U1, Bf1 : layouts of U / Bface
+ *   W       : [3][nz][ny][nx] upwind weight on the LOWER d-face of each cell (R6)
+ *   Fem     : [3][2][nz][ny][nx] the two induction fluxes kept for CT on that face:
+ *             d = x: (F_x[B_y], F_x[B_z]);  d = y: (F_y[B_z], F_y[B_x]);  d = z: (F_z[B_x], F_z[B_y])
+ *   Eedge   : [3][nz][ny][nx] Ex at (i, j-1/2, k-1/2), Ey at (i-1/2, j, k-1/2), Ez at (i-1/2, j-1/2, k)
+ * entries of inactive directions are zero. */
+int    pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem, double *Eedge);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,193 @@
+"""Thin ctypes binding of libpluto_b200.so (include/pluto.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device
+memory (the workspace the library computes in) and the stream it launches on.  There is no CPU
+fallback: a missing library or a missing device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB = os.path.join(_HERE, "libpluto_b200.so")
+
+OK, EINVAL, ESTATE, ECUDA, EPHYS, ENOMEM = 0, -1, -2, -3, -4, -5
+MINMOD, MC = 0, 1
+OPT_GRAPH = 1
+
+# every symbol include/pluto.h declares
+SYMBOLS = [
+    "pluto_init", "pluto_set_state", "pluto_step", "pluto_get_dt", "pluto_get_state",
+    "pluto_set_box", "pluto_step_fixed_dt", "pluto_get_time", "pluto_set_stream",
+    "pluto_workspace_bytes", "pluto_set_workspace", "pluto_finalize", "pluto_last_error",
+    "pluto_device_count", "pluto_step_async", "pluto_sync", "pluto_launch_count",
+    "pluto_set_option", "pluto_debug_euler",
+]
+
+
+class PlutoError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"pluto error {code}: {msg}")
+        self.code = code
+
+
+def load_library(build_if_missing: bool = True) -> C.CDLL:
+    if build_if_missing:
+        from . import build as _build
+        _build.build()
+    if not os.path.exists(LIB):
+        raise RuntimeError(f"{LIB} is missing: build it with `python -m paper_2511_20337_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB)
+    vp, dbl, i32 = C.c_void_p, C.c_double, C.c_int
+    L.pluto_init.argtypes = [i32, i32, i32, i32, dbl, dbl, i32]
+    L.pluto_set_state.argtypes = [vp, vp]
+    L.pluto_step.argtypes = [i32]
+    L.pluto_get_dt.restype = dbl
+    L.pluto_get_state.argtypes = [vp, vp]
+    L.pluto_set_box.argtypes = [dbl, dbl, dbl]
+    L.pluto_step_fixed_dt.argtypes = [i32, dbl]
+    L.pluto_get_time.restype = dbl
+    L.pluto_set_stream.argtypes = [vp]
+    L.pluto_workspace_bytes.argtypes = [i32, i32, i32, i32]
+    L.pluto_workspace_bytes.restype = C.c_size_t
+    L.pluto_set_workspace.argtypes = [vp, C.c_size_t]
+    L.pluto_last_error.restype = C.c_char_p
+    L.pluto_step_async.argtypes = [i32]
+    L.pluto_launch_count.restype = C.c_longlong
+    L.pluto_set_option.argtypes = [i32, i32]
+    L.pluto_debug_euler.argtypes = [dbl, vp, vp, vp, vp, vp]
+    return L
+
+
+def _addr(a):
+    """host numpy array or CUDA torch tensor -> raw address (the library tells host from device)"""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+        return a.ctypes.data
+    assert a.dtype.is_floating_point and a.element_size() == 8 and a.is_contiguous()
+    return a.data_ptr()
+
+
+class Pluto:
+    """pluto_* calls with the same names; arrays are numpy (host) or torch CUDA tensors (device)"""
+
+    def __init__(self, device: int = 0):
+        import torch
+        self.L = load_library()
+        if self.L.pluto_device_count() < 1 or not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: paper_2511_20337_b200 has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        torch.cuda.set_device(self.device)
+        self.stream = torch.cuda.Stream(device=self.device)
+        self._check(self.L.pluto_set_stream(self.stream.cuda_stream))
+        self.workspace = None
+        self.shape = None
+
+    def _check(self, rc):
+        if rc != 0:
+            raise PlutoError(rc, self.L.pluto_last_error().decode())
+        return rc
+
+    # ---- the five calls
+    def init(self, nx, ny, nz, ghost=2, gamma=5.0 / 3.0, cfl=0.4, limiter=MINMOD):
+        need = self.L.pluto_workspace_bytes(nx, ny, nz, ghost)
+        if need == 0:
+            raise PlutoError(EINVAL, "bad grid")
+        self.L.pluto_finalize()
+        if self.workspace is None or self.workspace.numel() < need:
+            self.workspace = None
+            self.workspace = self.torch.empty(need, dtype=self.torch.uint8, device=self.device)
+        self.torch.cuda.current_stream().synchronize()
+        self._check(self.L.pluto_set_workspace(self.workspace.data_ptr(), self.workspace.numel()))
+        self._check(self.L.pluto_init(nx, ny, nz, ghost, gamma, cfl, limiter))
+        self.shape = (nx, ny, nz)
+        return 0
+
+    def nface(self):
+        nx, ny, nz = self.shape
+        return (nx + 1) * ny * nz + nx * (ny + 1) * nz + (nx * ny * (nz + 1) if nz > 1 else 0)
+
+    def set_state(self, U, Bface):
+        if isinstance(U, np.ndarray):
+            U = np.ascontiguousarray(U, dtype=np.float64)
+            Bface = np.ascontiguousarray(Bface, dtype=np.float64)
+        else:
+            self.torch.cuda.current_stream().synchronize()
+        assert U.size == 8 * int(np.prod(self.shape)) if isinstance(U, np.ndarray) else U.numel() == 8 * int(np.prod(self.shape))
+        return self._check(self.L.pluto_set_state(_addr(U), _addr(Bface)))
+
+    def step(self, nsteps=1):
+        return self._check(self.L.pluto_step(nsteps))
+
+    def get_dt(self):
+        return self.L.pluto_get_dt()
+
+    def get_state(self, out_U=None, out_B=None, device=False):
+        nx, ny, nz = self.shape
+        if out_U is None:
+            if device:
+                out_U = self.torch.empty((8, nz, ny, nx), dtype=self.torch.float64, device=self.device)
+                out_B = self.torch.empty(self.nface(), dtype=self.torch.float64, device=self.device)
+                self.torch.cuda.current_stream().synchronize()
+            else:
+                out_U = np.empty((8, nz, ny, nx))
+                out_B = np.empty(self.nface())
+        self._check(self.L.pluto_get_state(_addr(out_U), _addr(out_B)))
+        return out_U, out_B
+
+    # ---- extensions
+    def set_box(self, Lx, Ly, Lz):
+        return self._check(self.L.pluto_set_box(Lx, Ly, Lz))
+
+    def step_fixed_dt(self, nsteps, dt):
+        return self._check(self.L.pluto_step_fixed_dt(nsteps, dt))
+
+    def get_time(self):
+        return self.L.pluto_get_time()
+
+    def step_async(self, nsteps):
+        return self._check(self.L.pluto_step_async(nsteps))
+
+    def sync(self):
+        return self._check(self.L.pluto_sync())
+
+    def launch_count(self):
+        return self.L.pluto_launch_count()
+
+    def set_option(self, opt, value):
+        return self.L.pluto_set_option(opt, value)
+
+    def finalize(self):
+        return self.L.pluto_finalize()
+
+    def load(self, w, ghost=2):
+        """init + set_box + set_state from a workloads.Workload (host arrays)"""
+        self.init(w.nx, w.ny, w.nz, ghost, w.gamma, w.cfl, w.limiter)
+        self.set_box(*w.box)
+        self.set_state(w.U, w.Bface)
+        return self
+
+    def debug_euler(self, dt, want=("U1", "Bf1", "W", "Fem", "E")):
+        nx, ny, nz = self.shape
+        out = {}
+        if "U1" in want:
+            out["U1"] = np.empty((8, nz, ny, nx))
+        if "Bf1" in want:
+            out["Bf1"] = np.empty(self.nface())
+        if "W" in want:
+            out["W"] = np.empty((3, nz, ny, nx))
+        if "Fem" in want:
+            out["Fem"] = np.empty((3, 2, nz, ny, nx))
+        if "E" in want:
+            out["E"] = np.empty((3, nz, ny, nx))
+        rc = self.L.pluto_debug_euler(dt, _addr(out.get("U1")), _addr(out.get("Bf1")), _addr(out.get("W")),
+                                      _addr(out.get("Fem")), _addr(out.get("E")))
+        out["rc"] = rc
+        return out

@@ -1,0 +1,83 @@
+// dt_kernel.cu -- CFL max-signal-speed reduction (a8, reading R8):
+//     dt = cfl / max_{zones, active d} ( (|v_d| + c_f,d) * (1/dx_d) )
+// This translation unit is compiled with -fmad=false and evaluates the per-zone expression in the
+// order DESIGN.md fixes (R15), so that for identical input the dt is bit-identical to an IEEE
+// evaluation without contraction.  The max itself is exact and order independent: warp shuffle ->
+// block shared memory -> atomicMax on the bit pattern (all candidates are positive doubles, for
+// which the IEEE ordering equals the unsigned integer ordering of the bits).
+#include "grid.h"
+#include <cuda_runtime.h>
+
+namespace pluto {
+
+__global__ void __launch_bounds__(256)
+k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
+{
+    const long long nzone = (long long)g.n[0] * g.n[1] * g.n[2];
+    double smax = 0.0;
+    int bad = 0;
+    for (long long z = blockIdx.x * (long long)blockDim.x + threadIdx.x; z < nzone;
+         z += (long long)gridDim.x * blockDim.x) {
+        int i = (int)(z % g.n[0]);
+        int j = (int)((z / g.n[0]) % g.n[1]);
+        int k = (int)(z / ((long long)g.n[0] * g.n[1]));
+        long long c = g.at(i, j, k);
+        double rho = U[c], mx = U[g.sa + c], my = U[2 * g.sa + c], mz = U[3 * g.sa + c];
+        double B[3] = { U[4 * g.sa + c], U[5 * g.sa + c], U[6 * g.sa + c] };
+        double E = U[7 * g.sa + c];
+        double v[3] = { mx / rho, my / rho, mz / rho };
+        double p = (g.gamma - 1.0) * (E - 0.5 * (mx * v[0] + my * v[1] + mz * v[2])
+                                        - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));
+        if (!(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p)) bad = 1;
+        double a2 = g.gamma * p / rho;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            if (!g.act[d]) continue;
+            const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+            double b2  = (B[d] * B[d] + B[t1] * B[t1] + B[t2] * B[t2]) / rho;
+            double bn2 = B[d] * B[d] / rho;
+            double s = a2 + b2;
+            double disc = s * s - 4.0 * a2 * bn2;
+            if (disc < 0.0) disc = 0.0;
+            double cf = sqrt(0.5 * (s + sqrt(disc)));
+            double sig = (fabs(v[d]) + cf) * g.idx[d];
+            if (sig > smax) smax = sig;
+        }
+    }
+    // warp max
+    for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+    __shared__ double wmax[8];
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = smax;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double m = threadIdx.x < (blockDim.x >> 5) ? wmax[threadIdx.x] : 0.0;
+        for (int o = 4; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (threadIdx.x == 0) atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(m));
+    }
+    if (bad) P->err = 1;
+}
+
+// mode 0: CFL dt for the step about to start; mode 1: imposed dt; mode 2: probe only (get_dt)
+__global__ void k_dtfinish(Grid g, StepParams *P, int mode)
+{
+    double smax = __longlong_as_double((long long)P->smax_bits);
+    P->smax_bits = 0ull;
+    double dt = (mode == 1) ? P->dt_fixed : g.cfl / smax;
+    if (mode == 2) { P->dt_probe = dt; return; }
+    P->dt = dt;
+    for (int d = 0; d < 3; d++) P->dtdx[d] = dt / g.dx[d];
+}
+
+__global__ void k_advance_time(StepParams *P) { P->time += P->dt; }
+
+void launch_dtmax(const Grid &g, const double *U, StepParams *P, int nblocks, cudaStream_t s)
+{
+    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, P);
+}
+void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s)
+{
+    k_dtfinish<<<1, 1, 0, s>>>(g, P, mode);
+}
+void launch_advance_time(StepParams *P, cudaStream_t s) { k_advance_time<<<1, 1, 0, s>>>(P); }
+
+} // namespace pluto

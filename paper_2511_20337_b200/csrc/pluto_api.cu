@@ -1,0 +1,565 @@
+// pluto_api.cu -- the C-ABI of include/pluto.h: context, memory, host<->device copies, and the
+// launch sequence of one RK2 step.  No CPU fallback: without a device every call fails loudly.
+#include "../../include/pluto.h"
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+namespace pluto {
+void launch_dtmax(const Grid &g, const double *U, StepParams *P, int nblocks, cudaStream_t s);
+void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s);
+void launch_advance_time(StepParams *P, cudaStream_t s);
+}
+
+using namespace pluto;
+
+namespace {
+
+struct Context {
+    bool init = false;
+    bool have_state = false;
+    bool stepped = false;
+    Grid g{};
+    double *base = nullptr;          // A_COUNT arrays
+    StepParams *P = nullptr;         // device scalars (inside the allocation)
+    bool own_mem = false;
+    void *ws = nullptr;              // registered workspace
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;   // stream in use (the caller's, or own_stream)
+    cudaStream_t own_stream = nullptr;
+    long long launches = 0;
+    long long per_step[2] = { 0, 0 };
+    int use_graph = 1;
+    cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step
+    int sm_count = 148;
+    char err[512] = "";
+};
+
+Context C;
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(C.err, sizeof C.err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(x)                                                                              \
+    do {                                                                                         \
+        cudaError_t e_ = (x);                                                                    \
+        if (e_ != cudaSuccess) return fail(PLUTO_ECUDA, "%s: %s", #x, cudaGetErrorString(e_));   \
+    } while (0)
+
+double *arr(int id) { return C.base + (long long)id * C.g.sa; }
+
+size_t layout_bytes(const Grid &g) { return (size_t)A_COUNT * g.sa * sizeof(double) + 256; }
+
+dim3 grid_for(const Box &b, int bx = 128)
+{
+    return dim3((b.hi[0] - b.lo[0] + bx - 1) / bx, b.hi[1] - b.lo[1], b.hi[2] - b.lo[2]);
+}
+
+// index box: per axis [lo, hi) if active, else [0, 1)
+Box make_box(const Grid &g, int lo0, int hi0, int lo1, int hi1, int lo2, int hi2)
+{
+    Box b;
+    int lo[3] = { lo0, lo1, lo2 }, hi[3] = { hi0, hi1, hi2 };
+    for (int a = 0; a < 3; a++) {
+        b.lo[a] = g.act[a] ? lo[a] : 0;
+        b.hi[a] = g.act[a] ? hi[a] : 1;
+    }
+    return b;
+}
+
+Box interior(const Grid &g) { return make_box(g, 0, g.n[0], 0, g.n[1], 0, g.n[2]); }
+
+void destroy_graphs()
+{
+    for (auto &gr : C.graph)
+        if (gr) { cudaGraphExecDestroy(gr); gr = nullptr; }
+}
+
+// ---------------------------------------------------------------- launch sequences
+
+void fill_ghosts(double *first, int narr)
+{
+    const Grid &g = C.g;
+    const int ngh = 2 * g.ng + 1;
+    cudaStream_t s = C.stream;
+    k_ghost<0><<<dim3(1, g.tot[1], g.tot[2] * narr), 64, 0, s>>>(g, first, narr);
+    k_ghost<1><<<dim3((g.tot[0] + 127) / 128, ngh, g.tot[2] * narr), 128, 0, s>>>(g, first, narr);
+    C.launches += 2;
+    if (g.act[2]) {
+        k_ghost<2><<<dim3((g.tot[0] + 127) / 128, g.tot[1], ngh * narr), 128, 0, s>>>(g, first, narr);
+        C.launches += 1;
+    }
+}
+
+template <int LIM>
+void launch_flux(const double *V, const double *bface)
+{
+    const Grid &g = C.g;
+    cudaStream_t s = C.stream;
+    // faces 0..n along the sweep, one ghost layer across it (CT needs the transverse neighbours)
+    Box bx = make_box(g, 0, g.n[0] + 1, -1, g.n[1] + 1, -1, g.n[2] + 1);
+    k_flux<0, LIM><<<grid_for(bx), 128, 0, s>>>(g, bx, V, bface + 0 * g.sa, arr(A_F + 0));
+    Box by = make_box(g, -1, g.n[0] + 1, 0, g.n[1] + 1, -1, g.n[2] + 1);
+    k_flux<1, LIM><<<grid_for(by), 128, 0, s>>>(g, by, V, bface + 1 * g.sa, arr(A_F + 8));
+    C.launches += 2;
+    if (g.act[2]) {
+        Box bz = make_box(g, -1, g.n[0] + 1, -1, g.n[1] + 1, 0, g.n[2] + 1);
+        k_flux<2, LIM><<<grid_for(bz), 128, 0, s>>>(g, bz, V, bface + 2 * g.sa, arr(A_F + 16));
+        C.launches += 1;
+    }
+}
+
+// One Euler stage (Uin, bin) -> (Uout, bout); combine: out <- (out + Euler(in)) / 2 in place.
+void enqueue_stage(int in_u, int in_b, int out_u, int out_b, bool combine)
+{
+    const Grid &g = C.g;
+    cudaStream_t s = C.stream;
+    Box in = interior(g);
+    k_prim<<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_V), C.P);
+    C.launches += 1;
+    fill_ghosts(arr(A_V), 8);
+    fill_ghosts(arr(in_b), g.ndim);
+    if (g.limiter == 0) launch_flux<0>(arr(A_V), arr(in_b));
+    else                launch_flux<1>(arr(A_V), arr(in_b));
+    if (combine) k_update<true><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P);
+    else         k_update<false><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P);
+    C.launches += 1;
+    // edge EMFs on all edges touching interior faces (indices 0..n in the two transverse directions)
+    if (g.act[2]) {
+        Box ex = make_box(g, 0, g.n[0], 0, g.n[1] + 1, 0, g.n[2] + 1);
+        k_emf<0><<<grid_for(ex), 128, 0, s>>>(g, ex, arr(A_V), arr(A_F), arr(A_EG));
+        Box ey = make_box(g, 0, g.n[0] + 1, 0, g.n[1], 0, g.n[2] + 1);
+        k_emf<1><<<grid_for(ey), 128, 0, s>>>(g, ey, arr(A_V), arr(A_F), arr(A_EG));
+        C.launches += 2;
+    }
+    Box ez = make_box(g, 0, g.n[0] + 1, 0, g.n[1] + 1, 0, g.n[2]);
+    k_emf<2><<<grid_for(ez), 128, 0, s>>>(g, ez, arr(A_V), arr(A_F), arr(A_EG));
+    C.launches += 1;
+    // faces 0..n (the duplicate upper face is computed, not copied: same inputs, same bits)
+    Box fx = make_box(g, 0, g.n[0] + 1, 0, g.n[1], 0, g.n[2]);
+    Box fy = make_box(g, 0, g.n[0], 0, g.n[1] + 1, 0, g.n[2]);
+    if (combine) {
+        k_ctface<0, true><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P);
+        k_ctface<1, true><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P);
+    } else {
+        k_ctface<0, false><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P);
+        k_ctface<1, false><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P);
+    }
+    C.launches += 2;
+    if (g.act[2]) {
+        Box fz = make_box(g, 0, g.n[0], 0, g.n[1], 0, g.n[2] + 1);
+        if (combine) k_ctface<2, true><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P);
+        else         k_ctface<2, false><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P);
+        C.launches += 1;
+    }
+    k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(out_b), arr(out_u));
+    C.launches += 1;
+}
+
+void enqueue_dt(int mode)
+{
+    if (mode != 1) {
+        launch_dtmax(C.g, arr(A_UA), C.P, C.sm_count * 8, C.stream);
+        C.launches += 1;
+    }
+    launch_dtfinish(C.g, C.P, mode, C.stream);
+    C.launches += 1;
+}
+
+void enqueue_step(bool fixed)
+{
+    enqueue_dt(fixed ? 1 : 0);
+    enqueue_stage(A_UA, A_BA, A_UB, A_BB, false);    // S^1 = S^n + L(S^n)
+    enqueue_stage(A_UB, A_BB, A_UA, A_BA, true);     // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
+    launch_advance_time(C.P, C.stream);
+    C.launches += 1;
+}
+
+int run_steps(int nsteps, bool fixed)
+{
+    const int gi = fixed ? 1 : 0;
+    if (C.use_graph && !C.graph[gi] && nsteps > 0) {
+        long long before = C.launches;
+        cudaGraph_t graph = nullptr;
+        CUDA_TRY(cudaStreamBeginCapture(C.stream, cudaStreamCaptureModeThreadLocal));
+        enqueue_step(fixed);
+        cudaError_t e = cudaStreamEndCapture(C.stream, &graph);
+        if (e != cudaSuccess) return fail(PLUTO_ECUDA, "graph capture: %s", cudaGetErrorString(e));
+        e = cudaGraphInstantiate(&C.graph[gi], graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return fail(PLUTO_ECUDA, "graph instantiate: %s", cudaGetErrorString(e));
+        C.per_step[gi] = C.launches - before;
+        C.launches = before;                      // capture enqueued nothing
+    }
+    for (int s = 0; s < nsteps; s++) {
+        if (C.use_graph) {
+            CUDA_TRY(cudaGraphLaunch(C.graph[gi], C.stream));
+            C.launches += C.per_step[gi];
+        } else {
+            enqueue_step(fixed);
+        }
+    }
+    CUDA_TRY(cudaGetLastError());
+    if (nsteps > 0) C.stepped = true;
+    return PLUTO_OK;
+}
+
+int finish()
+{
+    CUDA_TRY(cudaStreamSynchronize(C.stream));
+    int err = 0;
+    CUDA_TRY(cudaMemcpy(&err, &C.P->err, sizeof(int), cudaMemcpyDeviceToHost));
+    if (err) return fail(PLUTO_EPHYS, "non-finite or non-positive density/pressure met");
+    return PLUTO_OK;
+}
+
+bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// extents of the caller's array for the face family d (d = -1: cell array)
+void api_extent(const Grid &g, int d, int m[3])
+{
+    for (int a = 0; a < 3; a++) m[a] = g.n[a] + (a == d ? 1 : 0);
+}
+
+size_t api_count(const Grid &g, int d)
+{
+    int m[3];
+    api_extent(g, d, m);
+    return (size_t)m[0] * m[1] * m[2];
+}
+
+// staging buffer: the flux work arrays are free outside a step (24 arrays >= 11 interior arrays)
+double *staging() { return arr(A_F); }
+
+int copy_in(const double *src, size_t count, double **dev)
+{
+    if (is_device_ptr(src)) { *dev = const_cast<double *>(src); return PLUTO_OK; }
+    if (count * sizeof(double) > (size_t)24 * C.g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
+    CUDA_TRY(cudaMemcpyAsync(staging(), src, count * sizeof(double), cudaMemcpyHostToDevice, C.stream));
+    *dev = staging();
+    return PLUTO_OK;
+}
+
+} // namespace
+
+// ================================================================== C ABI
+
+extern "C" {
+
+const char *pluto_last_error(void) { return C.err; }
+
+int pluto_device_count(void)
+{
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return n;
+}
+
+size_t pluto_workspace_bytes(int nx, int ny, int nz, int ghost)
+{
+    Grid g;
+    if (!make_grid(g, nx, ny, nz, ghost)) return 0;
+    return layout_bytes(g);
+}
+
+int pluto_set_workspace(void *dev, size_t bytes)
+{
+    if (C.init && !C.own_mem) return fail(PLUTO_ESTATE, "workspace in use: call pluto_finalize first");
+    if (dev && !is_device_ptr(dev)) return fail(PLUTO_EINVAL, "workspace is not device memory");
+    if (dev && ((size_t)dev & 255)) return fail(PLUTO_EINVAL, "workspace must be 256-byte aligned");
+    C.ws = dev;
+    C.ws_bytes = dev ? bytes : 0;
+    return PLUTO_OK;
+}
+
+int pluto_set_stream(void *cuda_stream)
+{
+    if (C.init) cudaStreamSynchronize(C.stream);
+    if (!cuda_stream) {
+        // the legacy default stream cannot be captured into a graph: use a stream of our own
+        if (!C.own_stream && pluto_device_count() > 0)
+            if (cudaStreamCreateWithFlags(&C.own_stream, cudaStreamNonBlocking) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(PLUTO_ECUDA, "cannot create a stream");
+            }
+        C.stream = C.own_stream;
+    } else {
+        C.stream = (cudaStream_t)cuda_stream;
+    }
+    destroy_graphs();
+    return PLUTO_OK;
+}
+
+int pluto_finalize(void)
+{
+    if (C.init) {
+        cudaStreamSynchronize(C.stream);
+        destroy_graphs();
+        if (C.own_mem && C.base) cudaFree(C.base);
+    }
+    C.base = nullptr; C.P = nullptr; C.init = false; C.have_state = false; C.stepped = false; C.own_mem = false;
+    return PLUTO_OK;
+}
+
+int pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter)
+{
+    if (pluto_device_count() < 1) return fail(PLUTO_ECUDA, "no CUDA device: this library has no CPU fallback");
+    pluto_finalize();
+    if (!C.stream) { int rc = pluto_set_stream(nullptr); if (rc) return rc; }
+    Grid g;
+    if (!make_grid(g, nx, ny, nz, ghost))
+        return fail(PLUTO_EINVAL, "need nx >= 2, ny >= 2, nz >= 1, 2 <= ghost <= %d, active extents >= ghost", XOFF);
+    if (!(gamma > 1.0) || !(cfl > 0.0) || (limiter != PLUTO_MINMOD && limiter != PLUTO_MC))
+        return fail(PLUTO_EINVAL, "need gamma > 1, cfl > 0, limiter in {0,1}");
+    if ((long long)g.tot[2] * 8 > 65535 || g.tot[1] > 65535)
+        return fail(PLUTO_EINVAL, "extent too large for the launch grid");
+    g.gamma = gamma; g.cfl = cfl; g.limiter = limiter;
+    for (int a = 0; a < 3; a++) { g.dx[a] = 1.0 / nx; g.idx[a] = 1.0 / g.dx[a]; }   // R11: Lx = 1, cubic cells
+    size_t bytes = layout_bytes(g);
+    if (C.ws) {
+        if (C.ws_bytes < bytes) return fail(PLUTO_ENOMEM, "workspace has %zu bytes, need %zu", C.ws_bytes, bytes);
+        C.base = (double *)C.ws;
+        C.own_mem = false;
+    } else {
+        cudaError_t e = cudaMalloc((void **)&C.base, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); C.base = nullptr; return fail(PLUTO_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); }
+        C.own_mem = true;
+    }
+    C.g = g;
+    C.P = (StepParams *)(C.base + (long long)A_COUNT * g.sa);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&C.sm_count, cudaDevAttrMultiProcessorCount, dev);
+    CUDA_TRY(cudaMemsetAsync(C.base, 0, bytes, C.stream));
+    CUDA_TRY(cudaStreamSynchronize(C.stream));
+    C.init = true; C.have_state = false; C.stepped = false; C.launches = 0;
+    return PLUTO_OK;
+}
+
+int pluto_set_box(double Lx, double Ly, double Lz)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    if (!(Lx > 0.0) || !(Ly > 0.0) || !(Lz > 0.0)) return fail(PLUTO_EINVAL, "box lengths must be positive");
+    double L[3] = { Lx, Ly, Lz };
+    for (int a = 0; a < 3; a++) { C.g.dx[a] = L[a] / C.g.n[a]; C.g.idx[a] = 1.0 / C.g.dx[a]; }
+    destroy_graphs();          // kernels take the grid by value: captured copies are stale
+    return PLUTO_OK;
+}
+
+int pluto_set_option(int opt, int value)
+{
+    if (opt == PLUTO_OPT_GRAPH) { int old = C.use_graph; C.use_graph = value ? 1 : 0; return old; }
+    return fail(PLUTO_EINVAL, "unknown option %d", opt);
+}
+
+int pluto_set_state(const double *U, const double *Bface)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    if (!U || !Bface) return fail(PLUTO_EINVAL, "null pointer");
+    const Grid &g = C.g;
+    cudaStream_t s = C.stream;
+    double *dev = nullptr;
+    int rc = copy_in(U, 8 * api_count(g, -1), &dev);
+    if (rc) return rc;
+    Box in = interior(g);
+    for (int v = 0; v < 8; v++)
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + (size_t)v * api_count(g, -1), g.n[0], g.n[1], arr(A_UA + v));
+    CUDA_TRY(cudaStreamSynchronize(s));       // staging is reused below
+    size_t nface = 0;
+    for (int d = 0; d < g.ndim; d++) nface += api_count(g, d);
+    rc = copy_in(Bface, nface, &dev);
+    if (rc) return rc;
+    size_t off = 0;
+    for (int d = 0; d < g.ndim; d++) {
+        int m[3];
+        api_extent(g, d, m);
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + off, m[0], m[1], arr(A_BA + d));   // upper duplicate ignored
+        off += api_count(g, d);
+    }
+    fill_ghosts(arr(A_BA), g.ndim);                            // face n <- face 0 for the cell mean
+    k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_BA), arr(A_UA));
+    StepParams p0;
+    memset(&p0, 0, sizeof p0);
+    CUDA_TRY(cudaMemcpyAsync(C.P, &p0, sizeof p0, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    CUDA_TRY(cudaGetLastError());
+    C.launches += 8 + g.ndim + 1;
+    C.have_state = true; C.stepped = false;
+    return PLUTO_OK;
+}
+
+int pluto_get_state(double *U, double *Bface)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    const Grid &g = C.g;
+    cudaStream_t s = C.stream;
+    if (U) {
+        size_t n = api_count(g, -1);
+        bool dev = is_device_ptr(U);
+        double *dst = dev ? U : staging();
+        Box in = interior(g);
+        for (int v = 0; v < 8; v++)
+            k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_UA + v), g.n[0], g.n[1], dst + (size_t)v * n);
+        if (!dev) CUDA_TRY(cudaMemcpyAsync(U, dst, 8 * n * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(cudaStreamSynchronize(s));
+        C.launches += 8;
+    }
+    if (Bface) {
+        bool dev = is_device_ptr(Bface);
+        double *dst = dev ? Bface : staging();
+        size_t off = 0;
+        for (int d = 0; d < g.ndim; d++) {
+            int m[3];
+            api_extent(g, d, m);
+            Box b = make_box(g, 0, m[0], 0, m[1], 0, m[2]);
+            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_BA + d), m[0], m[1], dst + off);
+            off += api_count(g, d);
+        }
+        if (!dev) CUDA_TRY(cudaMemcpyAsync(Bface, dst, off * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(cudaStreamSynchronize(s));
+        C.launches += g.ndim;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return PLUTO_OK;
+}
+
+int pluto_step_async(int nsteps)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (nsteps < 0) return fail(PLUTO_EINVAL, "nsteps < 0");
+    return run_steps(nsteps, false);
+}
+
+int pluto_sync(void)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    return finish();
+}
+
+int pluto_step(int nsteps)
+{
+    int rc = pluto_step_async(nsteps);
+    return rc ? rc : finish();
+}
+
+int pluto_step_fixed_dt(int nsteps, double dt)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (nsteps < 0 || !(dt > 0.0)) return fail(PLUTO_EINVAL, "need nsteps >= 0 and dt > 0");
+    CUDA_TRY(cudaMemcpyAsync(&C.P->dt_fixed, &dt, sizeof dt, cudaMemcpyHostToDevice, C.stream));
+    CUDA_TRY(cudaStreamSynchronize(C.stream));
+    int rc = run_steps(nsteps, true);
+    return rc ? rc : finish();
+}
+
+double pluto_get_dt(void)
+{
+    if (!C.init || !C.have_state) return NAN;
+    double dt = NAN;
+    if (!C.stepped) {
+        enqueue_dt(2);
+        if (cudaMemcpyAsync(&dt, &C.P->dt_probe, sizeof dt, cudaMemcpyDeviceToHost, C.stream) != cudaSuccess) return NAN;
+    } else {
+        if (cudaMemcpyAsync(&dt, &C.P->dt, sizeof dt, cudaMemcpyDeviceToHost, C.stream) != cudaSuccess) return NAN;
+    }
+    if (cudaStreamSynchronize(C.stream) != cudaSuccess) return NAN;
+    return dt;
+}
+
+double pluto_get_time(void)
+{
+    if (!C.init || !C.have_state) return NAN;
+    double t = NAN;
+    if (cudaMemcpyAsync(&t, &C.P->time, sizeof t, cudaMemcpyDeviceToHost, C.stream) != cudaSuccess) return NAN;
+    if (cudaStreamSynchronize(C.stream) != cudaSuccess) return NAN;
+    return t;
+}
+
+long long pluto_launch_count(void) { return C.launches; }
+
+int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem, double *Eedge)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (!(dt > 0.0)) return fail(PLUTO_EINVAL, "dt must be positive");
+    const Grid &g = C.g;
+    cudaStream_t s = C.stream;
+    CUDA_TRY(cudaMemcpyAsync(&C.P->dt_fixed, &dt, sizeof dt, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    // keep dt/time of the real run intact: save and restore the scalars
+    StepParams saved;
+    CUDA_TRY(cudaMemcpy(&saved, C.P, sizeof saved, cudaMemcpyDeviceToHost));
+    launch_dtfinish(g, C.P, 1, s);
+    enqueue_stage(A_UA, A_BA, A_UB, A_BB, false);
+    CUDA_TRY(cudaStreamSynchronize(s));
+    CUDA_TRY(cudaGetLastError());
+    const size_t n = api_count(g, -1);
+    double *tmp = nullptr;                      // private staging: the flux arrays are being read
+    size_t maxcount = 8 * n + 3 * (n + (size_t)g.n[0] * g.n[1] + (size_t)g.n[1] * g.n[2] + (size_t)g.n[0] * g.n[2]);
+    CUDA_TRY(cudaMalloc((void **)&tmp, maxcount * sizeof(double)));
+    Box in = interior(g);
+    auto emit = [&](double *user, size_t count) -> int {
+        if (is_device_ptr(user)) return cudaMemcpy(user, tmp, count * sizeof(double), cudaMemcpyDeviceToDevice) == cudaSuccess ? 0 : 1;
+        return cudaMemcpy(user, tmp, count * sizeof(double), cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : 1;
+    };
+    int bad = 0;
+    if (U1) {
+        for (int v = 0; v < 8; v++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_UB + v), g.n[0], g.n[1], tmp + v * n);
+        cudaStreamSynchronize(s);
+        bad |= emit(U1, 8 * n);
+    }
+    if (Bf1) {
+        size_t off = 0;
+        for (int d = 0; d < g.ndim; d++) {
+            int m[3];
+            api_extent(g, d, m);
+            Box b = make_box(g, 0, m[0], 0, m[1], 0, m[2]);
+            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_BB + d), m[0], m[1], tmp + off);
+            off += api_count(g, d);
+        }
+        cudaStreamSynchronize(s);
+        bad |= emit(Bf1, off);
+    }
+    if (W) {
+        cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
+        for (int d = 0; d < g.ndim; d++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_F + 8 * d + 7), g.n[0], g.n[1], tmp + d * n);
+        cudaStreamSynchronize(s);
+        bad |= emit(W, 3 * n);
+    }
+    if (Fem) {
+        cudaMemsetAsync(tmp, 0, 6 * n * sizeof(double), s);
+        for (int d = 0; d < g.ndim; d++)
+            for (int q = 0; q < 2; q++)
+                k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_F + 8 * d + 5 + q), g.n[0], g.n[1], tmp + (2 * d + q) * n);
+        cudaStreamSynchronize(s);
+        bad |= emit(Fem, 6 * n);
+    }
+    if (Eedge) {
+        cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
+        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_EG + e), g.n[0], g.n[1], tmp + e * n);
+        cudaStreamSynchronize(s);
+        bad |= emit(Eedge, 3 * n);
+    }
+    cudaFree(tmp);
+    int err = 0;
+    CUDA_TRY(cudaMemcpy(&err, &C.P->err, sizeof(int), cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(C.P, &saved, sizeof saved, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaGetLastError());
+    if (bad) return fail(PLUTO_ECUDA, "debug copy failed");
+    return err ? PLUTO_EPHYS : PLUTO_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,314 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are the north_star's: fp64 max relative error <= 1e-10 after
+one step, L1 relative error <= 1e-8 after 100 steps, dt bit-exact for identical input state (R15)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2511_20337_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_1STEP_MAXREL = 1e-10
+TOL_100STEP_L1REL = 1e-8
+
+
+def maxrel(a, b):
+    """per component: max|a-b| / max|b| (R15); components identically zero in the oracle: absolute"""
+    out = []
+    for v in range(a.shape[0]):
+        ref = np.abs(b[v]).max()
+        d = np.abs(a[v] - b[v]).max()
+        out.append(d / ref if ref > 0 else d / 1.0)
+    return max(out)
+
+
+def l1rel(a, b):
+    out = []
+    for v in range(a.shape[0]):
+        ref = np.abs(b[v]).sum()
+        d = np.abs(a[v] - b[v]).sum()
+        out.append(d / ref if ref > 0 else d)
+    return max(out)
+
+
+def faces_as_components(Bf, w):
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    return [f[k].ravel() for k in sorted(f)]
+
+
+def compare_state(pl, orc, w, tol, norm=maxrel):
+    Ug, Bg = pl.get_state()
+    Uo, Bo = orc.get_state()
+    e_u = norm(Ug.reshape(8, -1), Uo.reshape(8, -1))
+    fg, fo = faces_as_components(Bg, w), faces_as_components(Bo, w)
+    e_b = max(norm(a[None], b[None]) for a, b in zip(fg, fo))
+    assert e_u <= tol and e_b <= tol, (e_u, e_b)
+    return e_u, e_b
+
+
+SMALL = [
+    ("2d_ragged_minmod", lambda: wl.random_smooth(37, 23, 1, seed=2, limiter=0, box=(1.0, 0.7, 1.0))),
+    ("2d_ragged_mc", lambda: wl.random_smooth(150, 21, 1, seed=4, limiter=1)),
+    ("3d_ragged_minmod", lambda: wl.random_smooth(19, 13, 11, seed=3, limiter=0, box=(1.0, 0.8, 1.1))),
+    ("3d_ragged_mc", lambda: wl.random_smooth(33, 9, 14, seed=5, limiter=1)),
+    ("3d_tiny", lambda: wl.random_smooth(2, 2, 2, seed=6)),
+    ("2d_tiny", lambda: wl.random_smooth(2, 3, 1, seed=7)),
+    ("blast_24", lambda: wl.blast_3d(24)),
+    ("ot_48", lambda: wl.orszag_tang_2d(48)),
+]
+
+
+@pytest.mark.parametrize("name,make", SMALL, ids=[s[0] for s in SMALL])
+def test_dt_is_bit_exact(pluto, oracle, name, make):
+    w = make()
+    pluto.load(w)
+    oracle.load(w)
+    assert pluto.get_dt() == oracle.get_dt()
+
+
+@pytest.mark.parametrize("name,make", SMALL, ids=[s[0] for s in SMALL])
+def test_euler_stage_pieces(pluto, oracle, name, make):
+    """per-kernel parity: upwind weights and induction fluxes (recon + HLLD), edge EMFs (CT average),
+    then the stage output (flux-difference update, face update, cell-B mean)"""
+    w = make()
+    pluto.load(w)
+    oracle.load(w)
+    dt = oracle.get_dt()
+    g = pluto.debug_euler(dt)
+    o = oracle.debug_euler(dt)
+    assert g["rc"] == 0 and o["rc"] == 0
+    nd = 3 if w.nz > 1 else 2
+    # induction fluxes kept for CT: d = x: (F_x[By], F_x[Bz]); y: (F_y[Bz], F_y[Bx]); z: (F_z[Bx], F_z[By])
+    scale = np.abs(o["F"]).max()
+    for d in range(nd):
+        t1, t2 = (d + 1) % 3, (d + 2) % 3
+        assert np.abs(g["Fem"][d, 0] - o["F"][d, 4 + t1]).max() <= 1e-12 * scale, d
+        assert np.abs(g["Fem"][d, 1] - o["F"][d, 4 + t2]).max() <= 1e-12 * scale, d
+        assert np.abs(g["W"][d] - o["W"][d]).max() <= 1e-9, d
+    for e in range(3):
+        assert np.abs(g["E"][e] - o["E"][e]).max() <= 1e-12 * max(np.abs(o["E"]).max(), 1e-300), e
+    assert maxrel(g["U1"].reshape(8, -1), o["U1"].reshape(8, -1)) <= 1e-12
+    assert maxrel(g["Bf1"][None], o["Bf1"][None]) <= 1e-12
+
+
+@pytest.mark.parametrize("name,make", SMALL, ids=[s[0] for s in SMALL])
+def test_one_step_max_rel(pluto, oracle, name, make):
+    w = make()
+    pluto.load(w)
+    oracle.load(w)
+    pluto.step(1)
+    assert oracle.step(1) == 0
+    assert pluto.get_dt() == oracle.get_dt()
+    assert abs(pluto.get_time() - oracle.get_time()) <= 1e-15
+    compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+
+
+def test_config0_100_steps(pluto, oracle):
+    """BASELINE.json configs[0]: 2D Orszag-Tang 128^2, minmod, CFL 0.4, 100 steps"""
+    w = wl.config(0)
+    pluto.load(w)
+    oracle.load(w)
+    assert pluto.get_dt() == oracle.get_dt()
+    pluto.step(1)
+    oracle.step(1)
+    compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+    pluto.step(99)
+    assert oracle.step(99) == 0
+    compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+    assert abs(pluto.get_time() - oracle.get_time()) <= 1e-12
+    # invariants on the GPU result itself
+    U, Bf = pluto.get_state()
+    for v in (0, 7):
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * abs(math.fsum(w.U[v].ravel()))
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    div = (f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) * w.nx + (f["by"][:, 1:, :] - f["by"][:, :-1, :]) * w.ny
+    assert np.abs(div).max() / w.nx <= 1e-12 * np.abs(Bf).max()
+    assert np.array_equal(f["bx"][:, :, 0], f["bx"][:, :, -1]) and np.array_equal(f["by"][:, 0, :], f["by"][:, -1, :])
+
+
+def _run_period(sim, w):
+    t, n = 0.0, 0
+    while True:
+        U, Bf = sim.get_state()
+        sim.set_state(U, Bf)                    # get_dt then returns the CFL dt of this state
+        dt = sim.get_dt()
+        if t + dt < w.t_end:
+            sim.step_fixed_dt(1, dt)
+            t += dt
+            n += 1
+        else:
+            sim.step_fixed_dt(1, w.t_end - t)
+            return n + 1
+
+
+def test_config1_one_period(pluto, oracle):
+    """configs[1]: oblique CP Alfven wave 64x32x32, MC, CFL 0.4, one period; L1 error vs exact"""
+    w = wl.config(1)
+    pluto.load(w)
+    oracle.load(w)
+    assert pluto.get_dt() == oracle.get_dt()
+    ng = _run_period(pluto, w)
+    no = _run_period(oracle, w)
+    assert ng == no
+    compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+    Ug, _ = pluto.get_state()
+    Uo, _ = oracle.get_state()
+    eg = math.sqrt(sum(np.abs(Ug[4 + s] - w.U[4 + s]).mean() ** 2 for s in range(3)))
+    eo = math.sqrt(sum(np.abs(Uo[4 + s] - w.U[4 + s]).mean() ** 2 for s in range(3)))
+    assert abs(eg - eo) <= 1e-9 and eg < 4e-3       # error vs the exact solution (the initial state)
+
+
+def test_cfl_steps_100_3d(pluto, oracle):
+    w = wl.blast_3d(32)
+    pluto.load(w)
+    oracle.load(w)
+    pluto.step(100)
+    assert oracle.step(100) == 0
+    compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+
+
+def _subbox_parity(pluto, oracle, w, centres, half=12, margin=7):
+    """sampled parity at full size: the step has a finite stencil (3 cells per stage, 6 per RK2 step),
+    so the oracle run on a periodic copy of a (2*half)^d sub-box with the GPU's dt reproduces the full
+    run in the sub-box's core (distance > margin from its boundary)."""
+    nd = w.ndim
+    pluto.load(w)
+    dt = pluto.get_dt()
+    pluto.step(1)
+    assert pluto.get_dt() == dt
+    Ug, Bg = pluto.get_state()
+    fg = wl.split_faces(Bg, w.nx, w.ny, w.nz)
+    f0 = wl.split_faces(w.Bface, w.nx, w.ny, w.nz)
+    worst = 0.0
+    # momentum can be pure round-off noise in a quiet sub-box (v = 0 background of the blast): floor its
+    # scale with rho * c_f of the initial data, an a-priori magnitude that does not come from either side
+    rho, B2 = w.U[0], w.U[4] ** 2 + w.U[5] ** 2 + w.U[6] ** 2
+    p0 = (w.gamma - 1) * (w.U[7] - 0.5 * (w.U[1] ** 2 + w.U[2] ** 2 + w.U[3] ** 2) / rho - 0.5 * B2)
+    mscale = float(rho.max() * np.sqrt((w.gamma * p0.max() + B2.max()) / rho.min()))
+    floor = {1: mscale, 2: mscale, 3: mscale}
+    for (ci, cj, ck) in centres:
+        ix = (np.arange(ci - half, ci + half)) % w.nx
+        iy = (np.arange(cj - half, cj + half)) % w.ny
+        iz = (np.arange(ck - half, ck + half)) % w.nz if nd == 3 else np.array([0])
+        sub = lambda a: a[np.ix_(iz, iy, ix)]
+        n = 2 * half
+        Us = np.stack([sub(w.U[v]) for v in range(8)])
+        faces = {}
+        for name in ("bx", "by", "bz")[:nd]:
+            a = f0[name]
+            core = sub(a[:w.nz, :w.ny, :w.nx])                  # lower faces of the sub-box cells
+            ax = {"bx": 2, "by": 1, "bz": 0}[name]
+            faces[name] = np.concatenate([core, np.take(core, [0], axis=ax)], axis=ax)
+        nzs = n if nd == 3 else 1
+        assert oracle.init(n, n, nzs, 2, w.gamma, w.cfl, w.limiter) == 0
+        oracle.set_box(n * w.box[0] / w.nx, n * w.box[1] / w.ny, (n * w.box[2] / w.nz) if nd == 3 else 1.0)
+        oracle.set_state(Us, wl.join_faces(faces, n, n, nzs))
+        assert oracle.step_fixed_dt(1, dt) == 0
+        Uo, Bo = oracle.get_state()
+        fo = wl.split_faces(Bo, n, n, nzs)
+        c = slice(margin, n - margin)
+        cz = c if nd == 3 else slice(0, 1)
+        for v in range(8):
+            ref = max(np.abs(Uo[v]).max(), floor.get(v, 0.0))
+            d = np.abs(sub(Ug[v])[cz, c, c] - Uo[v][cz, c, c]).max()
+            worst = max(worst, d / ref if ref > 0 else d)
+        for name in ("bx", "by", "bz")[:nd]:
+            d = np.abs(sub(fg[name][:w.nz, :w.ny, :w.nx])[cz, c, c] - fo[name][:nzs, :n, :n][cz, c, c]).max()
+            worst = max(worst, d / np.abs(fo[name]).max())
+    assert worst <= TOL_1STEP_MAXREL, worst
+    return Ug, Bg
+
+
+def test_config2_full_size_sampled(pluto, oracle):
+    """configs[2]: 2D Orszag-Tang 2048^2 at full size; sub-box parity + invariants"""
+    w = wl.config(2)
+    rng = np.random.default_rng(0)
+    centres = [(int(rng.integers(0, w.nx)), int(rng.integers(0, w.ny)), 0) for _ in range(6)] + [(0, 0, 0), (w.nx - 1, 5, 0)]
+    U, Bf = _subbox_parity(pluto, oracle, w, centres)
+    for v in (0, 7):
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * abs(math.fsum(w.U[v].ravel()))
+
+
+def test_config3_full_size_sampled(pluto, oracle):
+    """configs[3]: 3D blast 256^3 at full size; sub-boxes on the blast edge, at the corners, and random"""
+    w = wl.config(3)
+    r = int(0.1 * w.nx)
+    h = w.nx // 2
+    centres = [(h + r, h, h), (h, h - r, h), (h, h, h + r), (h, h, h), (0, 0, 0), (w.nx - 1, 3, w.nz - 2), (40, 200, 77)]
+    U, Bf = _subbox_parity(pluto, oracle, w, centres)
+    for v in (0, 7):
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * abs(math.fsum(w.U[v].ravel()))
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    div = ((f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) + (f["by"][:, 1:, :] - f["by"][:, :-1, :])
+           + (f["bz"][1:, :, :] - f["bz"][:-1, :, :]))
+    assert np.abs(div).max() <= 1e-12 * np.abs(Bf).max()
+
+
+def test_device_pointers_and_graph_equivalence(pluto, oracle):
+    """set/get with CUDA tensors; graph replay and plain launches give identical bits"""
+    import torch
+    from paper_2511_20337_b200 import binding
+    w = wl.random_smooth(40, 24, 12, seed=9)
+    pluto.load(w)
+    pluto.step(3)
+    U_a, B_a = pluto.get_state()
+    old = pluto.set_option(binding.OPT_GRAPH, 0)
+    assert old == 1
+    pluto.init(w.nx, w.ny, w.nz, 2, w.gamma, w.cfl, w.limiter)
+    pluto.set_box(*w.box)
+    pluto.set_state(torch.from_numpy(w.U).cuda(), torch.from_numpy(w.Bface).cuda())
+    pluto.step(3)
+    U_d, B_d = pluto.get_state(device=True)
+    pluto.set_option(binding.OPT_GRAPH, 1)
+    assert np.array_equal(U_d.cpu().numpy(), U_a) and np.array_equal(B_d.cpu().numpy(), B_a)
+    assert pluto.launch_count() > 0
+
+
+def test_ghost_layers_do_not_change_the_result(pluto):
+    w = wl.random_smooth(20, 18, 16, seed=12)
+    pluto.load(w, ghost=2)
+    pluto.step(2)
+    Ua, Ba = pluto.get_state()
+    pluto.load(w, ghost=4)
+    pluto.step(2)
+    Ub, Bb = pluto.get_state()
+    assert np.array_equal(Ua, Ub) and np.array_equal(Ba, Bb)
+
+
+def test_error_codes(pluto):
+    from paper_2511_20337_b200 import binding
+    with pytest.raises(binding.PlutoError) as e:
+        pluto.init(16, 16, 1, 1)
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.PlutoError) as e:
+        pluto.init(16, 16, 1, 2, gamma=1.0)
+    assert e.value.code == binding.EINVAL
+    w = wl.random_smooth(16, 16, 1, seed=1)
+    pluto.load(w)
+    with pytest.raises(binding.PlutoError) as e:
+        pluto.step_fixed_dt(1, -1.0)
+    assert e.value.code == binding.EINVAL
+    U = w.U.copy()
+    U[7, 0, 3, 3] = -5.0                           # negative pressure
+    pluto.set_state(U, w.Bface)
+    with pytest.raises(binding.PlutoError) as e:
+        pluto.step(1)
+    assert e.value.code == binding.EPHYS
+    pluto.set_state(w.U, w.Bface)                   # a fresh state clears the flag
+    pluto.step(1)
+
+
+def test_uniform_state_is_a_fixed_point(pluto):
+    nx, ny, nz = 12, 10, 8
+    shp = (nz, ny, nx)
+    v, B = (0.4, -0.3, 0.2), (0.5, 0.8, -0.6)
+    U = wl.conserved_from_fields(np.full(shp, 1.3), [np.full(shp, x) for x in v], [np.full(shp, x) for x in B],
+                                 np.full(shp, 0.7), 5.0 / 3.0)
+    Bf = wl.join_faces({nm: np.full(s, B["xyz".index(nm[1])]) for nm, s in wl.face_shapes(nx, ny, nz)}, nx, ny, nz)
+    pluto.init(nx, ny, nz, 2, 5.0 / 3.0, 0.3, 0)
+    pluto.set_state(U, Bf)
+    pluto.step(3)
+    U1, Bf1 = pluto.get_state()
+    assert np.abs(U1 - U).max() <= 1e-15 and np.abs(Bf1 - Bf).max() <= 1e-15
