@@ -88,6 +88,18 @@ int    pluto_sync(void);
 /* Number of kernel launches enqueued by this library since pluto_init (for bench.py's gpu_launches). */
 long long pluto_launch_count(void);
 
+/* Per-kernel device timing with CUDA events on the launching stream (for bench.py's roofline).
+ * pluto_profile(1) starts (plain launches, every launch bracketed by an event pair), pluto_profile(0)
+ * stops.  pluto_profile_get returns the accumulated time and launch count of kernel class `kernel`
+ * (0 <= kernel, pluto_kernel_name(kernel) != NULL). */
+int    pluto_profile(int on);
+int    pluto_profile_get(int kernel, double *total_ms, long long *launches);
+const char *pluto_kernel_name(int kernel);
+
+/* Measured fp64 FMA throughput of the device in GFLOP/s (2 flops per DFMA): a register-resident
+ * DFMA loop on every SM, timed with CUDA events.  The denominator of the "alu" roofline. */
+double pluto_probe_fp64_gflops(void);
+
 /* Tuning switches: opt = PLUTO_OPT_*, returns the previous value or PLUTO_EINVAL. */
 enum {
     PLUTO_OPT_GRAPH = 1    /* 1 (default): replay one captured CUDA graph per step; 0: plain launches */

@@ -24,7 +24,8 @@ SYMBOLS = [
     "pluto_set_box", "pluto_step_fixed_dt", "pluto_get_time", "pluto_set_stream",
     "pluto_workspace_bytes", "pluto_set_workspace", "pluto_finalize", "pluto_last_error",
     "pluto_device_count", "pluto_step_async", "pluto_sync", "pluto_launch_count",
-    "pluto_set_option", "pluto_debug_euler",
+    "pluto_set_option", "pluto_debug_euler", "pluto_profile", "pluto_profile_get", "pluto_kernel_name",
+    "pluto_probe_fp64_gflops",
 ]
 
 
@@ -60,6 +61,11 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pluto_launch_count.restype = C.c_longlong
     L.pluto_set_option.argtypes = [i32, i32]
     L.pluto_debug_euler.argtypes = [dbl, vp, vp, vp, vp, vp]
+    L.pluto_profile.argtypes = [i32]
+    L.pluto_profile_get.argtypes = [i32, C.POINTER(dbl), C.POINTER(C.c_longlong)]
+    L.pluto_kernel_name.argtypes = [i32]
+    L.pluto_kernel_name.restype = C.c_char_p
+    L.pluto_probe_fp64_gflops.restype = dbl
     return L
 
 
@@ -163,6 +169,24 @@ class Pluto:
 
     def set_option(self, opt, value):
         return self.L.pluto_set_option(opt, value)
+
+    def profile(self, on):
+        return self._check(self.L.pluto_profile(1 if on else 0))
+
+    def profile_report(self):
+        """{kernel name: (total ms, launches)} accumulated since profile(True)"""
+        out, k = {}, 0
+        while True:
+            name = self.L.pluto_kernel_name(k)
+            if name is None:
+                return out
+            ms, cnt = C.c_double(0.0), C.c_longlong(0)
+            self._check(self.L.pluto_profile_get(k, C.byref(ms), C.byref(cnt)))
+            out[name.decode()] = (ms.value, cnt.value)
+            k += 1
+
+    def probe_fp64_gflops(self):
+        return self.L.pluto_probe_fp64_gflops()
 
     def finalize(self):
         return self.L.pluto_finalize()

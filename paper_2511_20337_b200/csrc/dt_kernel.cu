@@ -81,3 +81,49 @@ void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s)
 void launch_advance_time(StepParams *P, cudaStream_t s) { k_advance_time<<<1, 1, 0, s>>>(P); }
 
 } // namespace pluto
+
+// ---------------------------------------------------------------- fp64 peak probe
+// 8 independent DFMA chains per thread, no memory traffic: measures what the fp64 pipe sustains.
+// (In this -fmad=false unit the FMAs are written explicitly with fma().)
+namespace pluto {
+
+__global__ void __launch_bounds__(256) k_fp64_probe(double *out, int iters, double seed)
+{
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-6;
+    for (int i = 0; i < iters; i++) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 123.456) out[0] = r;     // never true: keeps the loop alive
+}
+
+double probe_fp64_gflops(cudaStream_t s)
+{
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    double *out = nullptr;
+    if (cudaMalloc((void **)&out, 8) != cudaSuccess) return NAN;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 20000, blocks = sms * 8, threads = 256;
+    k_fp64_probe<<<blocks, threads, 0, s>>>(out, 2000, 1.0);          // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 5; rep++) {
+        cudaEventRecord(e0, s);
+        k_fp64_probe<<<blocks, threads, 0, s>>>(out, iters, 1.0);
+        cudaEventRecord(e1, s);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double gf = 2.0 * 8.0 * iters * (double)blocks * threads / (ms * 1e-3) * 1e-9;
+        if (gf > best) best = gf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    return cudaGetLastError() == cudaSuccess ? best : NAN;
+}
+
+} // namespace pluto

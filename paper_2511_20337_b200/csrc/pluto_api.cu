@@ -7,16 +7,24 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <vector>
 
 namespace pluto {
 void launch_dtmax(const Grid &g, const double *U, StepParams *P, int nblocks, cudaStream_t s);
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s);
 void launch_advance_time(StepParams *P, cudaStream_t s);
+double probe_fp64_gflops(cudaStream_t s);
 }
 
 using namespace pluto;
 
 namespace {
+
+enum KernelId { K_GHOST = 0, K_PRIM, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_UPDATE, K_EMF, K_CTFACE, K_CELLB,
+                K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
+const char *const kKernelNames[K_COUNT] = { "ghost_fill", "cons2prim", "plm_hlld_x", "plm_hlld_y", "plm_hlld_z",
+                                            "flux_update", "ct_edge_emf", "ct_face_update", "cell_b_mean",
+                                            "dt_max", "scalars", "pack_unpack" };
 
 struct Context {
     bool init = false;
@@ -36,6 +44,13 @@ struct Context {
     cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step
     int sm_count = 148;
     char err[512] = "";
+    // per-kernel CUDA-event timing (pluto_profile)
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_ev;    // pairs (start, stop)
+    std::vector<int> prof_kid;
+    size_t prof_used = 0;
+    double prof_ms[K_COUNT] = {};
+    long long prof_cnt[K_COUNT] = {};
 };
 
 Context C;
@@ -54,6 +69,38 @@ int fail(int code, const char *fmt, ...)
         cudaError_t e_ = (x);                                                                    \
         if (e_ != cudaSuccess) return fail(PLUTO_ECUDA, "%s: %s", #x, cudaGetErrorString(e_));   \
     } while (0)
+
+void prof_flush()
+{
+    if (!C.prof_used) return;
+    cudaStreamSynchronize(C.stream);
+    for (size_t n = 0; n < C.prof_used; n++) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, C.prof_ev[2 * n], C.prof_ev[2 * n + 1]) == cudaSuccess) {
+            C.prof_ms[C.prof_kid[n]] += ms;
+            C.prof_cnt[C.prof_kid[n]] += 1;
+        }
+    }
+    C.prof_used = 0;
+}
+
+// bracket one launch: counts it and, in profile mode, records an event pair on the launching stream
+struct Launch {
+    bool timed = false;
+    size_t slot = 0;
+    explicit Launch(int kid)
+    {
+        C.launches += 1;
+        if (!C.prof_on) return;
+        if (2 * (C.prof_used + 1) > C.prof_ev.size()) prof_flush();
+        slot = C.prof_used++;
+        C.prof_kid[slot] = kid;
+        cudaEventRecord(C.prof_ev[2 * slot], C.stream);
+        timed = true;
+    }
+    ~Launch() { if (timed) cudaEventRecord(C.prof_ev[2 * slot + 1], C.stream); }
+};
+#define LAUNCH(kid, ...) do { Launch l_(kid); __VA_ARGS__; } while (0)
 
 double *arr(int id) { return C.base + (long long)id * C.g.sa; }
 
@@ -91,13 +138,10 @@ void fill_ghosts(double *first, int narr)
     const Grid &g = C.g;
     const int ngh = 2 * g.ng + 1;
     cudaStream_t s = C.stream;
-    k_ghost<0><<<dim3(1, g.tot[1], g.tot[2] * narr), 64, 0, s>>>(g, first, narr);
-    k_ghost<1><<<dim3((g.tot[0] + 127) / 128, ngh, g.tot[2] * narr), 128, 0, s>>>(g, first, narr);
-    C.launches += 2;
-    if (g.act[2]) {
-        k_ghost<2><<<dim3((g.tot[0] + 127) / 128, g.tot[1], ngh * narr), 128, 0, s>>>(g, first, narr);
-        C.launches += 1;
-    }
+    LAUNCH(K_GHOST, k_ghost<0><<<dim3(1, g.tot[1], g.tot[2] * narr), 64, 0, s>>>(g, first, narr));
+    LAUNCH(K_GHOST, k_ghost<1><<<dim3((g.tot[0] + 127) / 128, ngh, g.tot[2] * narr), 128, 0, s>>>(g, first, narr));
+    if (g.act[2])
+        LAUNCH(K_GHOST, k_ghost<2><<<dim3((g.tot[0] + 127) / 128, g.tot[1], ngh * narr), 128, 0, s>>>(g, first, narr));
 }
 
 template <int LIM>
@@ -107,14 +151,12 @@ void launch_flux(const double *V, const double *bface)
     cudaStream_t s = C.stream;
     // faces 0..n along the sweep, one ghost layer across it (CT needs the transverse neighbours)
     Box bx = make_box(g, 0, g.n[0] + 1, -1, g.n[1] + 1, -1, g.n[2] + 1);
-    k_flux<0, LIM><<<grid_for(bx), 128, 0, s>>>(g, bx, V, bface + 0 * g.sa, arr(A_F + 0));
+    LAUNCH(K_FLUX_X, k_flux<0, LIM><<<grid_for(bx), 128, 0, s>>>(g, bx, V, bface + 0 * g.sa, arr(A_F + 0)));
     Box by = make_box(g, -1, g.n[0] + 1, 0, g.n[1] + 1, -1, g.n[2] + 1);
-    k_flux<1, LIM><<<grid_for(by), 128, 0, s>>>(g, by, V, bface + 1 * g.sa, arr(A_F + 8));
-    C.launches += 2;
+    LAUNCH(K_FLUX_Y, k_flux<1, LIM><<<grid_for(by), 128, 0, s>>>(g, by, V, bface + 1 * g.sa, arr(A_F + 8)));
     if (g.act[2]) {
         Box bz = make_box(g, -1, g.n[0] + 1, -1, g.n[1] + 1, 0, g.n[2] + 1);
-        k_flux<2, LIM><<<grid_for(bz), 128, 0, s>>>(g, bz, V, bface + 2 * g.sa, arr(A_F + 16));
-        C.launches += 1;
+        LAUNCH(K_FLUX_Z, k_flux<2, LIM><<<grid_for(bz), 128, 0, s>>>(g, bz, V, bface + 2 * g.sa, arr(A_F + 16)));
     }
 }
 
@@ -124,55 +166,42 @@ void enqueue_stage(int in_u, int in_b, int out_u, int out_b, bool combine)
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
     Box in = interior(g);
-    k_prim<<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_V), C.P);
-    C.launches += 1;
+    LAUNCH(K_PRIM, k_prim<<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_V), C.P));
     fill_ghosts(arr(A_V), 8);
     fill_ghosts(arr(in_b), g.ndim);
     if (g.limiter == 0) launch_flux<0>(arr(A_V), arr(in_b));
     else                launch_flux<1>(arr(A_V), arr(in_b));
-    if (combine) k_update<true><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P);
-    else         k_update<false><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P);
-    C.launches += 1;
+    if (combine) LAUNCH(K_UPDATE, k_update<true><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P));
+    else         LAUNCH(K_UPDATE, k_update<false><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P));
     // edge EMFs on all edges touching interior faces (indices 0..n in the two transverse directions)
     if (g.act[2]) {
         Box ex = make_box(g, 0, g.n[0], 0, g.n[1] + 1, 0, g.n[2] + 1);
-        k_emf<0><<<grid_for(ex), 128, 0, s>>>(g, ex, arr(A_V), arr(A_F), arr(A_EG));
+        LAUNCH(K_EMF, k_emf<0><<<grid_for(ex), 128, 0, s>>>(g, ex, arr(A_V), arr(A_F), arr(A_EG)));
         Box ey = make_box(g, 0, g.n[0] + 1, 0, g.n[1], 0, g.n[2] + 1);
-        k_emf<1><<<grid_for(ey), 128, 0, s>>>(g, ey, arr(A_V), arr(A_F), arr(A_EG));
-        C.launches += 2;
+        LAUNCH(K_EMF, k_emf<1><<<grid_for(ey), 128, 0, s>>>(g, ey, arr(A_V), arr(A_F), arr(A_EG)));
     }
     Box ez = make_box(g, 0, g.n[0] + 1, 0, g.n[1] + 1, 0, g.n[2]);
-    k_emf<2><<<grid_for(ez), 128, 0, s>>>(g, ez, arr(A_V), arr(A_F), arr(A_EG));
-    C.launches += 1;
+    LAUNCH(K_EMF, k_emf<2><<<grid_for(ez), 128, 0, s>>>(g, ez, arr(A_V), arr(A_F), arr(A_EG)));
     // faces 0..n (the duplicate upper face is computed, not copied: same inputs, same bits)
     Box fx = make_box(g, 0, g.n[0] + 1, 0, g.n[1], 0, g.n[2]);
     Box fy = make_box(g, 0, g.n[0], 0, g.n[1] + 1, 0, g.n[2]);
+    Box fz = make_box(g, 0, g.n[0], 0, g.n[1], 0, g.n[2] + 1);
     if (combine) {
-        k_ctface<0, true><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P);
-        k_ctface<1, true><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P);
+        LAUNCH(K_CTFACE, k_ctface<0, true><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P));
+        LAUNCH(K_CTFACE, k_ctface<1, true><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P));
+        if (g.act[2]) LAUNCH(K_CTFACE, k_ctface<2, true><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P));
     } else {
-        k_ctface<0, false><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P);
-        k_ctface<1, false><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P);
+        LAUNCH(K_CTFACE, k_ctface<0, false><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P));
+        LAUNCH(K_CTFACE, k_ctface<1, false><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P));
+        if (g.act[2]) LAUNCH(K_CTFACE, k_ctface<2, false><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P));
     }
-    C.launches += 2;
-    if (g.act[2]) {
-        Box fz = make_box(g, 0, g.n[0], 0, g.n[1], 0, g.n[2] + 1);
-        if (combine) k_ctface<2, true><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P);
-        else         k_ctface<2, false><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P);
-        C.launches += 1;
-    }
-    k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(out_b), arr(out_u));
-    C.launches += 1;
+    LAUNCH(K_CELLB, k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(out_b), arr(out_u)));
 }
 
 void enqueue_dt(int mode)
 {
-    if (mode != 1) {
-        launch_dtmax(C.g, arr(A_UA), C.P, C.sm_count * 8, C.stream);
-        C.launches += 1;
-    }
-    launch_dtfinish(C.g, C.P, mode, C.stream);
-    C.launches += 1;
+    if (mode != 1) LAUNCH(K_DTMAX, launch_dtmax(C.g, arr(A_UA), C.P, C.sm_count * 8, C.stream));
+    LAUNCH(K_SCALAR, launch_dtfinish(C.g, C.P, mode, C.stream));
 }
 
 void enqueue_step(bool fixed)
@@ -180,14 +209,14 @@ void enqueue_step(bool fixed)
     enqueue_dt(fixed ? 1 : 0);
     enqueue_stage(A_UA, A_BA, A_UB, A_BB, false);    // S^1 = S^n + L(S^n)
     enqueue_stage(A_UB, A_BB, A_UA, A_BA, true);     // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
-    launch_advance_time(C.P, C.stream);
-    C.launches += 1;
+    LAUNCH(K_SCALAR, launch_advance_time(C.P, C.stream));
 }
 
 int run_steps(int nsteps, bool fixed)
 {
     const int gi = fixed ? 1 : 0;
-    if (C.use_graph && !C.graph[gi] && nsteps > 0) {
+    const bool graph = C.use_graph && !C.prof_on;
+    if (graph && !C.graph[gi] && nsteps > 0) {
         long long before = C.launches;
         cudaGraph_t graph = nullptr;
         CUDA_TRY(cudaStreamBeginCapture(C.stream, cudaStreamCaptureModeThreadLocal));
@@ -201,7 +230,7 @@ int run_steps(int nsteps, bool fixed)
         C.launches = before;                      // capture enqueued nothing
     }
     for (int s = 0; s < nsteps; s++) {
-        if (C.use_graph) {
+        if (graph) {
             CUDA_TRY(cudaGraphLaunch(C.graph[gi], C.stream));
             C.launches += C.per_step[gi];
         } else {
@@ -490,6 +519,48 @@ double pluto_get_time(void)
 }
 
 long long pluto_launch_count(void) { return C.launches; }
+
+int pluto_profile(int on)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    if (on) {
+        const size_t pairs = 8192;
+        while (C.prof_ev.size() < 2 * pairs) {
+            cudaEvent_t e;
+            CUDA_TRY(cudaEventCreate(&e));
+            C.prof_ev.push_back(e);
+        }
+        C.prof_kid.assign(pairs, 0);
+        CUDA_TRY(cudaStreamSynchronize(C.stream));
+        C.prof_used = 0;
+        for (int k = 0; k < K_COUNT; k++) { C.prof_ms[k] = 0.0; C.prof_cnt[k] = 0; }
+        C.prof_on = true;
+    } else if (C.prof_on) {
+        prof_flush();
+        C.prof_on = false;
+    }
+    return PLUTO_OK;
+}
+
+int pluto_profile_get(int kernel, double *total_ms, long long *launches)
+{
+    if (kernel < 0 || kernel >= K_COUNT) return fail(PLUTO_EINVAL, "kernel id out of range");
+    if (C.prof_on) prof_flush();
+    if (total_ms) *total_ms = C.prof_ms[kernel];
+    if (launches) *launches = C.prof_cnt[kernel];
+    return PLUTO_OK;
+}
+
+const char *pluto_kernel_name(int kernel)
+{
+    return (kernel < 0 || kernel >= K_COUNT) ? nullptr : kKernelNames[kernel];
+}
+
+double pluto_probe_fp64_gflops(void)
+{
+    if (pluto_device_count() < 1) { fail(PLUTO_ECUDA, "no CUDA device"); return NAN; }
+    return pluto::probe_fp64_gflops(C.stream);
+}
 
 int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem, double *Eedge)
 {
