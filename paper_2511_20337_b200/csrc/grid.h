@@ -23,6 +23,7 @@ struct Grid {
     double dx[3];
     double idx[3];     // 1 / dx
     double gamma;
+    double igm1;       // 1 / (gamma - 1)
     double cfl;
     int limiter;
     int ndim;
@@ -66,16 +67,14 @@ inline bool make_grid(Grid &g, int nx, int ny, int nz, int ghost)
     return true;
 }
 
-// array ids inside the single allocation
+// array ids inside the single allocation (a state = 8 cell variables + 3 face fields, contiguous)
 enum ArrayId {
     A_UA = 0,        // 8: state S^n (and S^{n+1})
-    A_UB = 8,        // 8: stage state S^1
-    A_BA = 16,       // 3: faces of S^n
+    A_BA = 8,        // 3: faces of S^n
+    A_UB = 11,       // 8: stage state S^1
     A_BB = 19,       // 3: faces of S^1
-    A_V  = 22,       // 8: primitives of the stage input
-    A_F  = 30,       // 3 x 8: per direction rho, mx, my, mz, E flux, F[B_t1], F[B_t2], weight
-    A_EG = 54,       // 3: edge EMFs
-    A_COUNT = 57
+    A_CT = 22,       // 15: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3, CT_EG 3); staging outside a step
+    A_COUNT = 37
 };
 
 } // namespace pluto

@@ -1,5 +1,13 @@
-// kernels.cuh -- CUDA kernels of the MHD step (sm_100a), baseline multi-kernel form.
-// One thread per zone / face / edge, x fastest so every warp access is a contiguous 256 B row.
+// kernels.cuh -- CUDA kernels of the MHD step (sm_100a).
+//
+// Per RK stage:   k_ghost<0,1,2>   periodic ghost fill of the 8 cell variables + face fields (a1)
+//                 k_sweep_x        cons->prim + PLM + HLLD + flux difference along x (a2-a5), "flat pencil"
+//                 k_sweep_march<1> the same along y, each thread marching up its own column
+//                 k_sweep_march<2> the same along z
+//                 k_emf            CT edge EMFs from the face data the sweeps left (a6)
+//                 k_ctface         face-B curl update [+ RK2 combine] (a6, a7)
+//                 k_cellb          cell-centred B := face mean
+// x is the contiguous index everywhere, so every warp access is a contiguous row segment.
 #pragma once
 #include "grid.h"
 #include "mhd_device.cuh"
@@ -16,171 +24,331 @@ __device__ __forceinline__ bool thread_zone(const Box &b, int &i, int &j, int &k
     return i < b.hi[0];
 }
 
+__device__ __forceinline__ int wrap_m1(int i, int n) { return i == 0 ? n - 1 : i - 1; }
+__device__ __forceinline__ int wrap_p1(int i, int n) { return i == n - 1 ? 0 : i + 1; }
+
 // ---------------------------------------------------------------- periodic ghost fill (a1)
 // Fill the ghost layers of `narr` consecutive arrays along AXIS: index g in [-ng,0) <- g + n,
 // g in [n, n+ng] <- g - n (cells and faces alike; face n duplicates face 0).  Launched x, then y,
 // then z over the full padded extent of the other axes so edges and corners come out right
 // (the paper exchanges with diagonal neighbours for the same reason).
-template <int AXIS>
-__global__ void k_ghost(Grid g, double *__restrict__ base, int narr)
+__global__ void k_ghost_x(Grid g, double *__restrict__ base)
 {
-    // thread x runs over padded x (AXIS != 0) or over the 2*ng+1 ghost indices (AXIS == 0)
+    // one thread per padded row (j,k); the 2*ng+1 ghost cells of a row are strided by nothing
+    // useful, so each thread walks them itself
+    const long long rows = (long long)g.tot[1] * g.tot[2];
+    long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (r >= rows) return;
+    double *a = base + (long long)blockIdx.y * g.sa + r * g.st[1] + g.off[0];
+    const int n = g.n[0];
+    for (int s = 1; s <= g.ng; s++) a[-s] = a[n - s];
+    for (int s = 0; s <= g.ng; s++) a[n + s] = a[s];
+}
+
+template <int AXIS>   // AXIS = 1 or 2
+__global__ void k_ghost_yz(Grid g, double *__restrict__ base, int narr)
+{
     const int nghost = 2 * g.ng + 1;
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
-    int p[3];
-    if (AXIS == 0) {
-        if (t >= nghost) return;
-        p[0] = t; p[1] = blockIdx.y; p[2] = blockIdx.z % g.tot[2];
-    } else {
-        if (t >= g.tot[0]) return;
-        p[0] = t;
-        if (AXIS == 1) { p[1] = blockIdx.y; p[2] = blockIdx.z % g.tot[2]; }
-        else           { p[1] = blockIdx.y; p[2] = blockIdx.z % nghost; }
-    }
-    int arr = (AXIS == 2) ? blockIdx.z / nghost : blockIdx.z / g.tot[2];
+    int x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= g.tot[0]) return;
+    int slot, other, arr;
+    if (AXIS == 1) { slot = blockIdx.y; other = blockIdx.z % g.tot[2]; arr = blockIdx.z / g.tot[2]; }
+    else           { other = blockIdx.y; slot = blockIdx.z % nghost;   arr = blockIdx.z / nghost; }
     if (arr >= narr) return;
-    // ghost slot -> logical index along AXIS
-    int slot = p[AXIS];
-    int gi = slot < g.ng ? slot - g.ng : g.n[AXIS] + (slot - g.ng);
-    int src = gi < 0 ? gi + g.n[AXIS] : gi - g.n[AXIS];
-    long long o[3] = { p[0], p[1], p[2] };
-    long long dst_idx, src_idx;
-    o[AXIS] = gi + g.off[AXIS];
-    dst_idx = o[2] * g.st[2] + o[1] * g.st[1] + o[0];
-    o[AXIS] = src + g.off[AXIS];
-    src_idx = o[2] * g.st[2] + o[1] * g.st[1] + o[0];
-    double *a = base + (long long)arr * g.sa;
-    a[dst_idx] = a[src_idx];
-}
-
-// ---------------------------------------------------------------- cons -> prim (a2), Eq. 7
-__global__ void k_prim(Grid g, Box box, const double *__restrict__ U, double *__restrict__ V, StepParams *P)
-{
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
-    long long c = g.at(i, j, k);
-    double rho = U[c], mx = U[g.sa + c], my = U[2 * g.sa + c], mz = U[3 * g.sa + c];
-    double Bx = U[4 * g.sa + c], By = U[5 * g.sa + c], Bz = U[6 * g.sa + c], E = U[7 * g.sa + c];
-    double vx = mx / rho, vy = my / rho, vz = mz / rho;
-    double p = (g.gamma - 1.0) * (E - 0.5 * (mx * vx + my * vy + mz * vz) - 0.5 * (Bx * Bx + By * By + Bz * Bz));
-    V[c] = rho; V[g.sa + c] = vx; V[2 * g.sa + c] = vy; V[3 * g.sa + c] = vz;
-    V[4 * g.sa + c] = Bx; V[5 * g.sa + c] = By; V[6 * g.sa + c] = Bz; V[7 * g.sa + c] = p;
-    if (!(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p)) P->err = 1;
-}
-
-// ---------------------------------------------------------------- PLM + HLLD (a3, a4)
-// Thread = lower DIR-face of cell (i,j,k).  Reads the 7 reconstructed primitives of the four
-// cells c-2 .. c+1 along DIR and the face-normal field; writes the 5 hydro flux components in lab
-// order, the two induction fluxes CT needs and the upwind weight.
-template <int DIR, int LIM>
-__global__ void __launch_bounds__(128)
-k_flux(Grid g, Box box, const double *__restrict__ V, const double *__restrict__ bn, double *__restrict__ F)
-{
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
-    constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
-    const long long c = g.at(i, j, k), s = g.st[DIR], sa = g.sa;
-    const int comp[7] = { 0, 1 + DIR, 1 + T1, 1 + T2, 4 + T1, 4 + T2, 7 };
-    double l[7], r[7];
-#pragma unroll
-    for (int q = 0; q < 7; q++) {
-        const double *Q = V + comp[q] * sa + c;
-        double qm2 = Q[-2 * s], qm1 = Q[-s], q0 = Q[0], qp1 = Q[s];
-        double d0 = q0 - qm1;
-        l[q] = qm1 + 0.5 * plm_slope<LIM>(qm1 - qm2, d0);
-        r[q] = q0 - 0.5 * plm_slope<LIM>(d0, qp1 - q0);
+    const int n = g.n[AXIS];
+    int gi = slot < g.ng ? slot - g.ng : n + (slot - g.ng);
+    int src = gi < 0 ? gi + n : gi - n;
+    double *a = base + (long long)arr * g.sa + x;
+    if (AXIS == 1) {
+        a += (long long)other * g.st[2];
+        a[(long long)(gi + g.off[1]) * g.st[1]] = a[(long long)(src + g.off[1]) * g.st[1]];
+    } else {
+        a += (long long)other * g.st[1];
+        a[(long long)(gi + g.off[2]) * g.st[2]] = a[(long long)(src + g.off[2]) * g.st[2]];
     }
-    Side L = { l[0], l[1], l[2], l[3], l[4], l[5], l[6] };
-    Side R = { r[0], r[1], r[2], r[3], r[4], r[5], r[6] };
-    double f[7], w;
-    hlld(L, R, bn[c], g.gamma, f, w);
-    F[c] = f[0];
-    F[(1 + DIR) * sa + c] = f[1];
-    F[(1 + T1) * sa + c] = f[2];
-    F[(1 + T2) * sa + c] = f[3];
-    F[4 * sa + c] = f[6];
-    F[5 * sa + c] = f[4];
-    F[6 * sa + c] = f[5];
-    F[7 * sa + c] = w;
 }
 
-// ---------------------------------------------------------------- flux-difference update (a5) [+ RK2 combine (a7)]
-// Uout = Uin - sum_d dt/dx_d (F_d(+) - F_d(-)) for rho, m, E (and B_z in 2D, which has no faces).
-// COMBINE: Uout <- (Uout + that)/2 in place (Uout holds U^n) -- Eq. 5's form with R3.
-template <bool COMBINE>
-__global__ void k_update(Grid g, Box box, const double *__restrict__ Uin, const double *__restrict__ F,
-                         double *__restrict__ Uout, const StepParams *__restrict__ P)
+// ---------------------------------------------------------------- layout of the CT work arrays
+// ct + CT_FEM + 2*d + q : induction flux q of sweep d  (d = x: F_x[By], F_x[Bz]; y: F_y[Bz], F_y[Bx];
+//                         z: F_z[Bx], F_z[By]) on the lower d-face of each interior cell
+// ct + CT_W + d         : upwind weight on that face
+// ct + CT_EC + e        : cell-centred EMF component e, E^c = -(v x B)
+// ct + CT_EG + e        : edge EMF component e at the lower (a,b) edge of each interior cell
+enum { CT_FEM = 0, CT_W = 6, CT_EC = 9, CT_EG = 12, CT_COUNT = 15 };
+
+// ---------------------------------------------------------------- x sweep (a2-a5 fused)
+// The rows of the grid are laid end to end as one list of "items" (cells -2 .. nx+1 of each row).
+// A block takes NT consecutive items: every thread loads its cell and converts it to primitives in
+// shared memory, limits its own slopes from its two list neighbours, solves the Riemann problem on
+// its lower face with its left neighbour's q^L, and differences its flux with its right neighbour's.
+// Consecutive blocks overlap by 4 items, so no flux is computed twice inside a block and rows of any
+// length pack without a ragged tail.
+constexpr int SX_NT = 256;
+constexpr int SX_OUT = SX_NT - 4;
+
+template <int LIM, bool TWO_D>
+__global__ void __launch_bounds__(SX_NT, 2)
+k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx, double *Uout,
+          double *__restrict__ ct, StepParams *P, int combine)
 {
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
-    const long long c = g.at(i, j, k), sa = g.sa;
-    const int slot[5] = { 0, 1, 2, 3, 4 };        // flux slots of rho, mx, my, mz, E
-    const int var[5]  = { 0, 1, 2, 3, 7 };
+    __shared__ double sP[8][SX_NT];     // primitives; rows 0..5 are reused for the fluxes
+    __shared__ double sQ[7][SX_NT];     // q^L = q + slope/2 of each cell
+    const int t = threadIdx.x;
+    const int nx = g.n[0], M = nx + 4;
+    const long long sa = g.sa;
+    const long long nitems = (long long)M * g.n[1] * g.n[2];
+    const long long item = (long long)blockIdx.x * SX_OUT - 2 + t;
+    const bool valid = item >= 0 && item < nitems;
+    int f = -100;
+    long long c = 0;
+    double rho = 1.0, mx = 0, my = 0, mz = 0, En = 0, Bzc = 0;
+    double q[7] = { 1, 0, 0, 0, 0, 0, 1 };    // rho, vx, vy, vz, By, Bz, p
+    double Bxc = 0;
+    if (valid) {
+        long long row = item / M;
+        f = (int)(item - row * M) - 2;
+        int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]);
+        c = g.at(f, j, k);
+        rho = Uin[c]; mx = Uin[sa + c]; my = Uin[2 * sa + c]; mz = Uin[3 * sa + c];
+        Bxc = Uin[4 * sa + c];
+        double By = Uin[5 * sa + c];
+        Bzc = Uin[6 * sa + c];
+        En = Uin[7 * sa + c];
+        double ir = rcp_fast(rho);
+        q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = By; q[5] = Bzc;
+        q[6] = (g.gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3]) - 0.5 * (Bxc * Bxc + By * By + Bzc * Bzc));
+        if (f >= 0 && f < nx && (!(rho > 0.0) || !(q[6] > 0.0) || isinf(rho) || isinf(q[6]))) P->err = 1;
+    }
 #pragma unroll
-    for (int q = 0; q < 5; q++) {
-        double u = Uin[var[q] * sa + c];
-        for (int d = 0; d < 3; d++) {
-            if (!g.act[d]) continue;
-            const double *Fd = F + (long long)(d * 8 + slot[q]) * sa + c;
-            u -= P->dtdx[d] * (Fd[g.st[d]] - Fd[0]);
+    for (int v = 0; v < 7; v++) sP[v][t] = q[v];
+    __syncthreads();
+
+    // limited slopes of the own cell (needs both list neighbours, which lie in the same row)
+    const bool has_nb = valid && t >= 1 && t <= SX_NT - 2 && f >= -1 && f <= nx;
+    double qR[7];
+    if (has_nb) {
+#pragma unroll
+        for (int v = 0; v < 7; v++) {
+            double s = plm_slope<LIM>(q[v] - sP[v][t - 1], sP[v][t + 1] - q[v]);
+            sQ[v][t] = q[v] + 0.5 * s;
+            qR[v] = q[v] - 0.5 * s;
         }
-        Uout[var[q] * sa + c] = COMBINE ? 0.5 * (Uout[var[q] * sa + c] + u) : u;
     }
-    if (!g.act[2]) {
-        // 2D: B_z is cell centred and flux updated: F_x[B_z] is x's second induction flux, F_y[B_z] y's first
-        double u = Uin[6 * sa + c];
-        const double *Fx = F + (long long)(0 * 8 + 6) * sa + c;
-        const double *Fy = F + (long long)(1 * 8 + 5) * sa + c;
-        u -= P->dtdx[0] * (Fx[g.st[0]] - Fx[0]);
-        u -= P->dtdx[1] * (Fy[g.st[1]] - Fy[0]);
-        Uout[6 * sa + c] = COMBINE ? 0.5 * (Uout[6 * sa + c] + u) : u;
+    __syncthreads();
+
+    // Riemann problem on the lower face of cell f (faces 0 .. nx)
+    const bool face = has_nb && t >= 2 && f >= 0;
+    double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5;
+    if (face) {
+        Side L = { sQ[0][t - 1], sQ[1][t - 1], sQ[2][t - 1], sQ[3][t - 1], sQ[4][t - 1], sQ[5][t - 1], sQ[6][t - 1] };
+        Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
+        hlld(L, R, bx[c], g.gamma, g.igm1, F, w);
+        sP[0][t] = F[0]; sP[1][t] = F[1]; sP[2][t] = F[2]; sP[3][t] = F[3]; sP[4][t] = F[6];
+        if (TWO_D) sP[5][t] = F[5];
+    }
+    __syncthreads();
+
+    // cell f in [0, nx): flux difference with the right neighbour's face, CT data of the own face
+    if (face && f < nx && t <= SX_NT - 3) {
+        const double dtdx = P->dtdx[0];
+        double r0 = rho - dtdx * (sP[0][t + 1] - F[0]);
+        double r1 = mx - dtdx * (sP[1][t + 1] - F[1]);
+        double r2 = my - dtdx * (sP[2][t + 1] - F[2]);
+        double r3 = mz - dtdx * (sP[3][t + 1] - F[3]);
+        double r7 = En - dtdx * (sP[4][t + 1] - F[6]);
+        if (combine) {
+            r0 = 0.5 * (Uout[c] + r0); r1 = 0.5 * (Uout[sa + c] + r1); r2 = 0.5 * (Uout[2 * sa + c] + r2);
+            r3 = 0.5 * (Uout[3 * sa + c] + r3); r7 = 0.5 * (Uout[7 * sa + c] + r7);
+        }
+        Uout[c] = r0; Uout[sa + c] = r1; Uout[2 * sa + c] = r2; Uout[3 * sa + c] = r3; Uout[7 * sa + c] = r7;
+        if (TWO_D) {   // B_z has no faces in 2D: cell centred, flux updated
+            double r6 = Bzc - dtdx * (sP[5][t + 1] - F[5]);
+            Uout[6 * sa + c] = combine ? 0.5 * (Uout[6 * sa + c] + r6) : r6;
+        }
+        ct[(CT_FEM + 0) * sa + c] = F[4];
+        ct[(CT_FEM + 1) * sa + c] = F[5];
+        ct[(CT_W + 0) * sa + c] = w;
+        // cell-centred EMF  E^c = -(v x B)
+        ct[(CT_EC + 0) * sa + c] = q[3] * q[4] - q[2] * q[5];
+        ct[(CT_EC + 1) * sa + c] = q[1] * q[5] - q[3] * Bxc;
+        ct[(CT_EC + 2) * sa + c] = q[2] * Bxc - q[1] * q[4];
     }
 }
 
-// ---------------------------------------------------------------- CT: edge EMF (a6, R6)
-// Component EC of the edge EMF at (a-1/2, b-1/2) of cell c, (EC, a, b) cyclic: arithmetic mean of
-// the four face EMFs plus the upwinded half-cell differences to the cell-centred EMFs.
-template <int EC>
-__global__ void k_emf(Grid g, Box box, const double *__restrict__ V, const double *__restrict__ F,
-                      double *__restrict__ Eg)
+// ---------------------------------------------------------------- y / z sweep (a2-a5 fused), marching
+// Thread = one column (fixed i and transverse index), marching along DIR over `seglen` cells.  It
+// keeps the running q^L, the last two primitive states (as state + difference) and the previous
+// flux in registers, so every cell is loaded and converted once and every flux is computed once per
+// segment (+1 at the segment end).  Uout already holds the x-sweep result and is updated in place:
+//     Uout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (stage 1) or 1/2 (combine stage).
+template <int DIR>
+__device__ __forceinline__ void load_rot(const double *__restrict__ U, long long sa, long long c, double gamma,
+                                         double q[7], bool &bad)
 {
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
+    constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
+    double rho = U[c];
+    double m[3] = { U[sa + c], U[2 * sa + c], U[3 * sa + c] };
+    double B[3] = { U[4 * sa + c], U[5 * sa + c], U[6 * sa + c] };
+    double En = U[7 * sa + c];
+    double ir = rcp_fast(rho);
+    double v[3] = { m[0] * ir, m[1] * ir, m[2] * ir };
+    double p = (gamma - 1.0) * (En - 0.5 * (m[0] * v[0] + m[1] * v[1] + m[2] * v[2])
+                                   - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));
+    q[0] = rho; q[1] = v[DIR]; q[2] = v[T1]; q[3] = v[T2]; q[4] = B[T1]; q[5] = B[T2]; q[6] = p;
+    bad = !(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p);
+}
+
+template <int DIR, int LIM, bool TWO_D>
+__global__ void __launch_bounds__(128, 4)
+k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__ bn, double *Uout,
+              double *__restrict__ ct, StepParams *P, double scale, int seglen)
+{
+    constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.n[0]) return;
+    // DIR = 1: grid.y = segment, grid.z = k;   DIR = 2: grid.y = j, grid.z = segment
+    const int seg = DIR == 1 ? blockIdx.y : blockIdx.z;
+    const int tr = DIR == 1 ? blockIdx.z : blockIdx.y;
+    const int s0 = seg * seglen;
+    const int s1 = min(s0 + seglen, g.n[DIR]);
+    const long long sa = g.sa, st = g.st[DIR];
+    long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
+    const double gamma = g.gamma;
+    const double fac = scale * P->dtdx[DIR];
+    bool bad, anybad = false;
+
+    double qm[7], q0[7], d0[7], qL[7];
+    load_rot<DIR>(Uin, sa, c - 2 * st, gamma, qm, bad);
+    load_rot<DIR>(Uin, sa, c - st, gamma, q0, bad);
+#pragma unroll
+    for (int v = 0; v < 7; v++) d0[v] = q0[v] - qm[v];
+    load_rot<DIR>(Uin, sa, c, gamma, qm, bad);          // qm now holds cell s0
+    anybad |= bad;
+#pragma unroll
+    for (int v = 0; v < 7; v++) {
+        double d1 = qm[v] - q0[v];
+        qL[v] = q0[v] + 0.5 * plm_slope<LIM>(d0[v], d1);   // q^L of face s0 - 1/2
+        q0[v] = qm[v];
+        d0[v] = d1;
+    }
+    double Fp[6] = { 0, 0, 0, 0, 0, 0 };                // previous face: rho, m_n, m_t1, m_t2, E, (B_z in 2D)
+
+    for (int s = s0; s <= s1; s++, c += st) {
+        // cell s is in q0 (with d0 = q_s - q_{s-1}); fetch cell s+1
+        double q1[7];
+        load_rot<DIR>(Uin, sa, c + st, gamma, q1, bad);
+        if (s + 1 < s1) anybad |= bad;
+        double qR[7];
+#pragma unroll
+        for (int v = 0; v < 7; v++) {
+            double d1 = q1[v] - q0[v];
+            double sl = plm_slope<LIM>(d0[v], d1);
+            qR[v] = q0[v] - 0.5 * sl;
+            double nl = q0[v] + 0.5 * sl;
+            q0[v] = q1[v];
+            d0[v] = d1;
+            q1[v] = nl;                                   // q1 now carries the next q^L
+        }
+        Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
+        Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
+        double F[7], w;
+        hlld(L, R, bn[c], gamma, g.igm1, F, w);
+#pragma unroll
+        for (int v = 0; v < 7; v++) qL[v] = q1[v];
+        if (s > s0) {
+            const long long cm = c - st;                  // cell s-1
+            Uout[cm] -= fac * (F[0] - Fp[0]);
+            Uout[(1 + DIR) * sa + cm] -= fac * (F[1] - Fp[1]);
+            Uout[(1 + T1) * sa + cm] -= fac * (F[2] - Fp[2]);
+            Uout[(1 + T2) * sa + cm] -= fac * (F[3] - Fp[3]);
+            Uout[7 * sa + cm] -= fac * (F[6] - Fp[4]);
+            if (TWO_D && DIR == 1) Uout[6 * sa + cm] -= fac * (F[4] - Fp[5]);   // F_y[B_z]
+        }
+        if (s < s1) {
+            ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
+            ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
+            ct[(CT_W + DIR) * sa + c] = w;
+        }
+        Fp[0] = F[0]; Fp[1] = F[1]; Fp[2] = F[2]; Fp[3] = F[3]; Fp[4] = F[6]; Fp[5] = F[4];
+    }
+    if (anybad) P->err = 1;
+}
+
+// ---------------------------------------------------------------- CT: edge EMFs (a6, R6)
+// Thread = interior cell; computes the EMF components on its three lower edges (only E_z in 2D):
+// arithmetic mean of the four face EMFs plus the upwinded half-cell differences to the cell-centred
+// EMFs.  Neighbours are taken with periodic wrap, so the CT work arrays need no ghost layers.
+template <int EC>
+__device__ __forceinline__ double edge_emf(const Grid &g, const double *__restrict__ ct, int i, int j, int k)
+{
     constexpr int A = (EC + 1) % 3, B = (EC + 2) % 3;
-    const long long c = g.at(i, j, k), sa = g.sa, sA = g.st[A], sB = g.st[B];
-    const double *Fa = F + (long long)(A * 8 + 5) * sa;   // F_a[B_b]: first induction flux of sweep a
-    const double *Fb = F + (long long)(B * 8 + 6) * sa;   // F_b[B_a]: second induction flux of sweep b
-    const double *Wa = F + (long long)(A * 8 + 7) * sa;
-    const double *Wb = F + (long long)(B * 8 + 7) * sa;
-    const long long c11 = c, c01 = c - sA, c10 = c - sB, c00 = c - sA - sB;
-    auto ecell = [&](long long cc) {            // E^c = -(v x B) component EC = v_b B_a - v_a B_b
-        return V[(1 + B) * sa + cc] * V[(4 + A) * sa + cc] - V[(1 + A) * sa + cc] * V[(4 + B) * sa + cc];
-    };
+    const long long sa = g.sa;
+    int p[3] = { i, j, k };
+    int pa[3] = { i, j, k }, pb[3] = { i, j, k }, pab[3] = { i, j, k };
+    pa[A] = wrap_m1(p[A], g.n[A]);
+    pb[B] = wrap_m1(p[B], g.n[B]);
+    pab[A] = pa[A]; pab[B] = pb[B];
+    const long long c11 = g.at(p[0], p[1], p[2]), c01 = g.at(pa[0], pa[1], pa[2]);
+    const long long c10 = g.at(pb[0], pb[1], pb[2]), c00 = g.at(pab[0], pab[1], pab[2]);
+    const double *Fa = ct + (CT_FEM + 2 * A) * sa;       // F_a[B_b]: first induction flux of sweep a
+    const double *Fb = ct + (CT_FEM + 2 * B + 1) * sa;   // F_b[B_a]: second induction flux of sweep b
+    const double *Wa = ct + (CT_W + A) * sa, *Wb = ct + (CT_W + B) * sa;
+    const double *Ec = ct + (CT_EC + EC) * sa;
     double Ea_lo = -Fa[c10], Ea_hi = -Fa[c11];
     double Eb_lo =  Fb[c01], Eb_hi =  Fb[c11];
     double wa_lo = Wa[c10], wa_hi = Wa[c11], wb_lo = Wb[c01], wb_hi = Wb[c11];
-    double e00 = ecell(c00), e10 = ecell(c10), e01 = ecell(c01), e11 = ecell(c11);
+    double e00 = Ec[c00], e10 = Ec[c10], e01 = Ec[c01], e11 = Ec[c11];
     double t1 = wa_lo * (Eb_lo - e00) + (1.0 - wa_lo) * (Eb_hi - e10);
     double t2 = wa_hi * (e01 - Eb_lo) + (1.0 - wa_hi) * (e11 - Eb_hi);
     double t3 = wb_lo * (Ea_lo - e00) + (1.0 - wb_lo) * (Ea_hi - e01);
     double t4 = wb_hi * (e10 - Ea_lo) + (1.0 - wb_hi) * (e11 - Ea_hi);
-    Eg[EC * sa + c] = 0.25 * (Ea_lo + Ea_hi + Eb_lo + Eb_hi) + 0.25 * (t1 - t2) + 0.25 * (t3 - t4);
+    return 0.25 * (Ea_lo + Ea_hi + Eb_lo + Eb_hi) + 0.25 * (t1 - t2) + 0.25 * (t3 - t4);
 }
 
-// ---------------------------------------------------------------- CT: face update  db/dt = -curl E
-template <int DIR, bool COMBINE>
-__global__ void k_ctface(Grid g, Box box, const double *__restrict__ bin, const double *__restrict__ Eg,
-                         double *__restrict__ bout, const StepParams *__restrict__ P)
+__global__ void k_emf(Grid g, Box box, double *__restrict__ ct)
 {
     int i, j, k;
     if (!thread_zone(box, i, j, k)) return;
-    constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     const long long c = g.at(i, j, k), sa = g.sa;
-    double term1 = 0.0, term2 = 0.0;
-    if (g.act[T1]) { const double *E2 = Eg + T2 * sa + c; term1 = (E2[g.st[T1]] - E2[0]) / g.dx[T1]; }
-    if (g.act[T2]) { const double *E1 = Eg + T1 * sa + c; term2 = (E1[g.st[T2]] - E1[0]) / g.dx[T2]; }
-    double b = bin[DIR * sa + c] - P->dt * (term1 - term2);
-    bout[DIR * sa + c] = COMBINE ? 0.5 * (bout[DIR * sa + c] + b) : b;
+    double ez = edge_emf<2>(g, ct, i, j, k);
+    if (g.act[2]) {
+        double ex = edge_emf<0>(g, ct, i, j, k);
+        double ey = edge_emf<1>(g, ct, i, j, k);
+        ct[(CT_EG + 0) * sa + c] = ex;
+        ct[(CT_EG + 1) * sa + c] = ey;
+    }
+    ct[(CT_EG + 2) * sa + c] = ez;
+}
+
+// ---------------------------------------------------------------- CT: face update  db/dt = -curl E  [+ combine (a7)]
+// Thread = interior cell, updates its three lower faces; the +1 edge neighbours wrap periodically.
+// COMBINE: bout <- (bout + that)/2 in place (bout holds the faces of S^n).
+template <bool COMBINE>
+__global__ void k_ctface(Grid g, Box box, const double *__restrict__ bin, const double *__restrict__ ct,
+                         double *bout, const StepParams *__restrict__ P)
+{
+    int i, j, k;
+    if (!thread_zone(box, i, j, k)) return;
+    const long long c = g.at(i, j, k), sa = g.sa;
+    const double dt = P->dt;
+    const double *Ex = ct + (CT_EG + 0) * sa, *Ey = ct + (CT_EG + 1) * sa, *Ez = ct + (CT_EG + 2) * sa;
+    const long long cxp = g.at(wrap_p1(i, g.n[0]), j, k);
+    const long long cyp = g.at(i, wrap_p1(j, g.n[1]), k);
+    const double ez = Ez[c];
+    double bxn, byn;
+    if (g.act[2]) {
+        const long long czp = g.at(i, j, wrap_p1(k, g.n[2]));
+        const double ex = Ex[c], ey = Ey[c];
+        bxn = bin[c] - dt * ((Ez[cyp] - ez) / g.dx[1] - (Ey[czp] - ey) / g.dx[2]);
+        byn = bin[sa + c] - dt * ((Ex[czp] - ex) / g.dx[2] - (Ez[cxp] - ez) / g.dx[0]);
+        double bzn = bin[2 * sa + c] - dt * ((Ey[cxp] - ey) / g.dx[0] - (Ex[cyp] - ex) / g.dx[1]);
+        bout[2 * sa + c] = COMBINE ? 0.5 * (bout[2 * sa + c] + bzn) : bzn;
+    } else {
+        bxn = bin[c] - dt * ((Ez[cyp] - ez) / g.dx[1] - 0.0);
+        byn = bin[sa + c] - dt * (0.0 - (Ez[cxp] - ez) / g.dx[0]);
+    }
+    bout[c] = COMBINE ? 0.5 * (bout[c] + bxn) : bxn;
+    bout[sa + c] = COMBINE ? 0.5 * (bout[sa + c] + byn) : byn;
 }
 
 // ---------------------------------------------------------------- cell-centred B := face mean (R7)
@@ -189,8 +357,9 @@ __global__ void k_cellb(Grid g, Box box, const double *__restrict__ b, double *_
     int i, j, k;
     if (!thread_zone(box, i, j, k)) return;
     const long long c = g.at(i, j, k), sa = g.sa;
-    for (int d = 0; d < 3; d++)
-        if (g.act[d]) U[(4 + d) * sa + c] = 0.5 * (b[d * sa + c] + b[d * sa + c + g.st[d]]);
+    U[4 * sa + c] = 0.5 * (b[c] + b[g.at(wrap_p1(i, g.n[0]), j, k)]);
+    U[5 * sa + c] = 0.5 * (b[sa + c] + b[sa + g.at(i, wrap_p1(j, g.n[1]), k)]);
+    if (g.act[2]) U[6 * sa + c] = 0.5 * (b[2 * sa + c] + b[2 * sa + g.at(i, j, wrap_p1(k, g.n[2]))]);
 }
 
 // ---------------------------------------------------------------- API layout <-> padded layout
@@ -206,7 +375,7 @@ __global__ void k_pack(Grid g, Box box, const double *__restrict__ src, int m0, 
 {
     int i, j, k;
     if (!thread_zone(box, i, j, k)) return;
-    // periodic wrap so the duplicate upper face (index n) and interior-indexed work arrays both come out right
+    // periodic wrap: the duplicate upper face (index n) is face 0
     int ii = i % g.n[0], jj = j % g.n[1], kk = k % g.n[2];
     dst[((long long)k * m1 + j) * m0 + i] = src[g.at(ii, jj, kk)];
 }

@@ -12,6 +12,49 @@ namespace pluto {
 constexpr double kTheta = 1e-3;   // R6: |mass flux| >= theta * f_ref is fully upwinded
 constexpr double kDegen = 1e-8;   // R5: guard of the star-state denominator
 
+// ---------------------------------------------------------------- fp64 reciprocal / square root
+// IEEE division and sqrt cost ~9 fp64-pipe instructions each plus range checks and a slow-path call;
+// HLLD needs 9 reciprocals and 6 square roots per interface, about half of its arithmetic.  These
+// versions start from the hardware seed (MUFU.RCP64H / MUFU.RSQ64H, relative error <= 2^-22) and
+// refine it with a third-order / two second-order steps: results are within ~1 ulp of the IEEE
+// value for normal, finite, positive-range arguments, which is all this path produces (the error
+// flag catches non-positive density / pressure).  No denormal, zero or infinity handling.
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);          // e = 1 - x y,  |e| <= 2^-22
+    e = fma(e, e, e);                    // e + e^2
+    return fma(y, e, y);                 // y (1 + e + e^2): error ~ e^3
+}
+
+// s = sqrt(x), returns also r = 1/sqrt(x); x > 0
+__device__ __forceinline__ void sqrt_rsqrt_fast(double x, double &s, double &r)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double g = x * y, h = 0.5 * y;       // g -> sqrt(x), h -> 1/(2 sqrt(x))
+    double e = fma(-g, h, 0.5);
+    g = fma(g, e, g); h = fma(h, e, h);
+    e = fma(-g, h, 0.5);
+    s = fma(g, e, g);
+    r = 2.0 * fma(h, e, h);
+}
+
+__device__ __forceinline__ double sqrt_fast(double x)
+{
+    double s, r;
+    sqrt_rsqrt_fast(x, s, r);
+    return s;
+}
+
+// sqrt that tolerates x == 0 (the discriminant of the fast speed can vanish)
+__device__ __forceinline__ double sqrt_fast0(double x)
+{
+    double s = sqrt_fast(fmax(x, 1e-300));
+    return x > 0.0 ? s : 0.0;
+}
+
 template <int LIM>
 __device__ __forceinline__ double plm_slope(double dm, double dp)
 {
@@ -29,12 +72,11 @@ __device__ __forceinline__ double plm_slope(double dm, double dp)
 // fast magnetosonic speed from a^2*rho = gamma*p, B-normal^2 and |B|^2 (all divided by rho inside)
 __device__ __forceinline__ double fast_speed(double rho, double gp, double bn2, double b2)
 {
-    double ir  = 1.0 / rho;
+    double ir  = rcp_fast(rho);
     double a2  = gp * ir;
     double s   = a2 + b2 * ir;
     double disc = s * s - 4.0 * a2 * (bn2 * ir);
-    disc = disc < 0.0 ? 0.0 : disc;
-    return sqrt(0.5 * (s + sqrt(disc)));
+    return sqrt_fast(0.5 * (s + sqrt_fast0(disc)));
 }
 
 // One side of the Riemann fan in the rotated frame.
@@ -43,10 +85,9 @@ struct Side {
 };
 
 // HLLD flux.  Output f[7] = (rho, m_n, m_t1, m_t2, B_t1, B_t2, E) flux, wgt = upwind weight.
-__device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, double gamma,
+__device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, double gamma, double igm1,
                                      double f[7], double &wgt)
 {
-    const double igm1 = 1.0 / (gamma - 1.0);
     const double Bx2 = Bx * Bx;
 
     // left / right total pressure, v.B, energy, physical flux
@@ -65,7 +106,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
 
     // the side the interface lies in is decided by S_M; supersonic cases fall out of the same test
     double aL = L.rho * (SL - L.u), aR = R.rho * (SR - R.u);
-    double idenom = 1.0 / (aR - aL);
+    double idenom = rcp_fast(aR - aL);
     double SM  = (aR * R.u - aL * L.u - pTR + pTL) * idenom;
     double pTs = (aR * pTL - aL * pTR + aL * aR * (R.u - L.u)) * idenom;
 
@@ -73,13 +114,13 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     double rsL, vsL, wsL, BysL, BzsL, EsL, vBsL;
     double rsR, vsR, wsR, BysR, BzsR, EsR, vBsR;
     {
-        double dS = SL - SM, idS = 1.0 / dS;
+        double dS = SL - SM, idS = rcp_fast(dS);
         double D = aL * dS - Bx2;
         rsL = aL * idS;
         if (fabs(D) <= kDegen * pTs) {
             vsL = L.v; wsL = L.w; BysL = L.By; BzsL = L.Bz;
         } else {
-            double iD = 1.0 / D;
+            double iD = rcp_fast(D);
             double cv = Bx * (SM - L.u) * iD;
             double cb = (aL * (SL - L.u) - Bx2) * iD;
             vsL = L.v - cv * L.By; wsL = L.w - cv * L.Bz;
@@ -89,13 +130,13 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
         EsL = ((SL - L.u) * EL - pTL * L.u + pTs * SM + Bx * (vBL - vBsL)) * idS;
     }
     {
-        double dS = SR - SM, idS = 1.0 / dS;
+        double dS = SR - SM, idS = rcp_fast(dS);
         double D = aR * dS - Bx2;
         rsR = aR * idS;
         if (fabs(D) <= kDegen * pTs) {
             vsR = R.v; wsR = R.w; BysR = R.By; BzsR = R.Bz;
         } else {
-            double iD = 1.0 / D;
+            double iD = rcp_fast(D);
             double cv = Bx * (SM - R.u) * iD;
             double cb = (aR * (SR - R.u) - Bx2) * iD;
             vsR = R.v - cv * R.By; wsR = R.w - cv * R.Bz;
@@ -106,11 +147,13 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     }
 
     // Alfven waves and the double-star state
-    double rL = sqrt(rsL), rR = sqrt(rsR);
+    double rL, rR, irL, irR;
+    sqrt_rsqrt_fast(rsL, rL, irL);
+    sqrt_rsqrt_fast(rsR, rR, irR);
     double aBx = fabs(Bx);
-    double SaL = SM - aBx / rL, SaR = SM + aBx / rR;
+    double SaL = SM - aBx * irL, SaR = SM + aBx * irR;
     double sig = Bx > 0.0 ? 1.0 : (Bx < 0.0 ? -1.0 : 0.0);
-    double iR = 1.0 / (rL + rR);
+    double iR = rcp_fast(rL + rR);
     double vss  = (rL * vsL + rR * vsR + sig * (BysR - BysL)) * iR;
     double wss  = (rL * wsL + rR * wsR + sig * (BzsR - BzsL)) * iR;
     double Byss = (rL * BysR + rR * BysL + sig * rL * rR * (vsR - vsL)) * iR;
@@ -169,7 +212,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     f[0] = F0; f[1] = F1; f[2] = F2; f[3] = F3; f[4] = F5; f[5] = F6; f[6] = F7;
 
     double fref = 0.25 * (L.rho + R.rho) * (SR - SL);
-    double wv = 0.5 + 0.5 * F0 / (kTheta * fref);
+    double wv = 0.5 + 0.5 * F0 * rcp_fast(kTheta * fref);
     wgt = fmin(fmax(wv, 0.0), 1.0);
 }
 

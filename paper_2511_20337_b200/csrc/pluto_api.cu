@@ -20,10 +20,10 @@ using namespace pluto;
 
 namespace {
 
-enum KernelId { K_GHOST = 0, K_PRIM, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_UPDATE, K_EMF, K_CTFACE, K_CELLB,
+enum KernelId { K_GHOST = 0, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_EMF, K_CTFACE, K_CELLB,
                 K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
-const char *const kKernelNames[K_COUNT] = { "ghost_fill", "cons2prim", "plm_hlld_x", "plm_hlld_y", "plm_hlld_z",
-                                            "flux_update", "ct_edge_emf", "ct_face_update", "cell_b_mean",
+const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_x", "sweep_y", "sweep_z",
+                                            "ct_edge_emf", "ct_face_update", "cell_b_mean",
                                             "dt_max", "scalars", "pack_unpack" };
 
 struct Context {
@@ -133,30 +133,52 @@ void destroy_graphs()
 
 // ---------------------------------------------------------------- launch sequences
 
-void fill_ghosts(double *first, int narr)
+// ghost layers of the 8 cell variables + face fields of one state (11 contiguous arrays; 10 in 2D)
+void fill_ghosts(double *first)
 {
     const Grid &g = C.g;
     const int ngh = 2 * g.ng + 1;
+    const int narr = 8 + g.ndim;
     cudaStream_t s = C.stream;
-    LAUNCH(K_GHOST, k_ghost<0><<<dim3(1, g.tot[1], g.tot[2] * narr), 64, 0, s>>>(g, first, narr));
-    LAUNCH(K_GHOST, k_ghost<1><<<dim3((g.tot[0] + 127) / 128, ngh, g.tot[2] * narr), 128, 0, s>>>(g, first, narr));
+    const long long rows = (long long)g.tot[1] * g.tot[2];
+    LAUNCH(K_GHOST, k_ghost_x<<<dim3((unsigned)((rows + 127) / 128), narr), 128, 0, s>>>(g, first));
+    LAUNCH(K_GHOST, k_ghost_yz<1><<<dim3((g.tot[0] + 127) / 128, ngh, g.tot[2] * narr), 128, 0, s>>>(g, first, narr));
     if (g.act[2])
-        LAUNCH(K_GHOST, k_ghost<2><<<dim3((g.tot[0] + 127) / 128, g.tot[1], ngh * narr), 128, 0, s>>>(g, first, narr));
+        LAUNCH(K_GHOST, k_ghost_yz<2><<<dim3((g.tot[0] + 127) / 128, g.tot[1], ngh * narr), 128, 0, s>>>(g, first, narr));
 }
 
-template <int LIM>
-void launch_flux(const double *V, const double *bface)
+int march_seglen(int n, long long columns)
+{
+    // enough independent threads for ~8 waves of 16 warps per SM, segments no shorter than 16 cells
+    const long long want = (long long)C.sm_count * 16 * 32 * 8;
+    long long nseg = (want + columns - 1) / columns;
+    if (nseg < 1) nseg = 1;
+    int len = (int)((n + nseg - 1) / nseg);
+    if (len < 16) len = 16;
+    if (len > n) len = n;
+    return len;
+}
+
+template <int LIM, bool TWO_D>
+void launch_sweeps(const double *Uin, const double *bin, double *Uout, bool combine)
 {
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
-    // faces 0..n along the sweep, one ghost layer across it (CT needs the transverse neighbours)
-    Box bx = make_box(g, 0, g.n[0] + 1, -1, g.n[1] + 1, -1, g.n[2] + 1);
-    LAUNCH(K_FLUX_X, k_flux<0, LIM><<<grid_for(bx), 128, 0, s>>>(g, bx, V, bface + 0 * g.sa, arr(A_F + 0)));
-    Box by = make_box(g, -1, g.n[0] + 1, 0, g.n[1] + 1, -1, g.n[2] + 1);
-    LAUNCH(K_FLUX_Y, k_flux<1, LIM><<<grid_for(by), 128, 0, s>>>(g, by, V, bface + 1 * g.sa, arr(A_F + 8)));
-    if (g.act[2]) {
-        Box bz = make_box(g, -1, g.n[0] + 1, -1, g.n[1] + 1, 0, g.n[2] + 1);
-        LAUNCH(K_FLUX_Z, k_flux<2, LIM><<<grid_for(bz), 128, 0, s>>>(g, bz, V, bface + 2 * g.sa, arr(A_F + 16)));
+    double *ct = arr(A_CT);
+    const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
+    LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
+                         g, Uin, bin, Uout, ct, C.P, combine ? 1 : 0));
+    const double scale = combine ? 0.5 : 1.0;
+    const int bx = (g.n[0] + 127) / 128;
+    {
+        const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
+        dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
+        LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, 128, 0, s>>>(g, Uin, bin + g.sa, Uout, ct, C.P, scale, len));
+    }
+    if (!TWO_D) {
+        const int len = march_seglen(g.n[2], (long long)g.n[0] * g.n[1]);
+        dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
+        LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, 128, 0, s>>>(g, Uin, bin + 2 * g.sa, Uout, ct, C.P, scale, len));
     }
 }
 
@@ -166,35 +188,15 @@ void enqueue_stage(int in_u, int in_b, int out_u, int out_b, bool combine)
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
     Box in = interior(g);
-    LAUNCH(K_PRIM, k_prim<<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_V), C.P));
-    fill_ghosts(arr(A_V), 8);
-    fill_ghosts(arr(in_b), g.ndim);
-    if (g.limiter == 0) launch_flux<0>(arr(A_V), arr(in_b));
-    else                launch_flux<1>(arr(A_V), arr(in_b));
-    if (combine) LAUNCH(K_UPDATE, k_update<true><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P));
-    else         LAUNCH(K_UPDATE, k_update<false><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_u), arr(A_F), arr(out_u), C.P));
-    // edge EMFs on all edges touching interior faces (indices 0..n in the two transverse directions)
-    if (g.act[2]) {
-        Box ex = make_box(g, 0, g.n[0], 0, g.n[1] + 1, 0, g.n[2] + 1);
-        LAUNCH(K_EMF, k_emf<0><<<grid_for(ex), 128, 0, s>>>(g, ex, arr(A_V), arr(A_F), arr(A_EG)));
-        Box ey = make_box(g, 0, g.n[0] + 1, 0, g.n[1], 0, g.n[2] + 1);
-        LAUNCH(K_EMF, k_emf<1><<<grid_for(ey), 128, 0, s>>>(g, ey, arr(A_V), arr(A_F), arr(A_EG)));
-    }
-    Box ez = make_box(g, 0, g.n[0] + 1, 0, g.n[1] + 1, 0, g.n[2]);
-    LAUNCH(K_EMF, k_emf<2><<<grid_for(ez), 128, 0, s>>>(g, ez, arr(A_V), arr(A_F), arr(A_EG)));
-    // faces 0..n (the duplicate upper face is computed, not copied: same inputs, same bits)
-    Box fx = make_box(g, 0, g.n[0] + 1, 0, g.n[1], 0, g.n[2]);
-    Box fy = make_box(g, 0, g.n[0], 0, g.n[1] + 1, 0, g.n[2]);
-    Box fz = make_box(g, 0, g.n[0], 0, g.n[1], 0, g.n[2] + 1);
-    if (combine) {
-        LAUNCH(K_CTFACE, k_ctface<0, true><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P));
-        LAUNCH(K_CTFACE, k_ctface<1, true><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P));
-        if (g.act[2]) LAUNCH(K_CTFACE, k_ctface<2, true><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P));
-    } else {
-        LAUNCH(K_CTFACE, k_ctface<0, false><<<grid_for(fx), 128, 0, s>>>(g, fx, arr(in_b), arr(A_EG), arr(out_b), C.P));
-        LAUNCH(K_CTFACE, k_ctface<1, false><<<grid_for(fy), 128, 0, s>>>(g, fy, arr(in_b), arr(A_EG), arr(out_b), C.P));
-        if (g.act[2]) LAUNCH(K_CTFACE, k_ctface<2, false><<<grid_for(fz), 128, 0, s>>>(g, fz, arr(in_b), arr(A_EG), arr(out_b), C.P));
-    }
+    fill_ghosts(arr(in_u));
+    const bool two_d = !g.act[2];
+    if (g.limiter == 0) { if (two_d) launch_sweeps<0, true>(arr(in_u), arr(in_b), arr(out_u), combine);
+                          else       launch_sweeps<0, false>(arr(in_u), arr(in_b), arr(out_u), combine); }
+    else                { if (two_d) launch_sweeps<1, true>(arr(in_u), arr(in_b), arr(out_u), combine);
+                          else       launch_sweeps<1, false>(arr(in_u), arr(in_b), arr(out_u), combine); }
+    LAUNCH(K_EMF, k_emf<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT)));
+    if (combine) LAUNCH(K_CTFACE, k_ctface<true><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_b), arr(A_CT), arr(out_b), C.P));
+    else         LAUNCH(K_CTFACE, k_ctface<false><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_b), arr(A_CT), arr(out_b), C.P));
     LAUNCH(K_CELLB, k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(out_b), arr(out_u)));
 }
 
@@ -271,13 +273,13 @@ size_t api_count(const Grid &g, int d)
     return (size_t)m[0] * m[1] * m[2];
 }
 
-// staging buffer: the flux work arrays are free outside a step (24 arrays >= 11 interior arrays)
-double *staging() { return arr(A_F); }
+// staging buffer: the CT work arrays are free outside a step (15 arrays >= 11 interior arrays)
+double *staging() { return arr(A_CT); }
 
 int copy_in(const double *src, size_t count, double **dev)
 {
     if (is_device_ptr(src)) { *dev = const_cast<double *>(src); return PLUTO_OK; }
-    if (count * sizeof(double) > (size_t)24 * C.g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
+    if (count * sizeof(double) > (size_t)CT_COUNT * C.g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
     CUDA_TRY(cudaMemcpyAsync(staging(), src, count * sizeof(double), cudaMemcpyHostToDevice, C.stream));
     *dev = staging();
     return PLUTO_OK;
@@ -356,7 +358,7 @@ int pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int 
         return fail(PLUTO_EINVAL, "need gamma > 1, cfl > 0, limiter in {0,1}");
     if ((long long)g.tot[2] * 8 > 65535 || g.tot[1] > 65535)
         return fail(PLUTO_EINVAL, "extent too large for the launch grid");
-    g.gamma = gamma; g.cfl = cfl; g.limiter = limiter;
+    g.gamma = gamma; g.igm1 = 1.0 / (gamma - 1.0); g.cfl = cfl; g.limiter = limiter;
     for (int a = 0; a < 3; a++) { g.dx[a] = 1.0 / nx; g.idx[a] = 1.0 / g.dx[a]; }   // R11: Lx = 1, cubic cells
     size_t bytes = layout_bytes(g);
     if (C.ws) {
@@ -419,7 +421,6 @@ int pluto_set_state(const double *U, const double *Bface)
         k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + off, m[0], m[1], arr(A_BA + d));   // upper duplicate ignored
         off += api_count(g, d);
     }
-    fill_ghosts(arr(A_BA), g.ndim);                            // face n <- face 0 for the cell mean
     k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_BA), arr(A_UA));
     StepParams p0;
     memset(&p0, 0, sizeof p0);
@@ -606,7 +607,7 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     }
     if (W) {
         cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
-        for (int d = 0; d < g.ndim; d++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_F + 8 * d + 7), g.n[0], g.n[1], tmp + d * n);
+        for (int d = 0; d < g.ndim; d++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT + CT_W + d), g.n[0], g.n[1], tmp + d * n);
         cudaStreamSynchronize(s);
         bad |= emit(W, 3 * n);
     }
@@ -614,13 +615,13 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
         cudaMemsetAsync(tmp, 0, 6 * n * sizeof(double), s);
         for (int d = 0; d < g.ndim; d++)
             for (int q = 0; q < 2; q++)
-                k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_F + 8 * d + 5 + q), g.n[0], g.n[1], tmp + (2 * d + q) * n);
+                k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT + CT_FEM + 2 * d + q), g.n[0], g.n[1], tmp + (2 * d + q) * n);
         cudaStreamSynchronize(s);
         bad |= emit(Fem, 6 * n);
     }
     if (Eedge) {
         cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
-        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_EG + e), g.n[0], g.n[1], tmp + e * n);
+        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT + CT_EG + e), g.n[0], g.n[1], tmp + e * n);
         cudaStreamSynchronize(s);
         bad |= emit(Eedge, 3 * n);
     }
