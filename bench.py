@@ -35,8 +35,9 @@ METRIC = "zone-updates/sec (fp64 3D MHD step, 1 B200); achieved HBM GB/s vs peak
 UNIT = "zone-updates/s"
 
 # Algorithmic traffic of the dominant kernels, doubles per unit:
-#   plm_hlld_<d> : per face, read 7 primitives + 1 face field, write 5 fluxes + 2 induction fluxes + 1 weight
-ALGO_DOUBLES = {"plm_hlld_x": 16, "plm_hlld_y": 16, "plm_hlld_z": 16}
+#   sweep_x   : per zone, read U 8 + bx 1, write U' 5 + 2 induction fluxes + 1 weight + 3 cell EMFs  = 20
+#   sweep_y/z : per zone, read U 8 + b_d 1, read+write U' 5 + 5, write 2 induction fluxes + 1 weight = 22
+ALGO_DOUBLES = {"sweep_x": 20, "sweep_y": 22, "sweep_z": 22}
 
 
 def peaks():
@@ -225,10 +226,7 @@ def main():
     dom_ms, dom_cnt = rep[dom]
     hbm_peak, peak_src = peaks()
     # units one launch of the dominant kernel processes
-    faces = {"plm_hlld_x": (w.nx + 1) * (w.ny + 2) * (w.nz + 2 if w.nz > 1 else 1),
-             "plm_hlld_y": (w.nx + 2) * (w.ny + 1) * (w.nz + 2 if w.nz > 1 else 1),
-             "plm_hlld_z": (w.nx + 2) * (w.ny + 2) * (w.nz + 1)}
-    units = faces.get(dom, w.zones)
+    units = w.zones
     algo_bytes = ALGO_DOUBLES.get(dom, 0) * 8 * units
     dur = dom_ms * 1e-3 / max(dom_cnt, 1)
     achieved = algo_bytes / dur * 1e-9 if dur > 0 else 0.0

@@ -83,11 +83,11 @@ enum { CT_FEM = 0, CT_W = 6, CT_EC = 9, CT_EG = 12, CT_COUNT = 15 };
 // its lower face with its left neighbour's q^L, and differences its flux with its right neighbour's.
 // Consecutive blocks overlap by 4 items, so no flux is computed twice inside a block and rows of any
 // length pack without a ragged tail.
-constexpr int SX_NT = 256;
+constexpr int SX_NT = 128;
 constexpr int SX_OUT = SX_NT - 4;
 
 template <int LIM, bool TWO_D>
-__global__ void __launch_bounds__(SX_NT, 2)
+__global__ void __launch_bounds__(SX_NT, 4)
 k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx, double *Uout,
           double *__restrict__ ct, StepParams *P, int combine)
 {
@@ -103,7 +103,8 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
     long long c = 0;
     double rho = 1.0, mx = 0, my = 0, mz = 0, En = 0, Bzc = 0;
     double q[7] = { 1, 0, 0, 0, 0, 0, 1 };    // rho, vx, vy, vz, By, Bz, p
-    double Bxc = 0;
+    double Bxc = 0, bxf = 0;
+    double o0 = 0, o1 = 0, o2 = 0, o3 = 0, o6 = 0, o7 = 0;   // S^n of the cell (combine stage)
     if (valid) {
         long long row = item / M;
         f = (int)(item - row * M) - 2;
@@ -114,6 +115,11 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
         double By = Uin[5 * sa + c];
         Bzc = Uin[6 * sa + c];
         En = Uin[7 * sa + c];
+        bxf = bx[c];
+        if (combine && f >= 0 && f < nx) {     // issued with the other loads: one memory round trip per block
+            o0 = Uout[c]; o1 = Uout[sa + c]; o2 = Uout[2 * sa + c]; o3 = Uout[3 * sa + c]; o7 = Uout[7 * sa + c];
+            if (TWO_D) o6 = Uout[6 * sa + c];
+        }
         double ir = rcp_fast(rho);
         q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = By; q[5] = Bzc;
         q[6] = (g.gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3]) - 0.5 * (Bxc * Bxc + By * By + Bzc * Bzc));
@@ -142,7 +148,7 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
     if (face) {
         Side L = { sQ[0][t - 1], sQ[1][t - 1], sQ[2][t - 1], sQ[3][t - 1], sQ[4][t - 1], sQ[5][t - 1], sQ[6][t - 1] };
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-        hlld(L, R, bx[c], g.gamma, g.igm1, F, w);
+        hlld(L, R, bxf, g.gamma, g.igm1, F, w);
         sP[0][t] = F[0]; sP[1][t] = F[1]; sP[2][t] = F[2]; sP[3][t] = F[3]; sP[4][t] = F[6];
         if (TWO_D) sP[5][t] = F[5];
     }
@@ -157,13 +163,13 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
         double r3 = mz - dtdx * (sP[3][t + 1] - F[3]);
         double r7 = En - dtdx * (sP[4][t + 1] - F[6]);
         if (combine) {
-            r0 = 0.5 * (Uout[c] + r0); r1 = 0.5 * (Uout[sa + c] + r1); r2 = 0.5 * (Uout[2 * sa + c] + r2);
-            r3 = 0.5 * (Uout[3 * sa + c] + r3); r7 = 0.5 * (Uout[7 * sa + c] + r7);
+            r0 = 0.5 * (o0 + r0); r1 = 0.5 * (o1 + r1); r2 = 0.5 * (o2 + r2);
+            r3 = 0.5 * (o3 + r3); r7 = 0.5 * (o7 + r7);
         }
         Uout[c] = r0; Uout[sa + c] = r1; Uout[2 * sa + c] = r2; Uout[3 * sa + c] = r3; Uout[7 * sa + c] = r7;
         if (TWO_D) {   // B_z has no faces in 2D: cell centred, flux updated
             double r6 = Bzc - dtdx * (sP[5][t + 1] - F[5]);
-            Uout[6 * sa + c] = combine ? 0.5 * (Uout[6 * sa + c] + r6) : r6;
+            Uout[6 * sa + c] = combine ? 0.5 * (o6 + r6) : r6;
         }
         ct[(CT_FEM + 0) * sa + c] = F[4];
         ct[(CT_FEM + 1) * sa + c] = F[5];
@@ -181,15 +187,12 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
 // flux in registers, so every cell is loaded and converted once and every flux is computed once per
 // segment (+1 at the segment end).  Uout already holds the x-sweep result and is updated in place:
 //     Uout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (stage 1) or 1/2 (combine stage).
+// cons -> rotated primitives of one cell (Eq. 7)
 template <int DIR>
-__device__ __forceinline__ void load_rot(const double *__restrict__ U, long long sa, long long c, double gamma,
+__device__ __forceinline__ void prim_rot(double rho, const double m[3], const double B[3], double En, double gamma,
                                          double q[7], bool &bad)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
-    double rho = U[c];
-    double m[3] = { U[sa + c], U[2 * sa + c], U[3 * sa + c] };
-    double B[3] = { U[4 * sa + c], U[5 * sa + c], U[6 * sa + c] };
-    double En = U[7 * sa + c];
     double ir = rcp_fast(rho);
     double v[3] = { m[0] * ir, m[1] * ir, m[2] * ir };
     double p = (gamma - 1.0) * (En - 0.5 * (m[0] * v[0] + m[1] * v[1] + m[2] * v[2])
@@ -198,13 +201,39 @@ __device__ __forceinline__ void load_rot(const double *__restrict__ U, long long
     bad = !(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p);
 }
 
+template <int DIR>
+__device__ __forceinline__ void load_rot(const double *__restrict__ U, long long sa, long long c, double gamma,
+                                         double q[7], bool &bad)
+{
+    double m[3] = { U[sa + c], U[2 * sa + c], U[3 * sa + c] };
+    double B[3] = { U[4 * sa + c], U[5 * sa + c], U[6 * sa + c] };
+    prim_rot<DIR>(U[c], m, B, U[7 * sa + c], gamma, q, bad);
+}
+
+// 8-byte asynchronous global -> shared copy (LDGSTS): the data of the next march iteration is in
+// flight while the current interface is being solved, at no cost in registers
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
+{
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int MARCH_NT = 128;
+constexpr int MARCH_PF = 16;     // doubles prefetched per thread and iteration: U(s+1) 8, b_d 1, U'(s-1) 6
+
 template <int DIR, int LIM, bool TWO_D>
-__global__ void __launch_bounds__(128, 4)
+__global__ void __launch_bounds__(MARCH_NT, 4)
 k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__ bn, double *Uout,
               double *__restrict__ ct, StepParams *P, double scale, int seglen)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
+    __shared__ double pf[2][MARCH_PF][MARCH_NT];
+    const int t = threadIdx.x;
+    const int i = blockIdx.x * blockDim.x + t;
     if (i >= g.n[0]) return;
     // DIR = 1: grid.y = segment, grid.z = k;   DIR = 2: grid.y = j, grid.z = segment
     const int seg = DIR == 1 ? blockIdx.y : blockIdx.z;
@@ -216,6 +245,22 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
     const double gamma = g.gamma;
     const double fac = scale * P->dtdx[DIR];
     bool bad, anybad = false;
+
+    // what iteration s consumes: U of cell s+1, the face field on face s-1/2, U' of cell s-1
+    auto prefetch = [&](int slot, long long cs) {
+#pragma unroll
+        for (int v = 0; v < 8; v++) cp_async8(&pf[slot][v][t], Uin + v * sa + cs + st);
+        cp_async8(&pf[slot][8][t], bn + cs);
+        const long long cm = cs - st;
+        cp_async8(&pf[slot][9][t], Uout + cm);
+        cp_async8(&pf[slot][10][t], Uout + (1 + DIR) * sa + cm);
+        cp_async8(&pf[slot][11][t], Uout + (1 + T1) * sa + cm);
+        cp_async8(&pf[slot][12][t], Uout + (1 + T2) * sa + cm);
+        cp_async8(&pf[slot][13][t], Uout + 7 * sa + cm);
+        if (BZ2D) cp_async8(&pf[slot][14][t], Uout + 6 * sa + cm);
+        cp_async_commit();
+    };
+    prefetch(0, c);
 
     double qm[7], q0[7], d0[7], qL[7];
     load_rot<DIR>(Uin, sa, c - 2 * st, gamma, qm, bad);
@@ -234,9 +279,17 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
     double Fp[6] = { 0, 0, 0, 0, 0, 0 };                // previous face: rho, m_n, m_t1, m_t2, E, (B_z in 2D)
 
     for (int s = s0; s <= s1; s++, c += st) {
-        // cell s is in q0 (with d0 = q_s - q_{s-1}); fetch cell s+1
+        const int slot = (s - s0) & 1;
+        if (s < s1) { prefetch(slot ^ 1, c + st); cp_async_wait<1>(); }
+        else        { cp_async_wait<0>(); }
+        // cell s is in q0 (with d0 = q_s - q_{s-1}); cell s+1 arrives through shared memory
         double q1[7];
-        load_rot<DIR>(Uin, sa, c + st, gamma, q1, bad);
+        {
+            double m[3], B[3];
+            m[0] = pf[slot][1][t]; m[1] = pf[slot][2][t]; m[2] = pf[slot][3][t];
+            B[0] = pf[slot][4][t]; B[1] = pf[slot][5][t]; B[2] = pf[slot][6][t];
+            prim_rot<DIR>(pf[slot][0][t], m, B, pf[slot][7][t], gamma, q1, bad);
+        }
         if (s + 1 < s1) anybad |= bad;
         double qR[7];
 #pragma unroll
@@ -252,17 +305,17 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
         Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
         double F[7], w;
-        hlld(L, R, bn[c], gamma, g.igm1, F, w);
+        hlld(L, R, pf[slot][8][t], gamma, g.igm1, F, w);
 #pragma unroll
         for (int v = 0; v < 7; v++) qL[v] = q1[v];
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
-            Uout[cm] -= fac * (F[0] - Fp[0]);
-            Uout[(1 + DIR) * sa + cm] -= fac * (F[1] - Fp[1]);
-            Uout[(1 + T1) * sa + cm] -= fac * (F[2] - Fp[2]);
-            Uout[(1 + T2) * sa + cm] -= fac * (F[3] - Fp[3]);
-            Uout[7 * sa + cm] -= fac * (F[6] - Fp[4]);
-            if (TWO_D && DIR == 1) Uout[6 * sa + cm] -= fac * (F[4] - Fp[5]);   // F_y[B_z]
+            Uout[cm] = pf[slot][9][t] - fac * (F[0] - Fp[0]);
+            Uout[(1 + DIR) * sa + cm] = pf[slot][10][t] - fac * (F[1] - Fp[1]);
+            Uout[(1 + T1) * sa + cm] = pf[slot][11][t] - fac * (F[2] - Fp[2]);
+            Uout[(1 + T2) * sa + cm] = pf[slot][12][t] - fac * (F[3] - Fp[3]);
+            Uout[7 * sa + cm] = pf[slot][13][t] - fac * (F[6] - Fp[4]);
+            if (BZ2D) Uout[6 * sa + cm] = pf[slot][14][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
         }
         if (s < s1) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
