@@ -23,8 +23,13 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
         int k = (int)(z / ((long long)g.n[0] * g.n[1]));
         long long c = g.at(i, j, k);
         double rho = U[c], mx = U[g.sa + c], my = U[2 * g.sa + c], mz = U[3 * g.sa + c];
-        double B[3] = { U[4 * g.sa + c], U[5 * g.sa + c], U[6 * g.sa + c] };
-        double E = U[7 * g.sa + c];
+        double E = U[4 * g.sa + c];
+        // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
+        const double *b = U + S_B * g.sa;
+        double B[3] = { 0.5 * (b[c] + b[g.at(i + 1 == g.n[0] ? 0 : i + 1, j, k)]),
+                        0.5 * (b[g.sa + c] + b[g.sa + g.at(i, j + 1 == g.n[1] ? 0 : j + 1, k)]),
+                        g.act[2] ? 0.5 * (b[2 * g.sa + c] + b[2 * g.sa + g.at(i, j, k + 1 == g.n[2] ? 0 : k + 1)])
+                                 : b[2 * g.sa + c] };
         double v[3] = { mx / rho, my / rho, mz / rho };
         double p = (g.gamma - 1.0) * (E - 0.5 * (mx * v[0] + my * v[1] + mz * v[2])
                                         - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));

@@ -67,14 +67,17 @@ inline bool make_grid(Grid &g, int nx, int ny, int nz, int ghost)
     return true;
 }
 
-// array ids inside the single allocation (a state = 8 cell variables + 3 face fields, contiguous)
+// A state is 8 contiguous arrays: the five hydro variables and the three magnetic arrays.  Faces are
+// primary (R7): the cell-centred B of an active dimension is never stored, every consumer forms
+// 0.5 * (lower face + upper face) itself.  In 2D the third magnetic array holds the cell-centred B_z.
+enum StateVar { S_RHO = 0, S_MX = 1, S_MY = 2, S_MZ = 3, S_EN = 4, S_B = 5, S_COUNT = 8 };
+
+// array ids inside the single allocation
 enum ArrayId {
-    A_UA = 0,        // 8: state S^n (and S^{n+1})
-    A_BA = 8,        // 3: faces of S^n
-    A_UB = 11,       // 8: stage state S^1
-    A_BB = 19,       // 3: faces of S^1
-    A_CT = 22,       // 15: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3, CT_EG 3); staging outside a step
-    A_COUNT = 37
+    A_SA = 0,        // 8: state S^n (and S^{n+1})
+    A_SB = 8,        // 8: stage state S^1
+    A_CT = 16,       // 12: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3); staging outside a step
+    A_COUNT = 28
 };
 
 } // namespace pluto

@@ -1,13 +1,13 @@
 // kernels.cuh -- CUDA kernels of the MHD step (sm_100a).
 //
-// Per RK stage:   k_ghost<0,1,2>   periodic ghost fill of the 8 cell variables + face fields (a1)
+// Per RK stage:   k_ghost          periodic ghost fill of the 8 state arrays, one launch (a1)
 //                 k_sweep_x        cons->prim + PLM + HLLD + flux difference along x (a2-a5), "flat pencil"
 //                 k_sweep_march<1> the same along y, each thread marching up its own column
 //                 k_sweep_march<2> the same along z
-//                 k_emf            CT edge EMFs from the face data the sweeps left (a6)
-//                 k_ctface         face-B curl update [+ RK2 combine] (a6, a7)
-//                 k_cellb          cell-centred B := face mean
+//                 k_ct             CT: edge EMFs from the face data the sweeps left, face-B curl update
+//                                  [+ RK2 combine], marching along z with the edge EMFs in shared memory (a6, a7)
 // x is the contiguous index everywhere, so every warp access is a contiguous row segment.
+// A state is S[0..4] = rho, m_x, m_y, m_z, E and S[5..7] = b_x, b_y, b_z face fields (grid.h).
 #pragma once
 #include "grid.h"
 #include "mhd_device.cuh"
@@ -28,43 +28,51 @@ __device__ __forceinline__ int wrap_m1(int i, int n) { return i == 0 ? n - 1 : i
 __device__ __forceinline__ int wrap_p1(int i, int n) { return i == n - 1 ? 0 : i + 1; }
 
 // ---------------------------------------------------------------- periodic ghost fill (a1)
-// Fill the ghost layers of `narr` consecutive arrays along AXIS: index g in [-ng,0) <- g + n,
-// g in [n, n+ng] <- g - n (cells and faces alike; face n duplicates face 0).  Launched x, then y,
-// then z over the full padded extent of the other axes so edges and corners come out right
-// (the paper exchanges with diagonal neighbours for the same reason).
-__global__ void k_ghost_x(Grid g, double *__restrict__ base)
+// Every ghost position (index g in [-ng, 0) or [n, n+ng] along at least one active axis; cells and
+// faces alike, face n duplicates face 0) receives the value of its periodic image in the interior:
+// index g -> g + n or g - n along every axis at once.  Edges and corners therefore come out right in
+// ONE launch (the paper exchanges with diagonal neighbours for the same reason), and
+// sources are never written, so there is no ordering between positions.  The ghost set is walked as
+// three slab families: z-ghost planes (full padded rows), y-ghost rows of interior planes, x-ghost
+// ends of interior rows.
+__global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base, int narr)
 {
-    // one thread per padded row (j,k); the 2*ng+1 ghost cells of a row are strided by nothing
-    // useful, so each thread walks them itself
-    const long long rows = (long long)g.tot[1] * g.tot[2];
-    long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (r >= rows) return;
-    double *a = base + (long long)blockIdx.y * g.sa + r * g.st[1] + g.off[0];
-    const int n = g.n[0];
-    for (int s = 1; s <= g.ng; s++) a[-s] = a[n - s];
-    for (int s = 0; s <= g.ng; s++) a[n + s] = a[s];
-}
-
-template <int AXIS>   // AXIS = 1 or 2
-__global__ void k_ghost_yz(Grid g, double *__restrict__ base, int narr)
-{
-    const int nghost = 2 * g.ng + 1;
-    int x = blockIdx.x * blockDim.x + threadIdx.x;
-    if (x >= g.tot[0]) return;
-    int slot, other, arr;
-    if (AXIS == 1) { slot = blockIdx.y; other = blockIdx.z % g.tot[2]; arr = blockIdx.z / g.tot[2]; }
-    else           { other = blockIdx.y; slot = blockIdx.z % nghost;   arr = blockIdx.z / nghost; }
-    if (arr >= narr) return;
-    const int n = g.n[AXIS];
-    int gi = slot < g.ng ? slot - g.ng : n + (slot - g.ng);
-    int src = gi < 0 ? gi + n : gi - n;
-    double *a = base + (long long)arr * g.sa + x;
-    if (AXIS == 1) {
-        a += (long long)other * g.st[2];
-        a[(long long)(gi + g.off[1]) * g.st[1]] = a[(long long)(src + g.off[1]) * g.st[1]];
-    } else {
-        a += (long long)other * g.st[1];
-        a[(long long)(gi + g.off[2]) * g.st[2]] = a[(long long)(src + g.off[2]) * g.st[2]];
+    const int ng = g.ng, ngh = 2 * ng + 1;
+    const int gi = g.n[0] + ngh;                          // x positions -ng .. n+ng
+    const int gj = g.act[1] ? g.n[1] + ngh : 1;
+    const long long nZ = g.act[2] ? (long long)ngh * gj * gi : 0;
+    const long long nY = g.act[1] ? (long long)g.n[2] * ngh * gi : 0;
+    const long long nX = (long long)g.n[2] * g.n[1] * ngh;
+    const long long total = nZ + nY + nX;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        int i, j, k;
+        if (t < nZ) {
+            i = (int)(t % gi) - ng;
+            long long r = t / gi;
+            j = (int)(r % gj) - (g.act[1] ? ng : 0);
+            int s = (int)(r / gj);
+            k = s < ng ? s - ng : g.n[2] + (s - ng);
+        } else if (t < nZ + nY) {
+            long long u = t - nZ;
+            i = (int)(u % gi) - ng;
+            long long r = u / gi;
+            int s = (int)(r % ngh);
+            j = s < ng ? s - ng : g.n[1] + (s - ng);
+            k = (int)(r / ngh);
+        } else {
+            long long u = t - nZ - nY;
+            int s = (int)(u % ngh);
+            i = s < ng ? s - ng : g.n[0] + (s - ng);
+            long long r = u / ngh;
+            j = (int)(r % g.n[1]);
+            k = (int)(r / g.n[1]);
+        }
+        // (extents may be as small as ng, so index n+ng can need two periods)
+        const int si = (i + 2 * g.n[0]) % g.n[0], sj = (j + 2 * g.n[1]) % g.n[1], sk = (k + 2 * g.n[2]) % g.n[2];
+        const long long dst = g.at(i, j, k), src = g.at(si, sj, sk);
+#pragma unroll 8
+        for (int a = 0; a < narr; a++) base[a * g.sa + dst] = base[a * g.sa + src];
     }
 }
 
@@ -73,8 +81,16 @@ __global__ void k_ghost_yz(Grid g, double *__restrict__ base, int narr)
 //                         z: F_z[Bx], F_z[By]) on the lower d-face of each interior cell
 // ct + CT_W + d         : upwind weight on that face
 // ct + CT_EC + e        : cell-centred EMF component e, E^c = -(v x B)
-// ct + CT_EG + e        : edge EMF component e at the lower (a,b) edge of each interior cell
-enum { CT_FEM = 0, CT_W = 6, CT_EC = 9, CT_EG = 12, CT_COUNT = 15 };
+enum { CT_FEM = 0, CT_W = 6, CT_EC = 9, CT_COUNT = 12 };
+
+// cell-centred B of cell c from the face arrays b = S + S_B*sa (R7); 2D: b[2] is the cell-centred B_z
+template <bool TWO_D>
+__device__ __forceinline__ void cell_b(const Grid &g, const double *__restrict__ b, long long c, double B[3])
+{
+    B[0] = 0.5 * (b[c] + b[c + 1]);
+    B[1] = 0.5 * (b[g.sa + c] + b[g.sa + c + g.st[1]]);
+    B[2] = TWO_D ? b[2 * g.sa + c] : 0.5 * (b[2 * g.sa + c] + b[2 * g.sa + c + g.st[2]]);
+}
 
 // ---------------------------------------------------------------- x sweep (a2-a5 fused)
 // The rows of the grid are laid end to end as one list of "items" (cells -2 .. nx+1 of each row).
@@ -88,8 +104,7 @@ constexpr int SX_OUT = SX_NT - 4;
 
 template <int LIM, bool TWO_D>
 __global__ void __launch_bounds__(SX_NT, 4)
-k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx, double *Uout,
-          double *__restrict__ ct, StepParams *P, int combine)
+k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P, int combine)
 {
     __shared__ double sP[8][SX_NT];     // primitives; rows 0..5 are reused for the fluxes
     __shared__ double sQ[7][SX_NT];     // q^L = q + slope/2 of each cell
@@ -101,28 +116,27 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
     const bool valid = item >= 0 && item < nitems;
     int f = -100;
     long long c = 0;
-    double rho = 1.0, mx = 0, my = 0, mz = 0, En = 0, Bzc = 0;
+    double rho = 1.0, mx = 0, my = 0, mz = 0, En = 0;
     double q[7] = { 1, 0, 0, 0, 0, 0, 1 };    // rho, vx, vy, vz, By, Bz, p
-    double Bxc = 0, bxf = 0;
-    double o0 = 0, o1 = 0, o2 = 0, o3 = 0, o6 = 0, o7 = 0;   // S^n of the cell (combine stage)
+    double Bc[3] = { 0, 0, 0 }, bxf = 0;
+    double o0 = 0, o1 = 0, o2 = 0, o3 = 0, o4 = 0, o7 = 0;   // S^n of the cell (combine stage)
     if (valid) {
         long long row = item / M;
         f = (int)(item - row * M) - 2;
         int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]);
         c = g.at(f, j, k);
-        rho = Uin[c]; mx = Uin[sa + c]; my = Uin[2 * sa + c]; mz = Uin[3 * sa + c];
-        Bxc = Uin[4 * sa + c];
-        double By = Uin[5 * sa + c];
-        Bzc = Uin[6 * sa + c];
-        En = Uin[7 * sa + c];
-        bxf = bx[c];
+        rho = Sin[c]; mx = Sin[sa + c]; my = Sin[2 * sa + c]; mz = Sin[3 * sa + c];
+        En = Sin[4 * sa + c];
+        bxf = Sin[S_B * sa + c];
+        cell_b<TWO_D>(g, Sin + S_B * sa, c, Bc);
         if (combine && f >= 0 && f < nx) {     // issued with the other loads: one memory round trip per block
-            o0 = Uout[c]; o1 = Uout[sa + c]; o2 = Uout[2 * sa + c]; o3 = Uout[3 * sa + c]; o7 = Uout[7 * sa + c];
-            if (TWO_D) o6 = Uout[6 * sa + c];
+            o0 = Sout[c]; o1 = Sout[sa + c]; o2 = Sout[2 * sa + c]; o3 = Sout[3 * sa + c]; o4 = Sout[4 * sa + c];
+            if (TWO_D) o7 = Sout[7 * sa + c];
         }
         double ir = rcp_fast(rho);
-        q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = By; q[5] = Bzc;
-        q[6] = (g.gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3]) - 0.5 * (Bxc * Bxc + By * By + Bzc * Bzc));
+        q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = Bc[1]; q[5] = Bc[2];
+        q[6] = (g.gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3])
+                                     - 0.5 * (Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2]));
         if (f >= 0 && f < nx && (!(rho > 0.0) || !(q[6] > 0.0) || isinf(rho) || isinf(q[6]))) P->err = 1;
     }
 #pragma unroll
@@ -161,23 +175,23 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
         double r1 = mx - dtdx * (sP[1][t + 1] - F[1]);
         double r2 = my - dtdx * (sP[2][t + 1] - F[2]);
         double r3 = mz - dtdx * (sP[3][t + 1] - F[3]);
-        double r7 = En - dtdx * (sP[4][t + 1] - F[6]);
+        double r4 = En - dtdx * (sP[4][t + 1] - F[6]);
         if (combine) {
             r0 = 0.5 * (o0 + r0); r1 = 0.5 * (o1 + r1); r2 = 0.5 * (o2 + r2);
-            r3 = 0.5 * (o3 + r3); r7 = 0.5 * (o7 + r7);
+            r3 = 0.5 * (o3 + r3); r4 = 0.5 * (o4 + r4);
         }
-        Uout[c] = r0; Uout[sa + c] = r1; Uout[2 * sa + c] = r2; Uout[3 * sa + c] = r3; Uout[7 * sa + c] = r7;
+        Sout[c] = r0; Sout[sa + c] = r1; Sout[2 * sa + c] = r2; Sout[3 * sa + c] = r3; Sout[4 * sa + c] = r4;
         if (TWO_D) {   // B_z has no faces in 2D: cell centred, flux updated
-            double r6 = Bzc - dtdx * (sP[5][t + 1] - F[5]);
-            Uout[6 * sa + c] = combine ? 0.5 * (o6 + r6) : r6;
+            double r7 = Bc[2] - dtdx * (sP[5][t + 1] - F[5]);
+            Sout[7 * sa + c] = combine ? 0.5 * (o7 + r7) : r7;
         }
         ct[(CT_FEM + 0) * sa + c] = F[4];
         ct[(CT_FEM + 1) * sa + c] = F[5];
         ct[(CT_W + 0) * sa + c] = w;
         // cell-centred EMF  E^c = -(v x B)
         ct[(CT_EC + 0) * sa + c] = q[3] * q[4] - q[2] * q[5];
-        ct[(CT_EC + 1) * sa + c] = q[1] * q[5] - q[3] * Bxc;
-        ct[(CT_EC + 2) * sa + c] = q[2] * Bxc - q[1] * q[4];
+        ct[(CT_EC + 1) * sa + c] = q[1] * q[5] - q[3] * Bc[0];
+        ct[(CT_EC + 2) * sa + c] = q[2] * Bc[0] - q[1] * q[4];
     }
 }
 
@@ -185,9 +199,12 @@ k_sweep_x(Grid g, const double *__restrict__ Uin, const double *__restrict__ bx,
 // Thread = one column (fixed i and transverse index), marching along DIR over `seglen` cells.  It
 // keeps the running q^L, the last two primitive states (as state + difference) and the previous
 // flux in registers, so every cell is loaded and converted once and every flux is computed once per
-// segment (+1 at the segment end).  Uout already holds the x-sweep result and is updated in place:
-//     Uout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (stage 1) or 1/2 (combine stage).
-// cons -> rotated primitives of one cell (Eq. 7)
+// segment (+1 at the segment end).  Sout already holds the x-sweep result and is updated in place:
+//     Sout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (stage 1) or 1/2 (combine stage).
+// The operands of iteration s+1 travel global -> shared by 8-byte cp.async while interface s is
+// being solved (two slots per thread, no block synchronisation: a thread only reads what it copied).
+
+// cons -> rotated primitives of one cell (Eq. 7); B = cell-centred field
 template <int DIR>
 __device__ __forceinline__ void prim_rot(double rho, const double m[3], const double B[3], double En, double gamma,
                                          double q[7], bool &bad)
@@ -201,17 +218,17 @@ __device__ __forceinline__ void prim_rot(double rho, const double m[3], const do
     bad = !(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p);
 }
 
-template <int DIR>
-__device__ __forceinline__ void load_rot(const double *__restrict__ U, long long sa, long long c, double gamma,
-                                         double q[7], bool &bad)
+template <int DIR, bool TWO_D>
+__device__ __forceinline__ void load_rot(const Grid &g, const double *__restrict__ S, long long c, double q[7], bool &bad)
 {
-    double m[3] = { U[sa + c], U[2 * sa + c], U[3 * sa + c] };
-    double B[3] = { U[4 * sa + c], U[5 * sa + c], U[6 * sa + c] };
-    prim_rot<DIR>(U[c], m, B, U[7 * sa + c], gamma, q, bad);
+    const long long sa = g.sa;
+    double m[3] = { S[sa + c], S[2 * sa + c], S[3 * sa + c] };
+    double B[3];
+    cell_b<TWO_D>(g, S + S_B * sa, c, B);
+    prim_rot<DIR>(S[c], m, B, S[4 * sa + c], g.gamma, q, bad);
 }
 
-// 8-byte asynchronous global -> shared copy (LDGSTS): the data of the next march iteration is in
-// flight while the current interface is being solved, at no cost in registers
+// 8-byte asynchronous global -> shared copy (LDGSTS)
 __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
 {
     unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -222,12 +239,12 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 constexpr int MARCH_NT = 128;
-constexpr int MARCH_PF = 16;     // doubles prefetched per thread and iteration: U(s+1) 8, b_d 1, U'(s-1) 6
+constexpr int MARCH_PF = 16;     // doubles per thread and iteration: U(s+1) 5, faces 5, U'(s-1) 6
 
 template <int DIR, int LIM, bool TWO_D>
 __global__ void __launch_bounds__(MARCH_NT, 4)
-k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__ bn, double *Uout,
-              double *__restrict__ ct, StepParams *P, double scale, int seglen)
+k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
+              double scale, int seglen)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
@@ -244,30 +261,39 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
     long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
     const double gamma = g.gamma;
     const double fac = scale * P->dtdx[DIR];
+    const double *__restrict__ bn = Sin + (S_B + DIR) * sa;        // normal face field
+    const double *__restrict__ b1 = Sin + (S_B + T1) * sa;         // transverse fields
+    const double *__restrict__ b2 = Sin + (S_B + T2) * sa;
+    const long long st1 = g.st[T1], st2 = g.st[T2];
     bool bad, anybad = false;
 
-    // what iteration s consumes: U of cell s+1, the face field on face s-1/2, U' of cell s-1
+    // what iteration s consumes: U of cell s+1 and the faces around it, U' of cell s-1
     auto prefetch = [&](int slot, long long cs) {
+        const long long cn = cs + st;                    // cell s+1
 #pragma unroll
-        for (int v = 0; v < 8; v++) cp_async8(&pf[slot][v][t], Uin + v * sa + cs + st);
-        cp_async8(&pf[slot][8][t], bn + cs);
+        for (int v = 0; v < 5; v++) cp_async8(&pf[slot][v][t], Sin + v * sa + cn);
+        cp_async8(&pf[slot][5][t], bn + cn + st);        // upper normal face of cell s+1
+        cp_async8(&pf[slot][6][t], b1 + cn);             // (2D: the cell-centred B_z itself)
+        if (!(TWO_D && T1 == 2)) cp_async8(&pf[slot][7][t], b1 + cn + st1);
+        cp_async8(&pf[slot][8][t], b2 + cn);
+        if (!(TWO_D && T2 == 2)) cp_async8(&pf[slot][9][t], b2 + cn + st2);
         const long long cm = cs - st;
-        cp_async8(&pf[slot][9][t], Uout + cm);
-        cp_async8(&pf[slot][10][t], Uout + (1 + DIR) * sa + cm);
-        cp_async8(&pf[slot][11][t], Uout + (1 + T1) * sa + cm);
-        cp_async8(&pf[slot][12][t], Uout + (1 + T2) * sa + cm);
-        cp_async8(&pf[slot][13][t], Uout + 7 * sa + cm);
-        if (BZ2D) cp_async8(&pf[slot][14][t], Uout + 6 * sa + cm);
+        cp_async8(&pf[slot][10][t], Sout + cm);
+        cp_async8(&pf[slot][11][t], Sout + (1 + DIR) * sa + cm);
+        cp_async8(&pf[slot][12][t], Sout + (1 + T1) * sa + cm);
+        cp_async8(&pf[slot][13][t], Sout + (1 + T2) * sa + cm);
+        cp_async8(&pf[slot][14][t], Sout + 4 * sa + cm);
+        if (BZ2D) cp_async8(&pf[slot][15][t], Sout + 7 * sa + cm);
         cp_async_commit();
     };
     prefetch(0, c);
 
     double qm[7], q0[7], d0[7], qL[7];
-    load_rot<DIR>(Uin, sa, c - 2 * st, gamma, qm, bad);
-    load_rot<DIR>(Uin, sa, c - st, gamma, q0, bad);
+    load_rot<DIR, TWO_D>(g, Sin, c - 2 * st, qm, bad);
+    load_rot<DIR, TWO_D>(g, Sin, c - st, q0, bad);
 #pragma unroll
     for (int v = 0; v < 7; v++) d0[v] = q0[v] - qm[v];
-    load_rot<DIR>(Uin, sa, c, gamma, qm, bad);          // qm now holds cell s0
+    load_rot<DIR, TWO_D>(g, Sin, c, qm, bad);           // qm now holds cell s0
     anybad |= bad;
 #pragma unroll
     for (int v = 0; v < 7; v++) {
@@ -277,6 +303,8 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
         d0[v] = d1;
     }
     double Fp[6] = { 0, 0, 0, 0, 0, 0 };                // previous face: rho, m_n, m_t1, m_t2, E, (B_z in 2D)
+    double bface = bn[c];                               // normal field on face s - 1/2
+    double bnext = bn[c + st];                          // ... on face s + 1/2
 
     for (int s = s0; s <= s1; s++, c += st) {
         const int slot = (s - s0) & 1;
@@ -284,11 +312,14 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
         else        { cp_async_wait<0>(); }
         // cell s is in q0 (with d0 = q_s - q_{s-1}); cell s+1 arrives through shared memory
         double q1[7];
+        const double bup = pf[slot][5][t];
         {
             double m[3], B[3];
             m[0] = pf[slot][1][t]; m[1] = pf[slot][2][t]; m[2] = pf[slot][3][t];
-            B[0] = pf[slot][4][t]; B[1] = pf[slot][5][t]; B[2] = pf[slot][6][t];
-            prim_rot<DIR>(pf[slot][0][t], m, B, pf[slot][7][t], gamma, q1, bad);
+            B[DIR] = 0.5 * (bnext + bup);
+            B[T1] = (TWO_D && T1 == 2) ? pf[slot][6][t] : 0.5 * (pf[slot][6][t] + pf[slot][7][t]);
+            B[T2] = (TWO_D && T2 == 2) ? pf[slot][8][t] : 0.5 * (pf[slot][8][t] + pf[slot][9][t]);
+            prim_rot<DIR>(pf[slot][0][t], m, B, pf[slot][4][t], gamma, q1, bad);
         }
         if (s + 1 < s1) anybad |= bad;
         double qR[7];
@@ -305,17 +336,18 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
         Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
         double F[7], w;
-        hlld(L, R, pf[slot][8][t], gamma, g.igm1, F, w);
+        hlld(L, R, bface, gamma, g.igm1, F, w);
+        bface = bnext; bnext = bup;
 #pragma unroll
         for (int v = 0; v < 7; v++) qL[v] = q1[v];
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
-            Uout[cm] = pf[slot][9][t] - fac * (F[0] - Fp[0]);
-            Uout[(1 + DIR) * sa + cm] = pf[slot][10][t] - fac * (F[1] - Fp[1]);
-            Uout[(1 + T1) * sa + cm] = pf[slot][11][t] - fac * (F[2] - Fp[2]);
-            Uout[(1 + T2) * sa + cm] = pf[slot][12][t] - fac * (F[3] - Fp[3]);
-            Uout[7 * sa + cm] = pf[slot][13][t] - fac * (F[6] - Fp[4]);
-            if (BZ2D) Uout[6 * sa + cm] = pf[slot][14][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
+            Sout[cm] = pf[slot][10][t] - fac * (F[0] - Fp[0]);
+            Sout[(1 + DIR) * sa + cm] = pf[slot][11][t] - fac * (F[1] - Fp[1]);
+            Sout[(1 + T1) * sa + cm] = pf[slot][12][t] - fac * (F[2] - Fp[2]);
+            Sout[(1 + T2) * sa + cm] = pf[slot][13][t] - fac * (F[3] - Fp[3]);
+            Sout[4 * sa + cm] = pf[slot][14][t] - fac * (F[6] - Fp[4]);
+            if (BZ2D) Sout[7 * sa + cm] = pf[slot][15][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
         }
         if (s < s1) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
@@ -327,22 +359,16 @@ k_sweep_march(Grid g, const double *__restrict__ Uin, const double *__restrict__
     if (anybad) P->err = 1;
 }
 
-// ---------------------------------------------------------------- CT: edge EMFs (a6, R6)
-// Thread = interior cell; computes the EMF components on its three lower edges (only E_z in 2D):
-// arithmetic mean of the four face EMFs plus the upwinded half-cell differences to the cell-centred
-// EMFs.  Neighbours are taken with periodic wrap, so the CT work arrays need no ghost layers.
+// ---------------------------------------------------------------- CT (a6, R6) [+ RK2 combine of the faces (a7)]
+// Edge EMF component EC at the lower (A,B) edge of a cell, A = EC+1, B = EC+2 (cyclic): arithmetic
+// mean of the four face EMFs plus the upwinded half-cell differences to the cell-centred EMFs.
+// c11 = the cell, c01 = its neighbour at A-1, c10 = at B-1, c00 = at A-1,B-1 (periodic wrap done by
+// the caller, so the CT work arrays need no ghost layers).
 template <int EC>
-__device__ __forceinline__ double edge_emf(const Grid &g, const double *__restrict__ ct, int i, int j, int k)
+__device__ __forceinline__ double edge_emf(const double *__restrict__ ct, long long sa,
+                                           long long c11, long long c01, long long c10, long long c00)
 {
     constexpr int A = (EC + 1) % 3, B = (EC + 2) % 3;
-    const long long sa = g.sa;
-    int p[3] = { i, j, k };
-    int pa[3] = { i, j, k }, pb[3] = { i, j, k }, pab[3] = { i, j, k };
-    pa[A] = wrap_m1(p[A], g.n[A]);
-    pb[B] = wrap_m1(p[B], g.n[B]);
-    pab[A] = pa[A]; pab[B] = pb[B];
-    const long long c11 = g.at(p[0], p[1], p[2]), c01 = g.at(pa[0], pa[1], pa[2]);
-    const long long c10 = g.at(pb[0], pb[1], pb[2]), c00 = g.at(pab[0], pab[1], pab[2]);
     const double *Fa = ct + (CT_FEM + 2 * A) * sa;       // F_a[B_b]: first induction flux of sweep a
     const double *Fb = ct + (CT_FEM + 2 * B + 1) * sa;   // F_b[B_a]: second induction flux of sweep b
     const double *Wa = ct + (CT_W + A) * sa, *Wb = ct + (CT_W + B) * sa;
@@ -358,61 +384,95 @@ __device__ __forceinline__ double edge_emf(const Grid &g, const double *__restri
     return 0.25 * (Ea_lo + Ea_hi + Eb_lo + Eb_hi) + 0.25 * (t1 - t2) + 0.25 * (t3 - t4);
 }
 
-__global__ void k_emf(Grid g, Box box, double *__restrict__ ct)
-{
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
-    const long long c = g.at(i, j, k), sa = g.sa;
-    double ez = edge_emf<2>(g, ct, i, j, k);
-    if (g.act[2]) {
-        double ex = edge_emf<0>(g, ct, i, j, k);
-        double ey = edge_emf<1>(g, ct, i, j, k);
-        ct[(CT_EG + 0) * sa + c] = ex;
-        ct[(CT_EG + 1) * sa + c] = ey;
-    }
-    ct[(CT_EG + 2) * sa + c] = ez;
-}
+// in-plane offsets of a cell and of its x-1, y-1 and (x-1,y-1) neighbours (periodic)
+struct Nb { long long c, x, y, xy; };
 
-// ---------------------------------------------------------------- CT: face update  db/dt = -curl E  [+ combine (a7)]
-// Thread = interior cell, updates its three lower faces; the +1 edge neighbours wrap periodically.
-// COMBINE: bout <- (bout + that)/2 in place (bout holds the faces of S^n).
-template <bool COMBINE>
-__global__ void k_ctface(Grid g, Box box, const double *__restrict__ bin, const double *__restrict__ ct,
-                         double *bout, const StepParams *__restrict__ P)
+// Block = CT_TX x CT_TY columns marching along z over `seglen` planes.  Per plane k every thread
+// evaluates the three EMFs on the lower edges of its cell -- E_z(i-1/2, j-1/2, k) and, one plane
+// ahead, E_x(i, j-1/2, k+1/2), E_y(i-1/2, j, k+1/2) -- and leaves them in shared memory.  After one
+// barrier the lower faces of the cell are updated with  db/dt = -curl E  (COMBINE: bout <- (bout +
+// that)/2 in place, bout holding the faces of S^n).  E_x, E_y of plane k-1/2 stay in registers from
+// the previous iteration, so no edge EMF is ever stored in HBM.  Tiles overlap by one column and one
+// row: the threads of the last column / row only supply the edges just outside the tile, so all
+// threads run the same code (no divergent extra work) and each face is still written exactly once.
+constexpr int CT_TX = 32, CT_TY = 8;
+
+template <bool COMBINE, bool TWO_D>
+__global__ void __launch_bounds__(CT_TX * CT_TY, 3)
+k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, double *bout,
+     const StepParams *__restrict__ P, int seglen, double *__restrict__ dbg)
 {
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
-    const long long c = g.at(i, j, k), sa = g.sa;
+    __shared__ double sEz[2][CT_TY][CT_TX];
+    __shared__ double sEx[3][CT_TY][CT_TX];
+    __shared__ double sEy[3][CT_TY][CT_TX];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int i = blockIdx.x * (CT_TX - 1) + tx, j = blockIdx.y * (CT_TY - 1) + ty;
+    // cells i <= n0, j <= n1 supply edges (index n wraps to 0); faces are updated by the inner threads
+    const bool edge = i <= g.n[0] && j <= g.n[1];
+    const bool upd = tx < CT_TX - 1 && ty < CT_TY - 1 && i < g.n[0] && j < g.n[1];
+    const int k0 = blockIdx.z * seglen, k1 = min(k0 + seglen, g.n[2]);
+    const long long sa = g.sa, st2 = g.st[2];
     const double dt = P->dt;
-    const double *Ex = ct + (CT_EG + 0) * sa, *Ey = ct + (CT_EG + 1) * sa, *Ez = ct + (CT_EG + 2) * sa;
-    const long long cxp = g.at(wrap_p1(i, g.n[0]), j, k);
-    const long long cyp = g.at(i, wrap_p1(j, g.n[1]), k);
-    const double ez = Ez[c];
-    double bxn, byn;
-    if (g.act[2]) {
-        const long long czp = g.at(i, j, wrap_p1(k, g.n[2]));
-        const double ex = Ex[c], ey = Ey[c];
-        bxn = bin[c] - dt * ((Ez[cyp] - ez) / g.dx[1] - (Ey[czp] - ey) / g.dx[2]);
-        byn = bin[sa + c] - dt * ((Ex[czp] - ex) / g.dx[2] - (Ez[cxp] - ez) / g.dx[0]);
-        double bzn = bin[2 * sa + c] - dt * ((Ey[cxp] - ey) / g.dx[0] - (Ex[cyp] - ex) / g.dx[1]);
-        bout[2 * sa + c] = COMBINE ? 0.5 * (bout[2 * sa + c] + bzn) : bzn;
-    } else {
-        bxn = bin[c] - dt * ((Ez[cyp] - ez) / g.dx[1] - 0.0);
-        byn = bin[sa + c] - dt * (0.0 - (Ez[cxp] - ez) / g.dx[0]);
-    }
-    bout[c] = COMBINE ? 0.5 * (bout[c] + bxn) : bxn;
-    bout[sa + c] = COMBINE ? 0.5 * (bout[sa + c] + byn) : byn;
-}
 
-// ---------------------------------------------------------------- cell-centred B := face mean (R7)
-__global__ void k_cellb(Grid g, Box box, const double *__restrict__ b, double *__restrict__ U)
-{
-    int i, j, k;
-    if (!thread_zone(box, i, j, k)) return;
-    const long long c = g.at(i, j, k), sa = g.sa;
-    U[4 * sa + c] = 0.5 * (b[c] + b[g.at(wrap_p1(i, g.n[0]), j, k)]);
-    U[5 * sa + c] = 0.5 * (b[sa + c] + b[sa + g.at(i, wrap_p1(j, g.n[1]), k)]);
-    if (g.act[2]) U[6 * sa + c] = 0.5 * (b[2 * sa + c] + b[2 * sa + g.at(i, j, wrap_p1(k, g.n[2]))]);
+    // clamp the indices of idle threads so that every address below is legal
+    const int ii = edge ? (i == g.n[0] ? 0 : i) : 0, jj = edge ? (j == g.n[1] ? 0 : j) : 0;
+    const int im = wrap_m1(ii, g.n[0]), jm = wrap_m1(jj, g.n[1]);
+    const long long r0 = (long long)(jj + g.off[1]) * g.st[1] + g.off[0];
+    const long long rm = (long long)(jm + g.off[1]) * g.st[1] + g.off[0];
+    const Nb own = { r0 + ii, r0 + im, rm + ii, rm + im };
+
+    auto plane = [&](int k) { return (long long)(k + g.off[2]) * st2; };
+    auto Ez = [&](const Nb &n, long long pk) { return edge_emf<2>(ct, sa, pk + n.c, pk + n.x, pk + n.y, pk + n.xy); };
+    auto Ex = [&](const Nb &n, long long pk, long long pm) { return edge_emf<0>(ct, sa, pk + n.c, pk + n.y, pm + n.c, pm + n.y); };
+    auto Ey = [&](const Nb &n, long long pk, long long pm) { return edge_emf<1>(ct, sa, pk + n.c, pm + n.c, pk + n.x, pm + n.x); };
+
+    double exP = 0.0, eyP = 0.0;
+    if (!TWO_D && edge) {                                   // edges of plane k0 - 1/2
+        const long long pk = plane(k0), pm = plane(wrap_m1(k0, g.n[2]));
+        exP = Ex(own, pk, pm); eyP = Ey(own, pk, pm);
+        sEx[k0 % 3][ty][tx] = exP; sEy[k0 % 3][ty][tx] = eyP;
+    }
+
+    for (int k = k0; k < k1; k++) {
+        const long long pk = plane(k);
+        const long long c = pk + own.c;
+        const int sz = k & 1, sl = k % 3, sn = (k + 1) % 3;
+        double ez = 0.0, exN = 0.0, eyN = 0.0;
+        double b0 = 0.0, b1 = 0.0, b2 = 0.0, o0 = 0.0, o1 = 0.0, o2 = 0.0;
+        if (upd) {                                          // issued together with the CT loads below
+            b0 = bin[c]; b1 = bin[sa + c];
+            if (!TWO_D) b2 = bin[2 * sa + c];
+            if (COMBINE) { o0 = bout[c]; o1 = bout[sa + c]; if (!TWO_D) o2 = bout[2 * sa + c]; }
+        }
+        if (edge) {
+            ez = Ez(own, pk);
+            sEz[sz][ty][tx] = ez;
+            if (!TWO_D) {
+                const long long pn = plane(wrap_p1(k, g.n[2]));      // plane k+1; its lower neighbour is k
+                exN = Ex(own, pn, pk); eyN = Ey(own, pn, pk);
+                sEx[sn][ty][tx] = exN; sEy[sn][ty][tx] = eyN;
+            }
+        }
+        __syncthreads();
+        if (upd) {
+            const double ezy = sEz[sz][ty + 1][tx], ezx = sEz[sz][ty][tx + 1];
+            double bxn, byn;
+            if (!TWO_D) {
+                const double eyx = sEy[sl][ty][tx + 1], exy = sEx[sl][ty + 1][tx];
+                bxn = b0 - dt * ((ezy - ez) / g.dx[1] - (eyN - eyP) / g.dx[2]);
+                byn = b1 - dt * ((exN - exP) / g.dx[2] - (ezx - ez) / g.dx[0]);
+                double bzn = b2 - dt * ((eyx - eyP) / g.dx[0] - (exy - exP) / g.dx[1]);
+                bout[2 * sa + c] = COMBINE ? 0.5 * (o2 + bzn) : bzn;
+            } else {
+                bxn = b0 - dt * ((ezy - ez) / g.dx[1] - 0.0);
+                byn = b1 - dt * (0.0 - (ezx - ez) / g.dx[0]);
+            }
+            bout[c] = COMBINE ? 0.5 * (o0 + bxn) : bxn;
+            bout[sa + c] = COMBINE ? 0.5 * (o1 + byn) : byn;
+            if (dbg) { dbg[c] = exP; dbg[sa + c] = eyP; dbg[2 * sa + c] = ez; }
+        }
+        exP = exN; eyP = eyN;
+    }
 }
 
 // ---------------------------------------------------------------- API layout <-> padded layout
@@ -431,6 +491,18 @@ __global__ void k_pack(Grid g, Box box, const double *__restrict__ src, int m0, 
     // periodic wrap: the duplicate upper face (index n) is face 0
     int ii = i % g.n[0], jj = j % g.n[1], kk = k % g.n[2];
     dst[((long long)k * m1 + j) * m0 + i] = src[g.at(ii, jj, kk)];
+}
+
+// cell-centred B of the API's U[4..6]: the mean of the two faces (R7); 2D: U[6] is the stored B_z
+__global__ void k_pack_cellb(Grid g, Box box, const double *__restrict__ b, double *__restrict__ dst, long long n)
+{
+    int i, j, k;
+    if (!thread_zone(box, i, j, k)) return;
+    const long long sa = g.sa, c = g.at(i, j, k);
+    const long long o = ((long long)k * g.n[1] + j) * g.n[0] + i;
+    dst[o] = 0.5 * (b[c] + b[g.at(wrap_p1(i, g.n[0]), j, k)]);
+    dst[n + o] = 0.5 * (b[sa + c] + b[sa + g.at(i, wrap_p1(j, g.n[1]), k)]);
+    dst[2 * n + o] = g.act[2] ? 0.5 * (b[2 * sa + c] + b[2 * sa + g.at(i, j, wrap_p1(k, g.n[2]))]) : b[2 * sa + c];
 }
 
 } // namespace pluto

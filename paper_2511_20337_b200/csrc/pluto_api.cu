@@ -20,10 +20,8 @@ using namespace pluto;
 
 namespace {
 
-enum KernelId { K_GHOST = 0, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_EMF, K_CTFACE, K_CELLB,
-                K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
-const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_x", "sweep_y", "sweep_z",
-                                            "ct_edge_emf", "ct_face_update", "cell_b_mean",
+enum KernelId { K_GHOST = 0, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_CT, K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
+const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_x", "sweep_y", "sweep_z", "ct",
                                             "dt_max", "scalars", "pack_unpack" };
 
 struct Context {
@@ -133,23 +131,16 @@ void destroy_graphs()
 
 // ---------------------------------------------------------------- launch sequences
 
-// ghost layers of the 8 cell variables + face fields of one state (11 contiguous arrays; 10 in 2D)
-void fill_ghosts(double *first)
+// ghost layers of the 8 arrays of one state, one launch
+void fill_ghosts(double *state)
 {
-    const Grid &g = C.g;
-    const int ngh = 2 * g.ng + 1;
-    const int narr = 8 + g.ndim;
-    cudaStream_t s = C.stream;
-    const long long rows = (long long)g.tot[1] * g.tot[2];
-    LAUNCH(K_GHOST, k_ghost_x<<<dim3((unsigned)((rows + 127) / 128), narr), 128, 0, s>>>(g, first));
-    LAUNCH(K_GHOST, k_ghost_yz<1><<<dim3((g.tot[0] + 127) / 128, ngh, g.tot[2] * narr), 128, 0, s>>>(g, first, narr));
-    if (g.act[2])
-        LAUNCH(K_GHOST, k_ghost_yz<2><<<dim3((g.tot[0] + 127) / 128, g.tot[1], ngh * narr), 128, 0, s>>>(g, first, narr));
+    LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 8, 256, 0, C.stream>>>(C.g, state, S_COUNT));
 }
 
+// segments of a marching kernel: enough independent threads for ~8 waves of 16 warps per SM,
+// segments no shorter than 16 cells
 int march_seglen(int n, long long columns)
 {
-    // enough independent threads for ~8 waves of 16 warps per SM, segments no shorter than 16 cells
     const long long want = (long long)C.sm_count * 16 * 32 * 8;
     long long nseg = (want + columns - 1) / columns;
     if (nseg < 1) nseg = 1;
@@ -160,57 +151,70 @@ int march_seglen(int n, long long columns)
 }
 
 template <int LIM, bool TWO_D>
-void launch_sweeps(const double *Uin, const double *bin, double *Uout, bool combine)
+void launch_sweeps(const double *Sin, double *Sout, bool combine)
 {
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
     double *ct = arr(A_CT);
     const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
     LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
-                         g, Uin, bin, Uout, ct, C.P, combine ? 1 : 0));
+                         g, Sin, Sout, ct, C.P, combine ? 1 : 0));
     const double scale = combine ? 0.5 : 1.0;
-    const int bx = (g.n[0] + 127) / 128;
+    const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
     {
         const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
         dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
-        LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, 128, 0, s>>>(g, Uin, bin + g.sa, Uout, ct, C.P, scale, len));
+        LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
     if (!TWO_D) {
         const int len = march_seglen(g.n[2], (long long)g.n[0] * g.n[1]);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
-        LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, 128, 0, s>>>(g, Uin, bin + 2 * g.sa, Uout, ct, C.P, scale, len));
+        LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
 }
 
-// One Euler stage (Uin, bin) -> (Uout, bout); combine: out <- (out + Euler(in)) / 2 in place.
-void enqueue_stage(int in_u, int in_b, int out_u, int out_b, bool combine)
+// CT: edge EMFs + face update (+ combine) in one kernel; dbg (debug only) receives the edge EMFs
+void launch_ct(const double *bin, double *bout, bool combine, double *dbg)
 {
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
-    Box in = interior(g);
-    fill_ghosts(arr(in_u));
+    const int tiles_x = (g.n[0] + CT_TX - 2) / (CT_TX - 1), tiles_y = (g.n[1] + CT_TY - 2) / (CT_TY - 1);
+    const int len = march_seglen(g.n[2], (long long)tiles_x * tiles_y * CT_TX * CT_TY);
+    dim3 grid(tiles_x, tiles_y, (g.n[2] + len - 1) / len), block(CT_TX, CT_TY);
+    const double *ct = arr(A_CT);
+    if (g.act[2]) {
+        if (combine) LAUNCH(K_CT, k_ct<true, false><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        else         LAUNCH(K_CT, k_ct<false, false><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
+    } else {
+        if (combine) LAUNCH(K_CT, k_ct<true, true><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        else         LAUNCH(K_CT, k_ct<false, true><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
+    }
+}
+
+// One Euler stage Sin -> Sout; combine: Sout <- (Sout + Euler(Sin)) / 2 in place.
+void enqueue_stage(int in, int out, bool combine, double *dbg = nullptr)
+{
+    const Grid &g = C.g;
+    fill_ghosts(arr(in));
     const bool two_d = !g.act[2];
-    if (g.limiter == 0) { if (two_d) launch_sweeps<0, true>(arr(in_u), arr(in_b), arr(out_u), combine);
-                          else       launch_sweeps<0, false>(arr(in_u), arr(in_b), arr(out_u), combine); }
-    else                { if (two_d) launch_sweeps<1, true>(arr(in_u), arr(in_b), arr(out_u), combine);
-                          else       launch_sweeps<1, false>(arr(in_u), arr(in_b), arr(out_u), combine); }
-    LAUNCH(K_EMF, k_emf<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT)));
-    if (combine) LAUNCH(K_CTFACE, k_ctface<true><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_b), arr(A_CT), arr(out_b), C.P));
-    else         LAUNCH(K_CTFACE, k_ctface<false><<<grid_for(in), 128, 0, s>>>(g, in, arr(in_b), arr(A_CT), arr(out_b), C.P));
-    LAUNCH(K_CELLB, k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(out_b), arr(out_u)));
+    if (g.limiter == 0) { if (two_d) launch_sweeps<0, true>(arr(in), arr(out), combine);
+                          else       launch_sweeps<0, false>(arr(in), arr(out), combine); }
+    else                { if (two_d) launch_sweeps<1, true>(arr(in), arr(out), combine);
+                          else       launch_sweeps<1, false>(arr(in), arr(out), combine); }
+    launch_ct(arr(in + S_B), arr(out + S_B), combine, dbg);
 }
 
 void enqueue_dt(int mode)
 {
-    if (mode != 1) LAUNCH(K_DTMAX, launch_dtmax(C.g, arr(A_UA), C.P, C.sm_count * 8, C.stream));
+    if (mode != 1) LAUNCH(K_DTMAX, launch_dtmax(C.g, arr(A_SA), C.P, C.sm_count * 8, C.stream));
     LAUNCH(K_SCALAR, launch_dtfinish(C.g, C.P, mode, C.stream));
 }
 
 void enqueue_step(bool fixed)
 {
     enqueue_dt(fixed ? 1 : 0);
-    enqueue_stage(A_UA, A_BA, A_UB, A_BB, false);    // S^1 = S^n + L(S^n)
-    enqueue_stage(A_UB, A_BB, A_UA, A_BA, true);     // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
+    enqueue_stage(A_SA, A_SB, false);    // S^1 = S^n + L(S^n)
+    enqueue_stage(A_SB, A_SA, true);     // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
     LAUNCH(K_SCALAR, launch_advance_time(C.P, C.stream));
 }
 
@@ -273,7 +277,7 @@ size_t api_count(const Grid &g, int d)
     return (size_t)m[0] * m[1] * m[2];
 }
 
-// staging buffer: the CT work arrays are free outside a step (15 arrays >= 11 interior arrays)
+// staging buffer: the CT work arrays are free outside a step (12 padded arrays > 11 interior arrays)
 double *staging() { return arr(A_CT); }
 
 int copy_in(const double *src, size_t count, double **dev)
@@ -407,8 +411,14 @@ int pluto_set_state(const double *U, const double *Bface)
     int rc = copy_in(U, 8 * api_count(g, -1), &dev);
     if (rc) return rc;
     Box in = interior(g);
-    for (int v = 0; v < 8; v++)
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + (size_t)v * api_count(g, -1), g.n[0], g.n[1], arr(A_UA + v));
+    const size_t n = api_count(g, -1);
+    // U[0..3] -> rho, m; U[7] -> E; cell-centred B of an active dimension is not stored (R7: it IS the
+    // face mean); 2D: U[6] = B_z goes to the third magnetic array
+    const int src_of[5] = { 0, 1, 2, 3, 7 };
+    for (int v = 0; v < 5; v++)
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + (size_t)src_of[v] * n, g.n[0], g.n[1], arr(A_SA + v));
+    if (!g.act[2])
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + 6 * n, g.n[0], g.n[1], arr(A_SA + S_B + 2));
     CUDA_TRY(cudaStreamSynchronize(s));       // staging is reused below
     size_t nface = 0;
     for (int d = 0; d < g.ndim; d++) nface += api_count(g, d);
@@ -418,16 +428,15 @@ int pluto_set_state(const double *U, const double *Bface)
     for (int d = 0; d < g.ndim; d++) {
         int m[3];
         api_extent(g, d, m);
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + off, m[0], m[1], arr(A_BA + d));   // upper duplicate ignored
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + off, m[0], m[1], arr(A_SA + S_B + d));   // upper duplicate ignored
         off += api_count(g, d);
     }
-    k_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_BA), arr(A_UA));
     StepParams p0;
     memset(&p0, 0, sizeof p0);
     CUDA_TRY(cudaMemcpyAsync(C.P, &p0, sizeof p0, cudaMemcpyHostToDevice, s));
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
-    C.launches += 8 + g.ndim + 1;
+    C.launches += 6 + g.ndim;
     C.have_state = true; C.stepped = false;
     return PLUTO_OK;
 }
@@ -442,11 +451,13 @@ int pluto_get_state(double *U, double *Bface)
         bool dev = is_device_ptr(U);
         double *dst = dev ? U : staging();
         Box in = interior(g);
-        for (int v = 0; v < 8; v++)
-            k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_UA + v), g.n[0], g.n[1], dst + (size_t)v * n);
+        const int dst_of[5] = { 0, 1, 2, 3, 7 };
+        for (int v = 0; v < 5; v++)
+            k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SA + v), g.n[0], g.n[1], dst + (size_t)dst_of[v] * n);
+        k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SA + S_B), dst + 4 * n, (long long)n);
         if (!dev) CUDA_TRY(cudaMemcpyAsync(U, dst, 8 * n * sizeof(double), cudaMemcpyDeviceToHost, s));
         CUDA_TRY(cudaStreamSynchronize(s));
-        C.launches += 8;
+        C.launches += 6;
     }
     if (Bface) {
         bool dev = is_device_ptr(Bface);
@@ -456,7 +467,7 @@ int pluto_get_state(double *U, double *Bface)
             int m[3];
             api_extent(g, d, m);
             Box b = make_box(g, 0, m[0], 0, m[1], 0, m[2]);
-            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_BA + d), m[0], m[1], dst + off);
+            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_SA + S_B + d), m[0], m[1], dst + off);
             off += api_count(g, d);
         }
         if (!dev) CUDA_TRY(cudaMemcpyAsync(Bface, dst, off * sizeof(double), cudaMemcpyDeviceToHost, s));
@@ -575,7 +586,10 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     StepParams saved;
     CUDA_TRY(cudaMemcpy(&saved, C.P, sizeof saved, cudaMemcpyDeviceToHost));
     launch_dtfinish(g, C.P, 1, s);
-    enqueue_stage(A_UA, A_BA, A_UB, A_BB, false);
+    double *dbgE = nullptr;                     // edge EMFs are never stored by the production path
+    CUDA_TRY(cudaMalloc((void **)&dbgE, 3 * (size_t)g.sa * sizeof(double)));
+    CUDA_TRY(cudaMemsetAsync(dbgE, 0, 3 * (size_t)g.sa * sizeof(double), s));
+    enqueue_stage(A_SA, A_SB, false, dbgE);
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
     const size_t n = api_count(g, -1);
@@ -589,7 +603,9 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     };
     int bad = 0;
     if (U1) {
-        for (int v = 0; v < 8; v++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_UB + v), g.n[0], g.n[1], tmp + v * n);
+        const int dst_of[5] = { 0, 1, 2, 3, 7 };
+        for (int v = 0; v < 5; v++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SB + v), g.n[0], g.n[1], tmp + dst_of[v] * n);
+        k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SB + S_B), tmp + 4 * n, (long long)n);
         cudaStreamSynchronize(s);
         bad |= emit(U1, 8 * n);
     }
@@ -599,7 +615,7 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
             int m[3];
             api_extent(g, d, m);
             Box b = make_box(g, 0, m[0], 0, m[1], 0, m[2]);
-            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_BB + d), m[0], m[1], tmp + off);
+            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_SB + S_B + d), m[0], m[1], tmp + off);
             off += api_count(g, d);
         }
         cudaStreamSynchronize(s);
@@ -621,10 +637,11 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     }
     if (Eedge) {
         cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
-        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT + CT_EG + e), g.n[0], g.n[1], tmp + e * n);
+        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, dbgE + (size_t)e * g.sa, g.n[0], g.n[1], tmp + e * n);
         cudaStreamSynchronize(s);
         bad |= emit(Eedge, 3 * n);
     }
+    cudaFree(dbgE);
     cudaFree(tmp);
     int err = 0;
     CUDA_TRY(cudaMemcpy(&err, &C.P->err, sizeof(int), cudaMemcpyDeviceToHost));
