@@ -17,6 +17,7 @@ LIB = os.path.join(_HERE, "libpluto_b200.so")
 OK, EINVAL, ESTATE, ECUDA, EPHYS, ENOMEM = 0, -1, -2, -3, -4, -5
 MINMOD, MC = 0, 1
 OPT_GRAPH = 1
+OPT_FUSE_XY = 2
 
 # every symbol include/pluto.h declares
 SYMBOLS = [

@@ -30,6 +30,22 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
                         0.5 * (b[g.sa + c] + b[g.sa + g.at(i, j + 1 == g.n[1] ? 0 : j + 1, k)]),
                         g.act[2] ? 0.5 * (b[2 * g.sa + c] + b[2 * g.sa + g.at(i, j, k + 1 == g.n[2] ? 0 : k + 1)])
                                  : b[2 * g.sa + c] };
+        // Cheap upper bound first: c_f,d <= sqrt(a^2 + b^2) for every d, so
+        //     sig_d <= (|m_d|/rho + sqrt((gamma p + B^2)/rho)) / dx_d .
+        // A zone whose bound (with a 1e-9 margin for rounding) is below the thread's running
+        // maximum cannot raise it and skips the exact evaluation; the maximum found is unchanged.
+        {
+            double ir = 1.0 / rho;
+            double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
+            double pb = (g.gamma - 1.0) * (E - 0.5 * (mx * mx + my * my + mz * mz) * ir - 0.5 * B2);
+            bad |= !(rho > 0.0) || !(pb > 0.0) || isinf(rho) || isinf(pb);
+            double cb = sqrt((g.gamma * pb + B2) * ir);
+            double bound = 0.0;
+            if (g.act[0]) bound = fmax(bound, (fabs(mx) * ir + cb) * g.idx[0]);
+            if (g.act[1]) bound = fmax(bound, (fabs(my) * ir + cb) * g.idx[1]);
+            if (g.act[2]) bound = fmax(bound, (fabs(mz) * ir + cb) * g.idx[2]);
+            if (bound * (1.0 + 1e-9) < smax) continue;     // NaN or inf: falls through to the exact path
+        }
         double v[3] = { mx / rho, my / rho, mz / rho };
         double p = (g.gamma - 1.0) * (E - 0.5 * (mx * v[0] + my * v[1] + mz * v[2])
                                         - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));

@@ -359,6 +359,258 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     if (anybad) P->err = 1;
 }
 
+// ---------------------------------------------------------------- fused x + y sweep (a2-a5)
+// Block = NT consecutive cells of one x-row, marching along y over `seglen` rows.  Each arriving row
+// is converted to primitives once and kept in a three-row ring in shared memory.  The x interfaces of
+// a row are solved across the block (q^L and the fluxes are exchanged through shared memory, as in
+// k_sweep_x); the y interfaces are solved down each thread's own column from the ring (as in
+// k_sweep_march).  A cell is therefore read once and written once for both directions:
+//     S' = (S - dt/dx (Fx(+) - Fx(-))) - dt/dy (Fy(+) - Fy(-))      [combine: the RK2 average]
+// WRAP: the block spans the whole periodic row (NT = nx), neighbours wrap inside shared memory and
+// no lane is idle.  Otherwise blocks overlap by four cells like k_sweep_x.
+// Operands travel global -> shared by 8-byte cp.async one iteration ahead (group A: the row that
+// arrives next; group F: S and S^n of the row that is finished next).
+constexpr int XY_RING = 9;       // rho, vx, vy, vz, Bx, By, Bz, p (cell centred), b_x on the lower x-face
+constexpr int XY_PFA = 10;       // arriving row: U 5, bx 2, by 1 (upper), bz 2
+constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
+constexpr int XY_DOUBLES_PER_THREAD = 3 * XY_RING + XY_PFA + XY_PFF + 7;
+
+template <int LIM, bool TWO_D, bool WRAP>
+__global__ void __launch_bounds__(512, 1)
+k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
+           int combine, int seglen)
+{
+    extern __shared__ double xy_smem[];
+    const int NT = blockDim.x, t = threadIdx.x;
+    double *ring = xy_smem;                       // [3][XY_RING][NT]
+    double *pfa = ring + 3 * XY_RING * NT;        // [XY_PFA][NT]
+    double *pff = pfa + XY_PFA * NT;              // [XY_PFF][NT]
+    double *sQ = pff + XY_PFF * NT;               // [7][NT]: q^L along x, then the x fluxes
+    const int nx = g.n[0];
+    const int i = WRAP ? t : (int)blockIdx.x * (NT - 4) - 2 + t;
+    const bool valid = WRAP || i < nx + 2;
+    const int tl = WRAP ? (t == 0 ? NT - 1 : t - 1) : max(t - 1, 0);
+    const int tr = WRAP ? (t == NT - 1 ? 0 : t + 1) : min(t + 1, NT - 1);
+    const bool has_slope = WRAP || (valid && t >= 1 && t <= NT - 2 && i + 1 < nx + 2);
+    const bool xface = WRAP || (has_slope && t >= 2 && i <= nx);
+    const bool cell = WRAP || (xface && t <= NT - 3 && i < nx);     // this thread owns an interior cell
+    const int k = blockIdx.z;
+    const int s0 = blockIdx.y * seglen, s1 = min(s0 + seglen, g.n[1]);
+    const long long sa = g.sa, st = g.st[1], stz = g.st[2];
+    const double gamma = g.gamma;
+    const double dtdx = P->dtdx[0];
+    const double facy = (combine ? 0.5 : 1.0) * P->dtdx[1];
+    const double *__restrict__ bx = Sin + S_B * sa;
+    const double *__restrict__ by = Sin + (S_B + 1) * sa;
+    const double *__restrict__ bz = Sin + (S_B + 2) * sa;
+    long long c = g.at(valid ? i : 0, s0, k);                       // cell (i, s0, k)
+    bool anybad = false;
+
+    auto slot = [&](int r) { return ((r + 3) % 3) * XY_RING * NT; };
+    auto prefetch_arrive = [&](long long cr) {                      // cr = the arriving cell
+#pragma unroll
+        for (int v = 0; v < 5; v++) cp_async8(&pfa[v * NT + t], Sin + v * sa + cr);
+        cp_async8(&pfa[5 * NT + t], bx + cr);
+        cp_async8(&pfa[6 * NT + t], bx + cr + 1);
+        cp_async8(&pfa[7 * NT + t], by + cr + st);
+        cp_async8(&pfa[8 * NT + t], bz + cr);
+        if (!TWO_D) cp_async8(&pfa[9 * NT + t], bz + cr + stz);
+    };
+    auto prefetch_finish = [&](long long cf) {                      // cf = the cell finished next
+#pragma unroll
+        for (int v = 0; v < 5; v++) cp_async8(&pff[v * NT + t], Sin + v * sa + cf);
+        if (combine) {
+#pragma unroll
+            for (int v = 0; v < 5; v++) cp_async8(&pff[(5 + v) * NT + t], Sout + v * sa + cf);
+            if (TWO_D) cp_async8(&pff[10 * NT + t], Sout + 7 * sa + cf);
+        }
+    };
+    // primitives of one cell from its conserved variables and the faces around it
+    auto to_prim = [&](double rho, double mx, double my, double mz, double En, double B0, double B1, double B2,
+                       double q[8], bool &bad) {
+        double ir = rcp_fast(rho);
+        q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = B0; q[5] = B1; q[6] = B2;
+        q[7] = (gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3]) - 0.5 * (B0 * B0 + B1 * B1 + B2 * B2));
+        bad = !(rho > 0.0) || !(q[7] > 0.0) || isinf(rho) || isinf(q[7]);
+    };
+    auto load_prim = [&](long long cc, double q[8], double &bxf, bool &bad) {
+        double B[3];
+        cell_b<TWO_D>(g, bx, cc, B);
+        bxf = bx[cc];
+        to_prim(Sin[cc], Sin[sa + cc], Sin[2 * sa + cc], Sin[3 * sa + cc], Sin[4 * sa + cc], B[0], B[1], B[2], q, bad);
+    };
+
+    // ---- prologue: rows s0-2, s0-1, s0 straight from global; s0-1 and s0 enter the ring
+    double qLy[7];                                   // y-rotated q^L of face s - 1/2: rho, vy, vz, vx, Bz, Bx, p
+    double bface, bnext;                             // b_y on faces s - 1/2 and s + 1/2
+    {
+        double qa[8], qb[8], qc[8], f0, f1, f2;
+        bool bad;
+        if (valid) {
+            prefetch_arrive(c + st);
+            cp_async_commit();                       // group A(s0)
+            cp_async_commit();                       // group F(s0): empty
+            load_prim(c - 2 * st, qa, f0, bad);
+            load_prim(c - st, qb, f1, bad);
+            load_prim(c, qc, f2, bad);
+            if (cell) anybad |= bad;
+            bface = by[c]; bnext = by[c + st];
+        } else {
+            cp_async_commit(); cp_async_commit();
+#pragma unroll
+            for (int v = 0; v < 8; v++) { qa[v] = qb[v] = qc[v] = (v == 0 || v == 7) ? 1.0 : 0.0; }
+            f1 = f2 = 0.0; bface = bnext = 0.0;
+        }
+        const int rot[7] = { 0, 2, 3, 1, 6, 4, 7 };
+#pragma unroll
+        for (int v = 0; v < 7; v++) {
+            const int r = rot[v];
+            qLy[v] = qb[r] + 0.5 * plm_slope<LIM>(qb[r] - qa[r], qc[r] - qb[r]);
+        }
+        double *rb = ring + slot(s0 - 1), *rc = ring + slot(s0);
+#pragma unroll
+        for (int v = 0; v < 8; v++) { rb[v * NT + t] = qb[v]; rc[v * NT + t] = qc[v]; }
+        rb[8 * NT + t] = f1; rc[8 * NT + t] = f2;
+    }
+    double Fpy[6] = { 0, 0, 0, 0, 0, 0 };            // previous y-face: rho, m_y, m_z, m_x, E, (B_z in 2D)
+
+    for (int s = s0; s <= s1; s++, c += st) {
+        // ---- (1) the arriving row s+1: convert, ring
+        cp_async_wait<1>();                          // group A(s) has landed
+        double q1[8], byu = 0.0;
+        {
+            bool bad = false;
+            double bxf = 0.0;
+            if (valid) {
+                double B0 = 0.5 * (pfa[5 * NT + t] + pfa[6 * NT + t]);
+                byu = pfa[7 * NT + t];
+                double B1 = 0.5 * (bnext + byu);
+                double B2 = TWO_D ? pfa[8 * NT + t] : 0.5 * (pfa[8 * NT + t] + pfa[9 * NT + t]);
+                bxf = pfa[5 * NT + t];
+                to_prim(pfa[t], pfa[NT + t], pfa[2 * NT + t], pfa[3 * NT + t], pfa[4 * NT + t], B0, B1, B2, q1, bad);
+                if (cell && s + 1 < s1) anybad |= bad;
+                if (s < s1) prefetch_arrive(c + 2 * st);
+            } else {
+#pragma unroll
+                for (int v = 0; v < 8; v++) q1[v] = (v == 0 || v == 7) ? 1.0 : 0.0;
+            }
+            cp_async_commit();                       // group A(s+1)
+            double *rn = ring + slot(s + 1);
+#pragma unroll
+            for (int v = 0; v < 8; v++) rn[v * NT + t] = q1[v];
+            rn[8 * NT + t] = bxf;
+        }
+        __syncthreads();                             // B1: ring row s+1 visible, sQ free
+
+        // ---- (2) x interfaces of row s-1
+        double dUx[6] = { 0, 0, 0, 0, 0, 0 };
+        const double *rm = ring + slot(s - 1), *r0 = ring + slot(s);
+        if (s > s0) {
+            const int xv[7] = { 0, 1, 2, 3, 5, 6, 7 };              // rho, vx, vy, vz, By, Bz, p
+            double qR[7], qo[8];
+#pragma unroll
+            for (int v = 0; v < 8; v++) qo[v] = rm[v * NT + t];
+            if (has_slope) {
+#pragma unroll
+                for (int v = 0; v < 7; v++) {
+                    const int r = xv[v];
+                    double sl = plm_slope<LIM>(qo[r] - rm[r * NT + tl], rm[r * NT + tr] - qo[r]);
+                    sQ[v * NT + t] = qo[r] + 0.5 * sl;
+                    qR[v] = qo[r] - 0.5 * sl;
+                }
+            }
+            __syncthreads();                         // B2
+            Side L = { sQ[tl], sQ[NT + tl], sQ[2 * NT + tl], sQ[3 * NT + tl], sQ[4 * NT + tl], sQ[5 * NT + tl], sQ[6 * NT + tl] };
+            __syncthreads();                         // B2': everybody holds its L, sQ may take the fluxes
+            double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5;
+            if (xface) {
+                Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
+                hlld(L, R, rm[8 * NT + t], gamma, g.igm1, F, w);
+                sQ[t] = F[0]; sQ[NT + t] = F[1]; sQ[2 * NT + t] = F[2]; sQ[3 * NT + t] = F[3]; sQ[4 * NT + t] = F[6];
+                if (TWO_D) sQ[5 * NT + t] = F[5];
+            }
+            if (cell) {
+                const long long cm = c - st;
+                ct[(CT_FEM + 0) * sa + cm] = F[4];
+                ct[(CT_FEM + 1) * sa + cm] = F[5];
+                ct[(CT_W + 0) * sa + cm] = w;
+                // cell-centred EMF  E^c = -(v x B)
+                ct[(CT_EC + 0) * sa + cm] = qo[3] * qo[5] - qo[2] * qo[6];
+                ct[(CT_EC + 1) * sa + cm] = qo[1] * qo[6] - qo[3] * qo[4];
+                ct[(CT_EC + 2) * sa + cm] = qo[2] * qo[4] - qo[1] * qo[5];
+            }
+            __syncthreads();                         // B3
+            if (cell) {
+                dUx[0] = dtdx * (sQ[tr] - F[0]);
+                dUx[1] = dtdx * (sQ[NT + tr] - F[1]);
+                dUx[2] = dtdx * (sQ[2 * NT + tr] - F[2]);
+                dUx[3] = dtdx * (sQ[3 * NT + tr] - F[3]);
+                dUx[4] = dtdx * (sQ[4 * NT + tr] - F[6]);
+                if (TWO_D) dUx[5] = dtdx * (sQ[5 * NT + tr] - F[5]);
+            }
+        }
+
+        // ---- (3) y interface s - 1/2 down the own column
+        double Fy[7] = { 0, 0, 0, 0, 0, 0, 0 }, wy = 0.5;
+        {
+            const int rot[7] = { 0, 2, 3, 1, 6, 4, 7 };              // rho, vy, vz, vx, Bz, Bx, p
+            double qR[7], nl[7];
+#pragma unroll
+            for (int v = 0; v < 7; v++) {
+                const int r = rot[v];
+                double qs = r0[r * NT + t];
+                double sl = plm_slope<LIM>(qs - rm[r * NT + t], q1[r] - qs);
+                qR[v] = qs - 0.5 * sl;
+                nl[v] = qs + 0.5 * sl;
+            }
+            if (cell) {
+                Side L = { qLy[0], qLy[1], qLy[2], qLy[3], qLy[4], qLy[5], qLy[6] };
+                Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
+                hlld(L, R, bface, gamma, g.igm1, Fy, wy);
+            }
+#pragma unroll
+            for (int v = 0; v < 7; v++) qLy[v] = nl[v];
+        }
+
+        // ---- (4) finish row s-1; CT data of the y face
+        cp_async_wait<1>();                          // group F(s) has landed
+        if (s > s0 && cell) {
+            const long long cm = c - st;
+            double r0v = pff[t] - dUx[0];
+            double r1v = pff[NT + t] - dUx[1];
+            double r2v = pff[2 * NT + t] - dUx[2];
+            double r3v = pff[3 * NT + t] - dUx[3];
+            double r4v = pff[4 * NT + t] - dUx[4];
+            if (combine) {
+                r0v = 0.5 * (pff[5 * NT + t] + r0v); r1v = 0.5 * (pff[6 * NT + t] + r1v);
+                r2v = 0.5 * (pff[7 * NT + t] + r2v); r3v = 0.5 * (pff[8 * NT + t] + r3v);
+                r4v = 0.5 * (pff[9 * NT + t] + r4v);
+            }
+            // y-rotated flux: (rho, m_y, m_z, m_x, B_z, B_x, E)
+            Sout[cm] = r0v - facy * (Fy[0] - Fpy[0]);
+            Sout[2 * sa + cm] = r2v - facy * (Fy[1] - Fpy[1]);
+            Sout[3 * sa + cm] = r3v - facy * (Fy[2] - Fpy[2]);
+            Sout[sa + cm] = r1v - facy * (Fy[3] - Fpy[3]);
+            Sout[4 * sa + cm] = r4v - facy * (Fy[6] - Fpy[4]);
+            if (TWO_D) {
+                double r7v = rm[6 * NT + t] - dUx[5];
+                if (combine) r7v = 0.5 * (pff[10 * NT + t] + r7v);
+                Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
+            }
+        }
+        if (valid && s < s1) prefetch_finish(c);
+        cp_async_commit();                           // group F(s+1)
+        if (cell && s < s1) {
+            ct[(CT_FEM + 2) * sa + c] = Fy[4];
+            ct[(CT_FEM + 3) * sa + c] = Fy[5];
+            ct[(CT_W + 1) * sa + c] = wy;
+        }
+        Fpy[0] = Fy[0]; Fpy[1] = Fy[1]; Fpy[2] = Fy[2]; Fpy[3] = Fy[3]; Fpy[4] = Fy[6]; Fpy[5] = Fy[4];
+        bface = bnext; bnext = byu;
+    }
+    if (anybad) P->err = 1;
+}
+
 // ---------------------------------------------------------------- CT (a6, R6) [+ RK2 combine of the faces (a7)]
 // Edge EMF component EC at the lower (A,B) edge of a cell, A = EC+1, B = EC+2 (cyclic): arithmetic
 // mean of the four face EMFs plus the upwinded half-cell differences to the cell-centred EMFs.

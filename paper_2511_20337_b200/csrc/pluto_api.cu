@@ -20,8 +20,8 @@ using namespace pluto;
 
 namespace {
 
-enum KernelId { K_GHOST = 0, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_CT, K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
-const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_x", "sweep_y", "sweep_z", "ct",
+enum KernelId { K_GHOST = 0, K_FLUX_XY, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_CT, K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
+const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_xy", "sweep_x", "sweep_y", "sweep_z", "ct",
                                             "dt_max", "scalars", "pack_unpack" };
 
 struct Context {
@@ -39,6 +39,7 @@ struct Context {
     long long launches = 0;
     long long per_step[2] = { 0, 0 };
     int use_graph = 1;
+    int fuse_xy = 1;
     cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step
     int sm_count = 148;
     char err[512] = "";
@@ -156,17 +157,36 @@ void launch_sweeps(const double *Sin, double *Sout, bool combine)
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
     double *ct = arr(A_CT);
-    const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
-    LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
-                         g, Sin, Sout, ct, C.P, combine ? 1 : 0));
     const double scale = combine ? 0.5 : 1.0;
-    const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
-    {
+    if (C.fuse_xy) {
+        // fused x + y sweep: one block per x-row chunk and y-segment
+        const bool wrap = g.n[0] % 32 == 0 && g.n[0] <= 512;
+        const int nt = wrap ? g.n[0] : (g.n[0] >= 252 ? 256 : (int)round_up(g.n[0] + 4, 32));
+        const int chunks = wrap ? 1 : (g.n[0] + nt - 5) / (nt - 4);
+        const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
+        dim3 grid(chunks, (g.n[1] + len - 1) / len, g.n[2]);
+        const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double);
+        auto kw = k_sweep_xy<LIM, TWO_D, true>;
+        auto kc = k_sweep_xy<LIM, TWO_D, false>;
+        static bool attr_set = false;
+        if (!attr_set) {
+            cudaFuncSetAttribute(kw, cudaFuncAttributeMaxDynamicSharedMemorySize, XY_DOUBLES_PER_THREAD * 512 * 8);
+            cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, XY_DOUBLES_PER_THREAD * 512 * 8);
+            attr_set = true;
+        }
+        if (wrap) LAUNCH(K_FLUX_XY, kw<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, combine ? 1 : 0, len));
+        else      LAUNCH(K_FLUX_XY, kc<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, combine ? 1 : 0, len));
+    } else {
+        const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
+        LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
+                             g, Sin, Sout, ct, C.P, combine ? 1 : 0));
+        const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
         dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
         LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
     if (!TWO_D) {
+        const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[2], (long long)g.n[0] * g.n[1]);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
         LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
@@ -398,6 +418,12 @@ int pluto_set_box(double Lx, double Ly, double Lz)
 int pluto_set_option(int opt, int value)
 {
     if (opt == PLUTO_OPT_GRAPH) { int old = C.use_graph; C.use_graph = value ? 1 : 0; return old; }
+    if (opt == PLUTO_OPT_FUSE_XY) {
+        int old = C.fuse_xy;
+        C.fuse_xy = value ? 1 : 0;
+        destroy_graphs();
+        return old;
+    }
     return fail(PLUTO_EINVAL, "unknown option %d", opt);
 }
 

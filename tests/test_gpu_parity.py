@@ -266,6 +266,25 @@ def test_device_pointers_and_graph_equivalence(pluto, oracle):
     assert pluto.launch_count() > 0
 
 
+@pytest.mark.parametrize("shape", [(40, 24, 12), (64, 20, 1), (37, 23, 9), (300, 9, 1)])
+def test_fused_and_per_direction_sweeps_agree(pluto, shape):
+    """the fused x+y sweep (wrap and chunk modes) against one kernel per direction"""
+    from paper_2511_20337_b200 import binding
+    w = wl.random_smooth(*shape, seed=21, limiter=1)
+    pluto.load(w)
+    pluto.step(2)
+    Ua, Ba = pluto.get_state()
+    old = pluto.set_option(binding.OPT_FUSE_XY, 0)
+    try:
+        pluto.load(w)
+        pluto.step(2)
+        Ub, Bb = pluto.get_state()
+    finally:
+        pluto.set_option(binding.OPT_FUSE_XY, old)
+    assert maxrel(Ua.reshape(8, -1), Ub.reshape(8, -1)) <= 1e-13
+    assert maxrel(Ba[None], Bb[None]) <= 1e-13
+
+
 def test_ghost_layers_do_not_change_the_result(pluto):
     w = wl.random_smooth(20, 18, 16, seed=12)
     pluto.load(w, ghost=2)
