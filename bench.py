@@ -34,10 +34,13 @@ import numpy as np  # noqa: E402
 METRIC = "zone-updates/sec (fp64 3D MHD step, 1 B200); achieved HBM GB/s vs peak"
 UNIT = "zone-updates/s"
 
-# Algorithmic traffic of the dominant kernels, doubles per unit:
-#   sweep_x   : per zone, read U 8 + bx 1, write U' 5 + 2 induction fluxes + 1 weight + 3 cell EMFs  = 20
-#   sweep_y/z : per zone, read U 8 + b_d 1, read+write U' 5 + 5, write 2 induction fluxes + 1 weight = 22
-ALGO_DOUBLES = {"sweep_x": 20, "sweep_y": 22, "sweep_z": 22}
+# Algorithmic traffic of the sweep kernels, doubles per zone and launch; a
+# state is 5 hydro arrays + 3 face arrays (cell-centred B is never stored):
+#   sweep_xy  : read S 8, write S' 5, write CT data 9 (4 induction fluxes, 2 weights, 3 cell EMFs) = 22;
+#               the combine stage also reads S^n 5 = 27; the two launches of a step average 24.5
+#   sweep_x   : read S 8, write S' 5, CT data 6 (2 fluxes, 1 weight, 3 cell EMFs)                  = 19
+#   sweep_y/z : read S 8, read + write S' 5 + 5, CT data 3                                           = 21
+ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21}
 
 
 def peaks():
