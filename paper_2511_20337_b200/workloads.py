@@ -216,14 +216,14 @@ def cp_alfven_1d(nx=64, gamma=5.0 / 3.0, cfl=0.4, limiter=1, amp=0.1):
 # --------------------------------------------------------------------------- MHD blast (C3, C4)
 
 def blast_3d(n=256, nsteps=50, seed=511, noise=1e-3, gamma=5.0 / 3.0, cfl=0.3, limiter=0, name=None,
-             shape=None):
+             shape=None, p_in=10.0):
     nx, ny, nz = (n, n, n) if shape is None else shape
     L = (1.0, ny / nx, nz / nx)
     shp = (nz, ny, nx)
     xc, yc, zc = cell_centres(nx, L[0]), cell_centres(ny, L[1]), cell_centres(nz, L[2])
     r2 = ((xc[None, None, :] - 0.5 * L[0]) ** 2 + (yc[None, :, None] - 0.5 * L[1]) ** 2
           + (zc[:, None, None] - 0.5 * L[2]) ** 2)
-    p = np.where(r2 < 0.1 ** 2, 10.0, 0.1)
+    p = np.where(r2 < 0.1 ** 2, p_in, 0.1)
     u = counter_noise(seed, nx * ny * nz).reshape(shp)
     rho = 1.0 + noise * (2.0 * u - 1.0)
     b0 = 1.0 / np.sqrt(3.0)
