@@ -10,70 +10,122 @@
 
 namespace pluto {
 
+// exact per-zone candidates, IEEE operations in the oracle's order (R15)
+__device__ __forceinline__ double zone_sigma_exact(const Grid &g, double rho, double mx, double my, double mz,
+                                                   double E, const double B[3], int &bad)
+{
+    double v[3] = { mx / rho, my / rho, mz / rho };
+    double p = (g.gamma - 1.0) * (E - 0.5 * (mx * v[0] + my * v[1] + mz * v[2])
+                                    - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));
+    if (!(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p)) bad = 1;
+    double a2 = g.gamma * p / rho;
+    double smax = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        if (!g.act[d]) continue;
+        const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+        double b2  = (B[d] * B[d] + B[t1] * B[t1] + B[t2] * B[t2]) / rho;
+        double bn2 = B[d] * B[d] / rho;
+        double s = a2 + b2;
+        double disc = s * s - 4.0 * a2 * bn2;
+        if (disc < 0.0) disc = 0.0;
+        double cf = sqrt(0.5 * (s + sqrt(disc)));
+        double sig = (fabs(v[d]) + cf) * g.idx[d];
+        if (sig > smax) smax = sig;
+    }
+    return smax;
+}
+
+// Fast arithmetic for the two filters below (explicit fma: this unit is compiled with -fmad=false).
+__device__ __forceinline__ double rcp_nr(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    e = fma(e, e, e);
+    return fma(y, e, y);
+}
+__device__ __forceinline__ double sqrt_nr(double x)      // x > 0
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double gq = x * y, h = 0.5 * y;
+    double e = fma(-gq, h, 0.5);
+    gq = fma(gq, e, gq); h = fma(h, e, h);
+    e = fma(-gq, h, 0.5);
+    return fma(gq, e, gq);
+}
+
+// The maximum is exact, but most zones never reach the IEEE evaluation.  A zone is skipped when an
+// upper bound of its candidates lies below a value that is already known to be a lower bound of the
+// global maximum (`thr`: the exact candidates this thread has seen and the running global maximum
+// other warps have published).  Skipping never changes the result -- the zone that holds the maximum
+// has every bound >= the maximum >= thr -- so the dt stays bit-identical and order independent.
+//   filter 1:  c_f,d <= sqrt(a^2 + b^2)  =>  sig_d <= (|m_d|/rho + sqrt((gamma p + B^2)/rho)) / dx_d
+//   filter 2:  the candidates themselves in fast arithmetic (relative error <= 1e-8 even where the
+//              discriminant cancels), with a 1e-7 margin
+// One block walks whole rows (x contiguous); the running global maximum is re-read once per row.
 __global__ void __launch_bounds__(256)
 k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
 {
-    const long long nzone = (long long)g.n[0] * g.n[1] * g.n[2];
-    double smax = 0.0;
+    const int nrows = g.n[1] * g.n[2];
+    const long long sa = g.sa;
+    const double *__restrict__ b = U + S_B * sa;
+    const double gm1 = g.gamma - 1.0;
+    double smax = 0.0, published = 0.0;
     int bad = 0;
-    for (long long z = blockIdx.x * (long long)blockDim.x + threadIdx.x; z < nzone;
-         z += (long long)gridDim.x * blockDim.x) {
-        int i = (int)(z % g.n[0]);
-        int j = (int)((z / g.n[0]) % g.n[1]);
-        int k = (int)(z / ((long long)g.n[0] * g.n[1]));
-        long long c = g.at(i, j, k);
-        double rho = U[c], mx = U[g.sa + c], my = U[2 * g.sa + c], mz = U[3 * g.sa + c];
-        double E = U[4 * g.sa + c];
-        // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
-        const double *b = U + S_B * g.sa;
-        double B[3] = { 0.5 * (b[c] + b[g.at(i + 1 == g.n[0] ? 0 : i + 1, j, k)]),
-                        0.5 * (b[g.sa + c] + b[g.sa + g.at(i, j + 1 == g.n[1] ? 0 : j + 1, k)]),
-                        g.act[2] ? 0.5 * (b[2 * g.sa + c] + b[2 * g.sa + g.at(i, j, k + 1 == g.n[2] ? 0 : k + 1)])
-                                 : b[2 * g.sa + c] };
-        // Cheap upper bound first: c_f,d <= sqrt(a^2 + b^2) for every d, so
-        //     sig_d <= (|m_d|/rho + sqrt((gamma p + B^2)/rho)) / dx_d .
-        // A zone whose bound (with a 1e-9 margin for rounding) is below the thread's running
-        // maximum cannot raise it and skips the exact evaluation; the maximum found is unchanged.
-        {
-            double ir = 1.0 / rho;
-            double B2 = B[0] * B[0] + B[1] * B[1] + B[2] * B[2];
-            double pb = (g.gamma - 1.0) * (E - 0.5 * (mx * mx + my * my + mz * mz) * ir - 0.5 * B2);
-            bad |= !(rho > 0.0) || !(pb > 0.0) || isinf(rho) || isinf(pb);
-            double cb = sqrt((g.gamma * pb + B2) * ir);
-            double bound = 0.0;
-            if (g.act[0]) bound = fmax(bound, (fabs(mx) * ir + cb) * g.idx[0]);
-            if (g.act[1]) bound = fmax(bound, (fabs(my) * ir + cb) * g.idx[1]);
-            if (g.act[2]) bound = fmax(bound, (fabs(mz) * ir + cb) * g.idx[2]);
-            if (bound * (1.0 + 1e-9) < smax) continue;     // NaN or inf: falls through to the exact path
-        }
-        double v[3] = { mx / rho, my / rho, mz / rho };
-        double p = (g.gamma - 1.0) * (E - 0.5 * (mx * v[0] + my * v[1] + mz * v[2])
-                                        - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));
-        if (!(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p)) bad = 1;
-        double a2 = g.gamma * p / rho;
+    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
+        const int k = row / g.n[1], j = row - k * g.n[1];
+        const long long r0 = g.at(0, j, k);
+        const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
+        const long long upk = g.act[2] ? g.at(0, j, k + 1 == g.n[2] ? 0 : k + 1) - r0 : 0;
+        const double seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
+        double thr = fmax(smax, seen);
+        for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
+            const long long c = r0 + i;
+            const double rho = U[c], mx = U[sa + c], my = U[2 * sa + c], mz = U[3 * sa + c], E = U[4 * sa + c];
+            // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
+            const double B[3] = { 0.5 * (b[c] + b[r0 + (i + 1 == g.n[0] ? 0 : i + 1)]),
+                                  0.5 * (b[sa + c] + b[sa + c + upj]),
+                                  g.act[2] ? 0.5 * (b[2 * sa + c] + b[2 * sa + c + upk]) : b[2 * sa + c] };
+            const double ir = rcp_nr(rho);
+            const double B2 = fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2]));
+            const double vx = mx * ir, vy = my * ir, vz = mz * ir;
+            const double pf = gm1 * (E - 0.5 * fma(mx, vx, fma(my, vy, mz * vz)) - 0.5 * B2);
+            const double a2 = g.gamma * pf * ir;
+            // rho <= 0, p <= 0, NaN or inf: flag, and let the exact path decide what enters the maximum
+            const bool odd = (unsigned)(__double2hiint(rho) - 0x00100000) >= 0x7fe00000u ||
+                             (unsigned)(__double2hiint(pf) - 0x00100000) >= 0x7fe00000u;
+            if (!odd) {
+                const double cb = sqrt_nr(fma(B2, ir, a2));
+                double ub = 0.0;
+                if (g.act[0]) ub = fmax(ub, (fabs(vx) + cb) * g.idx[0]);
+                if (g.act[1]) ub = fmax(ub, (fabs(vy) + cb) * g.idx[1]);
+                if (g.act[2]) ub = fmax(ub, (fabs(vz) + cb) * g.idx[2]);
+                if (ub * (1.0 + 1e-9) < thr) continue;                       // filter 1
+                const double v[3] = { vx, vy, vz };
+                const double s = fma(B2, ir, a2);
+                double est = 0.0;
 #pragma unroll
-        for (int d = 0; d < 3; d++) {
-            if (!g.act[d]) continue;
-            const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
-            double b2  = (B[d] * B[d] + B[t1] * B[t1] + B[t2] * B[t2]) / rho;
-            double bn2 = B[d] * B[d] / rho;
-            double s = a2 + b2;
-            double disc = s * s - 4.0 * a2 * bn2;
-            if (disc < 0.0) disc = 0.0;
-            double cf = sqrt(0.5 * (s + sqrt(disc)));
-            double sig = (fabs(v[d]) + cf) * g.idx[d];
+                for (int d = 0; d < 3; d++) {
+                    if (!g.act[d]) continue;
+                    const double disc = fma(s, s, -4.0 * a2 * (B[d] * B[d] * ir));
+                    const double cf = sqrt_nr(0.5 * (s + sqrt_nr(fmax(disc, 1e-300))));
+                    est = fmax(est, (fabs(v[d]) + cf) * g.idx[d]);
+                }
+                if (est * (1.0 + 1e-7) < thr) continue;                      // filter 2
+            }
+            const double sig = zone_sigma_exact(g, rho, mx, my, mz, E, B, bad);
             if (sig > smax) smax = sig;
+            if (sig > thr) thr = sig;
         }
-    }
-    // warp max
-    for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
-    __shared__ double wmax[8];
-    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = smax;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        double m = threadIdx.x < (blockDim.x >> 5) ? wmax[threadIdx.x] : 0.0;
-        for (int o = 4; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-        if (threadIdx.x == 0) atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(m));
+        // publish the warp's maximum when it raises the global one (rare after the first rows)
+        double wm = smax;
+        for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
+        if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published)) {
+            atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
+            published = wm;
+        }
     }
     if (bad) P->err = 1;
 }

@@ -137,7 +137,7 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
         q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = Bc[1]; q[5] = Bc[2];
         q[6] = (g.gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3])
                                      - 0.5 * (Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2]));
-        if (f >= 0 && f < nx && (!(rho > 0.0) || !(q[6] > 0.0) || isinf(rho) || isinf(q[6]))) P->err = 1;
+        if (f >= 0 && f < nx && (unphysical(rho) || unphysical(q[6]))) P->err = 1;
     }
 #pragma unroll
     for (int v = 0; v < 7; v++) sP[v][t] = q[v];
@@ -149,9 +149,9 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     if (has_nb) {
 #pragma unroll
         for (int v = 0; v < 7; v++) {
-            double s = plm_slope<LIM>(q[v] - sP[v][t - 1], sP[v][t + 1] - q[v]);
-            sQ[v][t] = q[v] + 0.5 * s;
-            qR[v] = q[v] - 0.5 * s;
+            double hi;
+            plm_faces<LIM>(q[v], q[v] - sP[v][t - 1], sP[v][t + 1] - q[v], qR[v], hi);
+            sQ[v][t] = hi;
         }
     }
     __syncthreads();
@@ -215,7 +215,7 @@ __device__ __forceinline__ void prim_rot(double rho, const double m[3], const do
     double p = (gamma - 1.0) * (En - 0.5 * (m[0] * v[0] + m[1] * v[1] + m[2] * v[2])
                                    - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));
     q[0] = rho; q[1] = v[DIR]; q[2] = v[T1]; q[3] = v[T2]; q[4] = B[T1]; q[5] = B[T2]; q[6] = p;
-    bad = !(rho > 0.0) || !(p > 0.0) || isinf(rho) || isinf(p);
+    bad = unphysical(rho) || unphysical(p);
 }
 
 template <int DIR, bool TWO_D>
@@ -259,7 +259,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     const int s1 = min(s0 + seglen, g.n[DIR]);
     const long long sa = g.sa, st = g.st[DIR];
     long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
-    const double gamma = g.gamma;
+    const double gamma = g.gamma, igm1 = g.igm1;
     const double fac = scale * P->dtdx[DIR];
     const double *__restrict__ bn = Sin + (S_B + DIR) * sa;        // normal face field
     const double *__restrict__ b1 = Sin + (S_B + T1) * sa;         // transverse fields
@@ -288,26 +288,31 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     };
     prefetch(0, c);
 
-    double qm[7], q0[7], d0[7], qL[7];
-    load_rot<DIR, TWO_D>(g, Sin, c - 2 * st, qm, bad);
-    load_rot<DIR, TWO_D>(g, Sin, c - st, q0, bad);
+    // running state: q0 = primitives of cell s, d0 = q_s - q_{s-1}, qL = q^L of face s - 1/2,
+    // Fp = flux through face s - 1/2 of the previous iteration, bface / bnext = b_n on faces s -+ 1/2
+    double q0[7], d0[7], qL[7];
+    {
+        double qm[7];
+        load_rot<DIR, TWO_D>(g, Sin, c - 2 * st, qm, bad);
+        load_rot<DIR, TWO_D>(g, Sin, c - st, q0, bad);
 #pragma unroll
-    for (int v = 0; v < 7; v++) d0[v] = q0[v] - qm[v];
-    load_rot<DIR, TWO_D>(g, Sin, c, qm, bad);           // qm now holds cell s0
-    anybad |= bad;
+        for (int v = 0; v < 7; v++) d0[v] = q0[v] - qm[v];
+        load_rot<DIR, TWO_D>(g, Sin, c, qm, bad);           // qm now holds cell s0
+        anybad |= bad;
 #pragma unroll
-    for (int v = 0; v < 7; v++) {
-        double d1 = qm[v] - q0[v];
-        qL[v] = q0[v] + 0.5 * plm_slope<LIM>(d0[v], d1);   // q^L of face s0 - 1/2
-        q0[v] = qm[v];
-        d0[v] = d1;
+        for (int v = 0; v < 7; v++) {
+            double d1 = qm[v] - q0[v], lo;
+            plm_faces<LIM>(q0[v], d0[v], d1, lo, qL[v]);      // q^L of face s0 - 1/2
+            q0[v] = qm[v];
+            d0[v] = d1;
+        }
     }
     double Fp[6] = { 0, 0, 0, 0, 0, 0 };                // previous face: rho, m_n, m_t1, m_t2, E, (B_z in 2D)
     double bface = bn[c];                               // normal field on face s - 1/2
     double bnext = bn[c + st];                          // ... on face s + 1/2
 
-    for (int s = s0; s <= s1; s++, c += st) {
-        const int slot = (s - s0) & 1;
+    // one interface; SLOT is the prefetch buffer holding the operands of this iteration
+    auto iteration = [&](const int slot, const int s) {
         if (s < s1) { prefetch(slot ^ 1, c + st); cp_async_wait<1>(); }
         else        { cp_async_wait<0>(); }
         // cell s is in q0 (with d0 = q_s - q_{s-1}); cell s+1 arrives through shared memory
@@ -322,24 +327,19 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
             prim_rot<DIR>(pf[slot][0][t], m, B, pf[slot][4][t], gamma, q1, bad);
         }
         if (s + 1 < s1) anybad |= bad;
+        Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
         double qR[7];
 #pragma unroll
         for (int v = 0; v < 7; v++) {
             double d1 = q1[v] - q0[v];
-            double sl = plm_slope<LIM>(d0[v], d1);
-            qR[v] = q0[v] - 0.5 * sl;
-            double nl = q0[v] + 0.5 * sl;
+            plm_faces<LIM>(q0[v], d0[v], d1, qR[v], qL[v]);   // qL now carries the next q^L
             q0[v] = q1[v];
             d0[v] = d1;
-            q1[v] = nl;                                   // q1 now carries the next q^L
         }
-        Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
         double F[7], w;
-        hlld(L, R, bface, gamma, g.igm1, F, w);
+        hlld(L, R, bface, gamma, igm1, F, w);
         bface = bnext; bnext = bup;
-#pragma unroll
-        for (int v = 0; v < 7; v++) qL[v] = q1[v];
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
             Sout[cm] = pf[slot][10][t] - fac * (F[0] - Fp[0]);
@@ -355,7 +355,15 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
             ct[(CT_W + DIR) * sa + c] = w;
         }
         Fp[0] = F[0]; Fp[1] = F[1]; Fp[2] = F[2]; Fp[3] = F[3]; Fp[4] = F[6]; Fp[5] = F[4];
+        c += st;
+    };
+    // two interfaces per trip so that the running state needs no register rotation
+    int s = s0;
+    for (; s + 1 <= s1; s += 2) {
+        iteration(0, s);
+        iteration(1, s + 1);
     }
+    if (s <= s1) iteration(0, s);
     if (anybad) P->err = 1;
 }
 
@@ -431,7 +439,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         double ir = rcp_fast(rho);
         q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = B0; q[5] = B1; q[6] = B2;
         q[7] = (gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3]) - 0.5 * (B0 * B0 + B1 * B1 + B2 * B2));
-        bad = !(rho > 0.0) || !(q[7] > 0.0) || isinf(rho) || isinf(q[7]);
+        bad = unphysical(rho) || unphysical(q[7]);
     };
     auto load_prim = [&](long long cc, double q[8], double &bxf, bool &bad) {
         double B[3];
@@ -514,9 +522,9 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
 #pragma unroll
                 for (int v = 0; v < 7; v++) {
                     const int r = xv[v];
-                    double sl = plm_slope<LIM>(qo[r] - rm[r * NT + tl], rm[r * NT + tr] - qo[r]);
-                    sQ[v * NT + t] = qo[r] + 0.5 * sl;
-                    qR[v] = qo[r] - 0.5 * sl;
+                    double hi;
+                    plm_faces<LIM>(qo[r], qo[r] - rm[r * NT + tl], rm[r * NT + tr] - qo[r], qR[v], hi);
+                    sQ[v * NT + t] = hi;
                 }
             }
             __syncthreads();                         // B2
@@ -559,9 +567,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             for (int v = 0; v < 7; v++) {
                 const int r = rot[v];
                 double qs = r0[r * NT + t];
-                double sl = plm_slope<LIM>(qs - rm[r * NT + t], q1[r] - qs);
-                qR[v] = qs - 0.5 * sl;
-                nl[v] = qs + 0.5 * sl;
+                plm_faces<LIM>(qs, qs - rm[r * NT + t], q1[r] - qs, qR[v], nl[v]);
             }
             if (cell) {
                 Side L = { qLy[0], qLy[1], qLy[2], qLy[3], qLy[4], qLy[5], qLy[6] };

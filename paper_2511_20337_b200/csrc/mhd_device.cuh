@@ -55,28 +55,55 @@ __device__ __forceinline__ double sqrt_fast0(double x)
     return x > 0.0 ? s : 0.0;
 }
 
+// Limited slope (R4).  The sign test dm * dp > 0 is taken on the sign bits (integer pipe) instead
+// of a DMUL + DSETP: identical unless dm * dp underflows, where the slope is < 1e-154 anyway.
 template <int LIM>
 __device__ __forceinline__ double plm_slope(double dm, double dp)
 {
+    const bool same = (__double2hiint(dm) ^ __double2hiint(dp)) >= 0;
     if (LIM == 0) {
-        double s = fabs(dm) < fabs(dp) ? dm : dp;
-        return dm * dp > 0.0 ? s : 0.0;
+        double s = fabs(dm) < fabs(dp) ? dm : dp;     // a zero difference is returned as itself
+        return same ? s : 0.0;
     } else {
         double sum = dm + dp;
         double mag = fmin(2.0 * fmin(fabs(dm), fabs(dp)), 0.5 * fabs(sum));
-        double s = sum > 0.0 ? mag : -mag;
-        return dm * dp > 0.0 ? s : 0.0;
+        return same ? copysign(mag, dm) : 0.0;        // same sign: sign(dm + dp) = sign(dm)
     }
 }
 
-// fast magnetosonic speed from a^2*rho = gamma*p, B-normal^2 and |B|^2 (all divided by rho inside)
-__device__ __forceinline__ double fast_speed(double rho, double gp, double bn2, double b2)
+// Interface values of a cell with value q and one-sided differences dm, dp (Eq. 6):
+// lo = q - s/2 on its lower face, hi = q + s/2 on its upper face.  The zero-slope case multiplies by
+// a selected half-weight (0.5 or 0) instead of selecting the slope: one select fewer per variable.
+template <int LIM>
+__device__ __forceinline__ void plm_faces(double q, double dm, double dp, double &lo, double &hi)
+{
+    const bool same = (__double2hiint(dm) ^ __double2hiint(dp)) >= 0;
+    const double h = __hiloint2double(same ? 0x3fe00000 : 0, 0);      // 0.5 or 0.0
+    double s;
+    if (LIM == 0) {
+        s = fabs(dm) < fabs(dp) ? dm : dp;
+    } else {
+        double sum = dm + dp;
+        s = copysign(fmin(2.0 * fmin(fabs(dm), fabs(dp)), 0.5 * fabs(sum)), dm);
+    }
+    lo = fma(-h, s, q);
+    hi = fma(h, s, q);
+}
+
+// rho or p is unphysical: not a positive, finite, normal number (sign / exponent test on the high word)
+__device__ __forceinline__ bool unphysical(double x)
+{
+    return (unsigned)(__double2hiint(x) - 0x00100000) >= 0x7fe00000u;
+}
+
+// square of the fast magnetosonic speed from gp = gamma * p, B-normal^2 and |B|^2
+__device__ __forceinline__ double fast_speed2(double rho, double gp, double bn2, double b2)
 {
     double ir  = rcp_fast(rho);
     double a2  = gp * ir;
-    double s   = a2 + b2 * ir;
-    double disc = s * s - 4.0 * a2 * (bn2 * ir);
-    return sqrt_fast(0.5 * (s + sqrt_fast0(disc)));
+    double s   = fma(b2, ir, a2);
+    double disc = fma(s, s, -4.0 * a2 * (bn2 * ir));
+    return 0.5 * (s + sqrt_fast(fmax(disc, 1e-300)));   // max(0, disc) of R5 up to 1e-150
 }
 
 // One side of the Riemann fan in the rotated frame.
@@ -84,135 +111,109 @@ struct Side {
     double rho, u, v, w, By, Bz, p;     // reconstructed primitives (B-normal is shared)
 };
 
-// HLLD flux.  Output f[7] = (rho, m_n, m_t1, m_t2, B_t1, B_t2, E) flux, wgt = upwind weight.
+// HLLD flux (R5).  Output f[7] = (rho, m_n, m_t1, m_t2, B_t1, B_t2, E) flux, wgt = upwind weight (R6).
+//
+// The interface state is picked first -- the side by S_M, then U* or U** by the Alfven wave -- and the
+// flux is evaluated from that state, F = F(rho, S_M, v, w, By, Bz, E; pT*).  The HLLD states satisfy
+// the jump conditions S (U_b - U_a) = F_b - F_a with exactly these fluxes, so this equals the
+// jump form F_K + S_K (U* - U_K) [+ S* (U** - U*)] of the HLLD paper up to rounding (in the guarded
+// degenerate case the two differ by < 1e-8 pT* B_t |S_M - u|, second order small).  Only the chosen
+// side's energy chain is computed.  Supersonic fans take the rarely executed branch at the end.
 __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, double gamma, double igm1,
                                      double f[7], double &wgt)
 {
     const double Bx2 = Bx * Bx;
+    const double B2L = Bx2 + fma(L.By, L.By, L.Bz * L.Bz), B2R = Bx2 + fma(R.By, R.By, R.Bz * R.Bz);
+    const double pTL = fma(0.5, B2L, L.p), pTR = fma(0.5, B2R, R.p);
 
-    // left / right total pressure, v.B, energy, physical flux
-    double BtL2 = L.By * L.By + L.Bz * L.Bz, BtR2 = R.By * R.By + R.Bz * R.Bz;
-    double pTL = L.p + 0.5 * (Bx2 + BtL2), pTR = R.p + 0.5 * (Bx2 + BtR2);
-    double vBL = L.u * Bx + L.v * L.By + L.w * L.Bz;
-    double vBR = R.u * Bx + R.v * R.By + R.w * R.Bz;
-    double EL = L.p * igm1 + 0.5 * L.rho * (L.u * L.u + L.v * L.v + L.w * L.w) + 0.5 * (Bx2 + BtL2);
-    double ER = R.p * igm1 + 0.5 * R.rho * (R.u * R.u + R.v * R.v + R.w * R.w) + 0.5 * (Bx2 + BtR2);
+    const double cmax = sqrt_fast(fmax(fast_speed2(L.rho, gamma * L.p, Bx2, B2L),
+                                       fast_speed2(R.rho, gamma * R.p, Bx2, B2R)));
+    const double SL = fmin(L.u, R.u) - cmax, SR = fmax(L.u, R.u) + cmax;
+    const double dL = SL - L.u, dR = SR - R.u;              // S_a - u_a
+    const double aL = L.rho * dL, aR = R.rho * dR;
+    const double idenom = rcp_fast(aR - aL);
+    const double SM  = (aR * R.u - aL * L.u - pTR + pTL) * idenom;
+    const double pTs = (aR * pTL - aL * pTR + aL * aR * (R.u - L.u)) * idenom;
+    const double guard = kDegen * pTs;
 
-    double cfL = fast_speed(L.rho, gamma * L.p, Bx2, Bx2 + BtL2);
-    double cfR = fast_speed(R.rho, gamma * R.p, Bx2, Bx2 + BtR2);
-    double cmax = fmax(cfL, cfR);
-    double SL = fmin(L.u, R.u) - cmax;
-    double SR = fmax(L.u, R.u) + cmax;
-
-    // the side the interface lies in is decided by S_M; supersonic cases fall out of the same test
-    double aL = L.rho * (SL - L.u), aR = R.rho * (SR - R.u);
-    double idenom = rcp_fast(aR - aL);
-    double SM  = (aR * R.u - aL * L.u - pTR + pTL) * idenom;
-    double pTs = (aR * pTL - aL * pTR + aL * aR * (R.u - L.u)) * idenom;
-
-    // star states of both sides (transverse velocity and field, density, energy)
-    double rsL, vsL, wsL, BysL, BzsL, EsL, vBsL;
-    double rsR, vsR, wsR, BysR, BzsR, EsR, vBsR;
+    // star states: density and the transverse velocity / field of both sides
+    double rsL, vsL, wsL, BysL, BzsL, idSL;
+    double rsR, vsR, wsR, BysR, BzsR, idSR;
     {
-        double dS = SL - SM, idS = rcp_fast(dS);
-        double D = aL * dS - Bx2;
-        rsL = aL * idS;
-        if (fabs(D) <= kDegen * pTs) {
-            vsL = L.v; wsL = L.w; BysL = L.By; BzsL = L.Bz;
-        } else {
-            double iD = rcp_fast(D);
-            double cv = Bx * (SM - L.u) * iD;
-            double cb = (aL * (SL - L.u) - Bx2) * iD;
-            vsL = L.v - cv * L.By; wsL = L.w - cv * L.Bz;
-            BysL = L.By * cb;      BzsL = L.Bz * cb;
-        }
-        vBsL = SM * Bx + vsL * BysL + wsL * BzsL;
-        EsL = ((SL - L.u) * EL - pTL * L.u + pTs * SM + Bx * (vBL - vBsL)) * idS;
+        const double dS = SL - SM, D = fma(aL, dS, -Bx2);
+        idSL = rcp_fast(dS);
+        rsL = aL * idSL;
+        // (S_M - u)/D, zero in the guarded degenerate case: then v* = v, B_t* = B_t (R5)
+        const double m = fabs(D) <= guard ? 0.0 : (dL - dS) * rcp_fast(D);
+        const double cv = Bx * m, cb = aL * m;                      // B_t*/B_t = 1 + a (S_M - u)/D
+        vsL = fma(-cv, L.By, L.v); wsL = fma(-cv, L.Bz, L.w);
+        BysL = fma(L.By, cb, L.By); BzsL = fma(L.Bz, cb, L.Bz);
     }
     {
-        double dS = SR - SM, idS = rcp_fast(dS);
-        double D = aR * dS - Bx2;
-        rsR = aR * idS;
-        if (fabs(D) <= kDegen * pTs) {
-            vsR = R.v; wsR = R.w; BysR = R.By; BzsR = R.Bz;
-        } else {
-            double iD = rcp_fast(D);
-            double cv = Bx * (SM - R.u) * iD;
-            double cb = (aR * (SR - R.u) - Bx2) * iD;
-            vsR = R.v - cv * R.By; wsR = R.w - cv * R.Bz;
-            BysR = R.By * cb;      BzsR = R.Bz * cb;
-        }
-        vBsR = SM * Bx + vsR * BysR + wsR * BzsR;
-        EsR = ((SR - R.u) * ER - pTR * R.u + pTs * SM + Bx * (vBR - vBsR)) * idS;
+        const double dS = SR - SM, D = fma(aR, dS, -Bx2);
+        idSR = rcp_fast(dS);
+        rsR = aR * idSR;
+        const double m = fabs(D) <= guard ? 0.0 : (dR - dS) * rcp_fast(D);
+        const double cv = Bx * m, cb = aR * m;
+        vsR = fma(-cv, R.By, R.v); wsR = fma(-cv, R.Bz, R.w);
+        BysR = fma(R.By, cb, R.By); BzsR = fma(R.Bz, cb, R.Bz);
     }
 
-    // Alfven waves and the double-star state
-    double rL, rR, irL, irR;
-    sqrt_rsqrt_fast(rsL, rL, irL);
-    sqrt_rsqrt_fast(rsR, rR, irR);
-    double aBx = fabs(Bx);
-    double SaL = SM - aBx * irL, SaR = SM + aBx * irR;
-    double sig = Bx > 0.0 ? 1.0 : (Bx < 0.0 ? -1.0 : 0.0);
-    double iR = rcp_fast(rL + rR);
-    double vss  = (rL * vsL + rR * vsR + sig * (BysR - BysL)) * iR;
-    double wss  = (rL * wsL + rR * wsR + sig * (BzsR - BzsL)) * iR;
-    double Byss = (rL * BysR + rR * BysL + sig * rL * rR * (vsR - vsL)) * iR;
-    double Bzss = (rL * BzsR + rR * BzsL + sig * rL * rR * (wsR - wsL)) * iR;
-    double vBss = SM * Bx + vss * Byss + wss * Bzss;
+    // double-star state (common to both sides apart from density and energy)
+    const double rL = sqrt_fast(rsL), rR = sqrt_fast(rsR);
+    // sigma = sign(Bx); for Bx = 0 the double-star state is never selected (outer is always true)
+    const double sig = copysign(1.0, Bx);
+    const double iR = rcp_fast(rL + rR);
+    const double srr = sig * rL * rR;
+    const double vss  = (fma(rL, vsL, rR * vsR) + sig * (BysR - BysL)) * iR;
+    const double wss  = (fma(rL, wsL, rR * wsR) + sig * (BzsR - BzsL)) * iR;
+    const double Byss = (fma(rL, BysR, rR * BysL) + srr * (vsR - vsL)) * iR;
+    const double Bzss = (fma(rL, BzsR, rR * BzsL) + srr * (wsR - wsL)) * iR;
+    const double SMBx = SM * Bx;
+    const double vBss = fma(vss, Byss, fma(wss, Bzss, SMBx));
 
-    // pick the side, then the region on that side
-    // (test order of R5: S_L >= 0, S_R <= 0, S*_L >= 0, S_M >= 0, S*_R > 0; S*_L <= S_M always)
-    const bool supL = SL >= 0.0;
-    const bool supR = !supL && SR <= 0.0;
-    const bool supersonic = supL || supR;
-    const bool left = supL || (!supR && SM >= 0.0);
-    const bool outer = left ? (SaL >= 0.0) : !(SaR > 0.0);
+    // the side the interface lies in (test order of R5: ..., S*_L >= 0, S_M >= 0, S*_R > 0), and
+    // whether it lies outside the Alfven wave of that side:  S*_L = S_M - |Bx|/rL >= 0, S*_R = S_M + |Bx|/rR <= 0
+    const bool left = SM >= 0.0;
+    const double aBx = fabs(Bx);
+    const bool outer = left ? (SM * rL >= aBx) : (-SM * rR >= aBx);
 
-    const Side &K = left ? L : R;
-    double S   = left ? SL : SR;
-    double Sa  = left ? SaL : SaR;
-    double pT  = left ? pTL : pTR;
-    double vB  = left ? vBL : vBR;
-    double E   = left ? EL : ER;
-    double rs  = left ? rsL : rsR;
-    double vs  = left ? vsL : vsR,  ws  = left ? wsL : wsR;
-    double Bys = left ? BysL : BysR, Bzs = left ? BzsL : BzsR;
-    double Es  = left ? EsL : EsR,  vBs = left ? vBsL : vBsR;
-    double r   = left ? rL : rR;
-    double sg  = left ? -sig : sig;
+    const double rho = left ? L.rho : R.rho, u = left ? L.u : R.u, v = left ? L.v : R.v, w = left ? L.w : R.w;
+    const double By = left ? L.By : R.By, Bz = left ? L.Bz : R.Bz, p = left ? L.p : R.p;
+    const double B2 = left ? B2L : B2R, pT = left ? pTL : pTR, d = left ? dL : dR, idS = left ? idSL : idSR;
+    const double rs = left ? rsL : rsR, r = left ? rL : rR;
+    const double vs = left ? vsL : vsR, ws = left ? wsL : wsR, Bys = left ? BysL : BysR, Bzs = left ? BzsL : BzsR;
 
-    // physical flux of the chosen side (Eq. 2)
-    double F0 = K.rho * K.u;
-    double F1 = F0 * K.u + pT - Bx2;
-    double F2 = F0 * K.v - Bx * K.By;
-    double F3 = F0 * K.w - Bx * K.Bz;
-    double F5 = K.By * K.u - Bx * K.v;
-    double F6 = K.Bz * K.u - Bx * K.w;
-    double F7 = (E + pT) * K.u - Bx * vB;
+    // energy of the chosen side: U, U*, U**
+    const double E  = fma(p, igm1, 0.5 * fma(rho, fma(u, u, fma(v, v, w * w)), B2));
+    const double vB = fma(u, Bx, fma(v, By, w * Bz));
+    const double vBs = fma(vs, Bys, fma(ws, Bzs, SMBx));
+    const double Es = (fma(d, E, -pT * u) + fma(pTs, SM, Bx * (vB - vBs))) * idS;
+    const double sr = left ? -sig * r : sig * r;
+    const double Ess = fma(sr, vBs - vBss, Es);
 
-    if (!supersonic) {
-        // conserved vectors U (chosen side), U*, U**
-        double U0 = K.rho, U1 = K.rho * K.u, U2 = K.rho * K.v, U3 = K.rho * K.w;
-        double Us1 = rs * SM, Us2 = rs * vs, Us3 = rs * ws;
-        if (outer) {
-            F0 += S * (rs - U0);   F1 += S * (Us1 - U1);  F2 += S * (Us2 - U2);  F3 += S * (Us3 - U3);
-            F5 += S * (Bys - K.By); F6 += S * (Bzs - K.Bz); F7 += S * (Es - E);
-        } else {
-            double Ess = Es + sg * r * (vBs - vBss);
-            double c1 = Sa - S;     // F + Sa*U** - (Sa - S)*U* - S*U
-            F0 += Sa * rs - c1 * rs - S * U0;
-            F1 += Sa * (rs * SM) - c1 * Us1 - S * U1;
-            F2 += Sa * (rs * vss) - c1 * Us2 - S * U2;
-            F3 += Sa * (rs * wss) - c1 * Us3 - S * U3;
-            F5 += Sa * Byss - c1 * Bys - S * K.By;
-            F6 += Sa * Bzss - c1 * Bzs - S * K.Bz;
-            F7 += Sa * Ess - c1 * Es - S * E;
-        }
+    double rf = rs, uf = SM, pf = pTs;
+    double vf = outer ? vs : vss, wf = outer ? ws : wss, Byf = outer ? Bys : Byss, Bzf = outer ? Bzs : Bzss;
+    double Ef = outer ? Es : Ess, vBf = outer ? vBs : vBss;
+    if (__builtin_expect(SL >= 0.0 || SR <= 0.0, 0)) {          // one-sided fan: the upwind physical flux (Eq. 2)
+        const bool sl = SL >= 0.0;
+        rf = sl ? L.rho : R.rho; uf = sl ? L.u : R.u; vf = sl ? L.v : R.v; wf = sl ? L.w : R.w;
+        Byf = sl ? L.By : R.By; Bzf = sl ? L.Bz : R.Bz; pf = sl ? pTL : pTR;
+        const double pp = sl ? L.p : R.p, bb = sl ? B2L : B2R;
+        Ef = fma(pp, igm1, 0.5 * fma(rf, fma(uf, uf, fma(vf, vf, wf * wf)), bb));
+        vBf = fma(uf, Bx, fma(vf, Byf, wf * Bzf));
     }
-    f[0] = F0; f[1] = F1; f[2] = F2; f[3] = F3; f[4] = F5; f[5] = F6; f[6] = F7;
+    const double F0 = rf * uf;
+    f[0] = F0;
+    f[1] = fma(F0, uf, pf - Bx2);
+    f[2] = fma(F0, vf, -Bx * Byf);
+    f[3] = fma(F0, wf, -Bx * Bzf);
+    f[4] = fma(Byf, uf, -Bx * vf);
+    f[5] = fma(Bzf, uf, -Bx * wf);
+    f[6] = fma(Ef + pf, uf, -Bx * vBf);
 
-    double fref = 0.25 * (L.rho + R.rho) * (SR - SL);
-    double wv = 0.5 + 0.5 * F0 * rcp_fast(kTheta * fref);
+    // R6: w = clamp(1/2 + F[rho] / (2 theta f_ref)), f_ref = (rho_L + rho_R)(S_R - S_L) / 4
+    const double wv = fma(F0, rcp_fast((0.5 * kTheta) * ((L.rho + R.rho) * (SR - SL))), 0.5);
     wgt = fmin(fmax(wv, 0.0), 1.0);
 }
 
