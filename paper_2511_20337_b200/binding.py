@@ -12,7 +12,9 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB = os.path.join(_HERE, "libpluto_b200.so")
+# PLUTO_B200_LIB selects another build of the same library (kernel tuning experiments)
+LIB = os.environ.get("PLUTO_B200_LIB") or os.path.join(_HERE, "libpluto_b200.so")
+_DEFAULT_LIB = os.path.join(_HERE, "libpluto_b200.so")
 
 OK, EINVAL, ESTATE, ECUDA, EPHYS, ENOMEM = 0, -1, -2, -3, -4, -5
 MINMOD, MC = 0, 1
@@ -37,7 +39,7 @@ class PlutoError(RuntimeError):
 
 
 def load_library(build_if_missing: bool = True) -> C.CDLL:
-    if build_if_missing:
+    if build_if_missing and LIB == _DEFAULT_LIB:
         from . import build as _build
         _build.build()
     if not os.path.exists(LIB):

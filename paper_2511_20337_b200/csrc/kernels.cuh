@@ -383,13 +383,13 @@ constexpr int XY_PFA = 10;       // arriving row: U 5, bx 2, by 1 (upper), bz 2
 constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
 constexpr int XY_DOUBLES_PER_THREAD = 3 * XY_RING + XY_PFA + XY_PFF + 7;
 
-template <int LIM, bool TWO_D, bool WRAP>
-__global__ void __launch_bounds__(512, 1)
+template <int LIM, bool TWO_D, bool WRAP, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT)
 k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
            int combine, int seglen)
 {
     extern __shared__ double xy_smem[];
-    const int NT = blockDim.x, t = threadIdx.x;
+    const int t = threadIdx.x;
     double *ring = xy_smem;                       // [3][XY_RING][NT]
     double *pfa = ring + 3 * XY_RING * NT;        // [XY_PFA][NT]
     double *pff = pfa + XY_PFA * NT;              // [XY_PFF][NT]
@@ -414,7 +414,6 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     long long c = g.at(valid ? i : 0, s0, k);                       // cell (i, s0, k)
     bool anybad = false;
 
-    auto slot = [&](int r) { return ((r + 3) % 3) * XY_RING * NT; };
     auto prefetch_arrive = [&](long long cr) {                      // cr = the arriving cell
 #pragma unroll
         for (int v = 0; v < 5; v++) cp_async8(&pfa[v * NT + t], Sin + v * sa + cr);
@@ -475,12 +474,15 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             const int r = rot[v];
             qLy[v] = qb[r] + 0.5 * plm_slope<LIM>(qb[r] - qa[r], qc[r] - qb[r]);
         }
-        double *rb = ring + slot(s0 - 1), *rc = ring + slot(s0);
+        double *rb = ring + t, *rc = ring + XY_RING * NT + t;
 #pragma unroll
-        for (int v = 0; v < 8; v++) { rb[v * NT + t] = qb[v]; rc[v * NT + t] = qc[v]; }
-        rb[8 * NT + t] = f1; rc[8 * NT + t] = f2;
+        for (int v = 0; v < 8; v++) { rb[v * NT] = qb[v]; rc[v * NT] = qc[v]; }
+        rb[8 * NT] = f1; rc[8 * NT] = f2;
     }
     double Fpy[6] = { 0, 0, 0, 0, 0, 0 };            // previous y-face: rho, m_y, m_z, m_x, E, (B_z in 2D)
+    // ring rows s-1, s, s+1 (own column; neighbours at +-1): the three slots rotate every iteration
+    double *rm = ring + t, *r0 = ring + XY_RING * NT + t, *rn = ring + 2 * XY_RING * NT + t;
+    const int dl = tl - t, dr = tr - t;
 
     for (int s = s0; s <= s1; s++, c += st) {
         // ---- (1) the arriving row s+1: convert, ring
@@ -503,27 +505,26 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                 for (int v = 0; v < 8; v++) q1[v] = (v == 0 || v == 7) ? 1.0 : 0.0;
             }
             cp_async_commit();                       // group A(s+1)
-            double *rn = ring + slot(s + 1);
 #pragma unroll
-            for (int v = 0; v < 8; v++) rn[v * NT + t] = q1[v];
-            rn[8 * NT + t] = bxf;
+            for (int v = 0; v < 8; v++) rn[v * NT] = q1[v];
+            rn[8 * NT] = bxf;
         }
-        __syncthreads();                             // B1: ring row s+1 visible, sQ free
+        __syncthreads();                             // B1: sQ free (fluxes of the previous row consumed)
 
-        // ---- (2) x interfaces of row s-1
-        double dUx[6] = { 0, 0, 0, 0, 0, 0 };
-        const double *rm = ring + slot(s - 1), *r0 = ring + slot(s);
+        // ---- (2) x interfaces of row s-1; their flux difference goes straight into the prefetched S of
+        //      that row (group F(s), in shared memory), so nothing of it stays live across the y solve
+        cp_async_wait<1>();                          // group F(s) has landed
         if (s > s0) {
             const int xv[7] = { 0, 1, 2, 3, 5, 6, 7 };              // rho, vx, vy, vz, By, Bz, p
             double qR[7], qo[8];
 #pragma unroll
-            for (int v = 0; v < 8; v++) qo[v] = rm[v * NT + t];
+            for (int v = 0; v < 8; v++) qo[v] = rm[v * NT];
             if (has_slope) {
 #pragma unroll
                 for (int v = 0; v < 7; v++) {
                     const int r = xv[v];
                     double hi;
-                    plm_faces<LIM>(qo[r], qo[r] - rm[r * NT + tl], rm[r * NT + tr] - qo[r], qR[v], hi);
+                    plm_faces<LIM>(qo[r], qo[r] - rm[r * NT + dl], rm[r * NT + dr] - qo[r], qR[v], hi);
                     sQ[v * NT + t] = hi;
                 }
             }
@@ -533,7 +534,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5;
             if (xface) {
                 Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-                hlld(L, R, rm[8 * NT + t], gamma, g.igm1, F, w);
+                hlld(L, R, rm[8 * NT], gamma, g.igm1, F, w);
                 sQ[t] = F[0]; sQ[NT + t] = F[1]; sQ[2 * NT + t] = F[2]; sQ[3 * NT + t] = F[3]; sQ[4 * NT + t] = F[6];
                 if (TWO_D) sQ[5 * NT + t] = F[5];
             }
@@ -549,12 +550,12 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             }
             __syncthreads();                         // B3
             if (cell) {
-                dUx[0] = dtdx * (sQ[tr] - F[0]);
-                dUx[1] = dtdx * (sQ[NT + tr] - F[1]);
-                dUx[2] = dtdx * (sQ[2 * NT + tr] - F[2]);
-                dUx[3] = dtdx * (sQ[3 * NT + tr] - F[3]);
-                dUx[4] = dtdx * (sQ[4 * NT + tr] - F[6]);
-                if (TWO_D) dUx[5] = dtdx * (sQ[5 * NT + tr] - F[5]);
+                pff[t] -= dtdx * (sQ[tr] - F[0]);
+                pff[NT + t] -= dtdx * (sQ[NT + tr] - F[1]);
+                pff[2 * NT + t] -= dtdx * (sQ[2 * NT + tr] - F[2]);
+                pff[3 * NT + t] -= dtdx * (sQ[3 * NT + tr] - F[3]);
+                pff[4 * NT + t] -= dtdx * (sQ[4 * NT + tr] - F[6]);
+                if (TWO_D) sQ[6 * NT + t] = rm[6 * NT] - dtdx * (sQ[5 * NT + tr] - F[5]);   // own slot: B_z after x
             }
         }
 
@@ -566,8 +567,8 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
 #pragma unroll
             for (int v = 0; v < 7; v++) {
                 const int r = rot[v];
-                double qs = r0[r * NT + t];
-                plm_faces<LIM>(qs, qs - rm[r * NT + t], q1[r] - qs, qR[v], nl[v]);
+                double qs = r0[r * NT];
+                plm_faces<LIM>(qs, qs - rm[r * NT], rn[r * NT] - qs, qR[v], nl[v]);
             }
             if (cell) {
                 Side L = { qLy[0], qLy[1], qLy[2], qLy[3], qLy[4], qLy[5], qLy[6] };
@@ -579,14 +580,9 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         }
 
         // ---- (4) finish row s-1; CT data of the y face
-        cp_async_wait<1>();                          // group F(s) has landed
         if (s > s0 && cell) {
             const long long cm = c - st;
-            double r0v = pff[t] - dUx[0];
-            double r1v = pff[NT + t] - dUx[1];
-            double r2v = pff[2 * NT + t] - dUx[2];
-            double r3v = pff[3 * NT + t] - dUx[3];
-            double r4v = pff[4 * NT + t] - dUx[4];
+            double r0v = pff[t], r1v = pff[NT + t], r2v = pff[2 * NT + t], r3v = pff[3 * NT + t], r4v = pff[4 * NT + t];
             if (combine) {
                 r0v = 0.5 * (pff[5 * NT + t] + r0v); r1v = 0.5 * (pff[6 * NT + t] + r1v);
                 r2v = 0.5 * (pff[7 * NT + t] + r2v); r3v = 0.5 * (pff[8 * NT + t] + r3v);
@@ -599,7 +595,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             Sout[sa + cm] = r1v - facy * (Fy[3] - Fpy[3]);
             Sout[4 * sa + cm] = r4v - facy * (Fy[6] - Fpy[4]);
             if (TWO_D) {
-                double r7v = rm[6 * NT + t] - dUx[5];
+                double r7v = sQ[6 * NT + t];
                 if (combine) r7v = 0.5 * (pff[10 * NT + t] + r7v);
                 Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
             }
@@ -613,56 +609,65 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         }
         Fpy[0] = Fy[0]; Fpy[1] = Fy[1]; Fpy[2] = Fy[2]; Fpy[3] = Fy[3]; Fpy[4] = Fy[6]; Fpy[5] = Fy[4];
         bface = bnext; bnext = byu;
+        double *rt = rm; rm = r0; r0 = rn; rn = rt;
     }
     if (anybad) P->err = 1;
 }
 
 // ---------------------------------------------------------------- CT (a6, R6) [+ RK2 combine of the faces (a7)]
-// Edge EMF component EC at the lower (A,B) edge of a cell, A = EC+1, B = EC+2 (cyclic): arithmetic
+// Edge EMF at the lower (A,B) edge of a cell (component EC, A = EC+1, B = EC+2 cyclic): arithmetic
 // mean of the four face EMFs plus the upwinded half-cell differences to the cell-centred EMFs.
-// c11 = the cell, c01 = its neighbour at A-1, c10 = at B-1, c00 = at A-1,B-1 (periodic wrap done by
-// the caller, so the CT work arrays need no ghost layers).
-template <int EC>
-__device__ __forceinline__ double edge_emf(const double *__restrict__ ct, long long sa,
-                                           long long c11, long long c01, long long c10, long long c00)
+//   Ea_lo, Ea_hi : EMF on the two A-faces meeting at the edge (cells at B-1 and B)
+//   Eb_lo, Eb_hi : EMF on the two B-faces (cells at A-1 and A)
+//   wa_*, wb_*   : upwind weights on those faces
+//   e00, e10, e01, e11 : cell EMFs of (A-1,B-1), (A,B-1), (A-1,B), (A,B)
+__device__ __forceinline__ double edge_emf(double Ea_lo, double Ea_hi, double Eb_lo, double Eb_hi,
+                                           double wa_lo, double wa_hi, double wb_lo, double wb_hi,
+                                           double e00, double e10, double e01, double e11)
 {
-    constexpr int A = (EC + 1) % 3, B = (EC + 2) % 3;
-    const double *Fa = ct + (CT_FEM + 2 * A) * sa;       // F_a[B_b]: first induction flux of sweep a
-    const double *Fb = ct + (CT_FEM + 2 * B + 1) * sa;   // F_b[B_a]: second induction flux of sweep b
-    const double *Wa = ct + (CT_W + A) * sa, *Wb = ct + (CT_W + B) * sa;
-    const double *Ec = ct + (CT_EC + EC) * sa;
-    double Ea_lo = -Fa[c10], Ea_hi = -Fa[c11];
-    double Eb_lo =  Fb[c01], Eb_hi =  Fb[c11];
-    double wa_lo = Wa[c10], wa_hi = Wa[c11], wb_lo = Wb[c01], wb_hi = Wb[c11];
-    double e00 = Ec[c00], e10 = Ec[c10], e01 = Ec[c01], e11 = Ec[c11];
-    double t1 = wa_lo * (Eb_lo - e00) + (1.0 - wa_lo) * (Eb_hi - e10);
-    double t2 = wa_hi * (e01 - Eb_lo) + (1.0 - wa_hi) * (e11 - Eb_hi);
-    double t3 = wb_lo * (Ea_lo - e00) + (1.0 - wb_lo) * (Ea_hi - e01);
-    double t4 = wb_hi * (e10 - Ea_lo) + (1.0 - wb_hi) * (e11 - Ea_hi);
-    return 0.25 * (Ea_lo + Ea_hi + Eb_lo + Eb_hi) + 0.25 * (t1 - t2) + 0.25 * (t3 - t4);
+    // up(w; a, b) = w a + (1 - w) b = b + w (a - b)
+    const double a1 = Eb_lo - e00, b1 = Eb_hi - e10, a2 = e01 - Eb_lo, b2 = e11 - Eb_hi;
+    const double a3 = Ea_lo - e00, b3 = Ea_hi - e01, a4 = e10 - Ea_lo, b4 = e11 - Ea_hi;
+    const double t1 = fma(wa_lo, a1 - b1, b1), t2 = fma(wa_hi, a2 - b2, b2);
+    const double t3 = fma(wb_lo, a3 - b3, b3), t4 = fma(wb_hi, a4 - b4, b4);
+    return 0.25 * (((Ea_lo + Ea_hi) + (Eb_lo + Eb_hi)) + ((t1 - t2) + (t3 - t4)));
 }
 
-// in-plane offsets of a cell and of its x-1, y-1 and (x-1,y-1) neighbours (periodic)
-struct Nb { long long c, x, y, xy; };
-
-// Block = CT_TX x CT_TY columns marching along z over `seglen` planes.  Per plane k every thread
-// evaluates the three EMFs on the lower edges of its cell -- E_z(i-1/2, j-1/2, k) and, one plane
-// ahead, E_x(i, j-1/2, k+1/2), E_y(i-1/2, j, k+1/2) -- and leaves them in shared memory.  After one
-// barrier the lower faces of the cell are updated with  db/dt = -curl E  (COMBINE: bout <- (bout +
-// that)/2 in place, bout holding the faces of S^n).  E_x, E_y of plane k-1/2 stay in registers from
-// the previous iteration, so no edge EMF is ever stored in HBM.  Tiles overlap by one column and one
-// row: the threads of the last column / row only supply the edges just outside the tile, so all
-// threads run the same code (no divergent extra work) and each face is still written exactly once.
+// Block = CT_TX x CT_TY columns marching along z over `seglen` planes.  Iteration k forms
+// E_z(i-1/2, j-1/2, k) and, from plane k and the plane k-1 values kept in registers, E_x(i, j-1/2, k-1/2)
+// and E_y(i-1/2, j, k-1/2): 12 loads of the thread's own cell (HBM; prefetched into L1 two planes
+// ahead) and 13 of its x-1 / y-1 neighbours (L1 hits: the neighbour thread loads the same words).
+// The three EMFs are exchanged through shared memory (one barrier, double buffered) and the faces
+// b_z(k), b_x(k-1), b_y(k-1) are updated with  db/dt = -curl E  (COMBINE: bout <- (bout + that)/2
+// in place, bout holding the faces of S^n).  No edge EMF is ever stored in HBM.  Tiles overlap by
+// one column and one row: the threads of the last column / row only supply the edges just outside
+// the tile, so all threads run the same code and each face is written exactly once.
 constexpr int CT_TX = 32, CT_TY = 8;
 
+#ifndef CT_PF_DIST
+#define CT_PF_DIST 1
+#endif
+#ifndef CT_PF_L2
+#define CT_PF_L2 0
+#endif
+#ifndef CT_MINB
+#define CT_MINB 3
+#endif
+__device__ __forceinline__ void prefetch_l1(const void *p)
+{
+#if CT_PF_L2
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#else
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#endif
+}
+
 template <bool COMBINE, bool TWO_D>
-__global__ void __launch_bounds__(CT_TX * CT_TY, 3)
+__global__ void __launch_bounds__(CT_TX * CT_TY, CT_MINB)
 k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, double *bout,
      const StepParams *__restrict__ P, int seglen, double *__restrict__ dbg)
 {
-    __shared__ double sEz[2][CT_TY][CT_TX];
-    __shared__ double sEx[3][CT_TY][CT_TX];
-    __shared__ double sEy[3][CT_TY][CT_TX];
+    __shared__ double sE[2][3][CT_TY][CT_TX];
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int i = blockIdx.x * (CT_TX - 1) + tx, j = blockIdx.y * (CT_TY - 1) + ty;
     // cells i <= n0, j <= n1 supply edges (index n wraps to 0); faces are updated by the inner threads
@@ -670,64 +675,107 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
     const bool upd = tx < CT_TX - 1 && ty < CT_TY - 1 && i < g.n[0] && j < g.n[1];
     const int k0 = blockIdx.z * seglen, k1 = min(k0 + seglen, g.n[2]);
     const long long sa = g.sa, st2 = g.st[2];
-    const double dt = P->dt;
+    const double dtdx = P->dtdx[0], dtdy = P->dtdx[1], dtdz = P->dtdx[2];
 
     // clamp the indices of idle threads so that every address below is legal
     const int ii = edge ? (i == g.n[0] ? 0 : i) : 0, jj = edge ? (j == g.n[1] ? 0 : j) : 0;
     const int im = wrap_m1(ii, g.n[0]), jm = wrap_m1(jj, g.n[1]);
     const long long r0 = (long long)(jj + g.off[1]) * g.st[1] + g.off[0];
     const long long rm = (long long)(jm + g.off[1]) * g.st[1] + g.off[0];
-    const Nb own = { r0 + ii, r0 + im, rm + ii, rm + im };
+    const long long oc = r0 + ii;                                      // own cell, in-plane offset
+    const int XM = (int)(r0 + im - oc), YM = (int)(rm + ii - oc), XYM = (int)(rm + im - oc);   // neighbours
+    auto plane = [&](int k) { return (long long)((k == g.n[2] ? 0 : k) + g.off[2]) * st2; };
+    // the CT arrays: F_x[By] 0, F_x[Bz] 1, F_y[Bz] 2, F_y[Bx] 3, F_z[Bx] 4, F_z[By] 5, w_x 6, w_y 7, w_z 8, E^c 9-11
+    const double *__restrict__ A0 = ct + oc;
 
-    auto plane = [&](int k) { return (long long)(k + g.off[2]) * st2; };
-    auto Ez = [&](const Nb &n, long long pk) { return edge_emf<2>(ct, sa, pk + n.c, pk + n.x, pk + n.y, pk + n.xy); };
-    auto Ex = [&](const Nb &n, long long pk, long long pm) { return edge_emf<0>(ct, sa, pk + n.c, pk + n.y, pm + n.c, pm + n.y); };
-    auto Ey = [&](const Nb &n, long long pk, long long pm) { return edge_emf<1>(ct, sa, pk + n.c, pm + n.c, pk + n.x, pm + n.x); };
-
-    double exP = 0.0, eyP = 0.0;
-    if (!TWO_D && edge) {                                   // edges of plane k0 - 1/2
-        const long long pk = plane(k0), pm = plane(wrap_m1(k0, g.n[2]));
-        exP = Ex(own, pk, pm); eyP = Ey(own, pk, pm);
-        sEx[k0 % 3][ty][tx] = exP; sEy[k0 % 3][ty][tx] = eyP;
+    // plane k-1 values that enter E_x, E_y at k - 1/2
+    double fyz = 0, wyP = 0, excP = 0, excPm = 0, fxz = 0, wxP = 0, eycP = 0, eycPm = 0;
+    if (!TWO_D) {
+        const double *q = A0 + plane(wrap_m1(k0, g.n[2]));
+        fyz = q[2 * sa];  wyP = q[7 * sa];
+        excP = q[9 * sa]; excPm = q[9 * sa + YM];
+        fxz = q[1 * sa];  wxP = q[6 * sa];
+        eycP = q[10 * sa]; eycPm = q[10 * sa + XM];
+    }
+    double exP = 0.0, eyP = 0.0, dEzx = 0.0, dEzy = 0.0;
+    // faces to update next: b_z(k), b_x(k-1), b_y(k-1) (+ the S^n faces in the combine stage)
+    double pbx = 0, pby = 0, pbz = 0, qbx = 0, qby = 0, qbz = 0;
+    if (upd) {
+        const long long c = plane(k0) + oc;
+        if (TWO_D) {
+            pbx = bin[c]; pby = bin[sa + c];
+            if (COMBINE) { qbx = bout[c]; qby = bout[sa + c]; }
+        } else {
+            pbz = bin[2 * sa + c];
+            if (COMBINE) qbz = bout[2 * sa + c];
+        }
+    }
+    if (!TWO_D && CT_PF_DIST == 2 && k0 + 1 <= k1) {
+        const double *q = A0 + plane(k0 + 1);
+#pragma unroll
+        for (int a = 0; a < CT_COUNT; a++) prefetch_l1(q + a * sa);
     }
 
-    for (int k = k0; k < k1; k++) {
-        const long long pk = plane(k);
-        const long long c = pk + own.c;
-        const int sz = k & 1, sl = k % 3, sn = (k + 1) % 3;
-        double ez = 0.0, exN = 0.0, eyN = 0.0;
-        double b0 = 0.0, b1 = 0.0, b2 = 0.0, o0 = 0.0, o1 = 0.0, o2 = 0.0;
-        if (upd) {                                          // issued together with the CT loads below
-            b0 = bin[c]; b1 = bin[sa + c];
-            if (!TWO_D) b2 = bin[2 * sa + c];
-            if (COMBINE) { o0 = bout[c]; o1 = bout[sa + c]; if (!TWO_D) o2 = bout[2 * sa + c]; }
+    for (int k = k0; k <= (TWO_D ? k0 : k1); k++) {
+        const int buf = k & 1;
+        const double *__restrict__ v = A0 + plane(k);
+        if (!TWO_D && CT_PF_DIST > 0 && k + CT_PF_DIST <= k1) {        // own words of a later plane -> L1
+            const double *q = A0 + plane(k + CT_PF_DIST);
+#pragma unroll
+            for (int a = 0; a < CT_COUNT; a++) prefetch_l1(q + a * sa);
         }
-        if (edge) {
-            ez = Ez(own, pk);
-            sEz[sz][ty][tx] = ez;
-            if (!TWO_D) {
-                const long long pn = plane(wrap_p1(k, g.n[2]));      // plane k+1; its lower neighbour is k
-                exN = Ex(own, pn, pk); eyN = Ey(own, pn, pk);
-                sEx[sn][ty][tx] = exN; sEy[sn][ty][tx] = eyN;
-            }
+        auto S = [&](int a, int off) { return v[a * sa + off]; };
+        const double wx = S(6, 0), wy = S(7, 0);
+        // E_z(i-1/2, j-1/2, k): A = x, B = y
+        const double ez = edge_emf(-S(0, YM), -S(0, 0), S(3, XM), S(3, 0), S(6, YM), wx, S(7, XM), wy,
+                                   S(11, XYM), S(11, YM), S(11, XM), S(11, 0));
+        double exN = 0.0, eyN = 0.0;
+        sE[buf][0][ty][tx] = ez;
+        if (!TWO_D) {
+            const double wz = S(8, 0);
+            // E_x(i, j-1/2, k-1/2): A = y, B = z
+            const double fyzN = S(2, 0), excN = S(9, 0), excNm = S(9, YM);
+            exN = edge_emf(-fyz, -fyzN, S(5, YM), S(5, 0), wyP, wy, S(8, YM), wz, excPm, excP, excNm, excN);
+            // E_y(i-1/2, j, k-1/2): A = z, B = x
+            const double fxzN = S(1, 0), eycN = S(10, 0), eycNm = S(10, XM);
+            eyN = edge_emf(-S(4, XM), -S(4, 0), fxz, fxzN, S(8, XM), wz, wxP, wx, eycPm, eycNm, eycP, eycN);
+            sE[buf][1][ty][tx] = exN; sE[buf][2][ty][tx] = eyN;
+            fyz = fyzN; wyP = wy; excP = excN; excPm = excNm;
+            fxz = fxzN; wxP = wx; eycP = eycN; eycPm = eycNm;
         }
-        __syncthreads();
+        __syncthreads();                                      // edge EMFs of this iteration are visible
         if (upd) {
-            const double ezy = sEz[sz][ty + 1][tx], ezx = sEz[sz][ty][tx + 1];
-            double bxn, byn;
-            if (!TWO_D) {
-                const double eyx = sEy[sl][ty][tx + 1], exy = sEx[sl][ty + 1][tx];
-                bxn = b0 - dt * ((ezy - ez) / g.dx[1] - (eyN - eyP) / g.dx[2]);
-                byn = b1 - dt * ((exN - exP) / g.dx[2] - (ezx - ez) / g.dx[0]);
-                double bzn = b2 - dt * ((eyx - eyP) / g.dx[0] - (exy - exP) / g.dx[1]);
-                bout[2 * sa + c] = COMBINE ? 0.5 * (o2 + bzn) : bzn;
+            const double ezx = sE[buf][0][ty][tx + 1], ezy = sE[buf][0][ty + 1][tx];
+            const long long c = plane(k) + oc;
+            if (TWO_D) {
+                const double bxn = pbx - dtdy * (ezy - ez);
+                const double byn = pby + dtdx * (ezx - ez);
+                bout[c] = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                bout[sa + c] = COMBINE ? 0.5 * (qby + byn) : byn;
+                if (dbg) { dbg[c] = 0.0; dbg[sa + c] = 0.0; dbg[2 * sa + c] = ez; }
             } else {
-                bxn = b0 - dt * ((ezy - ez) / g.dx[1] - 0.0);
-                byn = b1 - dt * (0.0 - (ezx - ez) / g.dx[0]);
+                if (k > k0) {                                 // b_x, b_y of plane k-1
+                    const long long cm = plane(k - 1) + oc;
+                    const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
+                    const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
+                    bout[cm] = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    bout[sa + cm] = COMBINE ? 0.5 * (qby + byn) : byn;
+                }
+                if (k < k1) {                                 // b_z on the lower face of plane k
+                    const double eyx = sE[buf][2][ty][tx + 1], exy = sE[buf][1][ty + 1][tx];
+                    const double bzn = pbz - (dtdx * (eyx - eyN) - dtdy * (exy - exN));
+                    bout[2 * sa + c] = COMBINE ? 0.5 * (qbz + bzn) : bzn;
+                    if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
+                    // operands of the next iteration: b_x, b_y of this plane, b_z of the next
+                    pbx = bin[c]; pby = bin[sa + c];
+                    if (COMBINE) { qbx = bout[c]; qby = bout[sa + c]; }
+                    if (k + 1 < k1) {
+                        pbz = bin[2 * sa + c + st2];
+                        if (COMBINE) qbz = bout[2 * sa + c + st2];
+                    }
+                }
+                dEzx = ezx - ez; dEzy = ezy - ez;
             }
-            bout[c] = COMBINE ? 0.5 * (o0 + bxn) : bxn;
-            bout[sa + c] = COMBINE ? 0.5 * (o1 + byn) : byn;
-            if (dbg) { dbg[c] = exP; dbg[sa + c] = eyP; dbg[2 * sa + c] = ez; }
         }
         exP = exN; eyP = eyN;
     }

@@ -172,17 +172,19 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     const double SMBx = SM * Bx;
     const double vBss = fma(vss, Byss, fma(wss, Bzss, SMBx));
 
+#ifndef HLLD_VARIANT
+#define HLLD_VARIANT 0
+#endif
+#if HLLD_VARIANT == 0
     // the side the interface lies in (test order of R5: ..., S*_L >= 0, S_M >= 0, S*_R > 0), and
     // whether it lies outside the Alfven wave of that side:  S*_L = S_M - |Bx|/rL >= 0, S*_R = S_M + |Bx|/rR <= 0
     const bool left = SM >= 0.0;
-    const double aBx = fabs(Bx);
-    const bool outer = left ? (SM * rL >= aBx) : (-SM * rR >= aBx);
-
     const double rho = left ? L.rho : R.rho, u = left ? L.u : R.u, v = left ? L.v : R.v, w = left ? L.w : R.w;
     const double By = left ? L.By : R.By, Bz = left ? L.Bz : R.Bz, p = left ? L.p : R.p;
     const double B2 = left ? B2L : B2R, pT = left ? pTL : pTR, d = left ? dL : dR, idS = left ? idSL : idSR;
     const double rs = left ? rsL : rsR, r = left ? rL : rR;
     const double vs = left ? vsL : vsR, ws = left ? wsL : wsR, Bys = left ? BysL : BysR, Bzs = left ? BzsL : BzsR;
+    const bool outer = fabs(SM) * r >= fabs(Bx);
 
     // energy of the chosen side: U, U*, U**
     const double E  = fma(p, igm1, 0.5 * fma(rho, fma(u, u, fma(v, v, w * w)), B2));
@@ -192,18 +194,60 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     const double sr = left ? -sig * r : sig * r;
     const double Ess = fma(sr, vBs - vBss, Es);
 
-    double rf = rs, uf = SM, pf = pTs;
+    double rho_f = rs, uf = SM, pf = pTs;
     double vf = outer ? vs : vss, wf = outer ? ws : wss, Byf = outer ? Bys : Byss, Bzf = outer ? Bzs : Bzss;
     double Ef = outer ? Es : Ess, vBf = outer ? vBs : vBss;
+    const double EL = 0.0, ER = 0.0;
+#elif HLLD_VARIANT == 1
+    // energy chain of both sides up to the part that needs the star state:
+    //   E*_a (S_a - S_M) = G_a + pT* S_M - Bx (v.B)*_a,   G_a = (S_a - u_a) E_a - pT_a u_a + Bx (v.B)_a
+    const double EL = fma(L.p, igm1, 0.5 * fma(L.rho, fma(L.u, L.u, fma(L.v, L.v, L.w * L.w)), B2L));
+    const double ER = fma(R.p, igm1, 0.5 * fma(R.rho, fma(R.u, R.u, fma(R.v, R.v, R.w * R.w)), B2R));
+    const double GL = fma(dL, EL, fma(Bx, fma(L.u, Bx, fma(L.v, L.By, L.w * L.Bz)), -pTL * L.u));
+    const double GR = fma(dR, ER, fma(Bx, fma(R.u, Bx, fma(R.v, R.By, R.w * R.Bz)), -pTR * R.u));
+    const double vBsL = fma(vsL, BysL, fma(wsL, BzsL, SMBx)), vBsR = fma(vsR, BysR, fma(wsR, BzsR, SMBx));
+
+    // the side the interface lies in (test order of R5: ..., S*_L >= 0, S_M >= 0, S*_R > 0)
+    const bool left = SM >= 0.0;
+    const double rf = left ? rsL : rsR, r = left ? rL : rR, vBs = left ? vBsL : vBsR;
+    const double Es = (fma(pTs, SM, left ? GL : GR) - Bx * vBs) * (left ? idSL : idSR);
+    const double sr = left ? -sig * r : sig * r;
+
+    // inside the Alfven waves: the double-star state
+    double uf = SM, pf = pTs, rho_f = rf;
+    double vf = vss, wf = wss, Byf = Byss, Bzf = Bzss, vBf = vBss, Ef = fma(sr, vBs - vBss, Es);
+    // outside the Alfven wave of that side:  S*_L = S_M - |Bx|/rL >= 0  or  S*_R = S_M + |Bx|/rR <= 0
+    if (fabs(SM) * r >= fabs(Bx)) {
+        vf = left ? vsL : vsR; wf = left ? wsL : wsR; Byf = left ? BysL : BysR; Bzf = left ? BzsL : BzsR;
+        vBf = vBs; Ef = Es;
+    }
+#else
+    const double EL = fma(L.p, igm1, 0.5 * fma(L.rho, fma(L.u, L.u, fma(L.v, L.v, L.w * L.w)), B2L));
+    const double ER = fma(R.p, igm1, 0.5 * fma(R.rho, fma(R.u, R.u, fma(R.v, R.v, R.w * R.w)), B2R));
+    const double GL = fma(dL, EL, fma(Bx, fma(L.u, Bx, fma(L.v, L.By, L.w * L.Bz)), -pTL * L.u));
+    const double GR = fma(dR, ER, fma(Bx, fma(R.u, Bx, fma(R.v, R.By, R.w * R.Bz)), -pTR * R.u));
+    const double vBsL = fma(vsL, BysL, fma(wsL, BzsL, SMBx)), vBsR = fma(vsR, BysR, fma(wsR, BzsR, SMBx));
+    const bool left = SM >= 0.0;
+    const double rf = left ? rsL : rsR, r = left ? rL : rR, vBs = left ? vBsL : vBsR;
+    const double Es = (fma(pTs, SM, left ? GL : GR) - Bx * vBs) * (left ? idSL : idSR);
+    const double sr = left ? -sig * r : sig * r;
+    const bool outer = fabs(SM) * r >= fabs(Bx);
+    double uf = SM, pf = pTs, rho_f = rf;
+    double vf = outer ? (left ? vsL : vsR) : vss, wf = outer ? (left ? wsL : wsR) : wss;
+    double Byf = outer ? (left ? BysL : BysR) : Byss, Bzf = outer ? (left ? BzsL : BzsR) : Bzss;
+    double vBf = outer ? vBs : vBss, Ef = outer ? Es : fma(sr, vBs - vBss, Es);
+#endif
     if (__builtin_expect(SL >= 0.0 || SR <= 0.0, 0)) {          // one-sided fan: the upwind physical flux (Eq. 2)
         const bool sl = SL >= 0.0;
-        rf = sl ? L.rho : R.rho; uf = sl ? L.u : R.u; vf = sl ? L.v : R.v; wf = sl ? L.w : R.w;
+        rho_f = sl ? L.rho : R.rho; uf = sl ? L.u : R.u; vf = sl ? L.v : R.v; wf = sl ? L.w : R.w;
         Byf = sl ? L.By : R.By; Bzf = sl ? L.Bz : R.Bz; pf = sl ? pTL : pTR;
-        const double pp = sl ? L.p : R.p, bb = sl ? B2L : B2R;
-        Ef = fma(pp, igm1, 0.5 * fma(rf, fma(uf, uf, fma(vf, vf, wf * wf)), bb));
+        {
+            const double pp = sl ? L.p : R.p, bb = sl ? B2L : B2R;
+            Ef = fma(pp, igm1, 0.5 * fma(rho_f, fma(uf, uf, fma(vf, vf, wf * wf)), bb));
+        }
         vBf = fma(uf, Bx, fma(vf, Byf, wf * Bzf));
     }
-    const double F0 = rf * uf;
+    const double F0 = rho_f * uf;
     f[0] = F0;
     f[1] = fma(F0, uf, pf - Bx2);
     f[2] = fma(F0, vf, -Bx * Byf);

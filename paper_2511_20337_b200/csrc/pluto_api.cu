@@ -159,23 +159,22 @@ void launch_sweeps(const double *Sin, double *Sout, bool combine)
     double *ct = arr(A_CT);
     const double scale = combine ? 0.5 : 1.0;
     if (C.fuse_xy) {
-        // fused x + y sweep: one block per x-row chunk and y-segment
-        const bool wrap = g.n[0] % 32 == 0 && g.n[0] <= 512;
-        const int nt = wrap ? g.n[0] : (g.n[0] >= 252 ? 256 : (int)round_up(g.n[0] + 4, 32));
-        const int chunks = wrap ? 1 : (g.n[0] + nt - 5) / (nt - 4);
-        const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
+        // fused x + y sweep: one block per x-row chunk and y-segment.  The block width is a template
+        // parameter (shared-memory offsets become immediates): a whole periodic row when nx is one of
+        // the instantiated widths, else chunks of 128 or 256 threads that overlap by four cells.
+        const int nx = g.n[0];
+        const bool wrap = nx == 64 || nx == 128 || nx == 256 || nx == 512;
+        const int nt = wrap ? nx : (nx > 124 ? 256 : 128);
+        const int chunks = wrap ? 1 : (nx + nt - 5) / (nt - 4);
+        const int len = march_seglen(g.n[1], (long long)nx * g.n[2]);
         dim3 grid(chunks, (g.n[1] + len - 1) / len, g.n[2]);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double);
-        auto kw = k_sweep_xy<LIM, TWO_D, true>;
-        auto kc = k_sweep_xy<LIM, TWO_D, false>;
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaFuncSetAttribute(kw, cudaFuncAttributeMaxDynamicSharedMemorySize, XY_DOUBLES_PER_THREAD * 512 * 8);
-            cudaFuncSetAttribute(kc, cudaFuncAttributeMaxDynamicSharedMemorySize, XY_DOUBLES_PER_THREAD * 512 * 8);
-            attr_set = true;
-        }
-        if (wrap) LAUNCH(K_FLUX_XY, kw<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, combine ? 1 : 0, len));
-        else      LAUNCH(K_FLUX_XY, kc<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, combine ? 1 : 0, len));
+        void (*k)(Grid, const double *, double *, double *, StepParams *, int, int) =
+            wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
+                    : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
+                 : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
+        cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, combine ? 1 : 0, len));
     } else {
         const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
         LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
@@ -202,12 +201,13 @@ void launch_ct(const double *bin, double *bout, bool combine, double *dbg)
     const int len = march_seglen(g.n[2], (long long)tiles_x * tiles_y * CT_TX * CT_TY);
     dim3 grid(tiles_x, tiles_y, (g.n[2] + len - 1) / len), block(CT_TX, CT_TY);
     const double *ct = arr(A_CT);
+    const size_t smem = 0;
     if (g.act[2]) {
-        if (combine) LAUNCH(K_CT, k_ct<true, false><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
-        else         LAUNCH(K_CT, k_ct<false, false><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        if (combine) LAUNCH(K_CT, k_ct<true, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        else         LAUNCH(K_CT, k_ct<false, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
     } else {
-        if (combine) LAUNCH(K_CT, k_ct<true, true><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
-        else         LAUNCH(K_CT, k_ct<false, true><<<grid, block, 0, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        if (combine) LAUNCH(K_CT, k_ct<true, true><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        else         LAUNCH(K_CT, k_ct<false, true><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
     }
 }
 
