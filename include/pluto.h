@@ -103,7 +103,8 @@ double pluto_probe_fp64_gflops(void);
 /* Tuning switches: opt = PLUTO_OPT_*, returns the previous value or PLUTO_EINVAL. */
 enum {
     PLUTO_OPT_GRAPH = 1,   /* 1 (default): replay one captured CUDA graph per step; 0: plain launches */
-    PLUTO_OPT_FUSE_XY = 2  /* 1 (default): x and y sweeps fused in one kernel; 0: one kernel per direction */
+    PLUTO_OPT_FUSE_XY = 2, /* 1 (default): x and y sweeps fused in one kernel; 0: one kernel per direction */
+    PLUTO_OPT_CT_TMA = 3   /* 1 (default): CT operands staged by TMA (cp.async.bulk.tensor); 0: per-thread loads */
 };
 int    pluto_set_option(int opt, int value);
 

@@ -20,6 +20,7 @@ OK, EINVAL, ESTATE, ECUDA, EPHYS, ENOMEM = 0, -1, -2, -3, -4, -5
 MINMOD, MC = 0, 1
 OPT_GRAPH = 1
 OPT_FUSE_XY = 2
+OPT_CT_TMA = 3
 
 # every symbol include/pluto.h declares
 SYMBOLS = [

@@ -83,6 +83,11 @@ __global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base
 // ct + CT_EC + e        : cell-centred EMF component e, E^c = -(v x B)
 enum { CT_FEM = 0, CT_W = 6, CT_EC = 9, CT_COUNT = 12 };
 
+// The CT kernel reads the CT arrays one position beyond the interior in x (i = -1 and i = nx hold the
+// periodic copies of cells nx-1 and 0).  The sweep kernels write those copies with the value itself:
+// offset of the copy for cell i, or 0.
+__device__ __forceinline__ int ct_xdup(int i, int nx) { return i == 0 ? nx : (i == nx - 1 ? -nx : 0); }
+
 // cell-centred B of cell c from the face arrays b = S + S_B*sa (R7); 2D: b[2] is the cell-centred B_z
 template <bool TWO_D>
 __device__ __forceinline__ void cell_b(const Grid &g, const double *__restrict__ b, long long c, double B[3])
@@ -185,13 +190,24 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
             double r7 = Bc[2] - dtdx * (sP[5][t + 1] - F[5]);
             Sout[7 * sa + c] = combine ? 0.5 * (o7 + r7) : r7;
         }
+        // cell-centred EMF  E^c = -(v x B)
+        const double e0 = q[3] * q[4] - q[2] * q[5], e1 = q[1] * q[5] - q[3] * Bc[0], e2 = q[2] * Bc[0] - q[1] * q[4];
         ct[(CT_FEM + 0) * sa + c] = F[4];
         ct[(CT_FEM + 1) * sa + c] = F[5];
         ct[(CT_W + 0) * sa + c] = w;
-        // cell-centred EMF  E^c = -(v x B)
-        ct[(CT_EC + 0) * sa + c] = q[3] * q[4] - q[2] * q[5];
-        ct[(CT_EC + 1) * sa + c] = q[1] * q[5] - q[3] * Bc[0];
-        ct[(CT_EC + 2) * sa + c] = q[2] * Bc[0] - q[1] * q[4];
+        ct[(CT_EC + 0) * sa + c] = e0;
+        ct[(CT_EC + 1) * sa + c] = e1;
+        ct[(CT_EC + 2) * sa + c] = e2;
+        const int xdup = ct_xdup(f, nx);
+        if (xdup) {
+            const long long cd = c + xdup;
+            ct[(CT_FEM + 0) * sa + cd] = F[4];
+            ct[(CT_FEM + 1) * sa + cd] = F[5];
+            ct[(CT_W + 0) * sa + cd] = w;
+            ct[(CT_EC + 0) * sa + cd] = e0;
+            ct[(CT_EC + 1) * sa + cd] = e1;
+            ct[(CT_EC + 2) * sa + cd] = e2;
+        }
     }
 }
 
@@ -241,8 +257,13 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 constexpr int MARCH_NT = 128;
 constexpr int MARCH_PF = 16;     // doubles per thread and iteration: U(s+1) 5, faces 5, U'(s-1) 6
 
+// three blocks of 128 threads per SM: 168 registers per thread hold the running state without
+// spilling (measured: 4 blocks at 128 registers spill ~40 values per interface and run 20% slower)
+#ifndef MARCH_MINB
+#define MARCH_MINB 3
+#endif
 template <int DIR, int LIM, bool TWO_D>
-__global__ void __launch_bounds__(MARCH_NT, 4)
+__global__ void __launch_bounds__(MARCH_NT, MARCH_MINB)
 k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
               double scale, int seglen)
 {
@@ -353,6 +374,12 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;
+            const int xdup = ct_xdup(blockIdx.x * MARCH_NT + threadIdx.x, g.n[0]);
+            if (xdup) {
+                ct[(CT_FEM + 2 * DIR) * sa + c + xdup] = F[4];
+                ct[(CT_FEM + 2 * DIR + 1) * sa + c + xdup] = F[5];
+                ct[(CT_W + DIR) * sa + c + xdup] = w;
+            }
         }
         Fp[0] = F[0]; Fp[1] = F[1]; Fp[2] = F[2]; Fp[3] = F[3]; Fp[4] = F[6]; Fp[5] = F[4];
         c += st;
@@ -402,6 +429,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const bool has_slope = WRAP || (valid && t >= 1 && t <= NT - 2 && i + 1 < nx + 2);
     const bool xface = WRAP || (has_slope && t >= 2 && i <= nx);
     const bool cell = WRAP || (xface && t <= NT - 3 && i < nx);     // this thread owns an interior cell
+    const int xdup = cell ? ct_xdup(i, nx) : 0;
     const int k = blockIdx.z;
     const int s0 = blockIdx.y * seglen, s1 = min(s0 + seglen, g.n[1]);
     const long long sa = g.sa, st = g.st[1], stz = g.st[2];
@@ -540,13 +568,24 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             }
             if (cell) {
                 const long long cm = c - st;
+                // cell-centred EMF  E^c = -(v x B)
+                const double e0 = qo[3] * qo[5] - qo[2] * qo[6], e1 = qo[1] * qo[6] - qo[3] * qo[4],
+                             e2 = qo[2] * qo[4] - qo[1] * qo[5];
                 ct[(CT_FEM + 0) * sa + cm] = F[4];
                 ct[(CT_FEM + 1) * sa + cm] = F[5];
                 ct[(CT_W + 0) * sa + cm] = w;
-                // cell-centred EMF  E^c = -(v x B)
-                ct[(CT_EC + 0) * sa + cm] = qo[3] * qo[5] - qo[2] * qo[6];
-                ct[(CT_EC + 1) * sa + cm] = qo[1] * qo[6] - qo[3] * qo[4];
-                ct[(CT_EC + 2) * sa + cm] = qo[2] * qo[4] - qo[1] * qo[5];
+                ct[(CT_EC + 0) * sa + cm] = e0;
+                ct[(CT_EC + 1) * sa + cm] = e1;
+                ct[(CT_EC + 2) * sa + cm] = e2;
+                if (xdup) {
+                    const long long cd = cm + xdup;
+                    ct[(CT_FEM + 0) * sa + cd] = F[4];
+                    ct[(CT_FEM + 1) * sa + cd] = F[5];
+                    ct[(CT_W + 0) * sa + cd] = w;
+                    ct[(CT_EC + 0) * sa + cd] = e0;
+                    ct[(CT_EC + 1) * sa + cd] = e1;
+                    ct[(CT_EC + 2) * sa + cd] = e2;
+                }
             }
             __syncthreads();                         // B3
             if (cell) {
@@ -606,6 +645,11 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             ct[(CT_FEM + 2) * sa + c] = Fy[4];
             ct[(CT_FEM + 3) * sa + c] = Fy[5];
             ct[(CT_W + 1) * sa + c] = wy;
+            if (xdup) {
+                ct[(CT_FEM + 2) * sa + c + xdup] = Fy[4];
+                ct[(CT_FEM + 3) * sa + c + xdup] = Fy[5];
+                ct[(CT_W + 1) * sa + c + xdup] = wy;
+            }
         }
         Fpy[0] = Fy[0]; Fpy[1] = Fy[1]; Fpy[2] = Fy[2]; Fpy[3] = Fy[3]; Fpy[4] = Fy[6]; Fpy[5] = Fy[4];
         bface = bnext; bnext = byu;

@@ -2,6 +2,7 @@
 // launch sequence of one RK2 step.  No CPU fallback: without a device every call fails loudly.
 #include "../../include/pluto.h"
 #include "kernels.cuh"
+#include "ct_tma.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -20,9 +21,9 @@ using namespace pluto;
 
 namespace {
 
-enum KernelId { K_GHOST = 0, K_FLUX_XY, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_CT, K_DTMAX, K_SCALAR, K_PACK, K_COUNT };
+enum KernelId { K_GHOST = 0, K_FLUX_XY, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_CT, K_DTMAX, K_SCALAR, K_PACK, K_CT_HALO, K_COUNT };
 const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_xy", "sweep_x", "sweep_y", "sweep_z", "ct",
-                                            "dt_max", "scalars", "pack_unpack" };
+                                            "dt_max", "scalars", "pack_unpack", "ct_halo" };
 
 struct Context {
     bool init = false;
@@ -40,6 +41,8 @@ struct Context {
     long long per_step[2] = { 0, 0 };
     int use_graph = 1;
     int fuse_xy = 1;
+    int ct_tma = 1;
+    CUtensorMap ct_map{};            // the twelve CT arrays as one 4D tensor (x, y, z, array)
     cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step
     int sm_count = 148;
     char err[512] = "";
@@ -130,6 +133,32 @@ void destroy_graphs()
         if (gr) { cudaGraphExecDestroy(gr); gr = nullptr; }
 }
 
+// TMA descriptor of the CT work arrays: dims (pitch, tot1, tot2, CT_COUNT) doubles, box = one tile of
+// one array.  cuTensorMapEncodeTiled is taken from the driver through the runtime (no -lcuda).
+int make_ct_map()
+{
+    typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                 const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn)
+            return fail(PLUTO_ECUDA, "cuTensorMapEncodeTiled not available from the driver");
+        encode = (EncodeFn)fn;
+    }
+    const Grid &g = C.g;
+    cuuint64_t dims[4] = { (cuuint64_t)g.tot[0], (cuuint64_t)g.tot[1], (cuuint64_t)g.tot[2], (cuuint64_t)CT_COUNT };
+    cuuint64_t strides[3] = { (cuuint64_t)g.st[1] * 8, (cuuint64_t)g.st[2] * 8, (cuuint64_t)g.sa * 8 };
+    cuuint32_t box[4] = { CTM_COLS, CTM_ROWS, 1, 1 }, estr[4] = { 1, 1, 1, 1 };
+    CUresult r = encode(&C.ct_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, arr(A_CT), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(PLUTO_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return PLUTO_OK;
+}
+
 // ---------------------------------------------------------------- launch sequences
 
 // ghost layers of the 8 arrays of one state, one launch
@@ -201,6 +230,26 @@ void launch_ct(const double *bin, double *bout, bool combine, double *dbg)
     const int len = march_seglen(g.n[2], (long long)tiles_x * tiles_y * CT_TX * CT_TY);
     dim3 grid(tiles_x, tiles_y, (g.n[2] + len - 1) / len), block(CT_TX, CT_TY);
     const double *ct = arr(A_CT);
+    if (C.ct_tma) {
+        // periodic halo layer of the CT arrays, then the TMA-staged kernel
+        LAUNCH(K_CT_HALO, k_ct_halo<<<dim3(g.n[2], CT_COUNT), 256, 0, s>>>(g, arr(A_CT), g.act[2] ? 0 : 1));
+        static bool tma_attr = false;
+        if (!tma_attr) {
+            cudaFuncSetAttribute(k_ct_tma<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
+            cudaFuncSetAttribute(k_ct_tma<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
+            cudaFuncSetAttribute(k_ct_tma<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
+            cudaFuncSetAttribute(k_ct_tma<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
+            tma_attr = true;
+        }
+        if (g.act[2]) {
+            if (combine) LAUNCH(K_CT, k_ct_tma<true, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
+            else         LAUNCH(K_CT, k_ct_tma<false, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
+        } else {
+            if (combine) LAUNCH(K_CT, k_ct_tma<true, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
+            else         LAUNCH(K_CT, k_ct_tma<false, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
+        }
+        return;
+    }
     const size_t smem = 0;
     if (g.act[2]) {
         if (combine) LAUNCH(K_CT, k_ct<true, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
@@ -402,6 +451,8 @@ int pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int 
     CUDA_TRY(cudaMemsetAsync(C.base, 0, bytes, C.stream));
     CUDA_TRY(cudaStreamSynchronize(C.stream));
     C.init = true; C.have_state = false; C.stepped = false; C.launches = 0;
+    int rc = make_ct_map();
+    if (rc) { C.init = false; return rc; }
     return PLUTO_OK;
 }
 
@@ -418,6 +469,12 @@ int pluto_set_box(double Lx, double Ly, double Lz)
 int pluto_set_option(int opt, int value)
 {
     if (opt == PLUTO_OPT_GRAPH) { int old = C.use_graph; C.use_graph = value ? 1 : 0; return old; }
+    if (opt == PLUTO_OPT_CT_TMA) {
+        int old = C.ct_tma;
+        C.ct_tma = value ? 1 : 0;
+        destroy_graphs();
+        return old;
+    }
     if (opt == PLUTO_OPT_FUSE_XY) {
         int old = C.fuse_xy;
         C.fuse_xy = value ? 1 : 0;
