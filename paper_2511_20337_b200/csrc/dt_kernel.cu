@@ -10,7 +10,7 @@
 
 namespace pluto {
 
-// exact per-zone candidates, IEEE operations in the oracle's order (R15)
+// exact per-zone candidates, IEEE operations in the expression order DESIGN.md fixes (R15)
 __device__ __forceinline__ double zone_sigma_exact(const Grid &g, double rho, double mx, double my, double mz,
                                                    double E, const double B[3], int &bad)
 {
