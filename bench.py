@@ -40,7 +40,17 @@ UNIT = "zone-updates/s"
 #               the combine stage also reads S^n 5 = 27; the two launches of a step average 24.5
 #   sweep_x   : read S 8, write S' 5, CT data 6 (2 fluxes, 1 weight, 3 cell EMFs)                  = 19
 #   sweep_y/z : read S 8, read + write S' 5 + 5, CT data 3                                           = 21
-ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21}
+#   ct        : read CT data 12 + faces 3, write faces 3 = 18; the combine stage also reads S^n faces 3 = 21;
+#               the two launches of a step average 19.5
+ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21, "ct": 19.5}
+
+# From the committed ncu capture of the same workload (profiles/, `ncu --set full`, per launch, mean of the
+# stage-1 and stage-2 launches of a step): DRAM bytes moved and fp64-pipe instructions executed per zone.
+NCU = {
+    "sweep_xy": {"dram_bytes_per_launch": 3.47e9, "fp64_instr_per_zone": 572, "profile": "profiles/r1b_step_kernels.md"},
+    "sweep_z": {"dram_bytes_per_launch": 2.83e9, "fp64_instr_per_zone": 283, "profile": "profiles/r1b_step_kernels.md"},
+    "ct": {"dram_bytes_per_launch": 2.7e9, "fp64_instr_per_zone": 90, "profile": "profiles/r1b_step_kernels.md"},
+}
 
 
 def peaks():
@@ -239,6 +249,15 @@ def main():
                 "algorithmic_bytes_per_launch": algo_bytes,
                 "kernels_ms_per_step": {k: v[0] / K for k, v in rep.items() if v[1]},
                 "profiled_ms_per_step": ms_prof / K}
+    if dom in NCU:
+        roofline["traffic"] = NCU[dom]["dram_bytes_per_launch"] * (units / 256 ** 3)   # scaled from the 256^3 capture
+        roofline["traffic_source"] = NCU[dom]["profile"]
+        # the same kernel against the fp64 pipe: instructions executed per second vs the probed DFMA rate
+        fp64_peak = sim.probe_fp64_gflops() * 0.5e9            # DFMA/s (2 flops each)
+        rate = NCU[dom]["fp64_instr_per_zone"] * units / dur if dur > 0 else 0.0
+        roofline["alu"] = {"bound": "alu", "achieved": rate * 1e-12, "peak": fp64_peak * 1e-12, "unit": "T fp64-instr/s",
+                           "frac": rate / fp64_peak, "peak_source": "pluto_probe_fp64_gflops (register-resident DFMA loop, this run)",
+                           "fp64_instr_per_zone": NCU[dom]["fp64_instr_per_zone"]}
     # whole-step view: minimum traffic 320 B per zone-update
     roofline["step_hbm_frac_at_320B"] = value / world * 320.0 / (hbm_peak * 1e9)
 

@@ -246,6 +246,43 @@ def test_config3_full_size_sampled(pluto, oracle):
     assert np.abs(div).max() <= 1e-12 * np.abs(Bf).max()
 
 
+def test_config4_full_size_sampled(pluto, oracle):
+    """configs[4]: 3D blast 512^3 (134M zones, ~31 GB of library state) at full size, one step"""
+    w = wl.config(4)
+    r = int(0.1 * w.nx)
+    h = w.nx // 2
+    centres = [(h + r, h, h), (h, h, h - r), (0, 0, 0), (w.nx - 1, w.ny - 1, w.nz - 1), (100, 400, 333)]
+    U, Bf = _subbox_parity(pluto, oracle, w, centres)
+    for v in (0, 7):
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * abs(math.fsum(w.U[v].ravel()))
+    pluto.finalize()
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_dt_bit_exact_at_full_size(pluto, oracle, cfg):
+    """the filtered CFL reduction returns the oracle's dt bit for bit on the full-size initial states"""
+    w = wl.config(cfg)
+    pluto.load(w)
+    oracle.load(w)
+    assert pluto.get_dt() == oracle.get_dt()
+    oracle.finalize()
+
+
+def test_ct_tma_and_per_thread_paths_agree(pluto):
+    """the TMA-staged CT kernel and the per-thread-load CT kernel give identical bits"""
+    from paper_2511_20337_b200.binding import OPT_CT_TMA
+    for shape in [(40, 24, 12), (64, 20, 1), (37, 23, 9), (31, 7, 5), (63, 15, 3)]:
+        w = wl.random_smooth(*shape, seed=11, limiter=1)
+        out = []
+        for tma in (1, 0):
+            pluto.load(w)
+            pluto.set_option(OPT_CT_TMA, tma)
+            pluto.step(3)
+            out.append(pluto.get_state())
+        pluto.set_option(OPT_CT_TMA, 1)
+        assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]), shape
+
+
 def test_device_pointers_and_graph_equivalence(pluto, oracle):
     """set/get with CUDA tensors; graph replay and plain launches give identical bits"""
     import torch
