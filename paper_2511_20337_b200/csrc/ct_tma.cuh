@@ -189,7 +189,9 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
             if (TWO_D) {
                 const double bxn = pbx - dtdy * (ezy - ez);
                 const double byn = pby + dtdx * (ezx - ez);
-                bout[c] = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                bout[c] = bxo;
+                if (i == 0) bout[c + g.n[0]] = bxo;       // periodic copy: x-face n0 is face 0
                 bout[sa + c] = COMBINE ? 0.5 * (qby + byn) : byn;
                 if (dbg) { dbg[c] = 0.0; dbg[sa + c] = 0.0; dbg[2 * sa + c] = ez; }
             } else {
@@ -197,7 +199,9 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
                     const long long cm = (long long)zc(k - 1) * st2 + oc;
                     const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
                     const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
-                    bout[cm] = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    bout[cm] = bxo;
+                    if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
                     bout[sa + cm] = COMBINE ? 0.5 * (qby + byn) : byn;
                 }
                 if (k < k1) {                    // b_z on the lower face of plane k

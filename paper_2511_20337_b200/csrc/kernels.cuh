@@ -76,6 +76,32 @@ __global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base
     }
 }
 
+// Ghost rows and planes only (y and z slabs), as whole padded rows: used when no kernel reads an x ghost
+// except the x-face n0, which the CT kernel writes together with face 0.  grid.x = ghost row, grid.y =
+// array.  The rows are walked as: the ghost planes (every padded row j of planes -ng..-1, n2..n2+ng), then
+// the ghost rows of the interior planes.  A row is copied over the padded x range [-ng, n0+ng].
+__global__ void __launch_bounds__(128) k_ghost_yz(Grid g, double *__restrict__ base)
+{
+    const int ng = g.ng, ngh = 2 * ng + 1;
+    const int rows_z = g.act[2] ? ngh * (g.n[1] + ngh) : 0;
+    int r = blockIdx.x, j, k;
+    if (r < rows_z) {
+        const int pz = r / (g.n[1] + ngh);
+        j = r - pz * (g.n[1] + ngh) - ng;
+        k = pz < ng ? pz - ng : g.n[2] + (pz - ng);
+    } else {
+        r -= rows_z;
+        k = r / ngh;
+        const int py = r - k * ngh;
+        j = py < ng ? py - ng : g.n[1] + (py - ng);
+    }
+    const int sj = (j + 2 * g.n[1]) % g.n[1], sk = (k + 2 * g.n[2]) % g.n[2];
+    double *arr = base + (long long)blockIdx.y * g.sa;
+    double *dst = arr + g.at(-ng, j, k);
+    const double *src = arr + g.at(-ng, sj, sk);
+    for (int e = threadIdx.x; e < g.n[0] + ngh; e += blockDim.x) dst[e] = src[e];
+}
+
 // ---------------------------------------------------------------- layout of the CT work arrays
 // ct + CT_FEM + 2*d + q : induction flux q of sweep d  (d = x: F_x[By], F_x[Bz]; y: F_y[Bz], F_y[Bx];
 //                         z: F_z[Bx], F_z[By]) on the lower d-face of each interior cell
@@ -794,7 +820,9 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
             if (TWO_D) {
                 const double bxn = pbx - dtdy * (ezy - ez);
                 const double byn = pby + dtdx * (ezx - ez);
-                bout[c] = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                bout[c] = bxo;
+                if (i == 0) bout[c + g.n[0]] = bxo;       // periodic copy: x-face n0 is face 0
                 bout[sa + c] = COMBINE ? 0.5 * (qby + byn) : byn;
                 if (dbg) { dbg[c] = 0.0; dbg[sa + c] = 0.0; dbg[2 * sa + c] = ez; }
             } else {
@@ -802,7 +830,9 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
                     const long long cm = plane(k - 1) + oc;
                     const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
                     const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
-                    bout[cm] = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    bout[cm] = bxo;
+                    if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
                     bout[sa + cm] = COMBINE ? 0.5 * (qby + byn) : byn;
                 }
                 if (k < k1) {                                 // b_z on the lower face of plane k

@@ -162,9 +162,20 @@ int make_ct_map()
 // ---------------------------------------------------------------- launch sequences
 
 // ghost layers of the 8 arrays of one state, one launch
-void fill_ghosts(double *state)
+// widths for which the fused x+y sweep spans a whole periodic row: no kernel then reads an x ghost
+// other than the x-face n0 (kept equal to face 0 by the CT kernel)
+bool row_wraps(int nx) { return nx == 64 || nx == 128 || nx == 256 || nx == 512; }
+
+void fill_ghosts(double *state, bool all = false)
 {
-    LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 8, 256, 0, C.stream>>>(C.g, state, S_COUNT));
+    const Grid &g = C.g;
+    if (!all && C.fuse_xy && row_wraps(g.n[0])) {
+        const int ngh = 2 * g.ng + 1;
+        const int rows = (g.act[2] ? ngh * (g.n[1] + ngh) : 0) + g.n[2] * ngh;
+        LAUNCH(K_GHOST, k_ghost_yz<<<dim3(rows, S_COUNT), 128, 0, C.stream>>>(g, state));
+    } else {
+        LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 8, 256, 0, C.stream>>>(g, state, S_COUNT));
+    }
 }
 
 // segments of a marching kernel: enough independent threads for ~8 waves of 16 warps per SM,
@@ -192,7 +203,7 @@ void launch_sweeps(const double *Sin, double *Sout, bool combine)
         // parameter (shared-memory offsets become immediates): a whole periodic row when nx is one of
         // the instantiated widths, else chunks of 128 or 256 threads that overlap by four cells.
         const int nx = g.n[0];
-        const bool wrap = nx == 64 || nx == 128 || nx == 256 || nx == 512;
+        const bool wrap = row_wraps(nx);
         const int nt = wrap ? nx : (nx > 124 ? 256 : 128);
         const int chunks = wrap ? 1 : (nx + nt - 5) / (nt - 4);
         const int len = march_seglen(g.n[1], (long long)nx * g.n[2]);
@@ -514,6 +525,7 @@ int pluto_set_state(const double *U, const double *Bface)
         k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + off, m[0], m[1], arr(A_SA + S_B + d));   // upper duplicate ignored
         off += api_count(g, d);
     }
+    fill_ghosts(arr(A_SA), true);    // every ghost once (the per-stage fill may skip x: see fill_ghosts)
     StepParams p0;
     memset(&p0, 0, sizeof p0);
     CUDA_TRY(cudaMemcpyAsync(C.P, &p0, sizeof p0, cudaMemcpyHostToDevice, s));
