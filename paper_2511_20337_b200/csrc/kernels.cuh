@@ -27,6 +27,39 @@ __device__ __forceinline__ bool thread_zone(const Box &b, int &i, int &j, int &k
 __device__ __forceinline__ int wrap_m1(int i, int n) { return i == 0 ? n - 1 : i - 1; }
 __device__ __forceinline__ int wrap_p1(int i, int n) { return i == n - 1 ? 0 : i + 1; }
 
+// ---------------------------------------------------------------- mbarrier / TMA primitives (PTX)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(void *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void *bar, unsigned parity)
+{
+    const unsigned a = smem_u32(bar);
+    unsigned ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+// generic-proxy accesses to shared memory before this point are ordered before later async-proxy (TMA) writes
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// contiguous bytes global -> shared by the TMA engine (no tensor map; 16-byte aligned, size % 16 == 0),
+// completion counted in bytes on `bar`
+__device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigned bytes, void *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
 // ---------------------------------------------------------------- periodic ghost fill (a1)
 // Every ghost position (index g in [-ng, 0) or [n, n+ng] along at least one active axis; cells and
 // faces alike, face n duplicates face 0) receives the value of its periodic image in the interior:
@@ -429,24 +462,27 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
 //     S' = (S - dt/dx (Fx(+) - Fx(-))) - dt/dy (Fy(+) - Fy(-))      [combine: the RK2 average]
 // WRAP: the block spans the whole periodic row (NT = nx), neighbours wrap inside shared memory and
 // no lane is idle.  Otherwise blocks overlap by four cells like k_sweep_x.
-// Operands travel global -> shared by 8-byte cp.async one iteration ahead (group A: the row that
-// arrives next; group F: S and S^n of the row that is finished next).
+// Operands travel global -> shared as whole row segments by TMA bulk copies (cp.async.bulk + mbarrier)
+// issued by one thread: group A, the row that arrives next, one iteration ahead; group F, S and S^n of
+// the row that is finished in this iteration.  They bypass L1 and cost the other threads no instruction.
 constexpr int XY_RING = 9;       // rho, vx, vy, vz, Bx, By, Bz, p (cell centred), b_x on the lower x-face
-constexpr int XY_PFA = 10;       // arriving row: U 5, bx 2, by 1 (upper), bz 2
+constexpr int XY_PFA = 10;       // arriving row: U 5, bx (row 5; 6 unused), by upper 7, bz 8, bz upper 9
 constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
 constexpr int XY_DOUBLES_PER_THREAD = 3 * XY_RING + XY_PFA + XY_PFF + 7;
+constexpr int XY_SMEM_EXTRA = 16;   // two mbarriers behind the arrays
 
 template <int LIM, bool TWO_D, bool WRAP, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT)
 k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
            int combine, int seglen)
 {
-    extern __shared__ double xy_smem[];
+    extern __shared__ __align__(128) double xy_smem[];
     const int t = threadIdx.x;
     double *ring = xy_smem;                       // [3][XY_RING][NT]
     double *pfa = ring + 3 * XY_RING * NT;        // [XY_PFA][NT]
     double *pff = pfa + XY_PFA * NT;              // [XY_PFF][NT]
     double *sQ = pff + XY_PFF * NT;               // [7][NT]: q^L along x, then the x fluxes
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(sQ + 7 * NT);   // [2]: group A, group F
     const int nx = g.n[0];
     const int i = WRAP ? t : (int)blockIdx.x * (NT - 4) - 2 + t;
     const bool valid = WRAP || i < nx + 2;
@@ -468,24 +504,35 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     long long c = g.at(valid ? i : 0, s0, k);                       // cell (i, s0, k)
     bool anybad = false;
 
-    auto prefetch_arrive = [&](long long cr) {                      // cr = the arriving cell
+    // TMA row copies, issued by thread 0: the block's x range [i0, i0 + NT) of one row of each array
+    const long long row0 = g.at(WRAP ? 0 : (int)blockIdx.x * (NT - 4) - 2, s0, k);    // first cell of row s0
+    constexpr unsigned ROWB = NT * 8;
+    auto issue_arrive = [&](long long cr) {                         // cr = first cell of the arriving row
+        mbar_expect_tx(bars, (TWO_D ? 8 : 9) * ROWB);
 #pragma unroll
-        for (int v = 0; v < 5; v++) cp_async8(&pfa[v * NT + t], Sin + v * sa + cr);
-        cp_async8(&pfa[5 * NT + t], bx + cr);
-        cp_async8(&pfa[6 * NT + t], bx + cr + 1);
-        cp_async8(&pfa[7 * NT + t], by + cr + st);
-        cp_async8(&pfa[8 * NT + t], bz + cr);
-        if (!TWO_D) cp_async8(&pfa[9 * NT + t], bz + cr + stz);
+        for (int v = 0; v < 5; v++) tma_bulk_g2s(pfa + v * NT, Sin + v * sa + cr, ROWB, bars);
+        tma_bulk_g2s(pfa + 5 * NT, bx + cr, ROWB, bars);
+        tma_bulk_g2s(pfa + 7 * NT, by + cr + st, ROWB, bars);
+        tma_bulk_g2s(pfa + 8 * NT, bz + cr, ROWB, bars);
+        if (!TWO_D) tma_bulk_g2s(pfa + 9 * NT, bz + cr + stz, ROWB, bars);
     };
-    auto prefetch_finish = [&](long long cf) {                      // cf = the cell finished next
+    auto issue_finish = [&](long long cf) {                         // cf = first cell of the row finished next
+        mbar_expect_tx(bars + 1, (5 + (combine ? (TWO_D ? 6 : 5) : 0)) * ROWB);
 #pragma unroll
-        for (int v = 0; v < 5; v++) cp_async8(&pff[v * NT + t], Sin + v * sa + cf);
+        for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + v * NT, Sin + v * sa + cf, ROWB, bars + 1);
         if (combine) {
 #pragma unroll
-            for (int v = 0; v < 5; v++) cp_async8(&pff[(5 + v) * NT + t], Sout + v * sa + cf);
-            if (TWO_D) cp_async8(&pff[10 * NT + t], Sout + 7 * sa + cf);
+            for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + (5 + v) * NT, Sout + v * sa + cf, ROWB, bars + 1);
+            if (TWO_D) tma_bulk_g2s(pff + 10 * NT, Sout + 7 * sa + cf, ROWB, bars + 1);
         }
     };
+    if (t == 0) {
+        mbar_init(bars, 1);
+        mbar_init(bars + 1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (t == 0) issue_arrive(row0 + st);                            // group A(s0): row s0 + 1
     // primitives of one cell from its conserved variables and the faces around it
     auto to_prim = [&](double rho, double mx, double my, double mz, double En, double B0, double B1, double B2,
                        double q[8], bool &bad) {
@@ -508,16 +555,12 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         double qa[8], qb[8], qc[8], f0, f1, f2;
         bool bad;
         if (valid) {
-            prefetch_arrive(c + st);
-            cp_async_commit();                       // group A(s0)
-            cp_async_commit();                       // group F(s0): empty
             load_prim(c - 2 * st, qa, f0, bad);
             load_prim(c - st, qb, f1, bad);
             load_prim(c, qc, f2, bad);
             if (cell) anybad |= bad;
             bface = by[c]; bnext = by[c + st];
         } else {
-            cp_async_commit(); cp_async_commit();
 #pragma unroll
             for (int v = 0; v < 8; v++) { qa[v] = qb[v] = qc[v] = (v == 0 || v == 7) ? 1.0 : 0.0; }
             f1 = f2 = 0.0; bface = bnext = 0.0;
@@ -540,34 +583,37 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
 
     for (int s = s0; s <= s1; s++, c += st) {
         // ---- (1) the arriving row s+1: convert, ring
-        cp_async_wait<1>();                          // group A(s) has landed
+        mbar_wait(bars, (s - s0) & 1);               // group A(s) has landed
         double q1[8], byu = 0.0;
         {
             bool bad = false;
             double bxf = 0.0;
             if (valid) {
-                double B0 = 0.5 * (pfa[5 * NT + t] + pfa[6 * NT + t]);
+                double B0 = 0.5 * (pfa[5 * NT + t] + pfa[5 * NT + tr]);     // the upper x-face is the neighbour's
                 byu = pfa[7 * NT + t];
                 double B1 = 0.5 * (bnext + byu);
                 double B2 = TWO_D ? pfa[8 * NT + t] : 0.5 * (pfa[8 * NT + t] + pfa[9 * NT + t]);
                 bxf = pfa[5 * NT + t];
                 to_prim(pfa[t], pfa[NT + t], pfa[2 * NT + t], pfa[3 * NT + t], pfa[4 * NT + t], B0, B1, B2, q1, bad);
                 if (cell && s + 1 < s1) anybad |= bad;
-                if (s < s1) prefetch_arrive(c + 2 * st);
             } else {
 #pragma unroll
                 for (int v = 0; v < 8; v++) q1[v] = (v == 0 || v == 7) ? 1.0 : 0.0;
             }
-            cp_async_commit();                       // group A(s+1)
 #pragma unroll
             for (int v = 0; v < 8; v++) rn[v * NT] = q1[v];
             rn[8 * NT] = bxf;
         }
-        __syncthreads();                             // B1: sQ free (fluxes of the previous row consumed)
+        __syncthreads();                             // B1: sQ free; everybody has read group A(s) and finished row s-2
+        if (t == 0) {
+            fence_proxy_async();
+            const long long cr = row0 + (long long)(s - s0) * st;              // first cell of row s
+            if (s < s1) issue_arrive(cr + 2 * st);                              // group A(s+1): row s + 2
+            if (s > s0) issue_finish(cr - st);                                  // group F(s): row s - 1
+        }
 
         // ---- (2) x interfaces of row s-1; their flux difference goes straight into the prefetched S of
         //      that row (group F(s), in shared memory), so nothing of it stays live across the y solve
-        cp_async_wait<1>();                          // group F(s) has landed
         if (s > s0) {
             const int xv[7] = { 0, 1, 2, 3, 5, 6, 7 };              // rho, vx, vy, vz, By, Bz, p
             double qR[7], qo[8];
@@ -614,6 +660,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                 }
             }
             __syncthreads();                         // B3
+            mbar_wait(bars + 1, (s - s0 - 1) & 1);   // group F(s) has landed
             if (cell) {
                 pff[t] -= dtdx * (sQ[tr] - F[0]);
                 pff[NT + t] -= dtdx * (sQ[NT + tr] - F[1]);
@@ -665,8 +712,6 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                 Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
             }
         }
-        if (valid && s < s1) prefetch_finish(c);
-        cp_async_commit();                           // group F(s+1)
         if (cell && s < s1) {
             ct[(CT_FEM + 2) * sa + c] = Fy[4];
             ct[(CT_FEM + 3) * sa + c] = Fy[5];
