@@ -466,7 +466,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
 // issued by one thread: group A, the row that arrives next, one iteration ahead; group F, S and S^n of
 // the row that is finished in this iteration.  They bypass L1 and cost the other threads no instruction.
 constexpr int XY_RING = 9;       // rho, vx, vy, vz, Bx, By, Bz, p (cell centred), b_x on the lower x-face
-constexpr int XY_PFA = 10;       // arriving row: U 5, bx (row 5; 6 unused), by upper 7, bz 8, bz upper 9
+constexpr int XY_PFA = 10;       // arriving row: U 5, bx (NT + 2 faces in rows 5-6), by upper 7, bz 8, bz upper 9
 constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
 constexpr int XY_DOUBLES_PER_THREAD = 3 * XY_RING + XY_PFA + XY_PFF + 7;
 constexpr int XY_SMEM_EXTRA = 16;   // two mbarriers behind the arrays
@@ -508,10 +508,10 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const long long row0 = g.at(WRAP ? 0 : (int)blockIdx.x * (NT - 4) - 2, s0, k);    // first cell of row s0
     constexpr unsigned ROWB = NT * 8;
     auto issue_arrive = [&](long long cr) {                         // cr = first cell of the arriving row
-        mbar_expect_tx(bars, (TWO_D ? 8 : 9) * ROWB);
+        mbar_expect_tx(bars, (TWO_D ? 8 : 9) * ROWB + 16);
 #pragma unroll
         for (int v = 0; v < 5; v++) tma_bulk_g2s(pfa + v * NT, Sin + v * sa + cr, ROWB, bars);
-        tma_bulk_g2s(pfa + 5 * NT, bx + cr, ROWB, bars);
+        tma_bulk_g2s(pfa + 5 * NT, bx + cr, ROWB + 16, bars);         // NT + 2 faces: thread t also reads face t + 1
         tma_bulk_g2s(pfa + 7 * NT, by + cr + st, ROWB, bars);
         tma_bulk_g2s(pfa + 8 * NT, bz + cr, ROWB, bars);
         if (!TWO_D) tma_bulk_g2s(pfa + 9 * NT, bz + cr + stz, ROWB, bars);
@@ -589,7 +589,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             bool bad = false;
             double bxf = 0.0;
             if (valid) {
-                double B0 = 0.5 * (pfa[5 * NT + t] + pfa[5 * NT + tr]);     // the upper x-face is the neighbour's
+                double B0 = 0.5 * (pfa[5 * NT + t] + pfa[5 * NT + t + 1]);
                 byu = pfa[7 * NT + t];
                 double B1 = 0.5 * (bnext + byu);
                 double B2 = TWO_D ? pfa[8 * NT + t] : 0.5 * (pfa[8 * NT + t] + pfa[9 * NT + t]);
