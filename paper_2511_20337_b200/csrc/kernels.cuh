@@ -466,10 +466,11 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
 // issued by one thread: group A, the row that arrives next, one iteration ahead; group F, S and S^n of
 // the row that is finished in this iteration.  They bypass L1 and cost the other threads no instruction.
 constexpr int XY_RING = 9;       // rho, vx, vy, vz, Bx, By, Bz, p (cell centred), b_x on the lower x-face
-constexpr int XY_PFA = 10;       // arriving row: U 5, bx (NT + 2 faces in rows 5-6), by upper 7, bz 8, bz upper 9
+constexpr int XY_PFA = 10;       // arriving row: U 5, (rows 5, 6: carried y flux, see fpy), by upper 7, bz 8, bz upper 9
 constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
 constexpr int XY_DOUBLES_PER_THREAD = 3 * XY_RING + XY_PFA + XY_PFF + 7;
-constexpr int XY_SMEM_EXTRA = 16;   // two mbarriers behind the arrays
+constexpr int XY_BXROW_PAD = 2;     // the b_x row of the arriving row holds NT + 2 faces (thread t reads faces t, t + 1)
+constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 16; }   // b_x row + two mbarriers behind the arrays
 
 template <int LIM, bool TWO_D, bool WRAP, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT)
@@ -482,7 +483,13 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     double *pfa = ring + 3 * XY_RING * NT;        // [XY_PFA][NT]
     double *pff = pfa + XY_PFA * NT;              // [XY_PFF][NT]
     double *sQ = pff + XY_PFF * NT;               // [7][NT]: q^L along x, then the x fluxes
-    unsigned long long *bars = reinterpret_cast<unsigned long long *>(sQ + 7 * NT);   // [2]: group A, group F
+    double *bxrow = sQ + 7 * NT;                  // [NT + 2]: b_x faces of the arriving row
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(bxrow + NT + XY_BXROW_PAD);   // [2]: group A, group F
+    // The previous y flux is needed again only when its row is finished, a whole iteration later: its
+    // first components wait in otherwise unused shared-memory rows instead of registers (which would
+    // be spilled to local memory): pfa rows 5 and 6, and in 3D the sQ rows 5 and 6 that only 2D uses.
+    constexpr int NFPS = TWO_D ? 2 : 4;
+    double *const fpy[4] = { pfa + 5 * NT + t, pfa + 6 * NT + t, sQ + 5 * NT + t, sQ + 6 * NT + t };
     const int nx = g.n[0];
     const int i = WRAP ? t : (int)blockIdx.x * (NT - 4) - 2 + t;
     const bool valid = WRAP || i < nx + 2;
@@ -511,7 +518,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         mbar_expect_tx(bars, (TWO_D ? 8 : 9) * ROWB + 16);
 #pragma unroll
         for (int v = 0; v < 5; v++) tma_bulk_g2s(pfa + v * NT, Sin + v * sa + cr, ROWB, bars);
-        tma_bulk_g2s(pfa + 5 * NT, bx + cr, ROWB + 16, bars);         // NT + 2 faces: thread t also reads face t + 1
+        tma_bulk_g2s(bxrow, bx + cr, ROWB + 16, bars);                // NT + 2 faces: thread t also reads face t + 1
         tma_bulk_g2s(pfa + 7 * NT, by + cr + st, ROWB, bars);
         tma_bulk_g2s(pfa + 8 * NT, bz + cr, ROWB, bars);
         if (!TWO_D) tma_bulk_g2s(pfa + 9 * NT, bz + cr + stz, ROWB, bars);
@@ -576,7 +583,8 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         for (int v = 0; v < 8; v++) { rb[v * NT] = qb[v]; rc[v * NT] = qc[v]; }
         rb[8 * NT] = f1; rc[8 * NT] = f2;
     }
-    double Fpy[6] = { 0, 0, 0, 0, 0, 0 };            // previous y-face: rho, m_y, m_z, m_x, E, (B_z in 2D)
+    double Fpy[6] = { 0, 0, 0, 0, 0, 0 };            // previous y-face: rho, m_y, m_z, m_x, E, (B_z in 2D);
+                                                     // components < NFPS live in shared memory (fpy)
     // ring rows s-1, s, s+1 (own column; neighbours at +-1): the three slots rotate every iteration
     double *rm = ring + t, *r0 = ring + XY_RING * NT + t, *rn = ring + 2 * XY_RING * NT + t;
     const int dl = tl - t, dr = tr - t;
@@ -590,11 +598,11 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             bool bad = false;
             double bxf = 0.0;
             if (valid) {
-                double B0 = 0.5 * (pfa[5 * NT + t] + pfa[5 * NT + t + 1]);
+                double B0 = 0.5 * (bxrow[t] + bxrow[t + 1]);
                 byu = pfa[7 * NT + t];
                 double B1 = 0.5 * (bnext + byu);
                 double B2 = TWO_D ? pfa[8 * NT + t] : 0.5 * (pfa[8 * NT + t] + pfa[9 * NT + t]);
-                bxf = pfa[5 * NT + t];
+                bxf = bxrow[t];
                 to_prim(pfa[t], pfa[NT + t], pfa[2 * NT + t], pfa[3 * NT + t], pfa[4 * NT + t], B0, B1, B2, q1, bad);
                 if (cell && s + 1 < s1) anybad |= bad;
             } else {
@@ -705,6 +713,8 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                 r4v = 0.5 * (pff[9 * NT + t] + r4v);
             }
             // y-rotated flux: (rho, m_y, m_z, m_x, B_z, B_x, E)
+#pragma unroll
+            for (int n = 0; n < NFPS; n++) Fpy[n] = *fpy[n];
             Sout[cm] = r0v - facy * (Fy[0] - Fpy[0]);
             Sout[2 * sa + cm] = r2v - facy * (Fy[1] - Fpy[1]);
             Sout[3 * sa + cm] = r3v - facy * (Fy[2] - Fpy[2]);
@@ -726,7 +736,11 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                 ct[(CT_W + 1) * sa + c + xdup] = wy;
             }
         }
-        Fpy[0] = Fy[0]; Fpy[1] = Fy[1]; Fpy[2] = Fy[2]; Fpy[3] = Fy[3]; Fpy[4] = Fy[6]; Fpy[5] = Fy[4];
+        {
+            const double nf[6] = { Fy[0], Fy[1], Fy[2], Fy[3], Fy[6], Fy[4] };
+#pragma unroll
+            for (int n = 0; n < 6; n++) { if (n < NFPS) *fpy[n] = nf[n]; else Fpy[n] = nf[n]; }
+        }
         bface = bnext; bnext = byu;
         double *rt = rm; rm = r0; r0 = rn; rn = rt;
     }

@@ -208,7 +208,7 @@ void launch_sweeps(const double *Sin, double *Sout, bool combine)
         const int chunks = wrap ? 1 : (nx + nt - 5) / (nt - 4);
         const int len = march_seglen(g.n[1], (long long)nx * g.n[2]);
         dim3 grid(chunks, (g.n[1] + len - 1) / len, g.n[2]);
-        const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA;
+        const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
         void (*k)(Grid, const double *, double *, double *, StepParams *, int, int) =
             wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
                     : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
