@@ -47,6 +47,7 @@ class Oracle:
         L.oracle_get_dt.restype = C.c_double
         L.oracle_get_time.restype = C.c_double
         L.oracle_set_threads.argtypes = [C.c_int]
+        L.oracle_set_integrator.argtypes = [C.c_int]
         L.oracle_cons2prim.argtypes = [_dp, C.c_double, _dp]
         L.oracle_prim2cons.argtypes = [_dp, C.c_double, _dp]
         L.oracle_prim2cons.restype = None
@@ -107,6 +108,9 @@ class Oracle:
 
     def get_threads(self):
         return self.L.oracle_get_threads()
+
+    def set_integrator(self, order):
+        return self.L.oracle_set_integrator(order)
 
     def finalize(self):
         return self.L.oracle_finalize()

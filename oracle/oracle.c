@@ -44,6 +44,7 @@ typedef struct {
     double *V, *F, *W, *Eg, *Ec;
     double time, dt_last;
     int stepped;
+    int rk_order;          /* 2 (or 0: default) = SSP-RK2, 3 = SSP-RK3 */
     int err;
     int threads;
 } ctx_t;
@@ -594,6 +595,34 @@ static void one_step(double dt)
 {
     const size_t N = g.N;
     long c; int d;
+    if (g.rk_order == 3) {
+        /* Eq. 5, SSP-RK3 in Shu-Osher form; reading R17: the last stage carries 2 L**
+           (as printed, "+ L**", the weights of L do not sum to one):
+             U*  = U^n + L^n ;  U** = (3 U^n + U* + L*) / 4 ;  U^{n+1} = (U^n + 2 (U** + L**)) / 3 */
+        euler(g.U, g.b, dt, g.U1, g.b1);                 /* U1 = U*            */
+        euler(g.U1, g.b1, dt, g.U2, g.b2);               /* U2 = U* + L*       */
+#pragma omp parallel for
+        for (c = 0; c < (long)(8 * N); c++) g.U2[c] = (3.0 * g.U[c] + g.U2[c]) / 4.0;
+        for (d = 0; d < 3; d++) {
+            if (!g.act[d]) continue;
+#pragma omp parallel for
+            for (c = 0; c < (long)N; c++) g.b2[d][c] = (3.0 * g.b[d][c] + g.b2[d][c]) / 4.0;
+        }
+        cell_b_from_faces(g.U2, g.b2);                   /* U2 = U**           */
+        euler(g.U2, g.b2, dt, g.U1, g.b1);               /* U1 = U** + L**     */
+#pragma omp parallel for
+        for (c = 0; c < (long)(8 * N); c++) g.U[c] = (g.U[c] + 2.0 * g.U1[c]) / 3.0;
+        for (d = 0; d < 3; d++) {
+            if (!g.act[d]) continue;
+#pragma omp parallel for
+            for (c = 0; c < (long)N; c++) g.b[d][c] = (g.b[d][c] + 2.0 * g.b1[d][c]) / 3.0;
+        }
+        cell_b_from_faces(g.U, g.b);
+        g.time += dt;
+        g.dt_last = dt;
+        g.stepped = 1;
+        return;
+    }
     /* R3: U* = U^n + L^n ; U^{n+1} = (U^n + U* + L*) / 2, same dt in both stages */
     euler(g.U, g.b, dt, g.U1, g.b1);
     euler(g.U1, g.b1, dt, g.U2, g.b2);
@@ -608,6 +637,14 @@ static void one_step(double dt)
     g.time += dt;
     g.dt_last = dt;
     g.stepped = 1;
+}
+
+/* time integrator: 2 = SSP-RK2 (north_star, default), 3 = SSP-RK3 of Eq. 5 */
+int oracle_set_integrator(int order)
+{
+    if (order != 2 && order != 3) return ORACLE_EINVAL;
+    g.rk_order = order;
+    return ORACLE_OK;
 }
 
 int oracle_step(int nsteps)

@@ -38,6 +38,7 @@ double oracle_get_dt(void);
 double oracle_get_time(void);
 int    oracle_get_state(double *U, double *Bface);
 int    oracle_finalize(void);
+int    oracle_set_integrator(int order); /* after oracle_init: 2 = SSP-RK2 (default, R3), 3 = SSP-RK3 of Eq. 5 (R17) */
 int    oracle_set_threads(int n);      /* OpenMP threads (results do not depend on it) */
 int    oracle_get_threads(void);
 

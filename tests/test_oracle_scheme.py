@@ -362,3 +362,44 @@ def test_hydro_shock_tube_converges_to_exact_riemann_solution(oracle):
     # Toro's tabulated star values for Sod's problem (Riemann Solvers..., Table 4.2): p* = 0.30313, u* = 0.92745
     assert abs(ps - 0.30313) < 1e-5 and abs(us - 0.92745) < 1e-5
     assert e2 < 0.65 * e1 and e2 < 5e-3, (e1, e2)      # ~first order in L1 at discontinuities
+
+
+# --------------------------------------------------------------------------- SSP-RK3 (Eq. 5; R17)
+
+def _rk_state(oracle, w, order, n, T):
+    oracle.load(w)
+    assert oracle.set_integrator(order) == 0
+    assert oracle.step_fixed_dt(n, T / n) == 0
+    return oracle.get_state()[0].copy()
+
+
+def test_rk3_is_third_order_in_time(oracle):
+    """On a fixed mesh the error against a tiny-dt run falls by ~8x per halving of dt (RK2: 4x).  A wrong
+    stage weight (e.g. the '+ L**' of the extracted Eq. 5 instead of '+ 2 L**') is inconsistent: no decay."""
+    w = wl.random_smooth(24, 16, 1, seed=3, limiter=1, amp=0.2)
+    T = 0.04
+    err = {}
+    for order in (2, 3):
+        ref = _rk_state(oracle, w, order, 512, T)
+        err[order] = [np.abs(_rk_state(oracle, w, order, n, T) - ref).max() for n in (2, 4, 8)]
+    o2 = [math.log2(err[2][i] / err[2][i + 1]) for i in range(2)]
+    o3 = [math.log2(err[3][i] / err[3][i + 1]) for i in range(2)]
+    assert all(1.7 <= x <= 2.3 for x in o2), o2
+    assert all(x >= 2.7 for x in o3), o3
+    assert err[3][2] < 0.2 * err[2][2]
+    oracle.set_integrator(2)
+
+
+def test_rk3_conserves_and_keeps_divb(oracle):
+    w = wl.blast_3d(12)
+    oracle.load(w)
+    oracle.set_integrator(3)
+    assert oracle.step(10) == 0
+    U, Bf = oracle.get_state()
+    for v in (0, 7):
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * abs(math.fsum(w.U[v].ravel()))
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    div = ((f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) + (f["by"][:, 1:, :] - f["by"][:, :-1, :])
+           + (f["bz"][1:, :, :] - f["bz"][:-1, :, :]))
+    assert np.abs(div).max() <= 1e-12 * np.abs(Bf).max()
+    oracle.set_integrator(2)
