@@ -104,7 +104,8 @@ double pluto_probe_fp64_gflops(void);
 enum {
     PLUTO_OPT_GRAPH = 1,   /* 1 (default): replay one captured CUDA graph per step; 0: plain launches */
     PLUTO_OPT_FUSE_XY = 2, /* 1 (default): x and y sweeps fused in one kernel; 0: one kernel per direction */
-    PLUTO_OPT_CT_TMA = 3   /* 1 (default): CT operands staged by TMA (cp.async.bulk.tensor); 0: per-thread loads */
+    PLUTO_OPT_CT_TMA = 3,  /* 1 (default): CT operands staged by TMA (cp.async.bulk.tensor); 0: per-thread loads */
+    PLUTO_OPT_RK_ORDER = 4 /* 2 (default): SSP-RK2 (north star, reading R3); 3: SSP-RK3 of Eq. 5 (R17) */
 };
 int    pluto_set_option(int opt, int value);
 

@@ -21,6 +21,7 @@ MINMOD, MC = 0, 1
 OPT_GRAPH = 1
 OPT_FUSE_XY = 2
 OPT_CT_TMA = 3
+OPT_RK_ORDER = 4
 
 # every symbol include/pluto.h declares
 SYMBOLS = [
@@ -173,6 +174,13 @@ class Pluto:
 
     def set_option(self, opt, value):
         return self.L.pluto_set_option(opt, value)
+
+    def set_integrator(self, order):
+        """2: SSP-RK2 (default), 3: SSP-RK3 of Eq. 5; returns the previous order"""
+        old = self.L.pluto_set_option(OPT_RK_ORDER, order)
+        if old < 0:
+            raise PlutoError(old, self.L.pluto_last_error().decode())
+        return old
 
     def profile(self, on):
         return self._check(self.L.pluto_profile(1 if on else 0))

@@ -54,7 +54,7 @@ template <bool COMBINE, bool TWO_D>
 __global__ void __launch_bounds__(CT_TX * CT_TY, 3)
 k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restrict__ ct,
          const double *__restrict__ bin, double *bout, const StepParams *__restrict__ P, int seglen,
-         double *__restrict__ dbg)
+         double *__restrict__ dbg, Combine cb)
 {
     extern __shared__ __align__(128) unsigned char ctm_raw[];
     double *vals = reinterpret_cast<double *>(ctm_raw);                    // [2][CT_COUNT][CTM_TILE]
@@ -120,10 +120,10 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
         const long long c = (long long)zc(k0) * st2 + oc;
         if (TWO_D) {
             pbx = bin[c]; pby = bin[sa + c];
-            if (COMBINE) { qbx = bout[c]; qby = bout[sa + c]; }
+            if (COMBINE) { qbx = cb.Sn[c]; qby = cb.Sn[sa + c]; }
         } else {
             pbz = bin[2 * sa + c];
-            if (COMBINE) qbz = bout[2 * sa + c];
+            if (COMBINE) qbz = cb.Sn[2 * sa + c];
         }
     }
     const int so = (ty + 1) * CTM_COLS + tx + 1 + shift;                   // own position in a tile
@@ -164,32 +164,32 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
             if (TWO_D) {
                 const double bxn = pbx - dtdy * (ezy - ez);
                 const double byn = pby + dtdx * (ezx - ez);
-                const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                 bout[c] = bxo;
                 if (i == 0) bout[c + g.n[0]] = bxo;       // periodic copy: x-face n0 is face 0
-                bout[sa + c] = COMBINE ? 0.5 * (qby + byn) : byn;
+                bout[sa + c] = COMBINE ? fma(cb.wn, qby, cb.ws * byn) : byn;
                 if (dbg) { dbg[c] = 0.0; dbg[sa + c] = 0.0; dbg[2 * sa + c] = ez; }
             } else {
                 if (k > k0) {                    // b_x, b_y of plane k-1
                     const long long cm = (long long)zc(k - 1) * st2 + oc;
                     const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
                     const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
-                    const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                     bout[cm] = bxo;
                     if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
-                    bout[sa + cm] = COMBINE ? 0.5 * (qby + byn) : byn;
+                    bout[sa + cm] = COMBINE ? fma(cb.wn, qby, cb.ws * byn) : byn;
                 }
                 if (k < k1) {                    // b_z on the lower face of plane k
                     const double eyx = e[2 * CT_TX * CT_TY + 1], exy = e[CT_TX * CT_TY + CT_TX];
                     const double bzn = pbz - (dtdx * (eyx - eyN) - dtdy * (exy - exN));
-                    bout[2 * sa + c] = COMBINE ? 0.5 * (qbz + bzn) : bzn;
+                    bout[2 * sa + c] = COMBINE ? fma(cb.wn, qbz, cb.ws * bzn) : bzn;
                     if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
                     // operands of the next iteration: b_x, b_y of this plane, b_z of the next
                     pbx = bin[c]; pby = bin[sa + c];
-                    if (COMBINE) { qbx = bout[c]; qby = bout[sa + c]; }
+                    if (COMBINE) { qbx = cb.Sn[c]; qby = cb.Sn[sa + c]; }
                     if (k + 1 < k1) {
                         pbz = bin[2 * sa + c + st2];
-                        if (COMBINE) qbz = bout[2 * sa + c + st2];
+                        if (COMBINE) qbz = cb.Sn[2 * sa + c + st2];
                     }
                 }
                 dEzx = ezx - ez; dEzy = ezy - ez;

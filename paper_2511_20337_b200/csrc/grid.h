@@ -76,8 +76,9 @@ enum StateVar { S_RHO = 0, S_MX = 1, S_MY = 2, S_MZ = 3, S_EN = 4, S_B = 5, S_CO
 enum ArrayId {
     A_SA = 0,        // 8: state S^n (and S^{n+1})
     A_SB = 8,        // 8: stage state S^1
-    A_CT = 16,       // 12: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3); staging outside a step
-    A_COUNT = 28
+    A_SC = 16,       // 8: stage state S^2 (SSP-RK3 only)
+    A_CT = 24,       // 12: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3); staging outside a step
+    A_COUNT = 36
 };
 
 } // namespace pluto

@@ -16,6 +16,11 @@ namespace pluto {
 
 struct Box { int lo[3], hi[3]; };   // inclusive lo, exclusive hi
 
+// Runge-Kutta stage combine (a7): the stage writes  wn * S^n + ws * (S + L(S)).  Sn == nullptr: the plain
+// Euler stage S + L(S).  SSP-RK2 (R3): (1/2, 1/2).  SSP-RK3 (Eq. 5): (3/4, 1/4), (1/3, 2/3).
+// Sn may be the array the stage writes (each value is read before it is overwritten by the same thread).
+struct Combine { const double *Sn; double wn, ws; };
+
 __device__ __forceinline__ bool thread_zone(const Box &b, int &i, int &j, int &k)
 {
     i = b.lo[0] + blockIdx.x * blockDim.x + threadIdx.x;
@@ -168,7 +173,7 @@ constexpr int SX_OUT = SX_NT - 4;
 
 template <int LIM, bool TWO_D>
 __global__ void __launch_bounds__(SX_NT, 4)
-k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P, int combine)
+k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P, Combine cb)
 {
     __shared__ double sP[8][SX_NT];     // primitives; rows 0..5 are reused for the fluxes
     __shared__ double sQ[7][SX_NT];     // q^L = q + slope/2 of each cell
@@ -193,9 +198,10 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
         En = Sin[4 * sa + c];
         bxf = Sin[S_B * sa + c];
         cell_b<TWO_D>(g, Sin + S_B * sa, c, Bc);
-        if (combine && f >= 0 && f < nx) {     // issued with the other loads: one memory round trip per block
-            o0 = Sout[c]; o1 = Sout[sa + c]; o2 = Sout[2 * sa + c]; o3 = Sout[3 * sa + c]; o4 = Sout[4 * sa + c];
-            if (TWO_D) o7 = Sout[7 * sa + c];
+        if (cb.Sn && f >= 0 && f < nx) {       // issued with the other loads: one memory round trip per block
+            const double *Sn = cb.Sn;
+            o0 = Sn[c]; o1 = Sn[sa + c]; o2 = Sn[2 * sa + c]; o3 = Sn[3 * sa + c]; o4 = Sn[4 * sa + c];
+            if (TWO_D) o7 = Sn[7 * sa + c];
         }
         double ir = rcp_fast(rho);
         q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = Bc[1]; q[5] = Bc[2];
@@ -240,14 +246,14 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
         double r2 = my - dtdx * (sP[2][t + 1] - F[2]);
         double r3 = mz - dtdx * (sP[3][t + 1] - F[3]);
         double r4 = En - dtdx * (sP[4][t + 1] - F[6]);
-        if (combine) {
-            r0 = 0.5 * (o0 + r0); r1 = 0.5 * (o1 + r1); r2 = 0.5 * (o2 + r2);
-            r3 = 0.5 * (o3 + r3); r4 = 0.5 * (o4 + r4);
+        if (cb.Sn) {
+            r0 = fma(cb.wn, o0, cb.ws * r0); r1 = fma(cb.wn, o1, cb.ws * r1); r2 = fma(cb.wn, o2, cb.ws * r2);
+            r3 = fma(cb.wn, o3, cb.ws * r3); r4 = fma(cb.wn, o4, cb.ws * r4);
         }
         Sout[c] = r0; Sout[sa + c] = r1; Sout[2 * sa + c] = r2; Sout[3 * sa + c] = r3; Sout[4 * sa + c] = r4;
         if (TWO_D) {   // B_z has no faces in 2D: cell centred, flux updated
             double r7 = Bc[2] - dtdx * (sP[5][t + 1] - F[5]);
-            Sout[7 * sa + c] = combine ? 0.5 * (o7 + r7) : r7;
+            Sout[7 * sa + c] = cb.Sn ? fma(cb.wn, o7, cb.ws * r7) : r7;
         }
         // cell-centred EMF  E^c = -(v x B)
         const double e0 = q[3] * q[4] - q[2] * q[5], e1 = q[1] * q[5] - q[3] * Bc[0], e2 = q[2] * Bc[0] - q[1] * q[4];
@@ -275,7 +281,7 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
 // keeps the running q^L, the last two primitive states (as state + difference) and the previous
 // flux in registers, so every cell is loaded and converted once and every flux is computed once per
 // segment (+1 at the segment end).  Sout already holds the x-sweep result and is updated in place:
-//     Sout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (stage 1) or 1/2 (combine stage).
+//     Sout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (Euler stage) or the combine weight ws.
 // The operands of iteration s+1 travel global -> shared by 8-byte cp.async while interface s is
 // being solved (two slots per thread, no block synchronisation: a thread only reads what it copied).
 
@@ -459,7 +465,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
 // a row are solved across the block (q^L and the fluxes are exchanged through shared memory, as in
 // k_sweep_x); the y interfaces are solved down each thread's own column from the ring (as in
 // k_sweep_march).  A cell is therefore read once and written once for both directions:
-//     S' = (S - dt/dx (Fx(+) - Fx(-))) - dt/dy (Fy(+) - Fy(-))      [combine: the RK2 average]
+//     S' = (S - dt/dx (Fx(+) - Fx(-))) - dt/dy (Fy(+) - Fy(-))      [combine: wn S^n + ws S']
 // WRAP: the block spans the whole periodic row (NT = nx), neighbours wrap inside shared memory and
 // no lane is idle.  Otherwise blocks overlap by four cells like k_sweep_x.
 // Operands travel global -> shared as whole row segments by TMA bulk copies (cp.async.bulk + mbarrier)
@@ -479,7 +485,7 @@ constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 16; }   /
 template <int LIM, bool TWO_D, bool WRAP, int NT>
 __global__ void __launch_bounds__(NT, NT == 128 ? XY128_MINB : 512 / NT)
 k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-           int combine, int seglen)
+           Combine cb, int seglen)
 {
     extern __shared__ __align__(128) double xy_smem[];
     const int t = threadIdx.x;
@@ -508,7 +514,8 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const long long sa = g.sa, st = g.st[1], stz = g.st[2];
     const double gamma = g.gamma;
     const double dtdx = P->dtdx[0];
-    const double facy = (combine ? 0.5 : 1.0) * P->dtdx[1];
+    const bool combine = cb.Sn != nullptr;
+    const double facy = (combine ? cb.ws : 1.0) * P->dtdx[1];
     const double *__restrict__ bx = Sin + S_B * sa;
     const double *__restrict__ by = Sin + (S_B + 1) * sa;
     const double *__restrict__ bz = Sin + (S_B + 2) * sa;
@@ -533,8 +540,8 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + v * NT, Sin + v * sa + cf, ROWB, bars + 1);
         if (combine) {
 #pragma unroll
-            for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + (5 + v) * NT, Sout + v * sa + cf, ROWB, bars + 1);
-            if (TWO_D) tma_bulk_g2s(pff + 10 * NT, Sout + 7 * sa + cf, ROWB, bars + 1);
+            for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + (5 + v) * NT, cb.Sn + v * sa + cf, ROWB, bars + 1);
+            if (TWO_D) tma_bulk_g2s(pff + 10 * NT, cb.Sn + 7 * sa + cf, ROWB, bars + 1);
         }
     };
     if (t == 0) {
@@ -712,9 +719,9 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             const long long cm = c - st;
             double r0v = pff[t], r1v = pff[NT + t], r2v = pff[2 * NT + t], r3v = pff[3 * NT + t], r4v = pff[4 * NT + t];
             if (combine) {
-                r0v = 0.5 * (pff[5 * NT + t] + r0v); r1v = 0.5 * (pff[6 * NT + t] + r1v);
-                r2v = 0.5 * (pff[7 * NT + t] + r2v); r3v = 0.5 * (pff[8 * NT + t] + r3v);
-                r4v = 0.5 * (pff[9 * NT + t] + r4v);
+                r0v = fma(cb.wn, pff[5 * NT + t], cb.ws * r0v); r1v = fma(cb.wn, pff[6 * NT + t], cb.ws * r1v);
+                r2v = fma(cb.wn, pff[7 * NT + t], cb.ws * r2v); r3v = fma(cb.wn, pff[8 * NT + t], cb.ws * r3v);
+                r4v = fma(cb.wn, pff[9 * NT + t], cb.ws * r4v);
             }
             // y-rotated flux: (rho, m_y, m_z, m_x, B_z, B_x, E)
 #pragma unroll
@@ -726,7 +733,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             Sout[4 * sa + cm] = r4v - facy * (Fy[6] - Fpy[4]);
             if (TWO_D) {
                 double r7v = sQ[6 * NT + t];
-                if (combine) r7v = 0.5 * (pff[10 * NT + t] + r7v);
+                if (combine) r7v = fma(cb.wn, pff[10 * NT + t], cb.ws * r7v);
                 Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
             }
         }
@@ -802,7 +809,7 @@ __device__ __forceinline__ void prefetch_l1(const void *p)
 template <bool COMBINE, bool TWO_D>
 __global__ void __launch_bounds__(CT_TX * CT_TY, CT_MINB)
 k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, double *bout,
-     const StepParams *__restrict__ P, int seglen, double *__restrict__ dbg)
+     const StepParams *__restrict__ P, int seglen, double *__restrict__ dbg, Combine cb)
 {
     __shared__ double sE[2][3][CT_TY][CT_TX];
     const int tx = threadIdx.x, ty = threadIdx.y;
@@ -841,10 +848,10 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
         const long long c = plane(k0) + oc;
         if (TWO_D) {
             pbx = bin[c]; pby = bin[sa + c];
-            if (COMBINE) { qbx = bout[c]; qby = bout[sa + c]; }
+            if (COMBINE) { qbx = cb.Sn[c]; qby = cb.Sn[sa + c]; }
         } else {
             pbz = bin[2 * sa + c];
-            if (COMBINE) qbz = bout[2 * sa + c];
+            if (COMBINE) qbz = cb.Sn[2 * sa + c];
         }
     }
     if (!TWO_D && CT_PF_DIST == 2 && k0 + 1 <= k1) {
@@ -887,32 +894,32 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
             if (TWO_D) {
                 const double bxn = pbx - dtdy * (ezy - ez);
                 const double byn = pby + dtdx * (ezx - ez);
-                const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                 bout[c] = bxo;
                 if (i == 0) bout[c + g.n[0]] = bxo;       // periodic copy: x-face n0 is face 0
-                bout[sa + c] = COMBINE ? 0.5 * (qby + byn) : byn;
+                bout[sa + c] = COMBINE ? fma(cb.wn, qby, cb.ws * byn) : byn;
                 if (dbg) { dbg[c] = 0.0; dbg[sa + c] = 0.0; dbg[2 * sa + c] = ez; }
             } else {
                 if (k > k0) {                                 // b_x, b_y of plane k-1
                     const long long cm = plane(k - 1) + oc;
                     const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
                     const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
-                    const double bxo = COMBINE ? 0.5 * (qbx + bxn) : bxn;
+                    const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                     bout[cm] = bxo;
                     if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
-                    bout[sa + cm] = COMBINE ? 0.5 * (qby + byn) : byn;
+                    bout[sa + cm] = COMBINE ? fma(cb.wn, qby, cb.ws * byn) : byn;
                 }
                 if (k < k1) {                                 // b_z on the lower face of plane k
                     const double eyx = sE[buf][2][ty][tx + 1], exy = sE[buf][1][ty + 1][tx];
                     const double bzn = pbz - (dtdx * (eyx - eyN) - dtdy * (exy - exN));
-                    bout[2 * sa + c] = COMBINE ? 0.5 * (qbz + bzn) : bzn;
+                    bout[2 * sa + c] = COMBINE ? fma(cb.wn, qbz, cb.ws * bzn) : bzn;
                     if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
                     // operands of the next iteration: b_x, b_y of this plane, b_z of the next
                     pbx = bin[c]; pby = bin[sa + c];
-                    if (COMBINE) { qbx = bout[c]; qby = bout[sa + c]; }
+                    if (COMBINE) { qbx = cb.Sn[c]; qby = cb.Sn[sa + c]; }
                     if (k + 1 < k1) {
                         pbz = bin[2 * sa + c + st2];
-                        if (COMBINE) qbz = bout[2 * sa + c + st2];
+                        if (COMBINE) qbz = cb.Sn[2 * sa + c + st2];
                     }
                 }
                 dEzx = ezx - ez; dEzy = ezy - ez;

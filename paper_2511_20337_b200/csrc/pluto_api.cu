@@ -42,8 +42,9 @@ struct Context {
     int use_graph = 1;
     int fuse_xy = 1;
     int ct_tma = 1;
+    int rk_order = 2;                // 2: SSP-RK2 (R3), 3: SSP-RK3 (Eq. 5)
     CUtensorMap ct_map{};            // the twelve CT arrays as one 4D tensor (x, y, z, array)
-    cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step
+    cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step (of the current rk_order)
     int sm_count = 148;
     char err[512] = "";
     // per-kernel CUDA-event timing (pluto_profile)
@@ -192,12 +193,12 @@ int march_seglen(int n, long long columns)
 }
 
 template <int LIM, bool TWO_D>
-void launch_sweeps(const double *Sin, double *Sout, bool combine)
+void launch_sweeps(const double *Sin, double *Sout, Combine cb)
 {
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
     double *ct = arr(A_CT);
-    const double scale = combine ? 0.5 : 1.0;
+    const double scale = cb.Sn ? cb.ws : 1.0;
     if (C.fuse_xy) {
         // fused x + y sweep: one block per x-row chunk and y-segment.  The block width is a template
         // parameter (shared-memory offsets become immediates): a whole periodic row when nx is one of
@@ -209,16 +210,16 @@ void launch_sweeps(const double *Sin, double *Sout, bool combine)
         const int len = march_seglen(g.n[1], (long long)nx * g.n[2]);
         dim3 grid(chunks, (g.n[1] + len - 1) / len, g.n[2]);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
-        void (*k)(Grid, const double *, double *, double *, StepParams *, int, int) =
+        void (*k)(Grid, const double *, double *, double *, StepParams *, Combine, int) =
             wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
                     : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
                  : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, combine ? 1 : 0, len));
+        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len));
     } else {
         const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
         LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
-                             g, Sin, Sout, ct, C.P, combine ? 1 : 0));
+                             g, Sin, Sout, ct, C.P, cb));
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
         dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
@@ -233,8 +234,9 @@ void launch_sweeps(const double *Sin, double *Sout, bool combine)
 }
 
 // CT: edge EMFs + face update (+ combine) in one kernel; dbg (debug only) receives the edge EMFs
-void launch_ct(const double *bin, double *bout, bool combine, double *dbg)
+void launch_ct(const double *bin, double *bout, Combine cb, double *dbg)
 {
+    const bool combine = cb.Sn != nullptr;
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
     const int tiles_x = (g.n[0] + CT_TX - 2) / (CT_TX - 1), tiles_y = (g.n[1] + CT_TY - 2) / (CT_TY - 1);
@@ -253,35 +255,38 @@ void launch_ct(const double *bin, double *bout, bool combine, double *dbg)
             tma_attr = true;
         }
         if (g.act[2]) {
-            if (combine) LAUNCH(K_CT, k_ct_tma<true, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
-            else         LAUNCH(K_CT, k_ct_tma<false, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
+            if (combine) LAUNCH(K_CT, k_ct_tma<true, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
+            else         LAUNCH(K_CT, k_ct_tma<false, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
         } else {
-            if (combine) LAUNCH(K_CT, k_ct_tma<true, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
-            else         LAUNCH(K_CT, k_ct_tma<false, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg));
+            if (combine) LAUNCH(K_CT, k_ct_tma<true, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
+            else         LAUNCH(K_CT, k_ct_tma<false, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
         }
         return;
     }
     const size_t smem = 0;
     if (g.act[2]) {
-        if (combine) LAUNCH(K_CT, k_ct<true, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
-        else         LAUNCH(K_CT, k_ct<false, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        if (combine) LAUNCH(K_CT, k_ct<true, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg, cb));
+        else         LAUNCH(K_CT, k_ct<false, false><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg, cb));
     } else {
-        if (combine) LAUNCH(K_CT, k_ct<true, true><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
-        else         LAUNCH(K_CT, k_ct<false, true><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg));
+        if (combine) LAUNCH(K_CT, k_ct<true, true><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg, cb));
+        else         LAUNCH(K_CT, k_ct<false, true><<<grid, block, smem, s>>>(g, ct, bin, bout, C.P, len, dbg, cb));
     }
 }
 
-// One Euler stage Sin -> Sout; combine: Sout <- (Sout + Euler(Sin)) / 2 in place.
-void enqueue_stage(int in, int out, bool combine, double *dbg = nullptr)
+// One Runge-Kutta stage: Sout <- Euler(Sin), or with a combine  Sout <- wn * S^n + ws * Euler(Sin)
+// (sn < 0: no combine; sn may equal out: in place).
+void enqueue_stage(int in, int out, int sn = -1, double wn = 0.0, double ws = 1.0, double *dbg = nullptr)
 {
     const Grid &g = C.g;
     fill_ghosts(arr(in));
     const bool two_d = !g.act[2];
-    if (g.limiter == 0) { if (two_d) launch_sweeps<0, true>(arr(in), arr(out), combine);
-                          else       launch_sweeps<0, false>(arr(in), arr(out), combine); }
-    else                { if (two_d) launch_sweeps<1, true>(arr(in), arr(out), combine);
-                          else       launch_sweeps<1, false>(arr(in), arr(out), combine); }
-    launch_ct(arr(in + S_B), arr(out + S_B), combine, dbg);
+    const Combine cb = { sn >= 0 ? arr(sn) : nullptr, wn, ws };
+    if (g.limiter == 0) { if (two_d) launch_sweeps<0, true>(arr(in), arr(out), cb);
+                          else       launch_sweeps<0, false>(arr(in), arr(out), cb); }
+    else                { if (two_d) launch_sweeps<1, true>(arr(in), arr(out), cb);
+                          else       launch_sweeps<1, false>(arr(in), arr(out), cb); }
+    const Combine cbf = { sn >= 0 ? arr(sn + S_B) : nullptr, wn, ws };
+    launch_ct(arr(in + S_B), arr(out + S_B), cbf, dbg);
 }
 
 void enqueue_dt(int mode)
@@ -293,8 +298,15 @@ void enqueue_dt(int mode)
 void enqueue_step(bool fixed)
 {
     enqueue_dt(fixed ? 1 : 0);
-    enqueue_stage(A_SA, A_SB, false);    // S^1 = S^n + L(S^n)
-    enqueue_stage(A_SB, A_SA, true);     // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
+    if (C.rk_order == 3) {
+        // SSP-RK3, Eq. 5 (R17: the last stage carries 2 L**)
+        enqueue_stage(A_SA, A_SB);                                  // S*   = S^n + L(S^n)
+        enqueue_stage(A_SB, A_SC, A_SA, 0.75, 0.25);                // S**  = (3 S^n + S* + L(S*)) / 4
+        enqueue_stage(A_SC, A_SA, A_SA, 1.0 / 3.0, 2.0 / 3.0);      // S^{n+1} = (S^n + 2 (S** + L(S**))) / 3
+    } else {
+        enqueue_stage(A_SA, A_SB);                                  // S^1 = S^n + L(S^n)
+        enqueue_stage(A_SB, A_SA, A_SA, 0.5, 0.5);                  // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
+    }
     LAUNCH(K_SCALAR, launch_advance_time(C.P, C.stream));
 }
 
@@ -480,6 +492,13 @@ int pluto_set_box(double Lx, double Ly, double Lz)
 int pluto_set_option(int opt, int value)
 {
     if (opt == PLUTO_OPT_GRAPH) { int old = C.use_graph; C.use_graph = value ? 1 : 0; return old; }
+    if (opt == PLUTO_OPT_RK_ORDER) {
+        if (value != 2 && value != 3) return fail(PLUTO_EINVAL, "rk order must be 2 or 3");
+        int old = C.rk_order;
+        C.rk_order = value;
+        destroy_graphs();
+        return old;
+    }
     if (opt == PLUTO_OPT_CT_TMA) {
         int old = C.ct_tma;
         C.ct_tma = value ? 1 : 0;
@@ -684,7 +703,7 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     double *dbgE = nullptr;                     // edge EMFs are never stored by the production path
     CUDA_TRY(cudaMalloc((void **)&dbgE, 3 * (size_t)g.sa * sizeof(double)));
     CUDA_TRY(cudaMemsetAsync(dbgE, 0, 3 * (size_t)g.sa * sizeof(double), s));
-    enqueue_stage(A_SA, A_SB, false, dbgE);
+    enqueue_stage(A_SA, A_SB, -1, 0.0, 1.0, dbgE);
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
     const size_t n = api_count(g, -1);

@@ -283,6 +283,37 @@ def test_ct_tma_and_per_thread_paths_agree(pluto):
         assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]), shape
 
 
+RK3_CASES = [
+    ("2d_wrap", lambda: wl.random_smooth(64, 20, 1, seed=31, limiter=1)),
+    ("2d_chunk", lambda: wl.random_smooth(150, 21, 1, seed=32, limiter=0)),
+    ("3d_wrap", lambda: wl.random_smooth(64, 12, 10, seed=33, limiter=1, box=(1.0, 0.6, 0.5))),
+    ("3d_ragged", lambda: wl.random_smooth(37, 23, 9, seed=34, limiter=0)),
+    ("blast_24", lambda: wl.blast_3d(24)),
+]
+
+
+@pytest.mark.parametrize("name,make", RK3_CASES, ids=[s[0] for s in RK3_CASES])
+def test_rk3_parity(pluto, oracle, name, make):
+    """SSP-RK3 (Eq. 5; NEXT row 1 of SURVEY 8(f)): one step max-rel, 20 steps L1-rel"""
+    w = make()
+    pluto.set_integrator(3)
+    try:
+        pluto.load(w)
+        oracle.load(w)
+        assert oracle.set_integrator(3) == 0
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(1)
+        assert oracle.step(1) == 0
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+        pluto.step(19)
+        assert oracle.step(19) == 0
+        compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+        assert abs(pluto.get_time() - oracle.get_time()) <= 1e-12
+    finally:
+        pluto.set_integrator(2)
+        oracle.set_integrator(2)
+
+
 def test_device_pointers_and_graph_equivalence(pluto, oracle):
     """set/get with CUDA tensors; graph replay and plain launches give identical bits"""
     import torch
