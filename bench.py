@@ -108,13 +108,14 @@ class ClockSampler:
                 "power_w": statistics.median(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_throughput(workload_small, steps, threads=None):
+def oracle_throughput(workload_small, steps, threads=None, rk=2):
     """the oracle as it stands, timed on the host cores (zone-updates/s)"""
     from oracle import Oracle
     o = Oracle()
     if threads:
         o.set_threads(threads)
     o.load(workload_small)
+    o.set_integrator(rk)
     o.step(1)                                   # touch memory
     t0 = time.perf_counter()
     rc = o.step(steps)
@@ -128,6 +129,8 @@ def oracle_throughput(workload_small, steps, threads=None):
 def sample_workload(cfg):
     """bounded sample of configs[cfg] for the CPU legs: the same generator at a size the oracle steps in seconds"""
     from paper_2511_20337_b200 import workloads as wl
+    if cfg == 5:
+        return wl.orszag_tang_3d(128, noise=1e-3), "orszag_tang_3d 128^3 (1/8 of the zones of the 256^3 run)"
     if cfg in (3, 4):
         return wl.blast_3d(128, name="blast_3d_128 (1/8 of the zones of configs[3])"), "blast_3d 128^3, same recipe and seed as configs[3]"
     if cfg == 2:
@@ -143,6 +146,7 @@ def run_reference(args):
     from oracle import Oracle
     o = Oracle()
     o.load(w)
+    o.set_integrator(args.rk)
     for _ in range(args.warmup):
         o.step(1)
     t0 = time.perf_counter()
@@ -169,6 +173,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours")
+    ap.add_argument("--rk", type=int, default=2, help="2: SSP-RK2 (the north_star's step, default); 3: SSP-RK3 of Eq. 5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     args = ap.parse_args()
@@ -195,6 +200,7 @@ def main():
 
     w = wl.config(args.config)
     sim = Pluto(device=local)
+    sim.set_integrator(args.rk)
     sim.load(w)
     K, W = args.steps, max(args.warmup, 3)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -265,8 +271,8 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{args.config}] {w.name}", "grid": [w.nx, w.ny, w.nz], "zones": w.zones,
-                   "scheme": "PLM(%s)+HLLD+RK2+CT, CFL %.2g" % ("minmod" if w.limiter == 0 else "MC", w.cfl),
+        "config": {"workload": (f"configs[{args.config}] {w.name}" if args.config < 5 else f"paper section 4.1 workload (not a BASELINE config) {w.name}"), "grid": [w.nx, w.ny, w.nz], "zones": w.zones,
+                   "scheme": "PLM(%s)+HLLD+RK%d+CT, CFL %.2g" % ("minmod" if w.limiter == 0 else "MC", args.rk, w.cfl),
                    "l2": "inputs larger than L2 (state %.2f GB)" % (11 * w.zones * 8 / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline,
@@ -303,7 +309,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         ws, what = sample_workload(args.config)
         steps = 4 if ws.zones > 1_000_000 else 20
-        v, cores, secs = oracle_throughput(ws, steps)
+        v, cores, secs = oracle_throughput(ws, steps, rk=args.rk)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{what}, {steps} steps, {secs:.1f} s"}
     else:

@@ -153,6 +153,39 @@ def orszag_tang_2d(n=128, nsteps=100, seed=20337, noise=1e-3, gamma=5.0 / 3.0, c
                     nsteps, U, join_faces(faces, nx, ny, nz), seed=seed)
 
 
+# --------------------------------------------------------------------------- 3D Orszag-Tang vortex (the paper's own benchmark)
+
+def orszag_tang_3d(n=64, seed=4155, noise=0.0, gamma=5.0 / 3.0, cfl=0.3, limiter=1, name=None, shape=None):
+    """The 3D Orszag-Tang vortex of PAPER.md:254-258 (section 4.1): unit periodic cube, rho = 25/9, p = 5/3,
+    v = (-zeta sin 2 pi y, zeta sin 2 pi x, 0.2 sin 2 pi z), zeta = 1 + sin(2 pi z)/5, B = (-sin 2 pi y, sin 4 pi x, 0).
+    Face B is the discrete curl of A_z = cos(2 pi y)/(2 pi) + cos(4 pi x)/(4 pi); optional seeded density noise."""
+    nx, ny, nz = (n, n, n) if shape is None else shape
+    L = (1.0, ny / nx, nz / nx)
+    dx, dy = L[0] / nx, L[1] / ny
+    x, y, z = cell_centres(nx, L[0]), cell_centres(ny, L[1]), cell_centres(nz, L[2])
+    xf, yf = face_positions(nx, L[0]), face_positions(ny, L[1])
+    two_pi = 2.0 * np.pi
+    A = np.cos(two_pi * yf[:, None]) / two_pi + np.cos(2.0 * two_pi * xf[None, :]) / (2.0 * two_pi)   # (ny+1, nx+1)
+    bx = (A[1:, :] - A[:-1, :]) / dy
+    by = -(A[:, 1:] - A[:, :-1]) / dx
+    faces = {"bx": np.broadcast_to(bx[None], (nz, ny, nx + 1)).copy(),
+             "by": np.broadcast_to(by[None], (nz, ny + 1, nx)).copy(),
+             "bz": np.zeros((nz + 1, ny, nx))}
+    shp = (nz, ny, nx)
+    X = np.broadcast_to(x[None, None, :], shp)
+    Y = np.broadcast_to(y[None, :, None], shp)
+    Z = np.broadcast_to(z[:, None, None], shp)
+    zeta = 1.0 + np.sin(two_pi * Z) / 5.0
+    v = [-zeta * np.sin(two_pi * Y), zeta * np.sin(two_pi * X), 0.2 * np.sin(two_pi * Z)]
+    rho = np.full(shp, 25.0 / 9.0)
+    if noise:
+        rho = rho * (1.0 + noise * (2.0 * counter_noise(seed, nx * ny * nz).reshape(shp) - 1.0))
+    Bc = cell_mean_of_faces(faces, nx, ny, nz, [None, None, None])
+    U = conserved_from_fields(rho, v, Bc, np.full(shp, 5.0 / 3.0), gamma)
+    return Workload(name or f"orszag_tang_3d_{nx}x{ny}x{nz}", nx, ny, nz, L, gamma, cfl, limiter, 0, U,
+                    join_faces(faces, nx, ny, nz), t_end=0.5, seed=seed)
+
+
 # --------------------------------------------------------------------------- CP Alfven wave (C1)
 
 def cp_alfven_3d(nx=64, seed=2511, noise=1e-6, gamma=5.0 / 3.0, cfl=0.4, limiter=1, amp=0.1, name=None):
@@ -306,4 +339,6 @@ def config(idx: int) -> Workload:
         return blast_3d(256, nsteps=50, name="C3_blast_3d_256")
     if idx == 4:
         return blast_3d(512, nsteps=20, name="C4_blast_3d_512")
+    if idx == 5:    # not a BASELINE.json config: the paper's own 3D Orszag-Tang benchmark (section 4.1) at 256^3
+        return orszag_tang_3d(256, noise=1e-3, name="P1_orszag_tang_3d_256")
     raise ValueError(idx)

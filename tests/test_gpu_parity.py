@@ -283,6 +283,26 @@ def test_ct_tma_and_per_thread_paths_agree(pluto):
         assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]), shape
 
 
+def test_paper_orszag_tang_3d_rk3(pluto, oracle):
+    """the paper's own benchmark problem with its integrator (RK3), PLM/MC instead of WENOZ"""
+    w = wl.orszag_tang_3d(32, noise=1e-3)
+    pluto.set_integrator(3)
+    try:
+        pluto.load(w)
+        oracle.load(w)
+        oracle.set_integrator(3)
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(1)
+        assert oracle.step(1) == 0
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+        pluto.step(29)
+        assert oracle.step(29) == 0
+        compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+    finally:
+        pluto.set_integrator(2)
+        oracle.set_integrator(2)
+
+
 RK3_CASES = [
     ("2d_wrap", lambda: wl.random_smooth(64, 20, 1, seed=31, limiter=1)),
     ("2d_chunk", lambda: wl.random_smooth(150, 21, 1, seed=32, limiter=0)),

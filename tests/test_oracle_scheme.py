@@ -403,3 +403,49 @@ def test_rk3_conserves_and_keeps_divb(oracle):
            + (f["bz"][1:, :, :] - f["bz"][:-1, :, :]))
     assert np.abs(div).max() <= 1e-12 * np.abs(Bf).max()
     oracle.set_integrator(2)
+
+
+# --------------------------------------------------------------------------- the paper's 3D Orszag-Tang benchmark
+
+def test_orszag_tang_3d_initial_state_is_the_papers(oracle):
+    """rho = 25/9, p = 5/3, v and B as printed; face B divergence-free"""
+    w = wl.orszag_tang_3d(16)
+    x = wl.cell_centres(16, 1.0)
+    X, Y, Z = x[None, None, :], x[None, :, None], x[:, None, None]
+    zeta = 1 + np.sin(2 * np.pi * Z) / 5
+    rho = w.U[0]
+    assert np.allclose(rho, 25 / 9) and w.t_end == 0.5
+    assert np.allclose(w.U[1] / rho, -zeta * np.sin(2 * np.pi * Y) + 0 * X, atol=1e-14)
+    assert np.allclose(w.U[2] / rho, zeta * np.sin(2 * np.pi * X) + 0 * Y, atol=1e-14)
+    assert np.allclose(w.U[3] / rho, 0.2 * np.sin(2 * np.pi * Z) + 0 * X + 0 * Y, atol=1e-14)
+    # cell B = mean of faces of an exactly differenced potential: the printed field up to O(dx^2)
+    assert np.abs(w.U[4] - (-np.sin(2 * np.pi * Y) + 0 * X + 0 * Z)).max() < 0.03
+    assert np.abs(w.U[5] - (np.sin(4 * np.pi * X) + 0 * Y + 0 * Z)).max() < 0.11
+    V = np.empty(8)
+    assert oracle.L.oracle_cons2prim(np.ascontiguousarray(w.U[:, 3, 5, 7]).ctypes.data_as(oracle_dp()), w.gamma,
+                                     V.ctypes.data_as(oracle_dp())) == 0
+    assert abs(V[7] - 5 / 3) < 1e-13
+    f = wl.split_faces(w.Bface, w.nx, w.ny, w.nz)
+    div = ((f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) + (f["by"][:, 1:, :] - f["by"][:, :-1, :])
+           + (f["bz"][1:, :, :] - f["bz"][:-1, :, :]))
+    assert np.abs(div).max() < 1e-14
+
+
+def oracle_dp():
+    import ctypes
+    return ctypes.POINTER(ctypes.c_double)
+
+
+def test_orszag_tang_3d_keeps_its_point_symmetry_under_rk3(oracle):
+    """q(x, y, z) <-> q(1-x, 1-y, z): odd for v_x, v_y, B_x, B_y, even for the rest; 10 RK3 steps"""
+    w = wl.orszag_tang_3d(16)
+    oracle.load(w)
+    oracle.set_integrator(3)
+    assert oracle.step(10) == 0
+    oracle.set_integrator(2)
+    U, _ = oracle.get_state()
+    for v in range(8):
+        sign = -1.0 if v in (1, 2, 4, 5) else 1.0
+        assert np.abs(U[v] - sign * U[v][:, ::-1, ::-1]).max() <= 1e-12 * max(np.abs(U[v]).max(), 1.0), v
+    for v in (0, 7):
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * abs(math.fsum(w.U[v].ravel()))
