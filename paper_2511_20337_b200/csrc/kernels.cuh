@@ -779,7 +779,7 @@ __device__ __forceinline__ double edge_emf(double Ea_lo, double Ea_hi, double Eb
 
 // Block = CT_TX x CT_TY columns marching along z over `seglen` planes.  Iteration k forms
 // E_z(i-1/2, j-1/2, k) and, from plane k and the plane k-1 values kept in registers, E_x(i, j-1/2, k-1/2)
-// and E_y(i-1/2, j, k-1/2): 12 loads of the thread's own cell (HBM; prefetched into L1 two planes
+// and E_y(i-1/2, j, k-1/2): 12 loads of the thread's own cell (HBM; prefetched into L2 one plane
 // ahead) and 13 of its x-1 / y-1 neighbours (L1 hits: the neighbour thread loads the same words).
 // The three EMFs are exchanged through shared memory (one barrier, double buffered) and the faces
 // b_z(k), b_x(k-1), b_y(k-1) are updated with  db/dt = -curl E  (COMBINE: bout <- (bout + that)/2
@@ -788,26 +788,10 @@ __device__ __forceinline__ double edge_emf(double Ea_lo, double Ea_hi, double Eb
 // the tile, so all threads run the same code and each face is written exactly once.
 constexpr int CT_TX = 32, CT_TY = 8;
 
-#ifndef CT_PF_DIST
-#define CT_PF_DIST 1
-#endif
-#ifndef CT_PF_L2
-#define CT_PF_L2 0
-#endif
-#ifndef CT_MINB
-#define CT_MINB 3
-#endif
-__device__ __forceinline__ void prefetch_l1(const void *p)
-{
-#if CT_PF_L2
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-#else
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-#endif
-}
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 template <bool COMBINE, bool TWO_D>
-__global__ void __launch_bounds__(CT_TX * CT_TY, CT_MINB)
+__global__ void __launch_bounds__(CT_TX * CT_TY, 3)
 k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, double *bout,
      const StepParams *__restrict__ P, int seglen, double *__restrict__ dbg, Combine cb)
 {
@@ -854,19 +838,13 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
             if (COMBINE) qbz = cb.Sn[2 * sa + c];
         }
     }
-    if (!TWO_D && CT_PF_DIST == 2 && k0 + 1 <= k1) {
-        const double *q = A0 + plane(k0 + 1);
-#pragma unroll
-        for (int a = 0; a < CT_COUNT; a++) prefetch_l1(q + a * sa);
-    }
-
     for (int k = k0; k <= (TWO_D ? k0 : k1); k++) {
         const int buf = k & 1;
         const double *__restrict__ v = A0 + plane(k);
-        if (!TWO_D && CT_PF_DIST > 0 && k + CT_PF_DIST <= k1) {        // own words of a later plane -> L1
-            const double *q = A0 + plane(k + CT_PF_DIST);
+        if (!TWO_D && k + 1 <= k1) {                                   // own words of the next plane -> L2
+            const double *q = A0 + plane(k + 1);
 #pragma unroll
-            for (int a = 0; a < CT_COUNT; a++) prefetch_l1(q + a * sa);
+            for (int a = 0; a < CT_COUNT; a++) prefetch_l2(q + a * sa);
         }
         auto S = [&](int a, int off) { return v[a * sa + off]; };
         const double wx = S(6, 0), wy = S(7, 0);

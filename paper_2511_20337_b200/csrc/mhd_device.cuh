@@ -28,31 +28,16 @@ __device__ __forceinline__ double rcp_fast(double x)
     return fma(y, e, y);                 // y (1 + e + e^2): error ~ e^3
 }
 
-// s = sqrt(x), returns also r = 1/sqrt(x); x > 0
-__device__ __forceinline__ void sqrt_rsqrt_fast(double x, double &s, double &r)
+// sqrt(x), x > 0: two coupled Newton steps on (g, h) -> (sqrt x, 1 / (2 sqrt x))
+__device__ __forceinline__ double sqrt_fast(double x)
 {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double g = x * y, h = 0.5 * y;       // g -> sqrt(x), h -> 1/(2 sqrt(x))
+    double g = x * y, h = 0.5 * y;
     double e = fma(-g, h, 0.5);
     g = fma(g, e, g); h = fma(h, e, h);
     e = fma(-g, h, 0.5);
-    s = fma(g, e, g);
-    r = 2.0 * fma(h, e, h);
-}
-
-__device__ __forceinline__ double sqrt_fast(double x)
-{
-    double s, r;
-    sqrt_rsqrt_fast(x, s, r);
-    return s;
-}
-
-// sqrt that tolerates x == 0 (the discriminant of the fast speed can vanish)
-__device__ __forceinline__ double sqrt_fast0(double x)
-{
-    double s = sqrt_fast(fmax(x, 1e-300));
-    return x > 0.0 ? s : 0.0;
+    return fma(g, e, g);
 }
 
 // Limited slope (R4).  The sign test dm * dp > 0 is taken on the sign bits (integer pipe) instead
@@ -172,10 +157,6 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     const double SMBx = SM * Bx;
     const double vBss = fma(vss, Byss, fma(wss, Bzss, SMBx));
 
-#ifndef HLLD_VARIANT
-#define HLLD_VARIANT 0
-#endif
-#if HLLD_VARIANT == 0
     // the side the interface lies in (test order of R5: ..., S*_L >= 0, S_M >= 0, S*_R > 0), and
     // whether it lies outside the Alfven wave of that side:  S*_L = S_M - |Bx|/rL >= 0, S*_R = S_M + |Bx|/rR <= 0
     const bool left = SM >= 0.0;
@@ -197,46 +178,6 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     double rho_f = rs, uf = SM, pf = pTs;
     double vf = outer ? vs : vss, wf = outer ? ws : wss, Byf = outer ? Bys : Byss, Bzf = outer ? Bzs : Bzss;
     double Ef = outer ? Es : Ess, vBf = outer ? vBs : vBss;
-    const double EL = 0.0, ER = 0.0;
-#elif HLLD_VARIANT == 1
-    // energy chain of both sides up to the part that needs the star state:
-    //   E*_a (S_a - S_M) = G_a + pT* S_M - Bx (v.B)*_a,   G_a = (S_a - u_a) E_a - pT_a u_a + Bx (v.B)_a
-    const double EL = fma(L.p, igm1, 0.5 * fma(L.rho, fma(L.u, L.u, fma(L.v, L.v, L.w * L.w)), B2L));
-    const double ER = fma(R.p, igm1, 0.5 * fma(R.rho, fma(R.u, R.u, fma(R.v, R.v, R.w * R.w)), B2R));
-    const double GL = fma(dL, EL, fma(Bx, fma(L.u, Bx, fma(L.v, L.By, L.w * L.Bz)), -pTL * L.u));
-    const double GR = fma(dR, ER, fma(Bx, fma(R.u, Bx, fma(R.v, R.By, R.w * R.Bz)), -pTR * R.u));
-    const double vBsL = fma(vsL, BysL, fma(wsL, BzsL, SMBx)), vBsR = fma(vsR, BysR, fma(wsR, BzsR, SMBx));
-
-    // the side the interface lies in (test order of R5: ..., S*_L >= 0, S_M >= 0, S*_R > 0)
-    const bool left = SM >= 0.0;
-    const double rf = left ? rsL : rsR, r = left ? rL : rR, vBs = left ? vBsL : vBsR;
-    const double Es = (fma(pTs, SM, left ? GL : GR) - Bx * vBs) * (left ? idSL : idSR);
-    const double sr = left ? -sig * r : sig * r;
-
-    // inside the Alfven waves: the double-star state
-    double uf = SM, pf = pTs, rho_f = rf;
-    double vf = vss, wf = wss, Byf = Byss, Bzf = Bzss, vBf = vBss, Ef = fma(sr, vBs - vBss, Es);
-    // outside the Alfven wave of that side:  S*_L = S_M - |Bx|/rL >= 0  or  S*_R = S_M + |Bx|/rR <= 0
-    if (fabs(SM) * r >= fabs(Bx)) {
-        vf = left ? vsL : vsR; wf = left ? wsL : wsR; Byf = left ? BysL : BysR; Bzf = left ? BzsL : BzsR;
-        vBf = vBs; Ef = Es;
-    }
-#else
-    const double EL = fma(L.p, igm1, 0.5 * fma(L.rho, fma(L.u, L.u, fma(L.v, L.v, L.w * L.w)), B2L));
-    const double ER = fma(R.p, igm1, 0.5 * fma(R.rho, fma(R.u, R.u, fma(R.v, R.v, R.w * R.w)), B2R));
-    const double GL = fma(dL, EL, fma(Bx, fma(L.u, Bx, fma(L.v, L.By, L.w * L.Bz)), -pTL * L.u));
-    const double GR = fma(dR, ER, fma(Bx, fma(R.u, Bx, fma(R.v, R.By, R.w * R.Bz)), -pTR * R.u));
-    const double vBsL = fma(vsL, BysL, fma(wsL, BzsL, SMBx)), vBsR = fma(vsR, BysR, fma(wsR, BzsR, SMBx));
-    const bool left = SM >= 0.0;
-    const double rf = left ? rsL : rsR, r = left ? rL : rR, vBs = left ? vBsL : vBsR;
-    const double Es = (fma(pTs, SM, left ? GL : GR) - Bx * vBs) * (left ? idSL : idSR);
-    const double sr = left ? -sig * r : sig * r;
-    const bool outer = fabs(SM) * r >= fabs(Bx);
-    double uf = SM, pf = pTs, rho_f = rf;
-    double vf = outer ? (left ? vsL : vsR) : vss, wf = outer ? (left ? wsL : wsR) : wss;
-    double Byf = outer ? (left ? BysL : BysR) : Byss, Bzf = outer ? (left ? BzsL : BzsR) : Bzss;
-    double vBf = outer ? vBs : vBss, Ef = outer ? Es : fma(sr, vBs - vBss, Es);
-#endif
     if (__builtin_expect(SL >= 0.0 || SR <= 0.0, 0)) {          // one-sided fan: the upwind physical flux (Eq. 2)
         const bool sl = SL >= 0.0;
         rho_f = sl ? L.rho : R.rho; uf = sl ? L.u : R.u; vf = sl ? L.v : R.v; wf = sl ? L.w : R.w;
