@@ -48,6 +48,8 @@ class Oracle:
         L.oracle_get_time.restype = C.c_double
         L.oracle_set_threads.argtypes = [C.c_int]
         L.oracle_set_integrator.argtypes = [C.c_int]
+        L.oracle_wenoz.argtypes = [_dp]
+        L.oracle_wenoz.restype = C.c_double
         L.oracle_cons2prim.argtypes = [_dp, C.c_double, _dp]
         L.oracle_prim2cons.argtypes = [_dp, C.c_double, _dp]
         L.oracle_prim2cons.restype = None

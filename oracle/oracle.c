@@ -123,6 +123,30 @@ double oracle_plm_slope(double dm, double dp, int limiter)
     }
 }
 
+/* WENO-Z reconstruction of [51] (Borges, Carmona, Costa & Don 2008; named at PAPER.md:100,260; reading R18):
+   value at the UPPER face of the centre cell v[2] from the five-cell stencil v[0..4].
+   Candidate third-order values q_k, smoothness indicators beta_k (Jiang-Shu), global indicator
+   tau5 = |beta_0 - beta_2|, weights alpha_k = d_k (1 + tau5 / (beta_k + eps)), d = (1/10, 6/10, 3/10),
+   eps = 1e-40, power 1.  The value at the LOWER face is the same routine on the mirrored stencil. */
+double oracle_wenoz(const double v[5])
+{
+    const double eps = 1e-40;
+    double q0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) / 6.0;
+    double q1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) / 6.0;
+    double q2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) / 6.0;
+    double a0 = v[0] - 2.0 * v[1] + v[2], b0 = v[0] - 4.0 * v[1] + 3.0 * v[2];
+    double a1 = v[1] - 2.0 * v[2] + v[3], b1 = v[1] - v[3];
+    double a2 = v[2] - 2.0 * v[3] + v[4], b2 = 3.0 * v[2] - 4.0 * v[3] + v[4];
+    double be0 = 13.0 / 12.0 * a0 * a0 + 0.25 * b0 * b0;
+    double be1 = 13.0 / 12.0 * a1 * a1 + 0.25 * b1 * b1;
+    double be2 = 13.0 / 12.0 * a2 * a2 + 0.25 * b2 * b2;
+    double tau = fabs(be0 - be2);
+    double al0 = 0.1 * (1.0 + tau / (be0 + eps));
+    double al1 = 0.6 * (1.0 + tau / (be1 + eps));
+    double al2 = 0.3 * (1.0 + tau / (be2 + eps));
+    return (al0 * q0 + al1 * q1 + al2 * q2) / (al0 + al1 + al2);
+}
+
 /* rotated-frame conserved vector (rho, mn, mt1, mt2, Bn, Bt1, Bt2, E) from V = (rho,u,v,w,By,Bz,p) */
 static void rot_cons(const double V[7], double Bn, double gamma, double U[8])
 {
@@ -299,7 +323,7 @@ int oracle_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int
     if (g.init) free_all();
     g.threads = thr;
     if (nx < 1 || ny < 1 || nz < 1 || ghost < 2) return ORACLE_EINVAL;
-    if (!(gamma > 1.0) || !(cfl > 0.0) || (limiter != 0 && limiter != 1)) return ORACLE_EINVAL;
+    if (!(gamma > 1.0) || !(cfl > 0.0) || (limiter < 0 || limiter > 2)) return ORACLE_EINVAL;
     g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
     for (d = 0; d < 3; d++) g.act[d] = g.n[d] > 1;
     /* default box (R11): Lx = 1 and cubic cells */
@@ -486,13 +510,21 @@ static void euler(const double *Uin, double *const bin[3], double dt, double *Uo
 #pragma omp parallel for
         for (c = 0; c < (long)N; c++) {
             int i, j, k, q;
-            size_t cm2, cm1, c0, cp1;
+            size_t cm3, cm2, cm1, c0, cp1, cp2;
             double VL[7], VR[7], Fr[8], w;
             c2ijk((size_t)c, &i, &j, &k);
             cm2 = shift(i, j, k, d, -2); cm1 = shift(i, j, k, d, -1);
             c0 = (size_t)c;              cp1 = shift(i, j, k, d, +1);
+            cm3 = shift(i, j, k, d, -3); cp2 = shift(i, j, k, d, +2);
             for (q = 0; q < 7; q++) {
                 const double *Q = g.V + (size_t)qv[q] * N;
+                if (g.limiter == 2) {          /* WENOZ (R18): q^L from the stencil of cell c-1, q^R from cell c mirrored */
+                    double sl[5] = { Q[cm3], Q[cm2], Q[cm1], Q[c0], Q[cp1] };
+                    double sr[5] = { Q[cp2], Q[cp1], Q[c0], Q[cm1], Q[cm2] };
+                    VL[q] = oracle_wenoz(sl);
+                    VR[q] = oracle_wenoz(sr);
+                    continue;
+                }
                 /* slope of cell c-1 and of cell c (R4) */
                 double sm = oracle_plm_slope(Q[cm1] - Q[cm2], Q[c0] - Q[cm1], g.limiter);
                 double s0 = oracle_plm_slope(Q[c0] - Q[cm1], Q[cp1] - Q[c0], g.limiter);

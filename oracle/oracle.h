@@ -52,6 +52,9 @@ void   oracle_prim2cons(const double V[8], double gamma, double U[8]);
 double oracle_fast_speed(double rho, double p, double Bn, double Bt1, double Bt2, double gamma);
 /* limited slope from the two one-sided differences (R4); limiter 0 = minmod, 1 = MC */
 double oracle_plm_slope(double dm, double dp, int limiter);
+/* WENO-Z value at the upper face of the centre cell of a five-cell stencil ([51] named at PAPER.md:100; R18);
+   reconstruction id 2 of oracle_init's `limiter` argument */
+double oracle_wenoz(const double v[5]);
 /* physical flux of Eq. 2 in the rotated frame.
    V = (rho, u, v, w, By, Bz, p), Bn normal field. F = (rho, mn, mt1, mt2, 0, Bt1, Bt2, E) */
 void   oracle_physical_flux(const double V[7], double Bn, double gamma, double F[8]);

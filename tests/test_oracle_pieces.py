@@ -1,6 +1,8 @@
 """Pins for the pieces of the oracle (CPU only).  Each test checks oracle/oracle.c against something
 other than itself: a closed form, a textbook special case, a symmetry or a jump condition, chosen so
 that a dropped term, a wrong sign or a transposed operand fails one of them (SURVEY 8(c) pin table)."""
+import math
+
 import numpy as np
 import pytest
 
@@ -286,3 +288,47 @@ def test_upwind_weight_definition(oracle):
         assert abs(w - ref) < 1e-12
         seen_mid += 0.0 < w < 1.0
     assert seen_mid > 100
+
+
+# --------------------------------------------------------------------------- WENO-Z reconstruction ([51], R18)
+
+def _wenoz(oracle, v):
+    import ctypes
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    return oracle.L.oracle_wenoz(v.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+
+
+def test_wenoz_is_exact_for_quadratic_cell_averages(oracle):
+    """every candidate stencil reproduces a parabola's face value from its cell averages, so any convex
+    combination does: value at x = 1/2 of a + b x + c x^2 with averages a + b i + c (i^2 + 1/12)"""
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        a, b, c = rng.normal(size=3)
+        avg = [a + b * i + c * (i * i + 1.0 / 12.0) for i in range(-2, 3)]
+        exact = a + 0.5 * b + 0.25 * c
+        assert abs(_wenoz(oracle, avg) - exact) <= 1e-13 * (abs(a) + abs(b) + abs(c))
+
+
+def test_wenoz_is_fifth_order_on_smooth_data(oracle):
+    errs = []
+    for h in (0.1, 0.05, 0.025):
+        av = [(-math.cos(1 + (i + 0.5) * h) + math.cos(1 + (i - 0.5) * h)) / h for i in range(-2, 3)]
+        errs.append(abs(_wenoz(oracle, av) - math.sin(1 + 0.5 * h)))
+    assert math.log2(errs[0] / errs[1]) > 4.7 and math.log2(errs[1] / errs[2]) > 4.7
+
+
+def test_wenoz_takes_the_smooth_side_of_a_jump_and_stays_bounded(oracle):
+    assert abs(_wenoz(oracle, [0, 0, 0, 1, 1])) < 1e-30          # jump right of the face: left stencil only
+    assert abs(_wenoz(oracle, [0, 0, 1, 1, 1]) - 1.0) < 1e-30    # jump left of the cell
+    rng = np.random.default_rng(6)
+    for _ in range(200):
+        lo, hi = sorted(rng.normal(size=2))
+        k = rng.integers(1, 5)
+        v = [lo] * k + [hi] * (5 - k)
+        r = _wenoz(oracle, v)
+        assert lo - 1e-12 <= r <= hi + 1e-12
+    assert _wenoz(oracle, [2.5] * 5) == pytest.approx(2.5, abs=1e-15)
+    # mirror: the lower-face value of the mirrored data
+    v = rng.normal(size=5)
+    assert _wenoz(oracle, v[::-1]) != _wenoz(oracle, v)
+    assert _wenoz(oracle, -v) == pytest.approx(-_wenoz(oracle, v), rel=1e-14)
