@@ -143,6 +143,8 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     w, what = sample_workload(args.config)
+    if args.wenoz:
+        w.limiter = 2
     from oracle import Oracle
     o = Oracle()
     o.load(w)
@@ -173,6 +175,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours")
+    ap.add_argument("--wenoz", action="store_true", help="WENO-Z reconstruction instead of the config's PLM limiter")
     ap.add_argument("--rk", type=int, default=2, help="2: SSP-RK2 (the north_star's step, default); 3: SSP-RK3 of Eq. 5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -199,6 +202,8 @@ def main():
             dist.barrier()
 
     w = wl.config(args.config)
+    if args.wenoz:
+        w.limiter = 2
     sim = Pluto(device=local)
     sim.set_integrator(args.rk)
     sim.load(w)
@@ -272,7 +277,7 @@ def main():
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": (f"configs[{args.config}] {w.name}" if args.config < 5 else f"paper section 4.1 workload (not a BASELINE config) {w.name}"), "grid": [w.nx, w.ny, w.nz], "zones": w.zones,
-                   "scheme": "PLM(%s)+HLLD+RK%d+CT, CFL %.2g" % ("minmod" if w.limiter == 0 else "MC", args.rk, w.cfl),
+                   "scheme": "recon(%s)+HLLD+RK%d+CT, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], args.rk, w.cfl),
                    "l2": "inputs larger than L2 (state %.2f GB)" % (11 * w.zones * 8 / 1e9),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline,
@@ -308,6 +313,8 @@ def main():
     # ---------------- the oracle timed beside it (rank 0, N = 1 only)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         ws, what = sample_workload(args.config)
+        if args.wenoz:
+            ws.limiter = 2
         steps = 4 if ws.zones > 1_000_000 else 20
         v, cores, secs = oracle_throughput(ws, steps, rk=args.rk)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",

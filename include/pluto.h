@@ -42,12 +42,13 @@ enum {
     PLUTO_ENOMEM = -5    /* device allocation failed or registered workspace too small */
 };
 
-enum { PLUTO_MINMOD = 0, PLUTO_MC = 1 };
+/* reconstruction: PLM with the minmod / MC limiter (R4), or WENO-Z ([51]; R18; needs ghost >= 3) */
+enum { PLUTO_MINMOD = 0, PLUTO_MC = 1, PLUTO_WENOZ = 2 };
 
 /* Create (or re-create) the context for an nx x ny x nz periodic box of cubic cells with Lx = 1
  * (override with pluto_set_box).  ny >= 2 and nx >= 2 are required (2D when nz == 1, 3D when
  * nz >= 2); every active extent must be >= ghost.  ghost >= 2 layers are kept around the padded
- * device arrays (PLM needs 2).  gamma > 1 (Gamma of Eq. 3), cfl > 0, limiter PLUTO_MINMOD|PLUTO_MC.
+ * device arrays (PLM needs 2).  gamma > 1 (Gamma of Eq. 3), cfl > 0, limiter PLUTO_MINMOD|PLUTO_MC|PLUTO_WENOZ.
  * Allocates device memory unless a large enough workspace was registered before. */
 int    pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter);
 

@@ -17,7 +17,7 @@ LIB = os.environ.get("PLUTO_B200_LIB") or os.path.join(_HERE, "libpluto_b200.so"
 _DEFAULT_LIB = os.path.join(_HERE, "libpluto_b200.so")
 
 OK, EINVAL, ESTATE, ECUDA, EPHYS, ENOMEM = 0, -1, -2, -3, -4, -5
-MINMOD, MC = 0, 1
+MINMOD, MC, WENOZ = 0, 1, 2
 OPT_GRAPH = 1
 OPT_FUSE_XY = 2
 OPT_CT_TMA = 3
@@ -203,8 +203,10 @@ class Pluto:
     def finalize(self):
         return self.L.pluto_finalize()
 
-    def load(self, w, ghost=2):
+    def load(self, w, ghost=None):
         """init + set_box + set_state from a workloads.Workload (host arrays)"""
+        if ghost is None:
+            ghost = 3 if w.limiter == WENOZ else 2
         self.init(w.nx, w.ny, w.nz, ghost, w.gamma, w.cfl, w.limiter)
         self.set_box(*w.box)
         self.set_state(w.U, w.Bface)

@@ -169,7 +169,9 @@ __device__ __forceinline__ void cell_b(const Grid &g, const double *__restrict__
 // Consecutive blocks overlap by 4 items, so no flux is computed twice inside a block and rows of any
 // length pack without a ragged tail.
 constexpr int SX_NT = 128;
-constexpr int SX_OUT = SX_NT - 4;
+// halo cells on each side of a block's output range: 2 for PLM, 3 for the five-cell WENO-Z stencil
+__host__ __device__ constexpr int sx_halo(int lim) { return lim == 2 ? 3 : 2; }
+__host__ __device__ constexpr int sx_out(int lim) { return SX_NT - 2 * sx_halo(lim); }
 
 template <int LIM, bool TWO_D>
 __global__ void __launch_bounds__(SX_NT, 4)
@@ -178,10 +180,11 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     __shared__ double sP[8][SX_NT];     // primitives; rows 0..5 are reused for the fluxes
     __shared__ double sQ[7][SX_NT];     // q^L = q + slope/2 of each cell
     const int t = threadIdx.x;
-    const int nx = g.n[0], M = nx + 4;
+    constexpr int H = sx_halo(LIM);
+    const int nx = g.n[0], M = nx + 2 * H;
     const long long sa = g.sa;
     const long long nitems = (long long)M * g.n[1] * g.n[2];
-    const long long item = (long long)blockIdx.x * SX_OUT - 2 + t;
+    const long long item = (long long)blockIdx.x * sx_out(LIM) - H + t;
     const bool valid = item >= 0 && item < nitems;
     int f = -100;
     long long c = 0;
@@ -191,7 +194,7 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     double o0 = 0, o1 = 0, o2 = 0, o3 = 0, o4 = 0, o7 = 0;   // S^n of the cell (combine stage)
     if (valid) {
         long long row = item / M;
-        f = (int)(item - row * M) - 2;
+        f = (int)(item - row * M) - H;
         int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]);
         c = g.at(f, j, k);
         rho = Sin[c]; mx = Sin[sa + c]; my = Sin[2 * sa + c]; mz = Sin[3 * sa + c];
@@ -214,20 +217,21 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     __syncthreads();
 
     // limited slopes of the own cell (needs both list neighbours, which lie in the same row)
-    const bool has_nb = valid && t >= 1 && t <= SX_NT - 2 && f >= -1 && f <= nx;
+    const bool has_nb = valid && t >= H - 1 && t <= SX_NT - H && f >= -1 && f <= nx;
     double qR[7];
     if (has_nb) {
 #pragma unroll
         for (int v = 0; v < 7; v++) {
             double hi;
-            plm_faces<LIM>(q[v], q[v] - sP[v][t - 1], sP[v][t + 1] - q[v], qR[v], hi);
+            recon_faces<LIM>(LIM == 2 ? sP[v][t - 2] : 0.0, sP[v][t - 1], q[v], sP[v][t + 1],
+                             LIM == 2 ? sP[v][t + 2] : 0.0, qR[v], hi);
             sQ[v][t] = hi;
         }
     }
     __syncthreads();
 
     // Riemann problem on the lower face of cell f (faces 0 .. nx)
-    const bool face = has_nb && t >= 2 && f >= 0;
+    const bool face = has_nb && t >= H && f >= 0;
     double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5;
     if (face) {
         Side L = { sQ[0][t - 1], sQ[1][t - 1], sQ[2][t - 1], sQ[3][t - 1], sQ[4][t - 1], sQ[5][t - 1], sQ[6][t - 1] };
@@ -239,7 +243,7 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     __syncthreads();
 
     // cell f in [0, nx): flux difference with the right neighbour's face, CT data of the own face
-    if (face && f < nx && t <= SX_NT - 3) {
+    if (face && f < nx && t <= SX_NT - H - 1) {
         const double dtdx = P->dtdx[0];
         double r0 = rho - dtdx * (sP[0][t + 1] - F[0]);
         double r1 = mx - dtdx * (sP[1][t + 1] - F[1]);
@@ -456,6 +460,102 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
         iteration(1, s + 1);
     }
     if (s <= s1) iteration(0, s);
+    if (anybad) P->err = 1;
+}
+
+// ---------------------------------------------------------------- y / z sweep with the five-cell WENO-Z stencil
+// Same marching scheme as k_sweep_march, for the reconstruction of [51] (reading R18):
+// the primitives of cells s-2 .. s+2 live in a five-slot ring in shared memory (own column), iteration s
+// reconstructs both faces of cell s, solves interface s - 1/2 with the q^L kept from cell s-1 and
+// finishes cell s-1.  First version: operands are loaded directly (no prefetch ring).
+template <int DIR, bool TWO_D>
+__global__ void __launch_bounds__(MARCH_NT, 3)
+k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
+                 double scale, int seglen)
+{
+    constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
+    constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
+    __shared__ double ring[5][7][MARCH_NT];
+    const int t = threadIdx.x;
+    const int i = blockIdx.x * blockDim.x + t;
+    if (i >= g.n[0]) return;
+    const int seg = DIR == 1 ? blockIdx.y : blockIdx.z;
+    const int tr = DIR == 1 ? blockIdx.z : blockIdx.y;
+    const int s0 = seg * seglen;
+    const int s1 = min(s0 + seglen, g.n[DIR]);
+    const long long sa = g.sa, st = g.st[DIR];
+    long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
+    const double gamma = g.gamma, igm1 = g.igm1;
+    const double fac = scale * P->dtdx[DIR];
+    const double *__restrict__ bn = Sin + (S_B + DIR) * sa;        // normal face field
+    const int xdup = ct_xdup(i, g.n[0]);
+    bool bad, anybad = false;
+    auto slot = [](int m) { return ((m % 5) + 5) % 5; };
+
+    // prologue: cells s0-3 .. s0+1; q^L of face s0 - 1/2 comes from the stencil of cell s0-1
+    double qL[7];
+    {
+        double w[5][7];
+#pragma unroll
+        for (int m = 0; m < 5; m++) {
+            load_rot<DIR, TWO_D>(g, Sin, c + (m - 3) * st, w[m], bad);
+            if (m >= 3 && s0 + m - 3 < s1) anybad |= bad;
+        }
+#pragma unroll
+        for (int v = 0; v < 7; v++) {
+            double lo;
+            recon_faces<2>(w[0][v], w[1][v], w[2][v], w[3][v], w[4][v], lo, qL[v]);
+        }
+#pragma unroll
+        for (int m = 1; m < 5; m++) {
+            const int sl = slot(s0 + m - 3);
+#pragma unroll
+            for (int v = 0; v < 7; v++) ring[sl][v][t] = w[m][v];
+        }
+    }
+    double Fp[6] = { 0, 0, 0, 0, 0, 0 };                // previous face: rho, m_n, m_t1, m_t2, E, (B_z in 2D)
+
+    for (int s = s0; s <= s1; s++, c += st) {
+        {   // cell s+2 replaces cell s-3 in the ring
+            double qa[7];
+            load_rot<DIR, TWO_D>(g, Sin, c + 2 * st, qa, bad);
+            if (s + 2 < s1) anybad |= bad;
+            const int sl = slot(s + 2);
+#pragma unroll
+            for (int v = 0; v < 7; v++) ring[sl][v][t] = qa[v];
+        }
+        const int m2 = slot(s - 2), m1 = slot(s - 1), c0 = slot(s), p1 = slot(s + 1), p2 = slot(s + 2);
+        double qR[7], qLn[7];
+#pragma unroll
+        for (int v = 0; v < 7; v++)
+            recon_faces<2>(ring[m2][v][t], ring[m1][v][t], ring[c0][v][t], ring[p1][v][t], ring[p2][v][t], qR[v], qLn[v]);
+        Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
+        Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
+        double F[7], w;
+        hlld(L, R, bn[c], gamma, igm1, F, w);
+#pragma unroll
+        for (int v = 0; v < 7; v++) qL[v] = qLn[v];
+        if (s > s0) {
+            const long long cm = c - st;                  // cell s-1
+            Sout[cm] -= fac * (F[0] - Fp[0]);
+            Sout[(1 + DIR) * sa + cm] -= fac * (F[1] - Fp[1]);
+            Sout[(1 + T1) * sa + cm] -= fac * (F[2] - Fp[2]);
+            Sout[(1 + T2) * sa + cm] -= fac * (F[3] - Fp[3]);
+            Sout[4 * sa + cm] -= fac * (F[6] - Fp[4]);
+            if (BZ2D) Sout[7 * sa + cm] -= fac * (F[4] - Fp[5]);   // F_y[B_z]
+        }
+        if (s < s1) {
+            ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
+            ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
+            ct[(CT_W + DIR) * sa + c] = w;
+            if (xdup) {
+                ct[(CT_FEM + 2 * DIR) * sa + c + xdup] = F[4];
+                ct[(CT_FEM + 2 * DIR + 1) * sa + c + xdup] = F[5];
+                ct[(CT_W + DIR) * sa + c + xdup] = w;
+            }
+        }
+        Fp[0] = F[0]; Fp[1] = F[1]; Fp[2] = F[2]; Fp[3] = F[3]; Fp[4] = F[6]; Fp[5] = F[4];
+    }
     if (anybad) P->err = 1;
 }
 

@@ -170,7 +170,7 @@ bool row_wraps(int nx) { return nx == 64 || nx == 128 || nx == 256 || nx == 512;
 void fill_ghosts(double *state, bool all = false)
 {
     const Grid &g = C.g;
-    if (!all && C.fuse_xy && row_wraps(g.n[0])) {
+    if (!all && C.fuse_xy && g.limiter != 2 && row_wraps(g.n[0])) {
         const int ngh = 2 * g.ng + 1;
         const int rows = (g.act[2] ? ngh * (g.n[1] + ngh) : 0) + g.n[2] * ngh;
         LAUNCH(K_GHOST, k_ghost_yz<<<dim3(rows, S_COUNT), 128, 0, C.stream>>>(g, state));
@@ -199,7 +199,9 @@ void launch_sweeps(const double *Sin, double *Sout, Combine cb)
     cudaStream_t s = C.stream;
     double *ct = arr(A_CT);
     const double scale = cb.Sn ? cb.ws : 1.0;
-    if (C.fuse_xy) {
+    bool fused = false;
+    if constexpr (LIM != 2) if (C.fuse_xy) {
+        fused = true;
         // fused x + y sweep: one block per x-row chunk and y-segment.  The block width is a template
         // parameter (shared-memory offsets become immediates): a whole periodic row when nx is one of
         // the instantiated widths, else chunks of 128 or 256 threads that overlap by four cells.
@@ -216,20 +218,23 @@ void launch_sweeps(const double *Sin, double *Sout, Combine cb)
                  : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len));
-    } else {
-        const long long nitems = (long long)(g.n[0] + 4) * g.n[1] * g.n[2];
-        LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + SX_OUT - 1) / SX_OUT), SX_NT, 0, s>>>(
+    }
+    if (!fused) {
+        const long long nitems = (long long)(g.n[0] + 2 * sx_halo(LIM)) * g.n[1] * g.n[2];
+        LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + sx_out(LIM) - 1) / sx_out(LIM)), SX_NT, 0, s>>>(
                              g, Sin, Sout, ct, C.P, cb));
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
         dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
-        LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
     if (!TWO_D) {
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[2], (long long)g.n[0] * g.n[1]);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
-        LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        else LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
 }
 
@@ -281,10 +286,12 @@ void enqueue_stage(int in, int out, int sn = -1, double wn = 0.0, double ws = 1.
     fill_ghosts(arr(in));
     const bool two_d = !g.act[2];
     const Combine cb = { sn >= 0 ? arr(sn) : nullptr, wn, ws };
-    if (g.limiter == 0) { if (two_d) launch_sweeps<0, true>(arr(in), arr(out), cb);
-                          else       launch_sweeps<0, false>(arr(in), arr(out), cb); }
-    else                { if (two_d) launch_sweeps<1, true>(arr(in), arr(out), cb);
-                          else       launch_sweeps<1, false>(arr(in), arr(out), cb); }
+    if (g.limiter == 0)      { if (two_d) launch_sweeps<0, true>(arr(in), arr(out), cb);
+                               else       launch_sweeps<0, false>(arr(in), arr(out), cb); }
+    else if (g.limiter == 1) { if (two_d) launch_sweeps<1, true>(arr(in), arr(out), cb);
+                               else       launch_sweeps<1, false>(arr(in), arr(out), cb); }
+    else                     { if (two_d) launch_sweeps<2, true>(arr(in), arr(out), cb);
+                               else       launch_sweeps<2, false>(arr(in), arr(out), cb); }
     const Combine cbf = { sn >= 0 ? arr(sn + S_B) : nullptr, wn, ws };
     launch_ct(arr(in + S_B), arr(out + S_B), cbf, dbg);
 }
@@ -450,8 +457,10 @@ int pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int 
     Grid g;
     if (!make_grid(g, nx, ny, nz, ghost))
         return fail(PLUTO_EINVAL, "need nx >= 2, ny >= 2, nz >= 1, 2 <= ghost <= %d, active extents >= ghost", XOFF);
-    if (!(gamma > 1.0) || !(cfl > 0.0) || (limiter != PLUTO_MINMOD && limiter != PLUTO_MC))
-        return fail(PLUTO_EINVAL, "need gamma > 1, cfl > 0, limiter in {0,1}");
+    if (!(gamma > 1.0) || !(cfl > 0.0) || limiter < PLUTO_MINMOD || limiter > PLUTO_WENOZ)
+        return fail(PLUTO_EINVAL, "need gamma > 1, cfl > 0, limiter in {0,1,2}");
+    if (limiter == PLUTO_WENOZ && ghost < 3)
+        return fail(PLUTO_EINVAL, "the WENO-Z stencil needs ghost >= 3");
     if ((long long)g.tot[2] * 8 > 65535 || g.tot[1] > 65535)
         return fail(PLUTO_EINVAL, "extent too large for the launch grid");
     g.gamma = gamma; g.igm1 = 1.0 / (gamma - 1.0); g.cfl = cfl; g.limiter = limiter;
