@@ -468,6 +468,8 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
 // the primitives of cells s-2 .. s+2 live in a five-slot ring in shared memory (own column), iteration s
 // reconstructs both faces of cell s, solves interface s - 1/2 with the q^L kept from cell s-1 and
 // finishes cell s-1.  First version: operands are loaded directly (no prefetch ring).
+constexpr int WZ_PF = 17;        // doubles per thread and iteration: U(s+3) 5, faces 6, U'(s) 6
+
 template <int DIR, bool TWO_D>
 __global__ void __launch_bounds__(MARCH_NT, 3)
 k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
@@ -475,7 +477,9 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
-    __shared__ double ring[5][7][MARCH_NT];
+    extern __shared__ double wz_smem[];
+    double (*ring)[7][MARCH_NT] = reinterpret_cast<double (*)[7][MARCH_NT]>(wz_smem);                    // [5]
+    double (*pf)[WZ_PF][MARCH_NT] = reinterpret_cast<double (*)[WZ_PF][MARCH_NT]>(wz_smem + 5 * 7 * MARCH_NT);   // [2]
     const int t = threadIdx.x;
     const int i = blockIdx.x * blockDim.x + t;
     if (i >= g.n[0]) return;
@@ -488,9 +492,34 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     const double gamma = g.gamma, igm1 = g.igm1;
     const double fac = scale * P->dtdx[DIR];
     const double *__restrict__ bn = Sin + (S_B + DIR) * sa;        // normal face field
+    const double *__restrict__ b1 = Sin + (S_B + T1) * sa;         // transverse fields
+    const double *__restrict__ b2 = Sin + (S_B + T2) * sa;
+    const long long st1 = g.st[T1], st2 = g.st[T2];
     const int xdup = ct_xdup(i, g.n[0]);
     bool bad, anybad = false;
     auto slot = [](int m) { return ((m % 5) + 5) % 5; };
+
+    // what iteration s consumes: U of cell s+2 and the faces around it, U' of cell s-1 (cs = cell s)
+    auto prefetch = [&](int sl, long long cs) {
+        const long long cn = cs + 2 * st;
+#pragma unroll
+        for (int v = 0; v < 5; v++) cp_async8(&pf[sl][v][t], Sin + v * sa + cn);
+        cp_async8(&pf[sl][5][t], bn + cn);
+        cp_async8(&pf[sl][6][t], bn + cn + st);
+        cp_async8(&pf[sl][7][t], b1 + cn);               // (2D: the cell-centred B_z itself)
+        if (!(TWO_D && T1 == 2)) cp_async8(&pf[sl][8][t], b1 + cn + st1);
+        cp_async8(&pf[sl][9][t], b2 + cn);
+        if (!(TWO_D && T2 == 2)) cp_async8(&pf[sl][10][t], b2 + cn + st2);
+        const long long cm = cs - st;
+        cp_async8(&pf[sl][11][t], Sout + cm);
+        cp_async8(&pf[sl][12][t], Sout + (1 + DIR) * sa + cm);
+        cp_async8(&pf[sl][13][t], Sout + (1 + T1) * sa + cm);
+        cp_async8(&pf[sl][14][t], Sout + (1 + T2) * sa + cm);
+        cp_async8(&pf[sl][15][t], Sout + 4 * sa + cm);
+        if (BZ2D) cp_async8(&pf[sl][16][t], Sout + 7 * sa + cm);
+        cp_async_commit();
+    };
+    prefetch(0, c);
 
     // prologue: cells s0-3 .. s0+1; q^L of face s0 - 1/2 comes from the stencil of cell s0-1
     double qL[7];
@@ -516,9 +545,16 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     double Fp[6] = { 0, 0, 0, 0, 0, 0 };                // previous face: rho, m_n, m_t1, m_t2, E, (B_z in 2D)
 
     for (int s = s0; s <= s1; s++, c += st) {
+        const int ps = (s - s0) & 1;
+        if (s < s1) { prefetch(ps ^ 1, c + st); cp_async_wait<1>(); }
+        else        { cp_async_wait<0>(); }
         {   // cell s+2 replaces cell s-3 in the ring
-            double qa[7];
-            load_rot<DIR, TWO_D>(g, Sin, c + 2 * st, qa, bad);
+            double qa[7], m[3], B[3];
+            m[0] = pf[ps][1][t]; m[1] = pf[ps][2][t]; m[2] = pf[ps][3][t];
+            B[DIR] = 0.5 * (pf[ps][5][t] + pf[ps][6][t]);
+            B[T1] = (TWO_D && T1 == 2) ? pf[ps][7][t] : 0.5 * (pf[ps][7][t] + pf[ps][8][t]);
+            B[T2] = (TWO_D && T2 == 2) ? pf[ps][9][t] : 0.5 * (pf[ps][9][t] + pf[ps][10][t]);
+            prim_rot<DIR>(pf[ps][0][t], m, B, pf[ps][4][t], gamma, qa, bad);
             if (s + 2 < s1) anybad |= bad;
             const int sl = slot(s + 2);
 #pragma unroll
@@ -537,12 +573,12 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
         for (int v = 0; v < 7; v++) qL[v] = qLn[v];
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
-            Sout[cm] -= fac * (F[0] - Fp[0]);
-            Sout[(1 + DIR) * sa + cm] -= fac * (F[1] - Fp[1]);
-            Sout[(1 + T1) * sa + cm] -= fac * (F[2] - Fp[2]);
-            Sout[(1 + T2) * sa + cm] -= fac * (F[3] - Fp[3]);
-            Sout[4 * sa + cm] -= fac * (F[6] - Fp[4]);
-            if (BZ2D) Sout[7 * sa + cm] -= fac * (F[4] - Fp[5]);   // F_y[B_z]
+            Sout[cm] = pf[ps][11][t] - fac * (F[0] - Fp[0]);
+            Sout[(1 + DIR) * sa + cm] = pf[ps][12][t] - fac * (F[1] - Fp[1]);
+            Sout[(1 + T1) * sa + cm] = pf[ps][13][t] - fac * (F[2] - Fp[2]);
+            Sout[(1 + T2) * sa + cm] = pf[ps][14][t] - fac * (F[3] - Fp[3]);
+            Sout[4 * sa + cm] = pf[ps][15][t] - fac * (F[6] - Fp[4]);
+            if (BZ2D) Sout[7 * sa + cm] = pf[ps][16][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
         }
         if (s < s1) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
@@ -558,6 +594,7 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     }
     if (anybad) P->err = 1;
 }
+constexpr int WZ_SMEM_BYTES = (5 * 7 + 2 * WZ_PF) * MARCH_NT * 8;
 
 // ---------------------------------------------------------------- fused x + y sweep (a2-a5)
 // Block = NT consecutive cells of one x-row, marching along y over `seglen` rows.  Each arriving row

@@ -75,14 +75,13 @@ __device__ __forceinline__ void plm_faces(double q, double dm, double dp, double
     hi = fma(h, s, q);
 }
 
-// WENO-Z value at the upper face of the centre cell c of the stencil (a, b, c, d, e) ([51] named at
-// PAPER.md:100,260; reading R18: Jiang-Shu smoothness indicators, tau5 = |beta0 - beta2|,
-// alpha_k = d_k (1 + tau5 / (beta_k + 1e-40)), d = (1/10, 6/10, 3/10)).
-__device__ __forceinline__ double wenoz_face(double a, double b, double c, double d, double e)
+// WENO-Z values on both faces of the centre cell c of the stencil (a, b, c, d, e) ([51] named at
+// PAPER.md:100,260; reading R18: candidate values q_k, Jiang-Shu smoothness indicators beta_k,
+// tau5 = |beta0 - beta2|, alpha_k = d_k (1 + tau5 / (beta_k + 1e-40)), d = (1/10, 6/10, 3/10)).
+// The lower-face value is the same formula on the mirrored stencil: beta_0 and beta_2 swap, beta_1 and
+// tau5 are unchanged, so the indicators and the three quotients are formed once for both faces.
+__device__ __forceinline__ void wenoz_faces(double a, double b, double c, double d, double e, double &lo, double &hi)
 {
-    const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) * (1.0 / 6.0);
-    const double q1 = (-b + 5.0 * c + 2.0 * d) * (1.0 / 6.0);
-    const double q2 = (2.0 * c + 5.0 * d - e) * (1.0 / 6.0);
     const double a0 = a - 2.0 * b + c, b0 = a - 4.0 * b + 3.0 * c;
     const double a1 = b - 2.0 * c + d, b1 = b - d;
     const double a2 = c - 2.0 * d + e, b2 = 3.0 * c - 4.0 * d + e;
@@ -90,10 +89,25 @@ __device__ __forceinline__ double wenoz_face(double a, double b, double c, doubl
     const double be1 = fma(13.0 / 12.0 * a1, a1, 0.25 * b1 * b1);
     const double be2 = fma(13.0 / 12.0 * a2, a2, 0.25 * b2 * b2);
     const double tau = fabs(be0 - be2);
-    const double al0 = 0.1 * fma(tau, rcp_fast(be0 + 1e-40), 1.0);
-    const double al1 = 0.6 * fma(tau, rcp_fast(be1 + 1e-40), 1.0);
-    const double al2 = 0.3 * fma(tau, rcp_fast(be2 + 1e-40), 1.0);
-    return fma(al0, q0, fma(al1, q1, al2 * q2)) * rcp_fast(al0 + al1 + al2);
+    const double r0 = fma(tau, rcp_fast(be0 + 1e-40), 1.0);
+    const double r1 = 0.6 * fma(tau, rcp_fast(be1 + 1e-40), 1.0);
+    const double r2 = fma(tau, rcp_fast(be2 + 1e-40), 1.0);
+    // upper face: stencils (a,b,c), (b,c,d), (c,d,e) with d = (0.1, 0.6, 0.3)
+    {
+        const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) * (1.0 / 6.0);
+        const double q1 = (-b + 5.0 * c + 2.0 * d) * (1.0 / 6.0);
+        const double q2 = (2.0 * c + 5.0 * d - e) * (1.0 / 6.0);
+        const double al0 = 0.1 * r0, al2 = 0.3 * r2;
+        hi = fma(al0, q0, fma(r1, q1, al2 * q2)) * rcp_fast(al0 + r1 + al2);
+    }
+    // lower face: the mirrored stencils (e,d,c), (d,c,b), (c,b,a)
+    {
+        const double q0 = (2.0 * e - 7.0 * d + 11.0 * c) * (1.0 / 6.0);
+        const double q1 = (-d + 5.0 * c + 2.0 * b) * (1.0 / 6.0);
+        const double q2 = (2.0 * c + 5.0 * b - a) * (1.0 / 6.0);
+        const double al0 = 0.1 * r2, al2 = 0.3 * r0;
+        lo = fma(al0, q0, fma(r1, q1, al2 * q2)) * rcp_fast(al0 + r1 + al2);
+    }
 }
 
 // Interface values of the centre cell from its five-cell stencil: LIM 0/1 = PLM with minmod / MC
@@ -102,12 +116,8 @@ template <int LIM>
 __device__ __forceinline__ void recon_faces(double qm2, double qm1, double q0, double qp1, double qp2,
                                             double &lo, double &hi)
 {
-    if (LIM == 2) {
-        hi = wenoz_face(qm2, qm1, q0, qp1, qp2);
-        lo = wenoz_face(qp2, qp1, q0, qm1, qm2);
-    } else {
-        plm_faces<LIM == 2 ? 0 : LIM>(q0, q0 - qm1, qp1 - q0, lo, hi);
-    }
+    if (LIM == 2) wenoz_faces(qm2, qm1, q0, qp1, qp2, lo, hi);
+    else plm_faces<LIM == 2 ? 0 : LIM>(q0, q0 - qm1, qp1 - q0, lo, hi);
 }
 
 // rho or p is unphysical: not a positive, finite, normal number (sign / exponent test on the high word)

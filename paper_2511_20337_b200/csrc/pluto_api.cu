@@ -220,20 +220,24 @@ void launch_sweeps(const double *Sin, double *Sout, Combine cb)
         LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len));
     }
     if (!fused) {
+        if constexpr (LIM == 2) {
+            cudaFuncSetAttribute(k_sweep_march_wz<1, TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+        }
         const long long nitems = (long long)(g.n[0] + 2 * sx_halo(LIM)) * g.n[1] * g.n[2];
         LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + sx_out(LIM) - 1) / sx_out(LIM)), SX_NT, 0, s>>>(
                              g, Sin, Sout, ct, C.P, cb));
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
         dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len));
         else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
     if (!TWO_D) {
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = march_seglen(g.n[2], (long long)g.n[0] * g.n[1]);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len));
         else LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
     }
 }
