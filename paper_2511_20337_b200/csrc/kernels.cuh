@@ -54,6 +54,10 @@ __device__ __forceinline__ void mbar_wait(void *bar, unsigned parity)
                      : "=r"(ok) : "r"(a), "r"(parity) : "memory");
     } while (!ok);
 }
+__device__ __forceinline__ void mbar_arrive(void *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 // generic-proxy accesses to shared memory before this point are ordered before later async-proxy (TMA) writes
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
@@ -613,7 +617,7 @@ constexpr int XY_PFA = 10;       // arriving row: U 5, (rows 5, 6: carried y flu
 constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
 constexpr int XY_DOUBLES_PER_THREAD = 3 * XY_RING + XY_PFA + XY_PFF + 7;
 constexpr int XY_BXROW_PAD = 2;     // the b_x row of the arriving row holds NT + 2 faces (thread t reads faces t, t + 1)
-constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 16; }   // b_x row + two mbarriers behind the arrays
+constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 32; }   // b_x row + three mbarriers behind the arrays
 
 // 128-thread blocks run three per SM at 168 registers (measured 17% faster than four at 128)
 #ifndef XY128_MINB
@@ -631,7 +635,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     double *pff = pfa + XY_PFA * NT;              // [XY_PFF][NT]
     double *sQ = pff + XY_PFF * NT;               // [7][NT]: q^L along x, then the x fluxes
     double *bxrow = sQ + 7 * NT;                  // [NT + 2]: b_x faces of the arriving row
-    unsigned long long *bars = reinterpret_cast<unsigned long long *>(bxrow + NT + XY_BXROW_PAD);   // [2]: group A, group F
+    unsigned long long *bars = reinterpret_cast<unsigned long long *>(bxrow + NT + XY_BXROW_PAD);   // [3]: group A, group F, x fluxes
     // The previous y flux is needed again only when its row is finished, a whole iteration later: its
     // first components wait in otherwise unused shared-memory rows instead of registers (which would
     // be spilled to local memory): pfa rows 5 and 6, and in 3D the sQ rows 5 and 6 that only 2D uses.
@@ -684,6 +688,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     if (t == 0) {
         mbar_init(bars, 1);
         mbar_init(bars + 1, 1);
+        mbar_init(bars + 2, NT / 32);                               // one arrival per warp
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -819,16 +824,11 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                     ct[(CT_EC + 2) * sa + cd] = e2;
                 }
             }
-            __syncthreads();                         // B3
-            mbar_wait(bars + 1, (s - s0 - 1) & 1);   // group F(s) has landed
-            if (cell) {
-                pff[t] -= dtdx * (sQ[tr] - F[0]);
-                pff[NT + t] -= dtdx * (sQ[NT + tr] - F[1]);
-                pff[2 * NT + t] -= dtdx * (sQ[2 * NT + tr] - F[2]);
-                pff[3 * NT + t] -= dtdx * (sQ[3 * NT + tr] - F[3]);
-                pff[4 * NT + t] -= dtdx * (sQ[4 * NT + tr] - F[6]);
-                if (TWO_D) sQ[6 * NT + t] = rm[6 * NT] - dtdx * (sQ[5 * NT + tr] - F[5]);   // own slot: B_z after x
-            }
+            // split-phase barrier instead of a __syncthreads: every warp signals that its fluxes are in
+            // shared memory and goes on to the y solve; the neighbour's flux is read only when the row is
+            // finished, by which time every warp has long arrived (no waiting for the slowest x solve)
+            __syncwarp();
+            if ((t & 31) == 0) mbar_arrive(bars + 2);
         }
 
         // ---- (3) y interface s - 1/2 down the own column
@@ -852,9 +852,18 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         }
 
         // ---- (4) finish row s-1; CT data of the y face
+        if (s > s0) {
+            mbar_wait(bars + 2, (s - s0 - 1) & 1);   // all x fluxes of row s-1 are in shared memory
+            mbar_wait(bars + 1, (s - s0 - 1) & 1);   // group F(s) has landed
+        }
         if (s > s0 && cell) {
             const long long cm = c - st;
-            double r0v = pff[t], r1v = pff[NT + t], r2v = pff[2 * NT + t], r3v = pff[3 * NT + t], r4v = pff[4 * NT + t];
+            // S of row s-1 minus the x flux difference (own lower face, right neighbour's lower face)
+            double r0v = pff[t] - dtdx * (sQ[tr] - sQ[t]);
+            double r1v = pff[NT + t] - dtdx * (sQ[NT + tr] - sQ[NT + t]);
+            double r2v = pff[2 * NT + t] - dtdx * (sQ[2 * NT + tr] - sQ[2 * NT + t]);
+            double r3v = pff[3 * NT + t] - dtdx * (sQ[3 * NT + tr] - sQ[3 * NT + t]);
+            double r4v = pff[4 * NT + t] - dtdx * (sQ[4 * NT + tr] - sQ[4 * NT + t]);
             if (combine) {
                 r0v = fma(cb.wn, pff[5 * NT + t], cb.ws * r0v); r1v = fma(cb.wn, pff[6 * NT + t], cb.ws * r1v);
                 r2v = fma(cb.wn, pff[7 * NT + t], cb.ws * r2v); r3v = fma(cb.wn, pff[8 * NT + t], cb.ws * r3v);
@@ -869,7 +878,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             Sout[sa + cm] = r1v - facy * (Fy[3] - Fpy[3]);
             Sout[4 * sa + cm] = r4v - facy * (Fy[6] - Fpy[4]);
             if (TWO_D) {
-                double r7v = sQ[6 * NT + t];
+                double r7v = rm[6 * NT] - dtdx * (sQ[5 * NT + tr] - sQ[5 * NT + t]);
                 if (combine) r7v = fma(cb.wn, pff[10 * NT + t], cb.ws * r7v);
                 Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
             }
