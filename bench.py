@@ -108,8 +108,9 @@ class ClockSampler:
                 "power_w": statistics.median(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_throughput(workload_small, steps, threads=None, rk=2):
-    """the oracle as it stands, timed on the host cores (zone-updates/s)"""
+def oracle_throughput(workload_small, budget_s=12.0, threads=None, rk=2, max_steps=400):
+    """the oracle as it stands, timed on the host cores (zone-updates/s): whole steps until ~budget_s
+    seconds of CPU work are done"""
     from oracle import Oracle
     o = Oracle()
     if threads:
@@ -118,12 +119,16 @@ def oracle_throughput(workload_small, steps, threads=None, rk=2):
     o.set_integrator(rk)
     o.step(1)                                   # touch memory
     t0 = time.perf_counter()
-    rc = o.step(steps)
-    dt = time.perf_counter() - t0
-    assert rc == 0
+    steps = 0
+    while steps < max_steps:
+        assert o.step(1) == 0
+        steps += 1
+        dt = time.perf_counter() - t0
+        if dt >= budget_s:
+            break
     cores = o.get_threads()
     o.finalize()
-    return workload_small.zones * steps / dt, cores, dt
+    return workload_small.zones * steps / dt, cores, dt, steps
 
 
 def sample_workload(cfg):
@@ -315,8 +320,7 @@ def main():
         ws, what = sample_workload(args.config)
         if args.wenoz:
             ws.limiter = 2
-        steps = 4 if ws.zones > 1_000_000 else 20
-        v, cores, secs = oracle_throughput(ws, steps, rk=args.rk)
+        v, cores, secs, steps = oracle_throughput(ws, rk=args.rk)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{what}, {steps} steps, {secs:.1f} s"}
     else:
