@@ -72,14 +72,16 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
     const long long sa = g.sa;
     const double *__restrict__ b = U + S_B * sa;
     const double gm1 = g.gamma - 1.0;
-    double smax = 0.0, published = 0.0;
+    double smax = 0.0, published = 0.0, seen = 0.0;
+    int nrow = 0;
     int bad = 0;
     for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
         const int k = row / g.n[1], j = row - k * g.n[1];
         const long long r0 = g.at(0, j, k);
         const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
         const long long upk = g.act[2] ? g.at(0, j, k + 1 == g.n[2] ? 0 : k + 1) - r0 : 0;
-        const double seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
+        // the global running maximum is re-read (and the warp's own published) every eighth row
+        if ((nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
         double thr = fmax(smax, seen);
         for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
             const long long c = r0 + i;
@@ -120,12 +122,15 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
             if (sig > thr) thr = sig;
         }
         // publish the warp's maximum when it raises the global one (rare after the first rows)
-        double wm = smax;
-        for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
-        if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published)) {
-            atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
-            published = wm;
+        if ((nrow & 7) == 7 || row + (int)gridDim.x >= nrows) {
+            double wm = smax;
+            for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
+            if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published)) {
+                atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
+                published = wm;
+            }
         }
+        nrow++;
     }
     if (bad) P->err = 1;
 }
