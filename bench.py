@@ -53,6 +53,21 @@ NCU = {
 }
 
 
+def max_over_ranks(value, dist, device="cpu"):
+    """a time measured on every rank -> the maximum over ranks (a job is as slow as its slowest replica)"""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(zones_per_rank, steps, ms_max, world):
+    """whole-job zone-updates/s of `world` independent replicas (replicas only)"""
+    return world * zones_per_rank * steps / (ms_max * 1e-3)
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -234,11 +249,8 @@ def main():
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop(t0, t1)
     launches = sim.launch_count() - launches0
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * w.zones * K / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = aggregate_throughput(w.zones, K, ms, world)
 
     # ---------------- per-kernel timing of the same K steps (events around every launch)
     sim.profile(True)
@@ -307,10 +319,7 @@ def main():
             sim.get_state(Uon, Bon)             # device -> host read of the step's result
         torch.cuda.synchronize()
         te = (time.perf_counter() - tw0) / args.e2e_steps
-        if dist is not None:
-            t = torch.tensor([te], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
+        te = max_over_ranks(te, dist, "cuda")
         nbytes = (Uh.numel() + Bh.numel()) * 8
         line["e2e"] = {"value": world * w.zones / te, "unit": UNIT, "h2d_bytes_per_step": nbytes,
                        "d2h_bytes_per_step": nbytes, "ms_per_step": te * 1e3, "steps": args.e2e_steps}
