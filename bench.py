@@ -47,9 +47,9 @@ ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21, "
 # From the committed ncu capture of the same workload (profiles/, `ncu --set full`, per launch, mean of the
 # stage-1 and stage-2 launches of a step): DRAM bytes moved and fp64-pipe instructions executed per zone.
 NCU = {
-    "sweep_xy": {"dram_bytes_per_launch": 3.54e9, "fp64_instr_per_zone": 576, "profile": "profiles/r1b_step_kernels.md"},
-    "sweep_z": {"dram_bytes_per_launch": 2.88e9, "fp64_instr_per_zone": 285, "profile": "profiles/r1b_step_kernels.md"},
-    "ct": {"dram_bytes_per_launch": 2.89e9, "fp64_instr_per_zone": 117, "profile": "profiles/r1b_step_kernels.md"},
+    "sweep_xy": {"dram_bytes_per_launch": 3.54e9, "fp64_instr_per_zone": 576, "profile": "profiles/r1c_step_kernels.md"},
+    "sweep_z": {"dram_bytes_per_launch": 2.88e9, "fp64_instr_per_zone": 285, "profile": "profiles/r1c_step_kernels.md"},
+    "ct": {"dram_bytes_per_launch": 2.89e9, "fp64_instr_per_zone": 117, "profile": "profiles/r1c_step_kernels.md"},
 }
 
 
