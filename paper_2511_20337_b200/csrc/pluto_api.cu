@@ -180,14 +180,16 @@ void fill_ghosts(double *state, bool all = false)
 }
 
 // segments of a marching kernel: enough independent threads for ~8 waves of 16 warps per SM,
-// segments no shorter than 16 cells
+// segments no shorter than 16 cells -- or 4 cells when the grid is so small that 16-cell segments would
+// leave most SMs idle (configs 0 and 1: the step is then bound by the length of one segment's march)
 int march_seglen(int n, long long columns)
 {
     const long long want = (long long)C.sm_count * 16 * 32 * 8;
     long long nseg = (want + columns - 1) / columns;
     if (nseg < 1) nseg = 1;
     int len = (int)((n + nseg - 1) / nseg);
-    if (len < 16) len = 16;
+    const int minlen = columns * ((n + 15) / 16) < (long long)C.sm_count * 512 ? 4 : 16;
+    if (len < minlen) len = minlen;
     if (len > n) len = n;
     return len;
 }
