@@ -68,6 +68,11 @@ def aggregate_throughput(zones_per_rank, steps, ms_max, world):
     return world * zones_per_rank * steps / (ms_max * 1e-3)
 
 
+WORKLOAD_NAMES = {0: "configs[0] C0_orszag_tang_2d_128", 1: "configs[1] C1_cp_alfven_3d_64x32x32",
+                  2: "configs[2] C2_orszag_tang_2d_2048", 3: "configs[3] C3_blast_3d_256", 4: "configs[4] C4_blast_3d_512",
+                  5: "paper section 4.1 workload (not a BASELINE config) P1_orszag_tang_3d_256"}
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -181,7 +186,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{args.config}]", "sample": what},
+        "config": {"workload": WORKLOAD_NAMES.get(args.config, f"configs[{args.config}]"), "sample": what,
+                   "scheme": "recon(%s)+HLLD+RK%d+CT, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], args.rk, w.cfl)},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": f"{what}, {args.steps} steps"},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
