@@ -187,6 +187,9 @@ int march_seglen(int n, long long columns)
     const long long want = (long long)C.sm_count * 16 * 32 * 8;
     long long nseg = (want + columns - 1) / columns;
     if (nseg < 1) nseg = 1;
+    // equal segments when a slightly smaller count divides n (measured 2% faster at 256^3: 8 x 32 vs 10 x 26)
+    for (long long m = nseg; m >= 1 && 4 * m >= 3 * nseg; m--)
+        if (n % m == 0) { nseg = m; break; }
     int len = (int)((n + nseg - 1) / nseg);
     const int minlen = columns * ((n + 15) / 16) < (long long)C.sm_count * 512 ? 4 : 16;
     if (len < minlen) len = minlen;
