@@ -327,7 +327,9 @@ def main():
         te = (time.perf_counter() - tw0) / args.e2e_steps
         te = max_over_ranks(te, dist, "cuda")
         nbytes = (Uh.numel() + Bh.numel()) * 8
-        line["e2e"] = {"value": world * w.zones / te, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        # pluto_set_state does not copy U[4..6] of the active dimensions (the cell-centred B is the face mean)
+        h2d = (Uh.numel() // 8 * (5 if w.nz > 1 else 6) + Bh.numel()) * 8
+        line["e2e"] = {"value": world * w.zones / te, "unit": UNIT, "h2d_bytes_per_step": h2d,
                        "d2h_bytes_per_step": nbytes, "ms_per_step": te * 1e3, "steps": args.e2e_steps}
 
     # ---------------- the oracle timed beside it (rank 0, N = 1 only)

@@ -388,15 +388,6 @@ size_t api_count(const Grid &g, int d)
 // staging buffer: the CT work arrays are free outside a step (12 padded arrays > 11 interior arrays)
 double *staging() { return arr(A_CT); }
 
-int copy_in(const double *src, size_t count, double **dev)
-{
-    if (is_device_ptr(src)) { *dev = const_cast<double *>(src); return PLUTO_OK; }
-    if (count * sizeof(double) > (size_t)CT_COUNT * C.g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
-    CUDA_TRY(cudaMemcpyAsync(staging(), src, count * sizeof(double), cudaMemcpyHostToDevice, C.stream));
-    *dev = staging();
-    return PLUTO_OK;
-}
-
 } // namespace
 
 // ================================================================== C ABI
@@ -538,23 +529,32 @@ int pluto_set_state(const double *U, const double *Bface)
     if (!U || !Bface) return fail(PLUTO_EINVAL, "null pointer");
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
-    double *dev = nullptr;
-    int rc = copy_in(U, 8 * api_count(g, -1), &dev);
-    if (rc) return rc;
     Box in = interior(g);
     const size_t n = api_count(g, -1);
-    // U[0..3] -> rho, m; U[7] -> E; cell-centred B of an active dimension is not stored (R7: it IS the
-    // face mean); 2D: U[6] = B_z goes to the third magnetic array
-    const int src_of[5] = { 0, 1, 2, 3, 7 };
-    for (int v = 0; v < 5; v++)
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + (size_t)src_of[v] * n, g.n[0], g.n[1], arr(A_SA + v));
-    if (!g.act[2])
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + 6 * n, g.n[0], g.n[1], arr(A_SA + S_B + 2));
-    CUDA_TRY(cudaStreamSynchronize(s));       // staging is reused below
     size_t nface = 0;
     for (int d = 0; d < g.ndim; d++) nface += api_count(g, d);
-    rc = copy_in(Bface, nface, &dev);
-    if (rc) return rc;
+    // Host arrays are staged in the CT work arrays (free outside a step): U at offset 0, Bface behind it.
+    // U[4..6], the cell-centred B of the active dimensions, is never read (R7: it IS the face mean) and
+    // is not even copied; 2D: U[6] = B_z goes to the third magnetic array.
+    const double *dU = U, *dB = Bface;
+    if (!is_device_ptr(U)) {
+        if ((8 * n + nface) * sizeof(double) > (size_t)CT_COUNT * g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
+        CUDA_TRY(cudaMemcpyAsync(staging(), U, 4 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        if (!g.act[2]) CUDA_TRY(cudaMemcpyAsync(staging() + 6 * n, U + 6 * n, n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaMemcpyAsync(staging() + 7 * n, U + 7 * n, n * sizeof(double), cudaMemcpyHostToDevice, s));
+        dU = staging();
+    }
+    if (!is_device_ptr(Bface)) {
+        if ((8 * n + nface) * sizeof(double) > (size_t)CT_COUNT * g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
+        CUDA_TRY(cudaMemcpyAsync(staging() + 8 * n, Bface, nface * sizeof(double), cudaMemcpyHostToDevice, s));
+        dB = staging() + 8 * n;
+    }
+    const int src_of[5] = { 0, 1, 2, 3, 7 };
+    for (int v = 0; v < 5; v++)
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + (size_t)src_of[v] * n, g.n[0], g.n[1], arr(A_SA + v));
+    if (!g.act[2])
+        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + 6 * n, g.n[0], g.n[1], arr(A_SA + S_B + 2));
+    const double *dev = dB;
     size_t off = 0;
     for (int d = 0; d < g.ndim; d++) {
         int m[3];
@@ -578,8 +578,8 @@ int pluto_get_state(double *U, double *Bface)
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
     const Grid &g = C.g;
     cudaStream_t s = C.stream;
+    const size_t n = api_count(g, -1);
     if (U) {
-        size_t n = api_count(g, -1);
         bool dev = is_device_ptr(U);
         double *dst = dev ? U : staging();
         Box in = interior(g);
@@ -588,12 +588,11 @@ int pluto_get_state(double *U, double *Bface)
             k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SA + v), g.n[0], g.n[1], dst + (size_t)dst_of[v] * n);
         k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SA + S_B), dst + 4 * n, (long long)n);
         if (!dev) CUDA_TRY(cudaMemcpyAsync(U, dst, 8 * n * sizeof(double), cudaMemcpyDeviceToHost, s));
-        CUDA_TRY(cudaStreamSynchronize(s));
         C.launches += 6;
     }
     if (Bface) {
         bool dev = is_device_ptr(Bface);
-        double *dst = dev ? Bface : staging();
+        double *dst = dev ? Bface : staging() + 8 * n;      // behind U's staging: both copies overlap the packing
         size_t off = 0;
         for (int d = 0; d < g.ndim; d++) {
             int m[3];
@@ -603,9 +602,9 @@ int pluto_get_state(double *U, double *Bface)
             off += api_count(g, d);
         }
         if (!dev) CUDA_TRY(cudaMemcpyAsync(Bface, dst, off * sizeof(double), cudaMemcpyDeviceToHost, s));
-        CUDA_TRY(cudaStreamSynchronize(s));
         C.launches += g.ndim;
     }
+    CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
     return PLUTO_OK;
 }
