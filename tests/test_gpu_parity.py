@@ -395,6 +395,44 @@ def test_rk3_parity(pluto, oracle, name, make):
         oracle.set_integrator(2)
 
 
+def _random_cases(count=24, seed=2024):
+    rng = np.random.default_rng(seed)
+    cases = []
+    while len(cases) < count:
+        three_d = rng.random() < 0.6
+        nx = int(rng.choice([3, 5, 8, 17, 31, 32, 33, 64, 65, 100, 127, 128, 129, 200, 256, 260]))
+        ny = int(rng.integers(3, 20))
+        nz = int(rng.integers(3, 12)) if three_d else 1
+        lim = int(rng.integers(0, 3))
+        ghost = int(rng.integers(3 if lim == 2 else 2, 5))
+        if min(nx, ny, nz if three_d else 99) < ghost:
+            continue
+        rk = int(rng.choice([2, 3]))
+        box = (1.0, float(rng.uniform(0.5, 1.5)), float(rng.uniform(0.5, 1.5)))
+        cases.append((nx, ny, nz, lim, ghost, rk, box, int(rng.integers(1, 10**6))))
+    return cases
+
+
+@pytest.mark.parametrize("case", _random_cases(), ids=lambda c: "%dx%dx%d_l%d_g%d_rk%d" % c[:6])
+def test_random_shapes_two_steps(pluto, oracle, case):
+    """seeded random extents (wrap widths, chunk widths, ragged tails, tiny grids), ghost counts, box shapes,
+    reconstructions and integrators: two CFL steps against the oracle"""
+    nx, ny, nz, lim, ghost, rk, box, seed = case
+    w = wl.random_smooth(nx, ny, nz, seed=seed, limiter=lim, box=box, amp=0.15)
+    pluto.set_integrator(rk)
+    try:
+        pluto.load(w, ghost=ghost)
+        oracle.load(w)
+        oracle.set_integrator(rk)
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(2)
+        assert oracle.step(2) == 0
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+    finally:
+        pluto.set_integrator(2)
+        oracle.set_integrator(2)
+
+
 def test_device_pointers_and_graph_equivalence(pluto, oracle):
     """set/get with CUDA tensors; graph replay and plain launches give identical bits"""
     import torch
