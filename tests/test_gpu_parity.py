@@ -395,6 +395,27 @@ def test_rk3_parity(pluto, oracle, name, make):
         oracle.set_integrator(2)
 
 
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_config_run_keeps_the_invariants(pluto, cfg):
+    """configs[2] (200 steps) and configs[3] (50 steps) run to their full length on the GPU: mass and energy
+    conserved to 1e-12, face field divergence-free to round-off, periodic duplicates equal, no unphysical zone"""
+    w = wl.config(cfg)
+    pluto.load(w)
+    pluto.step(w.nsteps)
+    U, Bf = pluto.get_state()
+    assert np.isfinite(U).all() and U[0].min() > 0
+    for v in (0, 7):
+        tot0 = math.fsum(w.U[v].ravel())
+        assert abs(math.fsum(U[v].ravel()) - tot0) <= 1e-12 * abs(tot0)
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    div = (f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) + (f["by"][:, 1:, :] - f["by"][:, :-1, :])
+    if w.nz > 1:
+        div = div + (f["bz"][1:, :, :] - f["bz"][:-1, :, :])
+        assert np.array_equal(f["bz"][0], f["bz"][-1])
+    assert np.abs(div).max() <= 1e-12 * np.abs(Bf).max()
+    assert np.array_equal(f["bx"][:, :, 0], f["bx"][:, :, -1]) and np.array_equal(f["by"][:, 0, :], f["by"][:, -1, :])
+
+
 def _random_cases(count=24, seed=2024):
     rng = np.random.default_rng(seed)
     cases = []
