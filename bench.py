@@ -42,7 +42,8 @@ UNIT = "zone-updates/s"
 #   sweep_y/z : read S 8, read + write S' 5 + 5, CT data 3                                           = 21
 #   ct        : read CT data 12 + faces 3, write faces 3 = 18; the combine stage also reads S^n faces 3 = 21;
 #               the two launches of a step average 19.5
-ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21, "ct": 19.5}
+#   dt_max    : read S 8
+ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21, "ct": 19.5, "dt_max": 8}
 
 # From the committed ncu capture of the same workload (profiles/, `ncu --set full`, per launch, mean of the
 # stage-1 and stage-2 launches of a step): DRAM bytes moved and fp64-pipe instructions executed per zone.
@@ -283,6 +284,10 @@ def main():
                 "algorithmic_bytes_per_launch": algo_bytes,
                 "kernels_ms_per_step": {k: v[0] / K for k, v in rep.items() if v[1]},
                 "profiled_ms_per_step": ms_prof / K}
+    # the same HBM view for every kernel of the step (algorithmic bytes / live launch time / HBM peak)
+    roofline["all_kernels_hbm_frac"] = {
+        k: round(ALGO_DOUBLES[k] * 8 * units / (v[0] * 1e-3 / v[1]) * 1e-9 / hbm_peak, 4)
+        for k, v in rep.items() if v[1] and k in ALGO_DOUBLES}
     if dom in NCU:
         roofline["traffic"] = NCU[dom]["dram_bytes_per_launch"] * (units / 256 ** 3)   # scaled from the 256^3 capture
         roofline["traffic_source"] = NCU[dom]["profile"]
