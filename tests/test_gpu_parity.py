@@ -416,6 +416,43 @@ def test_full_config_run_keeps_the_invariants(pluto, cfg):
     assert np.array_equal(f["bx"][:, :, 0], f["bx"][:, :, -1]) and np.array_equal(f["by"][:, 0, :], f["by"][:, -1, :])
 
 
+@pytest.mark.parametrize("lim,rk", [(0, 2), (1, 3), (2, 3)])
+def test_scaled_units(pluto, oracle, lim, rk):
+    """the same flow in units far from 1 (rho ~ 1e-12, p ~ 1e-8, B ~ 1e-4, v ~ 1e2, L ~ 1e10): the Newton
+    reciprocals / square roots, the 1e-40 of WENO-Z and the relative guards keep the tolerances"""
+    w = wl.random_smooth(40, 18, 12, seed=77, limiter=lim, amp=0.2)
+    a, b, c = 1e-12, 1e-8, 1e10                      # density, pressure and length units
+    vu, Bu = math.sqrt(b / a), math.sqrt(b)
+    U = w.U.copy()
+    U[0] *= a
+    U[1:4] *= a * vu
+    U[4:7] *= Bu
+    U[7] *= b
+    w2 = wl.Workload("scaled", w.nx, w.ny, w.nz, tuple(c * L for L in w.box), w.gamma, w.cfl, lim, 0, U, w.Bface * Bu)
+    pluto.set_integrator(rk)
+    try:
+        pluto.load(w2)
+        oracle.load(w2)
+        oracle.set_integrator(rk)
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(3)
+        assert oracle.step(3) == 0
+        compare_state(pluto, oracle, w2, TOL_1STEP_MAXREL)
+        # and it is the same flow: the unscaled run agrees to round-off after rescaling
+        pluto.load(w)
+        pluto.step(3)
+        U1, _ = pluto.get_state()
+        oracle.load(w2)
+        oracle.set_integrator(rk)
+        oracle.step(3)
+        U2, _ = oracle.get_state()
+        scale = np.array([a, a * vu, a * vu, a * vu, Bu, Bu, Bu, b]).reshape(8, 1, 1, 1)
+        assert maxrel((U2 / scale).reshape(8, -1), U1.reshape(8, -1)) <= 1e-9
+    finally:
+        pluto.set_integrator(2)
+        oracle.set_integrator(2)
+
+
 def _random_cases(count=24, seed=2024):
     rng = np.random.default_rng(seed)
     cases = []
