@@ -416,6 +416,52 @@ def test_full_config_run_keeps_the_invariants(pluto, cfg):
     assert np.array_equal(f["bx"][:, :, 0], f["bx"][:, :, -1]) and np.array_equal(f["by"][:, 0, :], f["by"][:, -1, :])
 
 
+def _special_state(kind, n=(24, 16, 10), gamma=5.0 / 3.0):
+    """flows that exercise the special branches of HLLD: no field at all, no normal field, a field along one
+    axis only (the guarded degenerate star state), supersonic one-sided fans, exactly zero velocity"""
+    nx, ny, nz = n
+    base = wl.random_smooth(nx, ny, nz, seed=91, amp=0.1)
+    shp = (nz, ny, nx)
+    x = wl.cell_centres(nx, 1.0)[None, None, :] + np.zeros(shp)
+    y = wl.cell_centres(ny, base.box[1])[None, :, None] / base.box[1] + np.zeros(shp)
+    z = wl.cell_centres(nz, base.box[2])[:, None, None] / base.box[2] + np.zeros(shp)
+    s2 = lambda a: np.sin(2 * np.pi * a)
+    rho = 1.0 + 0.3 * s2(x) * np.cos(2 * np.pi * y)
+    p = 0.6 + 0.2 * np.cos(2 * np.pi * (x + z))
+    v = [0.3 * s2(y), 0.2 * s2(z), 0.1 * s2(x)]
+    faces = {nm: np.zeros(sh) for nm, sh in wl.face_shapes(nx, ny, nz)}
+    if kind == "hydro_supersonic":
+        v = [3.0 + 0.5 * s2(y), -2.5 + 0.3 * s2(x), 2.0 * s2(x + y)]
+    elif kind == "no_normal_field_x":            # B = (0, By(x), Bz(x)): B_x = 0 on every x-face, div B = 0
+        faces["by"] += 0.5 + 0.2 * s2(np.broadcast_to(wl.cell_centres(nx, 1.0)[None, None, :], faces["by"].shape))
+        faces["bz"] += -0.3 + 0.1 * np.cos(2 * np.pi * np.broadcast_to(wl.cell_centres(nx, 1.0)[None, None, :], faces["bz"].shape))
+    elif kind == "axis_aligned_field":           # B = (1.2, 0, 0): transverse field exactly zero, c_f = c_a > a
+        faces["bx"] += 1.2
+        p = 0.2 + 0.05 * np.cos(2 * np.pi * x)
+    elif kind == "static":
+        v = [np.zeros(shp)] * 3
+        faces["bx"] += 0.4; faces["by"] += -0.2; faces["bz"] += 0.7
+    Bc = wl.cell_mean_of_faces(faces, nx, ny, nz, [None, None, None])
+    U = wl.conserved_from_fields(rho, v, Bc, p, gamma)
+    return wl.Workload(kind, nx, ny, nz, base.box, gamma, 0.3, 0, 0, U, wl.join_faces(faces, nx, ny, nz))
+
+
+@pytest.mark.parametrize("kind", ["hydro_supersonic", "no_normal_field_x", "axis_aligned_field", "static"])
+@pytest.mark.parametrize("lim", [0, 1])
+def test_special_field_configurations(pluto, oracle, kind, lim):
+    w = _special_state(kind)
+    w.limiter = lim
+    pluto.load(w)
+    oracle.load(w)
+    assert pluto.get_dt() == oracle.get_dt()
+    pluto.step(1)
+    assert oracle.step(1) == 0
+    compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+    pluto.step(9)
+    assert oracle.step(9) == 0
+    compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+
+
 @pytest.mark.parametrize("lim,rk", [(0, 2), (1, 3), (2, 3)])
 def test_scaled_units(pluto, oracle, lim, rk):
     """the same flow in units far from 1 (rho ~ 1e-12, p ~ 1e-8, B ~ 1e-4, v ~ 1e2, L ~ 1e10): the Newton
