@@ -47,27 +47,45 @@ enum {
 /* reconstruction: PLM with the minmod / MC limiter (R4), or WENO-Z ([51]; R18; needs ghost >= 3) */
 enum { PLUTO_MINMOD = 0, PLUTO_MC = 1, PLUTO_WENOZ = 2 };
 
-/* Create (or re-create) the context for an nx x ny x nz periodic box of cubic cells with Lx = 1
- * (override with pluto_set_box).  ny >= 2 and nx >= 2 are required (2D when nz == 1, 3D when
- * nz >= 2); every active extent must be >= ghost.  ghost >= 2 layers are kept around the padded
- * device arrays (PLM needs 2).  gamma > 1 (Gamma of Eq. 3), cfl > 0, limiter PLUTO_MINMOD|PLUTO_MC|PLUTO_WENOZ.
- * Allocates device memory unless a large enough workspace was registered before. */
+/* pluto_init -- the mesh and the scheme (uniform Cartesian mesh of Eq. 4; periodic box,
+ * PAPER.md:254,360; Gamma-law gas, Eq. 3).
+ * Creates (or re-creates) the one global context for an nx x ny x nz periodic box of cubic cells with
+ * Lx = 1 (override with pluto_set_box).  nx >= 2 and ny >= 2 (2D when nz == 1, 3D when nz >= 2); every
+ * active extent >= ghost.  ghost = layers kept around the padded device arrays: >= 2 for PLM, >= 3 for
+ * WENO-Z (R9), at most 16.  gamma > 1, cfl > 0 (R8), limiter = PLUTO_MINMOD | PLUTO_MC | PLUTO_WENOZ (R4, R18).
+ * Memory: allocates pluto_workspace_bytes(...) of device memory itself unless a workspace of at least that
+ * size was registered with pluto_set_workspace (then the caller keeps ownership and must keep it alive
+ * until pluto_finalize).  Errors: PLUTO_ECUDA (no device: there is no CPU fallback), PLUTO_EINVAL
+ * (arguments), PLUTO_ENOMEM. */
 int    pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter);
 
-/* Copy a state in.  Cell-centred B of every active dimension is OVERWRITTEN by the mean of its two
- * faces (reading R7); E is taken as given.  Resets the time to 0. */
+/* pluto_set_state -- the conserved state U of Eq. 2 and the staggered face field of the
+ * constrained-transport method.
+ * U: 8*nz*ny*nx doubles, Bface: the concatenated face arrays (layouts at the top of this file); each may
+ * be a HOST or a DEVICE pointer, is only read, and is not kept after the call returns.  The cell-centred
+ * B of every active dimension in U is ignored and replaced by the mean of its two faces (R7); E is taken
+ * as given; the duplicate upper-boundary faces are ignored.  Resets the time to 0 and fills every ghost
+ * zone (a1).  Errors: PLUTO_ESTATE (no pluto_init), PLUTO_EINVAL (NULL), PLUTO_ECUDA. */
 int    pluto_set_state(const double *U, const double *Bface);
 
-/* Advance nsteps full SSP-RK2 steps, each with its own CFL dt computed on the device from the
- * state at the start of the step.  Returns after the work has completed on the stream.
- * PLUTO_EPHYS if an unphysical zone was met (state then undefined). */
+/* pluto_step -- nsteps full time steps of the semi-discrete scheme of Eq. 4 integrated
+ * with SSP Runge-Kutta (Eq. 5; RK2 by default, R3): per stage ghost fill, cons->prim
+ * (Eq. 7), reconstruction (Eq. 6), HLLD flux (Eq. 8), flux-difference update, CT; per step the CFL dt (R8)
+ * computed on the device from the state at the start of the step.  Blocks until the work has completed on
+ * the stream.  Errors: PLUTO_ESTATE (no state), PLUTO_EINVAL (nsteps < 0), PLUTO_EPHYS (a non-finite or
+ * non-positive density / pressure was met: the state is then undefined, R13), PLUTO_ECUDA. */
 int    pluto_step(int nsteps);
 
-/* dt used by the most recent step; before any step since set_state: the dt the next step will
- * use.  NaN if not initialised. */
+/* pluto_get_dt -- the CFL time step (R8; the paper does not print its rule): dt used by the most recent
+ * step; before any step since pluto_set_state, the dt the next step will use (computed now).  Bit-identical
+ * to an IEEE evaluation of dt = cfl / max_{zones, d} ((|v_d| + c_f,d) / dx_d) without contraction (R15).
+ * NaN if there is no state. */
 double pluto_get_dt(void);
 
-/* Copy the state out (either pointer may be NULL). */
+/* pluto_get_state -- copy the state out in the layouts of pluto_set_state.  U, Bface: HOST or DEVICE
+ * pointers to caller-owned memory of 8*nz*ny*nx and (sum of the face arrays) doubles; either may be
+ * NULL.  U[4..6] of the active dimensions is the face mean (R7); the duplicate upper-boundary faces are
+ * written equal to face 0.  Errors: PLUTO_ESTATE, PLUTO_ECUDA. */
 int    pluto_get_state(double *U, double *Bface);
 
 /* ---- extensions the five calls cannot express ---- */
