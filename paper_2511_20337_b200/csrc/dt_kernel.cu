@@ -80,8 +80,9 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
         const long long r0 = g.at(0, j, k);
         const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
         const long long upk = g.act[2] ? g.at(0, j, k + 1 == g.n[2] ? 0 : k + 1) - r0 : 0;
-        // the global running maximum is re-read (and the warp's own published) every eighth row
-        if ((nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
+        // the global running maximum is re-read (and the warp's own published) on each of a block's first
+        // eight rows, while it is still rising fast, then every eighth row
+        if (nrow < 8 || (nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
         double thr = fmax(smax, seen);
         for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
             const long long c = r0 + i;
@@ -122,7 +123,7 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
             if (sig > thr) thr = sig;
         }
         // publish the warp's maximum when it raises the global one (rare after the first rows)
-        if ((nrow & 7) == 7 || row + (int)gridDim.x >= nrows) {
+        if (nrow < 8 || (nrow & 7) == 7 || row + (int)gridDim.x >= nrows) {
             double wm = smax;
             for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
             if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published)) {
