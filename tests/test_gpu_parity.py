@@ -610,6 +610,47 @@ def test_error_codes(pluto):
     pluto.step(1)
 
 
+def test_c_abi_memory_and_call_order(pluto, oracle):
+    """raw C ABI: call order errors, a too-small registered workspace, and the library's own allocation and
+    stream (no torch memory, no torch stream) giving the same step as the bound path"""
+    import ctypes
+    import torch
+    from paper_2511_20337_b200 import binding
+    L = pluto.L
+    w = wl.random_smooth(20, 12, 6, seed=5)
+    pluto.load(w)
+    pluto.step(2)
+    ref = pluto.get_state()
+    assert L.pluto_finalize() == 0
+    assert L.pluto_step(1) == binding.ESTATE and L.pluto_get_dt() != L.pluto_get_dt()
+    assert L.pluto_set_state(None, None) == binding.ESTATE
+    # a registered workspace that is too small
+    need = L.pluto_workspace_bytes(w.nx, w.ny, w.nz, 2)
+    small = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+    assert L.pluto_set_workspace(small.data_ptr(), small.numel()) == 0
+    assert L.pluto_init(w.nx, w.ny, w.nz, 2, w.gamma, w.cfl, w.limiter) == binding.ENOMEM
+    assert L.pluto_set_workspace(ctypes.c_void_p(1234567 * 256 + 8), 10) == binding.EINVAL
+    # the library allocates for itself and runs on its own stream
+    assert L.pluto_set_workspace(None, 0) == 0
+    assert L.pluto_set_stream(None) == 0
+    assert L.pluto_init(w.nx, w.ny, w.nz, 2, w.gamma, w.cfl, w.limiter) == 0
+    assert L.pluto_set_box(*w.box) == 0
+    assert L.pluto_step(1) == binding.ESTATE                      # no state yet
+    U = np.ascontiguousarray(w.U)
+    assert L.pluto_set_state(U.ctypes.data, w.Bface.ctypes.data) == 0
+    assert L.pluto_step(2) == 0
+    Uo, Bo = np.empty_like(U), np.empty_like(w.Bface)
+    assert L.pluto_get_state(Uo.ctypes.data, Bo.ctypes.data) == 0
+    assert np.array_equal(Uo, ref[0]) and np.array_equal(Bo, ref[1])
+    assert L.pluto_get_state(None, None) == 0
+    assert L.pluto_finalize() == 0
+    # hand the session fixture its stream back
+    assert L.pluto_set_stream(pluto.stream.cuda_stream) == 0
+    pluto.workspace = None
+    pluto.load(w)
+    pluto.step(1)
+
+
 def test_uniform_state_is_a_fixed_point(pluto):
     nx, ny, nz = 12, 10, 8
     shp = (nz, ny, nx)
