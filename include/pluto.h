@@ -14,6 +14,10 @@
  * Beyond the north-star step: SSP-RK3 (Eq. 5 itself; PLUTO_OPT_RK_ORDER, reading R17) and WENO-Z
  * reconstruction ([51] named at PAPER.md:100,260; limiter PLUTO_WENOZ, reading R18).
  *
+ * Beyond one GPU: the box cut into z slabs, one or more per process, with the ghost planes pulled out of
+ * the neighbour slab's memory and one max for dt (section 3.4 "Multi GPU communication", PAPER.md:208-244,
+ * Fig. 4; pluto_init_slabs and the calls below it).
+ *
  * Everything is fp64.  One global context (the five north-star calls carry no handle).
  * All entry points return 0 (PLUTO_OK) or a negative error code; no exceptions, aborts or stdout.
  * There is NO CPU fallback: without a CUDA device every compute entry point returns PLUTO_ECUDA.
@@ -93,12 +97,61 @@ int    pluto_get_state(double *U, double *Bface);
 int    pluto_set_box(double Lx, double Ly, double Lz);      /* cell sizes dx_d = L_d / n_d (R11) */
 int    pluto_step_fixed_dt(int nsteps, double dt);          /* same step with dt imposed (R8: 1D pin, clipping) */
 double pluto_get_time(void);                                /* sum of dt since set_state */
-int    pluto_set_stream(void *cuda_stream);                 /* cudaStream_t to launch on (NULL: default) */
+int    pluto_set_stream(void *cuda_stream);                 /* cudaStream_t to launch on (NULL: a stream of the library's own on the current device) */
+/* Device memory one context needs (SSP-RK2; SSP-RK3 keeps a third state, which the library allocates itself on
+ * first use unless the workspace was sized with pluto_workspace_bytes_slabs(..., rk_order = 3) and the
+ * integrator was selected before pluto_init).  0 for sizes the library does not take. */
 size_t pluto_workspace_bytes(int nx, int ny, int nz, int ghost);
-int    pluto_set_workspace(void *dev, size_t bytes);        /* caller-owned device memory, used by the next pluto_init */
+/* caller-owned device memory (256-byte aligned) used by the next pluto_init / pluto_init_slabs; the
+ * registration ends at pluto_finalize (the memory may then be freed); NULL: the library allocates */
+int    pluto_set_workspace(void *dev, size_t bytes);
 int    pluto_finalize(void);
 const char *pluto_last_error(void);
 int    pluto_device_count(void);                            /* 0 without a usable CUDA device */
+
+/* ---- z-slab domain decomposition (section 3.4, Fig. 4) ----
+ *
+ * The nz planes of the box are cut into nslab slabs (the first nz % nslab slabs hold one plane more); every
+ * slab has at least ghost + 1 planes.  This process holds slabs first .. first + count - 1:
+ *   count == nslab : the whole box in one process, on one GPU.  Every other call of this header works
+ *                    unchanged (pluto_step replays the whole step); results are bit-identical to
+ *                    pluto_init for any nslab.
+ *   count <  nslab : one process per GPU (count = 1, first = rank).  U / Bface of pluto_set_state and
+ *                    pluto_get_state then cover only the planes held here ([bz] has local planes + 1), the
+ *                    two outer neighbours are attached with pluto_attach_peer, and the step is driven in
+ *                    phases so that the caller can place its collectives between them:
+ *                        pluto_step_begin(0)            local part of the CFL max (a8)
+ *                        [all-reduce MAX of the 8 bytes at pluto_dt_max_bits() over the processes]
+ *                        pluto_step_stage(0, 0)         dt = cfl / max; ghost planes pulled from the peers; stage 1
+ *                        [barrier: every process has finished its stage]
+ *                        pluto_step_stage(1, 0) ...     one call per Runge-Kutta stage
+ *                    The only data-path exchange is the ghost-plane pull inside the ghost-fill kernel (peer
+ *                    loads over NVLink, no pack / unpack buffers: Fig. 4's Isend / Irecv pairs)
+ *                    and the one max for dt.
+ * Errors: as pluto_init; PLUTO_EINVAL for a slab thinner than ghost + 1 planes or nz < 2. */
+int    pluto_init_slabs(int nslab, int first, int count, int nx, int ny, int nz, int ghost,
+                        double gamma, double cfl, int limiter);
+size_t pluto_workspace_bytes_slabs(int nslab, int first, int count, int nx, int ny, int nz, int ghost, int rk_order);
+/* planes of slab `slab` when nz planes are cut into nslab slabs: first plane and count (no device needed) */
+int    pluto_slab_planes(int nz, int nslab, int slab, int *k0, int *planes);
+/* first global plane and number of planes this process holds */
+int    pluto_local_planes(int *k0, int *nz_local);
+/* The memory of the lowest (side 0) or highest (side 1) slab held here, for the neighbour process to attach:
+ * a 64-byte CUDA IPC handle (ipc_handle64, may be NULL; only for memory the library allocated itself), the
+ * device pointer (device_ptr, for a neighbour in the same process or with peer access), the array stride
+ * in doubles and the number of interior planes.  Any output pointer may be NULL. */
+int    pluto_export_slab(int side, void *ipc_handle64, void **device_ptr, long long *array_stride, int *planes);
+/* Attach the slab below (side 0) or above (side 1) the planes held here: either its IPC handle (opened with
+ * peer access enabled; closed at pluto_finalize) or a device pointer valid in this process. */
+int    pluto_attach_peer(int side, const void *ipc_handle64, void *device_ptr, long long array_stride, int planes);
+/* fill every ghost zone of the current state (a1) once all processes have set their state */
+int    pluto_fill_ghosts(void);
+/* Phases of one step (see above).  fixed_dt > 0: impose dt (no reduction); pass fixed = 1 to pluto_step_stage.
+ * Nothing here waits for the device: the calls enqueue on the stream; pluto_sync reports errors. */
+int    pluto_step_begin(double fixed_dt);
+void  *pluto_dt_max_bits(void);        /* DEVICE pointer to the running max of (|v_d| + c_f,d)/dx_d as the bit
+                                          pattern of a positive double (an order-preserving unsigned 64-bit integer) */
+int    pluto_step_stage(int stage, int fixed);
 
 /* Enqueue nsteps steps without waiting (no error check, no host synchronisation); used for timing
  * with CUDA events on the stream given to pluto_set_stream.  pluto_sync waits and returns

@@ -12,9 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# PLUTO_B200_LIB selects another build of the same library (kernel tuning experiments)
-LIB = os.environ.get("PLUTO_B200_LIB") or os.path.join(_HERE, "libpluto_b200.so")
-_DEFAULT_LIB = os.path.join(_HERE, "libpluto_b200.so")
+LIB = os.path.join(_HERE, "libpluto_b200.so")
 
 OK, EINVAL, ESTATE, ECUDA, EPHYS, ENOMEM = 0, -1, -2, -3, -4, -5
 MINMOD, MC, WENOZ = 0, 1, 2
@@ -31,6 +29,8 @@ SYMBOLS = [
     "pluto_device_count", "pluto_step_async", "pluto_sync", "pluto_launch_count",
     "pluto_set_option", "pluto_debug_euler", "pluto_profile", "pluto_profile_get", "pluto_kernel_name",
     "pluto_probe_fp64_gflops",
+    "pluto_init_slabs", "pluto_workspace_bytes_slabs", "pluto_local_planes", "pluto_export_slab",
+    "pluto_attach_peer", "pluto_fill_ghosts", "pluto_slab_planes", "pluto_step_begin", "pluto_dt_max_bits", "pluto_step_stage",
 ]
 
 
@@ -41,7 +41,7 @@ class PlutoError(RuntimeError):
 
 
 def load_library(build_if_missing: bool = True) -> C.CDLL:
-    if build_if_missing and LIB == _DEFAULT_LIB:
+    if build_if_missing:
         from . import build as _build
         _build.build()
     if not os.path.exists(LIB):
@@ -71,6 +71,16 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pluto_kernel_name.argtypes = [i32]
     L.pluto_kernel_name.restype = C.c_char_p
     L.pluto_probe_fp64_gflops.restype = dbl
+    L.pluto_init_slabs.argtypes = [i32, i32, i32, i32, i32, i32, i32, dbl, dbl, i32]
+    L.pluto_workspace_bytes_slabs.argtypes = [i32] * 8
+    L.pluto_workspace_bytes_slabs.restype = C.c_size_t
+    L.pluto_local_planes.argtypes = [C.POINTER(i32), C.POINTER(i32)]
+    L.pluto_slab_planes.argtypes = [i32, i32, i32, C.POINTER(i32), C.POINTER(i32)]
+    L.pluto_export_slab.argtypes = [i32, vp, C.POINTER(vp), C.POINTER(C.c_longlong), C.POINTER(i32)]
+    L.pluto_attach_peer.argtypes = [i32, vp, vp, C.c_longlong, i32]
+    L.pluto_step_begin.argtypes = [dbl]
+    L.pluto_dt_max_bits.restype = vp
+    L.pluto_step_stage.argtypes = [i32, i32]
     return L
 
 
@@ -100,6 +110,7 @@ class Pluto:
         self._check(self.L.pluto_set_stream(self.stream.cuda_stream))
         self.workspace = None
         self.shape = None
+        self.rk_order = 2
 
     def _check(self, rc):
         if rc != 0:
@@ -107,8 +118,9 @@ class Pluto:
         return rc
 
     # ---- the five calls
-    def init(self, nx, ny, nz, ghost=2, gamma=5.0 / 3.0, cfl=0.4, limiter=MINMOD):
-        need = self.L.pluto_workspace_bytes(nx, ny, nz, ghost)
+    def init(self, nx, ny, nz, ghost=2, gamma=5.0 / 3.0, cfl=0.4, limiter=MINMOD, nslab=1):
+        """nslab > 1: the box cut into nslab z slabs, all of them on this GPU (pluto_init_slabs)"""
+        need = self.L.pluto_workspace_bytes_slabs(nslab, 0, nslab, nx, ny, nz, ghost, self.rk_order)
         if need == 0:
             raise PlutoError(EINVAL, "bad grid")
         self.L.pluto_finalize()
@@ -117,7 +129,10 @@ class Pluto:
             self.workspace = self.torch.empty(need, dtype=self.torch.uint8, device=self.device)
         self.torch.cuda.current_stream().synchronize()
         self._check(self.L.pluto_set_workspace(self.workspace.data_ptr(), self.workspace.numel()))
-        self._check(self.L.pluto_init(nx, ny, nz, ghost, gamma, cfl, limiter))
+        if nslab == 1:
+            self._check(self.L.pluto_init(nx, ny, nz, ghost, gamma, cfl, limiter))
+        else:
+            self._check(self.L.pluto_init_slabs(nslab, 0, nslab, nx, ny, nz, ghost, gamma, cfl, limiter))
         self.shape = (nx, ny, nz)
         return 0
 
@@ -180,6 +195,7 @@ class Pluto:
         old = self.L.pluto_set_option(OPT_RK_ORDER, order)
         if old < 0:
             raise PlutoError(old, self.L.pluto_last_error().decode())
+        self.rk_order = order
         return old
 
     def profile(self, on):
@@ -203,11 +219,11 @@ class Pluto:
     def finalize(self):
         return self.L.pluto_finalize()
 
-    def load(self, w, ghost=None):
+    def load(self, w, ghost=None, nslab=1):
         """init + set_box + set_state from a workloads.Workload (host arrays)"""
         if ghost is None:
             ghost = 3 if w.limiter == WENOZ else 2
-        self.init(w.nx, w.ny, w.nz, ghost, w.gamma, w.cfl, w.limiter)
+        self.init(w.nx, w.ny, w.nz, ghost, w.gamma, w.cfl, w.limiter, nslab=nslab)
         self.set_box(*w.box)
         self.set_state(w.U, w.Bface)
         return self

@@ -40,20 +40,20 @@ def _sources():
     return out
 
 
-def build(force: bool = False, verbose: bool = False, defines=(), out: str | None = None) -> str:
-    """defines / out: build a tuning variant (-DNAME=VALUE ...) into another file"""
-    lib = out or LIB
+def build(force: bool = False, verbose: bool = False) -> str:
+    """verbose: also print the ptxas resource table (-Xptxas=-v) of every kernel"""
+    lib = LIB
     newest = max(os.path.getmtime(s) for s in _sources())
-    if not force and not defines and os.path.exists(lib) and os.path.getmtime(lib) >= newest:
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= newest:
         return lib
     nvcc = _nvcc()
-    objdir = _OBJ if not out else _OBJ + "_" + os.path.basename(out)
+    objdir = _OBJ
     os.makedirs(objdir, exist_ok=True)
     objs = []
     procs = []
     for unit, extra in UNITS.items():
         obj = os.path.join(objdir, unit.replace(".cu", ".o"))
-        cmd = [nvcc, *ARCH, *COMMON, *extra, *[f"-D{d}" for d in defines], "-c", os.path.join(_CSRC, unit), "-o", obj]
+        cmd = [nvcc, *ARCH, *COMMON, *extra, "-c", os.path.join(_CSRC, unit), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
@@ -70,6 +70,4 @@ def build(force: bool = False, verbose: bool = False, defines=(), out: str | Non
 
 
 if __name__ == "__main__":
-    defs = [a[2:] for a in sys.argv[1:] if a.startswith("-D")]
-    outs = [a[2:] for a in sys.argv[1:] if a.startswith("-o")]
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=defs, out=outs[0] if outs else None))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -20,13 +20,13 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
 }
 
 // ---------------------------------------------------------------- periodic halo rows of the CT arrays
-// Rows j = -1 and j = n1 of every interior plane receive the rows n1-1 and 0 (positions i = -1 .. n0:
-// the sweep kernels have already written the x copies, kernels.cuh ct_xdup).  grid.x = plane,
-// grid.y = array; contiguous row copies.
+// Rows j = -1 and j = n1 of every plane the CT kernel reads (3D: -1 .. nz) receive the rows n1-1 and 0
+// (positions i = -1 .. n0: the sweep kernels have already written the x copies, kernels.cuh ct_xdup).
+// grid.x = plane, grid.y = array; contiguous row copies.
 __global__ void __launch_bounds__(256) k_ct_halo(Grid g, double *__restrict__ ct, int two_d)
 {
     const int n0 = g.n[0], n1 = g.n[1];
-    const int a = blockIdx.y, k = blockIdx.x;
+    const int a = blockIdx.y, k = (int)blockIdx.x - (two_d ? 0 : 1);
     if (two_d && !(a == 0 || a == 3 || a == 6 || a == 7 || a == 11)) return;     // arrays the 2D path reads
     double *arr = ct + (long long)a * g.sa + (long long)(k + g.off[2]) * g.st[2] + g.off[0] - 1;
     const long long st1 = g.st[1];
@@ -71,7 +71,7 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
     const int k0 = blockIdx.z * seglen, k1 = min(k0 + seglen, g.n[2]);
     const long long sa = g.sa, st1 = g.st[1], st2 = g.st[2];
     const double dtdx = P->dtdx[0], dtdy = P->dtdx[1], dtdz = P->dtdx[2];
-    auto zc = [&](int k) { return (k == g.n[2] ? 0 : k) + g.off[2]; };     // padded z coordinate of plane k
+    auto zc = [&](int k) { return k + g.off[2]; };     // padded z coordinate of plane k (no z wrap: see k_ct)
     // in-plane offset of the own cell (idle threads are clamped onto a legal address)
     const long long oc = (long long)((edge ? j : 0) + g.off[1]) * st1 + (edge ? i : 0) + g.off[0];
 
@@ -107,7 +107,7 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
     // plane k-1 values that enter E_x, E_y at k - 1/2
     double fyz = 0, wyP = 0, excP = 0, excPm = 0, fxz = 0, wxP = 0, eycP = 0, eycPm = 0;
     if (!TWO_D) {
-        const double *q = ct + (long long)zc(wrap_m1(k0, g.n[2])) * st2 + oc;
+        const double *q = ct + (long long)zc(k0 - 1) * st2 + oc;
         fyz = q[2 * sa];  wyP = q[7 * sa];
         excP = q[9 * sa]; excPm = q[9 * sa - st1];
         fxz = q[1 * sa];  wxP = q[6 * sa];

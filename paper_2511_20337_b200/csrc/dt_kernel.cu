@@ -61,36 +61,46 @@ __device__ __forceinline__ double sqrt_nr(double x)      // x > 0
 // global maximum (`thr`: the exact candidates this thread has seen and the running global maximum
 // other warps have published).  Skipping never changes the result -- the zone that holds the maximum
 // has every bound >= the maximum >= thr -- so the dt stays bit-identical and order independent.
+//   filter 0:  whole rows, from the bound grid the last stage of the previous step left behind (an upper
+//              bound of every candidate of the row's zones, kernels.cuh sigma_bound): rows that cannot
+//              hold the maximum are never read
 //   filter 1:  c_f,d <= sqrt(a^2 + b^2)  =>  sig_d <= (|m_d|/rho + sqrt((gamma p + B^2)/rho)) / dx_d
 //   filter 2:  the candidates themselves in fast arithmetic (relative error <= 1e-8 even where the
 //              discriminant cancels), with a 1e-7 margin
 // One block walks whole rows (x contiguous); the running global maximum is re-read once per row.
+// bz_up: the b_z array holding the upper face of the last plane in its plane 0 (the slab above in a
+// z-slab decomposition; the state itself in a periodic single domain).
 __global__ void __launch_bounds__(256)
-k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
+k_dtmax(Grid g, const double *__restrict__ U, const double *__restrict__ bz_up, StepParams *P, BoundGrid bg)
 {
     const int nrows = g.n[1] * g.n[2];
     const long long sa = g.sa;
     const double *__restrict__ b = U + S_B * sa;
     const double gm1 = g.gamma - 1.0;
-    double smax = 0.0, published = 0.0, seen = 0.0;
-    int nrow = 0;
+    double smax = 0.0, published = 0.0, seen = 0.0;      // published, seen: uniform across the warp
+    int nrow = 0;                                        // rows this block has visited
     int bad = 0;
     for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
         const int k = row / g.n[1], j = row - k * g.n[1];
+        // the global running maximum is re-read on each of a block's first eight visited rows, while it is
+        // still rising fast, then every eighth row
+        if (nrow < 8 || (nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
+        if (bg.b) {                                                              // filter 0 (warp uniform)
+            const double bound = __longlong_as_double((long long)bg.b[(long long)(k / bg.bk) * bg.nbj + j / bg.bj]);
+            if (bound < fmax(seen, published)) continue;
+        }
         const long long r0 = g.at(0, j, k);
         const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
-        const long long upk = g.act[2] ? g.at(0, j, k + 1 == g.n[2] ? 0 : k + 1) - r0 : 0;
-        // the global running maximum is re-read (and the warp's own published) on each of a block's first
-        // eight rows, while it is still rising fast, then every eighth row
-        if (nrow < 8 || (nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
-        double thr = fmax(smax, seen);
+        const bool top = g.act[2] && k + 1 == g.n[2];
+        const double *__restrict__ bzu = top ? bz_up + g.at(0, j, 0) : b + 2 * sa + r0 + g.st[2];
+        double thr = fmax(smax, fmax(seen, published));
         for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
             const long long c = r0 + i;
             const double rho = U[c], mx = U[sa + c], my = U[2 * sa + c], mz = U[3 * sa + c], E = U[4 * sa + c];
             // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
             const double B[3] = { 0.5 * (b[c] + b[r0 + (i + 1 == g.n[0] ? 0 : i + 1)]),
                                   0.5 * (b[sa + c] + b[sa + c + upj]),
-                                  g.act[2] ? 0.5 * (b[2 * sa + c] + b[2 * sa + c + upk]) : b[2 * sa + c] };
+                                  g.act[2] ? 0.5 * (b[2 * sa + c] + bzu[i]) : b[2 * sa + c] };
             const double ir = rcp_nr(rho);
             const double B2 = fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2]));
             const double vx = mx * ir, vy = my * ir, vz = mz * ir;
@@ -123,15 +133,20 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P)
             if (sig > thr) thr = sig;
         }
         // publish the warp's maximum when it raises the global one (rare after the first rows)
-        if (nrow < 8 || (nrow & 7) == 7 || row + (int)gridDim.x >= nrows) {
+        if (nrow < 8 || (nrow & 7) == 7) {
             double wm = smax;
             for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
-            if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published)) {
+            if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published))
                 atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
-                published = wm;
-            }
+            published = fmax(published, wm);
         }
         nrow++;
+    }
+    {
+        double wm = smax;
+        for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
+        if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published))
+            atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
     }
     if (bad) P->err = 1;
 }
@@ -149,9 +164,9 @@ __global__ void k_dtfinish(Grid g, StepParams *P, int mode)
 
 __global__ void k_advance_time(StepParams *P) { P->time += P->dt; }
 
-void launch_dtmax(const Grid &g, const double *U, StepParams *P, int nblocks, cudaStream_t s)
+void launch_dtmax(const Grid &g, const double *U, const double *bz_up, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s)
 {
-    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, P);
+    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, bz_up, P, bg);
 }
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s)
 {

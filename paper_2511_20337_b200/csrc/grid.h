@@ -45,6 +45,14 @@ struct StepParams {
     int pad;
 };
 
+// Coarse grid of CFL upper bounds left by the kernel that writes the final hydro variables of a step
+// (kernels.cuh "CFL pre-filter"), read by the exact reduction (dt_kernel.cu): cell (j / bj, k / bk).
+struct BoundGrid {
+    unsigned long long *b;      // IEEE bit patterns of non-negative doubles; nullptr: none
+    int bj, bk, nbj;            // nbj cells per plane row
+    double cfac;                // max(gamma (gamma - 1), 2)
+};
+
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
 // Fill the layout part of a Grid.  Returns false for sizes this library does not take.
@@ -76,8 +84,9 @@ enum StateVar { S_RHO = 0, S_MX = 1, S_MY = 2, S_MZ = 3, S_EN = 4, S_B = 5, S_CO
 enum ArrayId {
     A_SA = 0,        // 8: state S^n (and S^{n+1})
     A_SB = 8,        // 8: stage state S^1
-    A_SC = 16,       // 8: stage state S^2 (SSP-RK3 only)
-    A_CT = 24,       // 12: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3); staging outside a step
+    A_CT = 16,       // 12: CT work arrays (kernels.cuh: CT_FEM 6, CT_W 3, CT_EC 3); staging outside a step
+    A_SC = 28,       // 8: stage state S^2 (SSP-RK3 only: allocated when the integrator asks for it)
+    A_COUNT_RK2 = 28,
     A_COUNT = 36
 };
 

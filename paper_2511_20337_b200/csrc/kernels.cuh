@@ -69,15 +69,36 @@ __device__ __forceinline__ void tma_bulk_g2s(void *dst, const void *src, unsigne
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// ---------------------------------------------------------------- periodic ghost fill (a1)
+// ---------------------------------------------------------------- ghost fill (a1)
+// Where the z-ghost planes of a state come from.  A periodic single domain is its own neighbour on
+// both sides (lo = hi = the state itself).  In a z-slab decomposition (Fig. 4) lo / hi
+// are the same state of the slab below / above -- in this process or, peer-mapped, on another GPU: the
+// ghost kernel PULLS the planes it needs straight out of the neighbour's interior (no pack / unpack
+// buffers).  x and y stay periodic inside every slab.  All slabs share nx, ny and the ghost count, so
+// the in-plane strides agree; the plane count and the array stride may differ.
+struct ZSrc {
+    const double *lo, *hi;      // array 0 of the neighbour states
+    long long lo_sa, hi_sa;     // elements per array there
+    int lo_n2, hi_n2;           // interior planes there
+};
+
+// source of z-ghost plane k (k < 0 or k >= n2) of array a: pointer to the start of the neighbour's
+// array and the interior plane index there (modular: a domain thinner than the ghost depth wraps twice)
+__device__ __forceinline__ const double *zsrc_plane(const Grid &g, const ZSrc &z, int a, int k, int &sk)
+{
+    if (k < 0) { sk = ((k % z.lo_n2) + z.lo_n2) % z.lo_n2; return z.lo + (long long)a * z.lo_sa; }
+    sk = (k - g.n[2]) % z.hi_n2;
+    return z.hi + (long long)a * z.hi_sa;
+}
+
 // Every ghost position (index g in [-ng, 0) or [n, n+ng] along at least one active axis; cells and
 // faces alike, face n duplicates face 0) receives the value of its periodic image in the interior:
-// index g -> g + n or g - n along every axis at once.  Edges and corners therefore come out right in
-// ONE launch (the paper exchanges with diagonal neighbours for the same reason), and
-// sources are never written, so there is no ordering between positions.  The ghost set is walked as
-// three slab families: z-ghost planes (full padded rows), y-ghost rows of interior planes, x-ghost
-// ends of interior rows.
-__global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base, int narr)
+// index g -> g + n or g - n along every axis at once (along z: the image lies in the neighbour slab).
+// Edges and corners therefore come out right in ONE launch (the paper exchanges with diagonal
+// neighbours for the same reason), and sources are never written, so there is no
+// ordering between positions.  The ghost set is walked as three slab families: z-ghost planes (full
+// padded rows), y-ghost rows of interior planes, x-ghost ends of interior rows.
+__global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base, int narr, ZSrc zs)
 {
     const int ng = g.ng, ngh = 2 * ng + 1;
     const int gi = g.n[0] + ngh;                          // x positions -ng .. n+ng
@@ -111,10 +132,20 @@ __global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base
             k = (int)(r / g.n[1]);
         }
         // (extents may be as small as ng, so index n+ng can need two periods)
-        const int si = (i + 2 * g.n[0]) % g.n[0], sj = (j + 2 * g.n[1]) % g.n[1], sk = (k + 2 * g.n[2]) % g.n[2];
-        const long long dst = g.at(i, j, k), src = g.at(si, sj, sk);
+        const int si = (i + 2 * g.n[0]) % g.n[0], sj = (j + 2 * g.n[1]) % g.n[1];
+        const long long dst = g.at(i, j, k);
+        if (t < nZ) {
+            int sk;
 #pragma unroll 8
-        for (int a = 0; a < narr; a++) base[a * g.sa + dst] = base[a * g.sa + src];
+            for (int a = 0; a < narr; a++) {
+                const double *src = zsrc_plane(g, zs, a, k, sk);
+                base[a * g.sa + dst] = src[g.at(si, sj, sk)];
+            }
+        } else {
+            const long long src = g.at(si, sj, k);
+#pragma unroll 8
+            for (int a = 0; a < narr; a++) base[a * g.sa + dst] = base[a * g.sa + src];
+        }
     }
 }
 
@@ -122,25 +153,29 @@ __global__ void __launch_bounds__(256) k_ghost(Grid g, double *__restrict__ base
 // except the x-face n0, which the CT kernel writes together with face 0.  grid.x = ghost row, grid.y =
 // array.  The rows are walked as: the ghost planes (every padded row j of planes -ng..-1, n2..n2+ng), then
 // the ghost rows of the interior planes.  A row is copied over the padded x range [-ng, n0+ng].
-__global__ void __launch_bounds__(128) k_ghost_yz(Grid g, double *__restrict__ base)
+__global__ void __launch_bounds__(128) k_ghost_yz(Grid g, double *__restrict__ base, ZSrc zs)
 {
     const int ng = g.ng, ngh = 2 * ng + 1;
     const int rows_z = g.act[2] ? ngh * (g.n[1] + ngh) : 0;
     int r = blockIdx.x, j, k;
+    double *arr = base + (long long)blockIdx.y * g.sa;
+    const double *srcarr = arr;
+    int sk;
     if (r < rows_z) {
         const int pz = r / (g.n[1] + ngh);
         j = r - pz * (g.n[1] + ngh) - ng;
         k = pz < ng ? pz - ng : g.n[2] + (pz - ng);
+        srcarr = zsrc_plane(g, zs, blockIdx.y, k, sk);
     } else {
         r -= rows_z;
         k = r / ngh;
         const int py = r - k * ngh;
         j = py < ng ? py - ng : g.n[1] + (py - ng);
+        sk = k;
     }
-    const int sj = (j + 2 * g.n[1]) % g.n[1], sk = (k + 2 * g.n[2]) % g.n[2];
-    double *arr = base + (long long)blockIdx.y * g.sa;
+    const int sj = (j + 2 * g.n[1]) % g.n[1];
     double *dst = arr + g.at(-ng, j, k);
-    const double *src = arr + g.at(-ng, sj, sk);
+    const double *src = srcarr + g.at(-ng, sj, sk);
     for (int e = threadIdx.x; e < g.n[0] + ngh; e += blockDim.x) dst[e] = src[e];
 }
 
@@ -165,6 +200,32 @@ __device__ __forceinline__ void cell_b(const Grid &g, const double *__restrict__
     B[2] = TWO_D ? b[2 * g.sa + c] : 0.5 * (b[2 * g.sa + c] + b[2 * g.sa + c + g.st[2]]);
 }
 
+// ---------------------------------------------------------------- CFL pre-filter written by the last stage (a8)
+// The kernel that writes the final hydro variables of a step also leaves, per cell of a coarse "bound
+// grid" (one cell = the part of a row-march segment a thread covers: bj rows x bk planes), an UPPER BOUND
+// of every CFL candidate (|v_d| + c_f,d)/dx_d of the zones in it.  The exact reduction of the next step
+// (dt_kernel.cu) then only visits rows whose bound can still hold the maximum; the dt stays bit-exact
+// because a skipped row provably cannot raise it.  The bound needs no magnetic field (the final faces are
+// written later by the CT kernel):  c_f,d^2 <= (gamma p + B^2)/rho  and, with p >= 0,
+// B^2 <= 2 (E - K), K = |m|^2/(2 rho), so  gamma p + B^2 <= max(gamma (gamma-1), 2) (E - K).
+__device__ __forceinline__ double sigma_bound(const Grid &g, double cfac, double rho, double mx, double my, double mz, double En)
+{
+    const double ir = rcp_fast(rho);
+    const double eint = En - 0.5 * ir * fma(mx, mx, fma(my, my, mz * mz));
+    if (unphysical(rho) || unphysical(eint)) return __longlong_as_double(0x7fe0000000000000ll);   // visit it
+    const double cs = sqrt_fast(cfac * eint * ir);
+    double b = 0.0;
+    if (g.act[0]) b = fmax(b, fma(fabs(mx), ir, cs) * g.idx[0]);
+    if (g.act[1]) b = fmax(b, fma(fabs(my), ir, cs) * g.idx[1]);
+    if (g.act[2]) b = fmax(b, fma(fabs(mz), ir, cs) * g.idx[2]);
+    return b * (1.0 + 1e-9);
+}
+
+__device__ __forceinline__ void bound_publish(const BoundGrid &bg, int j, int k, double b)
+{
+    atomicMax(bg.b + (long long)(k / bg.bk) * bg.nbj + j / bg.bj, (unsigned long long)__double_as_longlong(b));
+}
+
 // ---------------------------------------------------------------- x sweep (a2-a5 fused)
 // The rows of the grid are laid end to end as one list of "items" (cells -2 .. nx+1 of each row).
 // A block takes NT consecutive items: every thread loads its cell and converts it to primitives in
@@ -187,7 +248,9 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     constexpr int H = sx_halo(LIM);
     const int nx = g.n[0], M = nx + 2 * H;
     const long long sa = g.sa;
-    const long long nitems = (long long)M * g.n[1] * g.n[2];
+    // 3D: planes -1 .. nz -- the CT kernel reads the x-face data one plane beyond the interior (no z wrap)
+    const int nzp = TWO_D ? 1 : g.n[2] + 2, kz0 = TWO_D ? 0 : -1;
+    const long long nitems = (long long)M * g.n[1] * nzp;
     const long long item = (long long)blockIdx.x * sx_out(LIM) - H + t;
     const bool valid = item >= 0 && item < nitems;
     int f = -100;
@@ -199,7 +262,7 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     if (valid) {
         long long row = item / M;
         f = (int)(item - row * M) - H;
-        int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]);
+        int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]) + kz0;
         c = g.at(f, j, k);
         rho = Sin[c]; mx = Sin[sa + c]; my = Sin[2 * sa + c]; mz = Sin[3 * sa + c];
         En = Sin[4 * sa + c];
@@ -332,13 +395,11 @@ constexpr int MARCH_PF = 16;     // doubles per thread and iteration: U(s+1) 5, 
 
 // three blocks of 128 threads per SM: 168 registers per thread hold the running state without
 // spilling (measured: 4 blocks at 128 registers spill ~40 values per interface and run 20% slower)
-#ifndef MARCH_MINB
-#define MARCH_MINB 3
-#endif
+constexpr int MARCH_MINB = 3;
 template <int DIR, int LIM, bool TWO_D>
 __global__ void __launch_bounds__(MARCH_NT, MARCH_MINB)
 k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-              double scale, int seglen)
+              double scale, int seglen, int tr0, BoundGrid bg)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
@@ -348,9 +409,14 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     if (i >= g.n[0]) return;
     // DIR = 1: grid.y = segment, grid.z = k;   DIR = 2: grid.y = j, grid.z = segment
     const int seg = DIR == 1 ? blockIdx.y : blockIdx.z;
-    const int tr = DIR == 1 ? blockIdx.z : blockIdx.y;
+    // transverse index; the y sweep of a 3D run also covers planes -1 and nz (tr0 = -1): the CT kernel
+    // reads the y-face data one plane beyond the interior (no z wrap)
+    const int tr = (DIR == 1 ? blockIdx.z : blockIdx.y) + tr0;
     const int s0 = seg * seglen;
     const int s1 = min(s0 + seglen, g.n[DIR]);
+    // the z sweep also leaves the CT data of the upper boundary face n (a periodic single domain gets
+    // the same bits as on face 0; a z slab gets the face it shares with the slab above)
+    const int sct = (DIR == 2 && s1 == g.n[2]) ? s1 + 1 : s1;
     const long long sa = g.sa, st = g.st[DIR];
     long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
     const double gamma = g.gamma, igm1 = g.igm1;
@@ -360,6 +426,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     const double *__restrict__ b2 = Sin + (S_B + T2) * sa;
     const long long st1 = g.st[T1], st2 = g.st[T2];
     bool bad, anybad = false;
+    double bmax = 0.0;                                   // dt bound of the zones this thread finishes (last stage)
 
     // what iteration s consumes: U of cell s+1 and the faces around it, U' of cell s-1
     auto prefetch = [&](int slot, long long cs) {
@@ -436,14 +503,21 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
         bface = bnext; bnext = bup;
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
-            Sout[cm] = pf[slot][10][t] - fac * (F[0] - Fp[0]);
-            Sout[(1 + DIR) * sa + cm] = pf[slot][11][t] - fac * (F[1] - Fp[1]);
-            Sout[(1 + T1) * sa + cm] = pf[slot][12][t] - fac * (F[2] - Fp[2]);
-            Sout[(1 + T2) * sa + cm] = pf[slot][13][t] - fac * (F[3] - Fp[3]);
-            Sout[4 * sa + cm] = pf[slot][14][t] - fac * (F[6] - Fp[4]);
+            double m[3];
+            const double r0 = pf[slot][10][t] - fac * (F[0] - Fp[0]);
+            m[DIR] = pf[slot][11][t] - fac * (F[1] - Fp[1]);
+            m[T1] = pf[slot][12][t] - fac * (F[2] - Fp[2]);
+            m[T2] = pf[slot][13][t] - fac * (F[3] - Fp[3]);
+            const double r4 = pf[slot][14][t] - fac * (F[6] - Fp[4]);
+            Sout[cm] = r0;
+            Sout[(1 + DIR) * sa + cm] = m[DIR];
+            Sout[(1 + T1) * sa + cm] = m[T1];
+            Sout[(1 + T2) * sa + cm] = m[T2];
+            Sout[4 * sa + cm] = r4;
             if (BZ2D) Sout[7 * sa + cm] = pf[slot][15][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
+            if (bg.b) bmax = fmax(bmax, sigma_bound(g, bg.cfac, r0, m[0], m[1], m[2], r4));
         }
-        if (s < s1) {
+        if (s < sct) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;
@@ -465,6 +539,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     }
     if (s <= s1) iteration(0, s);
     if (anybad) P->err = 1;
+    if (bg.b) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, bmax);
 }
 
 // ---------------------------------------------------------------- y / z sweep with the five-cell WENO-Z stencil
@@ -477,7 +552,7 @@ constexpr int WZ_PF = 17;        // doubles per thread and iteration: U(s+3) 5, 
 template <int DIR, bool TWO_D>
 __global__ void __launch_bounds__(MARCH_NT, 3)
 k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-                 double scale, int seglen)
+                 double scale, int seglen, int tr0, BoundGrid bg)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
@@ -488,9 +563,10 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     const int i = blockIdx.x * blockDim.x + t;
     if (i >= g.n[0]) return;
     const int seg = DIR == 1 ? blockIdx.y : blockIdx.z;
-    const int tr = DIR == 1 ? blockIdx.z : blockIdx.y;
+    const int tr = (DIR == 1 ? blockIdx.z : blockIdx.y) + tr0;    // see k_sweep_march
     const int s0 = seg * seglen;
     const int s1 = min(s0 + seglen, g.n[DIR]);
+    const int sct = (DIR == 2 && s1 == g.n[2]) ? s1 + 1 : s1;     // CT data of the upper boundary face too
     const long long sa = g.sa, st = g.st[DIR];
     long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
     const double gamma = g.gamma, igm1 = g.igm1;
@@ -501,6 +577,7 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     const long long st1 = g.st[T1], st2 = g.st[T2];
     const int xdup = ct_xdup(i, g.n[0]);
     bool bad, anybad = false;
+    double bmax = 0.0;
     auto slot = [](int m) { return ((m % 5) + 5) % 5; };
 
     // what iteration s consumes: U of cell s+2 and the faces around it, U' of cell s-1 (cs = cell s)
@@ -577,14 +654,21 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
         for (int v = 0; v < 7; v++) qL[v] = qLn[v];
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
-            Sout[cm] = pf[ps][11][t] - fac * (F[0] - Fp[0]);
-            Sout[(1 + DIR) * sa + cm] = pf[ps][12][t] - fac * (F[1] - Fp[1]);
-            Sout[(1 + T1) * sa + cm] = pf[ps][13][t] - fac * (F[2] - Fp[2]);
-            Sout[(1 + T2) * sa + cm] = pf[ps][14][t] - fac * (F[3] - Fp[3]);
-            Sout[4 * sa + cm] = pf[ps][15][t] - fac * (F[6] - Fp[4]);
+            double m[3];
+            const double r0 = pf[ps][11][t] - fac * (F[0] - Fp[0]);
+            m[DIR] = pf[ps][12][t] - fac * (F[1] - Fp[1]);
+            m[T1] = pf[ps][13][t] - fac * (F[2] - Fp[2]);
+            m[T2] = pf[ps][14][t] - fac * (F[3] - Fp[3]);
+            const double r4 = pf[ps][15][t] - fac * (F[6] - Fp[4]);
+            Sout[cm] = r0;
+            Sout[(1 + DIR) * sa + cm] = m[DIR];
+            Sout[(1 + T1) * sa + cm] = m[T1];
+            Sout[(1 + T2) * sa + cm] = m[T2];
+            Sout[4 * sa + cm] = r4;
             if (BZ2D) Sout[7 * sa + cm] = pf[ps][16][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
+            if (bg.b) bmax = fmax(bmax, sigma_bound(g, bg.cfac, r0, m[0], m[1], m[2], r4));
         }
-        if (s < s1) {
+        if (s < sct) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;
@@ -597,6 +681,7 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
         Fp[0] = F[0]; Fp[1] = F[1]; Fp[2] = F[2]; Fp[3] = F[3]; Fp[4] = F[6]; Fp[5] = F[4];
     }
     if (anybad) P->err = 1;
+    if (bg.b) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, bmax);
 }
 constexpr int WZ_SMEM_BYTES = (5 * 7 + 2 * WZ_PF) * MARCH_NT * 8;
 
@@ -620,13 +705,11 @@ constexpr int XY_BXROW_PAD = 2;     // the b_x row of the arriving row holds NT 
 constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 32; }   // b_x row + three mbarriers behind the arrays
 
 // 128-thread blocks run three per SM at 168 registers (measured 17% faster than four at 128)
-#ifndef XY128_MINB
-#define XY128_MINB 3
-#endif
+constexpr int XY128_MINB = 3;
 template <int LIM, bool TWO_D, bool WRAP, int NT>
 __global__ void __launch_bounds__(NT, NT == 128 ? XY128_MINB : 512 / NT)
 k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-           Combine cb, int seglen)
+           Combine cb, int seglen, int kz0, BoundGrid bg)
 {
     extern __shared__ __align__(128) double xy_smem[];
     const int t = threadIdx.x;
@@ -650,7 +733,11 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const bool xface = WRAP || (has_slope && t >= 2 && i <= nx);
     const bool cell = WRAP || (xface && t <= NT - 3 && i < nx);     // this thread owns an interior cell
     const int xdup = cell ? ct_xdup(i, nx) : 0;
-    const int k = blockIdx.z;
+    // 3D: kz0 = -1 and the grid covers planes -1 .. nz: the CT kernel reads the x- and y-face data one plane
+    // beyond the interior (no z wrap: a z slab's neighbour planes are not its own); only the CT data of
+    // those two planes is kept, their hydro update is not stored
+    const int k = (int)blockIdx.z + kz0;
+    const bool kin = TWO_D || (k >= 0 && k < g.n[2]);
     const int s0 = blockIdx.y * seglen, s1 = min(s0 + seglen, g.n[1]);
     const long long sa = g.sa, st = g.st[1], stz = g.st[2];
     const double gamma = g.gamma;
@@ -662,6 +749,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const double *__restrict__ bz = Sin + (S_B + 2) * sa;
     long long c = g.at(valid ? i : 0, s0, k);                       // cell (i, s0, k)
     bool anybad = false;
+    double bmax = 0.0;
 
     // TMA row copies, issued by thread 0: the block's x range [i0, i0 + NT) of one row of each array
     const long long row0 = g.at(WRAP ? 0 : (int)blockIdx.x * (NT - 4) - 2, s0, k);    // first cell of row s0
@@ -856,7 +944,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             mbar_wait(bars + 2, (s - s0 - 1) & 1);   // all x fluxes of row s-1 are in shared memory
             mbar_wait(bars + 1, (s - s0 - 1) & 1);   // group F(s) has landed
         }
-        if (s > s0 && cell) {
+        if (s > s0 && cell && kin) {
             const long long cm = c - st;
             // S of row s-1 minus the x flux difference (own lower face, right neighbour's lower face)
             double r0v = pff[t] - dtdx * (sQ[tr] - sQ[t]);
@@ -872,15 +960,22 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             // y-rotated flux: (rho, m_y, m_z, m_x, B_z, B_x, E)
 #pragma unroll
             for (int n = 0; n < NFPS; n++) Fpy[n] = *fpy[n];
-            Sout[cm] = r0v - facy * (Fy[0] - Fpy[0]);
-            Sout[2 * sa + cm] = r2v - facy * (Fy[1] - Fpy[1]);
-            Sout[3 * sa + cm] = r3v - facy * (Fy[2] - Fpy[2]);
-            Sout[sa + cm] = r1v - facy * (Fy[3] - Fpy[3]);
-            Sout[4 * sa + cm] = r4v - facy * (Fy[6] - Fpy[4]);
+            r0v -= facy * (Fy[0] - Fpy[0]);
+            r2v -= facy * (Fy[1] - Fpy[1]);
+            r3v -= facy * (Fy[2] - Fpy[2]);
+            r1v -= facy * (Fy[3] - Fpy[3]);
+            r4v -= facy * (Fy[6] - Fpy[4]);
+            Sout[cm] = r0v;
+            Sout[2 * sa + cm] = r2v;
+            Sout[3 * sa + cm] = r3v;
+            Sout[sa + cm] = r1v;
+            Sout[4 * sa + cm] = r4v;
             if (TWO_D) {
                 double r7v = rm[6 * NT] - dtdx * (sQ[5 * NT + tr] - sQ[5 * NT + t]);
                 if (combine) r7v = fma(cb.wn, pff[10 * NT + t], cb.ws * r7v);
                 Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
+                // 2D: this kernel writes the final hydro variables of the step
+                if (bg.b) bmax = fmax(bmax, sigma_bound(g, bg.cfac, r0v, r1v, r2v, r3v, r4v));
             }
         }
         if (cell && s < s1) {
@@ -901,7 +996,8 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         bface = bnext; bnext = byu;
         double *rt = rm; rm = r0; r0 = rn; rn = rt;
     }
-    if (anybad) P->err = 1;
+    if (anybad && kin) P->err = 1;
+    if (TWO_D && bg.b && cell) bound_publish(bg, s0, 0, bmax);
 }
 
 // ---------------------------------------------------------------- CT (a6, R6) [+ RK2 combine of the faces (a7)]
@@ -923,7 +1019,8 @@ __device__ __forceinline__ double edge_emf(double Ea_lo, double Ea_hi, double Eb
     return 0.25 * (((Ea_lo + Ea_hi) + (Eb_lo + Eb_hi)) + ((t1 - t2) + (t3 - t4)));
 }
 
-// Block = CT_TX x CT_TY columns marching along z over `seglen` planes.  Iteration k forms
+// Block = CT_TX x CT_TY columns marching along z over `seglen` planes (k = k0 .. k1; the CT data of
+// planes k0 - 1 and k1 is read too: -1 and nz lie in the ghost planes, written by the sweeps).  Iteration k forms
 // E_z(i-1/2, j-1/2, k) and, from plane k and the plane k-1 values kept in registers, E_x(i, j-1/2, k-1/2)
 // and E_y(i-1/2, j, k-1/2): 12 loads of the thread's own cell (HBM; prefetched into L2 one plane
 // ahead) and 13 of its x-1 / y-1 neighbours (L1 hits: the neighbour thread loads the same words).
@@ -958,14 +1055,15 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
     const long long rm = (long long)(jm + g.off[1]) * g.st[1] + g.off[0];
     const long long oc = r0 + ii;                                      // own cell, in-plane offset
     const int XM = (int)(r0 + im - oc), YM = (int)(rm + ii - oc), XYM = (int)(rm + im - oc);   // neighbours
-    auto plane = [&](int k) { return (long long)((k == g.n[2] ? 0 : k) + g.off[2]) * st2; };
+    // no z wrap: the sweeps leave the CT data of planes -1 and nz (and of the z face nz) as well
+    auto plane = [&](int k) { return (long long)(k + g.off[2]) * st2; };
     // the CT arrays: F_x[By] 0, F_x[Bz] 1, F_y[Bz] 2, F_y[Bx] 3, F_z[Bx] 4, F_z[By] 5, w_x 6, w_y 7, w_z 8, E^c 9-11
     const double *__restrict__ A0 = ct + oc;
 
     // plane k-1 values that enter E_x, E_y at k - 1/2
     double fyz = 0, wyP = 0, excP = 0, excPm = 0, fxz = 0, wxP = 0, eycP = 0, eycPm = 0;
     if (!TWO_D) {
-        const double *q = A0 + plane(wrap_m1(k0, g.n[2]));
+        const double *q = A0 + plane(k0 - 1);
         fyz = q[2 * sa];  wyP = q[7 * sa];
         excP = q[9 * sa]; excPm = q[9 * sa + YM];
         fxz = q[1 * sa];  wxP = q[6 * sa];
@@ -1054,33 +1152,40 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
 }
 
 // ---------------------------------------------------------------- API layout <-> padded layout
-// The caller's interior-only array (extent m[] = n[] + face bump) <-> padded array.
-__global__ void k_unpack(Grid g, Box box, const double *__restrict__ src, int m0, int m1, double *__restrict__ dst)
+// The caller's interior-only array (extent m0 x m1 x ..., planes counted from the first plane this
+// process holds) <-> the padded array of one slab; kofs = the slab's first plane in the caller's array.
+__global__ void k_unpack(Grid g, Box box, const double *__restrict__ src, int m0, int m1, int kofs, double *__restrict__ dst)
 {
     int i, j, k;
     if (!thread_zone(box, i, j, k)) return;
-    dst[g.at(i, j, k)] = src[((long long)k * m1 + j) * m0 + i];
+    dst[g.at(i, j, k)] = src[((long long)(k + kofs) * m1 + j) * m0 + i];
 }
 
-__global__ void k_pack(Grid g, Box box, const double *__restrict__ src, int m0, int m1, double *__restrict__ dst)
+// sk0 >= 0: every plane of the box is read from plane sk0 of src (the duplicate upper z face of the
+// box comes from plane 0 of the slab above / of the periodic image)
+__global__ void k_pack(Grid g, Box box, const double *__restrict__ src, int m0, int m1, int kofs, int sk0, double *__restrict__ dst)
 {
     int i, j, k;
     if (!thread_zone(box, i, j, k)) return;
-    // periodic wrap: the duplicate upper face (index n) is face 0
-    int ii = i % g.n[0], jj = j % g.n[1], kk = k % g.n[2];
-    dst[((long long)k * m1 + j) * m0 + i] = src[g.at(ii, jj, kk)];
+    // periodic wrap in x and y: the duplicate upper face (index n) is face 0
+    int ii = i % g.n[0], jj = j % g.n[1];
+    dst[((long long)(k + kofs) * m1 + j) * m0 + i] = src[g.at(ii, jj, sk0 >= 0 ? sk0 : k)];
 }
 
-// cell-centred B of the API's U[4..6]: the mean of the two faces (R7); 2D: U[6] is the stored B_z
-__global__ void k_pack_cellb(Grid g, Box box, const double *__restrict__ b, double *__restrict__ dst, long long n)
+// cell-centred B of the API's U[4..6]: the mean of the two faces (R7); 2D: U[6] is the stored B_z.
+// bz_up: the b_z array whose plane 0 is the upper face of this slab's last plane (the slab above; the
+// array itself in a periodic single domain).  n = zones of the caller's array, kofs as above.
+__global__ void k_pack_cellb(Grid g, Box box, const double *__restrict__ b, const double *__restrict__ bz_up,
+                             double *__restrict__ dst, long long n, int kofs)
 {
     int i, j, k;
     if (!thread_zone(box, i, j, k)) return;
     const long long sa = g.sa, c = g.at(i, j, k);
-    const long long o = ((long long)k * g.n[1] + j) * g.n[0] + i;
+    const long long o = ((long long)(k + kofs) * g.n[1] + j) * g.n[0] + i;
     dst[o] = 0.5 * (b[c] + b[g.at(wrap_p1(i, g.n[0]), j, k)]);
     dst[n + o] = 0.5 * (b[sa + c] + b[sa + g.at(i, wrap_p1(j, g.n[1]), k)]);
-    dst[2 * n + o] = g.act[2] ? 0.5 * (b[2 * sa + c] + b[2 * sa + g.at(i, j, wrap_p1(k, g.n[2]))]) : b[2 * sa + c];
+    if (!g.act[2]) dst[2 * n + o] = b[2 * sa + c];
+    else dst[2 * n + o] = 0.5 * (b[2 * sa + c] + (k + 1 < g.n[2] ? b[2 * sa + c + g.st[2]] : bz_up[g.at(i, j, 0)]));
 }
 
 } // namespace pluto

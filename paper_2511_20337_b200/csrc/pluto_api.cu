@@ -1,5 +1,10 @@
 // pluto_api.cu -- the C-ABI of include/pluto.h: context, memory, host<->device copies, and the
-// launch sequence of one RK2 step.  No CPU fallback: without a device every call fails loudly.
+// launch sequence of one Runge-Kutta step.  No CPU fallback: without a device every call fails loudly.
+//
+// The box is held as one or more z-slabs ("domains", section 3.4): a periodic single
+// domain is the special case of one slab that is its own neighbour.  Every kernel works on one slab; the
+// only places where slabs meet are the ghost fill (z-ghost planes are pulled out of the neighbour slab's
+// interior, in this process or peer-mapped from another GPU) and the single max that fixes dt.
 #include "../../include/pluto.h"
 #include "kernels.cuh"
 #include "ct_tma.cuh"
@@ -11,7 +16,7 @@
 #include <vector>
 
 namespace pluto {
-void launch_dtmax(const Grid &g, const double *U, StepParams *P, int nblocks, cudaStream_t s);
+void launch_dtmax(const Grid &g, const double *U, const double *bz_up, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s);
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s);
 void launch_advance_time(StepParams *P, cudaStream_t s);
 double probe_fp64_gflops(cudaStream_t s);
@@ -25,25 +30,48 @@ enum KernelId { K_GHOST = 0, K_FLUX_XY, K_FLUX_X, K_FLUX_Y, K_FLUX_Z, K_CT, K_DT
 const char *const kKernelNames[K_COUNT] = { "ghost_fill", "sweep_xy", "sweep_x", "sweep_y", "sweep_z", "ct",
                                             "dt_max", "scalars", "pack_unpack", "ct_halo" };
 
+// where a neighbour slab's arrays live (this process or a peer-mapped allocation)
+struct Peer {
+    double *base = nullptr;     // array 0 of the neighbour's allocation (same array order)
+    double *sc = nullptr;       // its S^2 arrays (RK3), if it keeps them outside `base`
+    long long sa = 0;
+    int n2 = 0;
+    void *ipc_mapping = nullptr;    // cudaIpcOpenMemHandle result to close, if any
+    unsigned char ipc_handle[64] = {};
+};
+
+struct Domain {
+    Grid g{};
+    int kz0 = 0;                     // first plane of the slab inside this process's part of the box
+    double *base = nullptr;          // A_COUNT_RK2 (or A_COUNT) arrays, then the scalars / bound grid of slab 0
+    double *sc = nullptr;            // S^2 (8 arrays) when it was allocated after pluto_init
+    bool own_mem = false, own_sc = false;
+    int narrays = A_COUNT_RK2;
+    unsigned long long *bound = nullptr;     // dt bound grid: n1 * n2 cells at most
+    CUtensorMap ct_map{};
+    Peer nb[2];                      // [0] the slab below, [1] the slab above
+};
+
 struct Context {
     bool init = false;
     bool have_state = false;
     bool stepped = false;
-    Grid g{};
-    double *base = nullptr;          // A_COUNT arrays
-    StepParams *P = nullptr;         // device scalars (inside the allocation)
-    bool own_mem = false;
+    std::vector<Domain> dom;
+    int nslab = 1, first = 0;        // slabs of the whole box / first slab held here
+    int nzg = 1;                     // planes of the whole box
+    int nzloc = 1;                   // planes this process holds
+    StepParams *P = nullptr;         // device scalars (inside slab 0's allocation), shared by the slabs here
     void *ws = nullptr;              // registered workspace
     size_t ws_bytes = 0;
     cudaStream_t stream = nullptr;   // stream in use (the caller's, or own_stream)
     cudaStream_t own_stream = nullptr;
+    int own_stream_dev = -1;
     long long launches = 0;
     long long per_step[2] = { 0, 0 };
     int use_graph = 1;
     int fuse_xy = 1;
     int ct_tma = 1;
     int rk_order = 2;                // 2: SSP-RK2 (R3), 3: SSP-RK3 (Eq. 5)
-    CUtensorMap ct_map{};            // the twelve CT arrays as one 4D tensor (x, y, z, array)
     cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step (of the current rk_order)
     int sm_count = 148;
     char err[512] = "";
@@ -54,6 +82,7 @@ struct Context {
     size_t prof_used = 0;
     double prof_ms[K_COUNT] = {};
     long long prof_cnt[K_COUNT] = {};
+    bool whole() const { return (int)dom.size() == nslab; }     // every slab of the box is in this process
 };
 
 Context C;
@@ -105,9 +134,35 @@ struct Launch {
 };
 #define LAUNCH(kid, ...) do { Launch l_(kid); __VA_ARGS__; } while (0)
 
-double *arr(int id) { return C.base + (long long)id * C.g.sa; }
+double *arr(const Domain &d, int id)
+{
+    if (id >= A_SC && d.sc) return d.sc + (long long)(id - A_SC) * d.g.sa;
+    return d.base + (long long)id * d.g.sa;
+}
 
-size_t layout_bytes(const Grid &g) { return (size_t)A_COUNT * g.sa * sizeof(double) + 256; }
+// the same array of a neighbour slab
+double *peer_arr(const Peer &p, int id)
+{
+    if (id >= A_SC && p.sc) return p.sc + (long long)(id - A_SC) * p.sa;
+    return p.base + (long long)id * p.sa;
+}
+
+ZSrc zsrc(const Domain &d, int state)
+{
+    ZSrc z;
+    z.lo = peer_arr(d.nb[0], state); z.hi = peer_arr(d.nb[1], state);
+    z.lo_sa = d.nb[0].sa; z.hi_sa = d.nb[1].sa;
+    z.lo_n2 = d.nb[0].n2; z.hi_n2 = d.nb[1].n2;
+    return z;
+}
+
+size_t bound_cells(const Grid &g) { return (size_t)g.n[1] * g.n[2]; }
+
+// bytes of one slab: the arrays, then 256 bytes of scalars and the dt bound grid
+size_t layout_bytes(const Grid &g, int narrays)
+{
+    return (size_t)narrays * g.sa * sizeof(double) + 256 + round_up((long long)bound_cells(g) * 8, 256);
+}
 
 dim3 grid_for(const Box &b, int bx = 128)
 {
@@ -134,9 +189,17 @@ void destroy_graphs()
         if (gr) { cudaGraphExecDestroy(gr); gr = nullptr; }
 }
 
+// planes of slab s when nz planes are cut into nslab slabs (the first nz % nslab slabs get one more)
+void slab_range(int nz, int nslab, int s, int &k0, int &n)
+{
+    const int q = nz / nslab, r = nz % nslab;
+    n = q + (s < r ? 1 : 0);
+    k0 = s * q + (s < r ? s : r);
+}
+
 // TMA descriptor of the CT work arrays: dims (pitch, tot1, tot2, CT_COUNT) doubles, box = one tile of
 // one array.  cuTensorMapEncodeTiled is taken from the driver through the runtime (no -lcuda).
-int make_ct_map()
+int make_ct_map(Domain &d)
 {
     typedef CUresult (*EncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -149,11 +212,11 @@ int make_ct_map()
             return fail(PLUTO_ECUDA, "cuTensorMapEncodeTiled not available from the driver");
         encode = (EncodeFn)fn;
     }
-    const Grid &g = C.g;
+    const Grid &g = d.g;
     cuuint64_t dims[4] = { (cuuint64_t)g.tot[0], (cuuint64_t)g.tot[1], (cuuint64_t)g.tot[2], (cuuint64_t)CT_COUNT };
     cuuint64_t strides[3] = { (cuuint64_t)g.st[1] * 8, (cuuint64_t)g.st[2] * 8, (cuuint64_t)g.sa * 8 };
     cuuint32_t box[4] = { CTM_COLS, CTM_ROWS, 1, 1 }, estr[4] = { 1, 1, 1, 1 };
-    CUresult r = encode(&C.ct_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, arr(A_CT), dims, strides, box, estr,
+    CUresult r = encode(&d.ct_map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, arr(d, A_CT), dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(PLUTO_ECUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
@@ -162,20 +225,21 @@ int make_ct_map()
 
 // ---------------------------------------------------------------- launch sequences
 
-// ghost layers of the 8 arrays of one state, one launch
-// widths for which the fused x+y sweep spans a whole periodic row: no kernel then reads an x ghost
-// other than the x-face n0 (kept equal to face 0 by the CT kernel)
+// The fused x+y sweep spans a whole periodic row when nx is one of the instantiated block widths: no
+// kernel then reads an x ghost other than the x-face n0 (kept equal to face 0 by the CT kernel).
 bool row_wraps(int nx) { return nx == 64 || nx == 128 || nx == 256 || nx == 512; }
 
-void fill_ghosts(double *state, bool all = false)
+// ghost layers of the 8 arrays of one state of one slab, one launch (z planes from the neighbour slabs)
+void fill_ghosts(const Domain &d, int state, bool all = false)
 {
-    const Grid &g = C.g;
+    const Grid &g = d.g;
+    const ZSrc zs = zsrc(d, state);
     if (!all && C.fuse_xy && g.limiter != 2 && row_wraps(g.n[0])) {
         const int ngh = 2 * g.ng + 1;
         const int rows = (g.act[2] ? ngh * (g.n[1] + ngh) : 0) + g.n[2] * ngh;
-        LAUNCH(K_GHOST, k_ghost_yz<<<dim3(rows, S_COUNT), 128, 0, C.stream>>>(g, state));
+        LAUNCH(K_GHOST, k_ghost_yz<<<dim3(rows, S_COUNT), 128, 0, C.stream>>>(g, arr(d, state), zs));
     } else {
-        LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 8, 256, 0, C.stream>>>(g, state, S_COUNT));
+        LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 8, 256, 0, C.stream>>>(g, arr(d, state), S_COUNT, zs));
     }
 }
 
@@ -197,13 +261,38 @@ int march_seglen(int n, long long columns)
     return len;
 }
 
-template <int LIM, bool TWO_D>
-void launch_sweeps(const double *Sin, double *Sout, Combine cb)
+// The sweep that writes the final hydro variables of a stage is the z sweep (3D) or the y part of the
+// x+y sweep (2D); in the last stage of a step it also fills the dt bound grid (kernels.cuh sigma_bound).
+BoundGrid bound_grid(const Domain &d, bool last, int bj, int bk)
 {
-    const Grid &g = C.g;
+    BoundGrid bg;
+    bg.b = last ? d.bound : nullptr;
+    bg.bj = bj; bg.bk = bk; bg.nbj = (d.g.n[1] + bj - 1) / bj;
+    bg.cfac = fmax(d.g.gamma * (d.g.gamma - 1.0), 2.0);
+    return bg;
+}
+
+// segment lengths of the marching sweeps (functions of the slab alone: the dt kernel must find the bound
+// grid in the shape the last stage of the previous step wrote it, whatever path wrote it)
+int seglen_y(const Grid &g) { return march_seglen(g.n[1], (long long)g.n[0] * g.n[2]); }
+int seglen_z(const Grid &g) { return march_seglen(g.n[2], (long long)g.n[0] * g.n[1]); }
+
+// the bound grid of the slab: one cell per (row, z segment) in 3D, per y segment in 2D
+BoundGrid final_bound_grid(const Domain &d, bool last)
+{
+    return d.g.act[2] ? bound_grid(d, last, 1, seglen_z(d.g)) : bound_grid(d, last, seglen_y(d.g), 1);
+}
+
+template <int LIM, bool TWO_D>
+void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb, bool last)
+{
+    const Grid &g = d.g;
     cudaStream_t s = C.stream;
-    double *ct = arr(A_CT);
+    double *ct = arr(d, A_CT);
     const double scale = cb.Sn ? cb.ws : 1.0;
+    const int kz0 = TWO_D ? 0 : -1;                      // 3D: the x and y sweeps cover planes -1 .. nz
+    const int nplanes = TWO_D ? 1 : g.n[2] + 2;
+    const BoundGrid none = bound_grid(d, false, 1, 1);
     bool fused = false;
     if constexpr (LIM != 2) if (C.fuse_xy) {
         fused = true;
@@ -214,66 +303,61 @@ void launch_sweeps(const double *Sin, double *Sout, Combine cb)
         const bool wrap = row_wraps(nx);
         const int nt = wrap ? nx : (nx > 124 ? 256 : 128);
         const int chunks = wrap ? 1 : (nx + nt - 5) / (nt - 4);
-        const int len = march_seglen(g.n[1], (long long)nx * g.n[2]);
-        dim3 grid(chunks, (g.n[1] + len - 1) / len, g.n[2]);
+        const int len = seglen_y(g);
+        dim3 grid(chunks, (g.n[1] + len - 1) / len, nplanes);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
-        void (*k)(Grid, const double *, double *, double *, StepParams *, Combine, int) =
+        void (*k)(Grid, const double *, double *, double *, StepParams *, Combine, int, int, BoundGrid) =
             wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
                     : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
                  : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len));
+        const BoundGrid bg = TWO_D ? final_bound_grid(d, last) : none;
+        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len, kz0, bg));
     }
     if (!fused) {
         if constexpr (LIM == 2) {
             cudaFuncSetAttribute(k_sweep_march_wz<1, TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
             cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
         }
-        const long long nitems = (long long)(g.n[0] + 2 * sx_halo(LIM)) * g.n[1] * g.n[2];
+        const long long nitems = (long long)(g.n[0] + 2 * sx_halo(LIM)) * g.n[1] * nplanes;
         LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + sx_out(LIM) - 1) / sx_out(LIM)), SX_NT, 0, s>>>(
                              g, Sin, Sout, ct, C.P, cb));
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
-        const int len = march_seglen(g.n[1], (long long)g.n[0] * g.n[2]);
-        dim3 grid(bx, (g.n[1] + len - 1) / len, g.n[2]);
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len));
-        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        const int len = seglen_y(g);
+        dim3 grid(bx, (g.n[1] + len - 1) / len, nplanes);
+        const BoundGrid bg = TWO_D ? final_bound_grid(d, last) : none;
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, bg));
+        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, bg));
     }
     if (!TWO_D) {
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
-        const int len = march_seglen(g.n[2], (long long)g.n[0] * g.n[1]);
+        const int len = seglen_z(g);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len));
-        else LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len));
+        const BoundGrid bg = final_bound_grid(d, last);
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+        else LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
     }
 }
 
 // CT: edge EMFs + face update (+ combine) in one kernel; dbg (debug only) receives the edge EMFs
-void launch_ct(const double *bin, double *bout, Combine cb, double *dbg)
+void launch_ct(const Domain &d, const double *bin, double *bout, Combine cb, double *dbg)
 {
     const bool combine = cb.Sn != nullptr;
-    const Grid &g = C.g;
+    const Grid &g = d.g;
     cudaStream_t s = C.stream;
     const int tiles_x = (g.n[0] + CT_TX - 2) / (CT_TX - 1), tiles_y = (g.n[1] + CT_TY - 2) / (CT_TY - 1);
     const int len = march_seglen(g.n[2], (long long)tiles_x * tiles_y * CT_TX * CT_TY);
     dim3 grid(tiles_x, tiles_y, (g.n[2] + len - 1) / len), block(CT_TX, CT_TY);
-    const double *ct = arr(A_CT);
+    const double *ct = arr(d, A_CT);
     if (C.ct_tma) {
-        // periodic halo layer of the CT arrays, then the TMA-staged kernel
-        LAUNCH(K_CT_HALO, k_ct_halo<<<dim3(g.n[2], CT_COUNT), 256, 0, s>>>(g, arr(A_CT), g.act[2] ? 0 : 1));
-        static bool tma_attr = false;
-        if (!tma_attr) {
-            cudaFuncSetAttribute(k_ct_tma<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
-            cudaFuncSetAttribute(k_ct_tma<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
-            cudaFuncSetAttribute(k_ct_tma<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
-            cudaFuncSetAttribute(k_ct_tma<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES);
-            tma_attr = true;
-        }
+        // periodic halo rows of the CT arrays (3D: planes -1 .. nz), then the TMA-staged kernel
+        LAUNCH(K_CT_HALO, k_ct_halo<<<dim3(g.act[2] ? g.n[2] + 2 : 1, CT_COUNT), 256, 0, s>>>(g, arr(d, A_CT), g.act[2] ? 0 : 1));
         if (g.act[2]) {
-            if (combine) LAUNCH(K_CT, k_ct_tma<true, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
-            else         LAUNCH(K_CT, k_ct_tma<false, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
+            if (combine) LAUNCH(K_CT, k_ct_tma<true, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, d.ct_map, ct, bin, bout, C.P, len, dbg, cb));
+            else         LAUNCH(K_CT, k_ct_tma<false, false><<<grid, block, CTM_SMEM_BYTES, s>>>(g, d.ct_map, ct, bin, bout, C.P, len, dbg, cb));
         } else {
-            if (combine) LAUNCH(K_CT, k_ct_tma<true, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
-            else         LAUNCH(K_CT, k_ct_tma<false, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, C.ct_map, ct, bin, bout, C.P, len, dbg, cb));
+            if (combine) LAUNCH(K_CT, k_ct_tma<true, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, d.ct_map, ct, bin, bout, C.P, len, dbg, cb));
+            else         LAUNCH(K_CT, k_ct_tma<false, true><<<grid, block, CTM_SMEM_BYTES, s>>>(g, d.ct_map, ct, bin, bout, C.P, len, dbg, cb));
         }
         return;
     }
@@ -287,47 +371,90 @@ void launch_ct(const double *bin, double *bout, Combine cb, double *dbg)
     }
 }
 
-// One Runge-Kutta stage: Sout <- Euler(Sin), or with a combine  Sout <- wn * S^n + ws * Euler(Sin)
-// (sn < 0: no combine; sn may equal out: in place).
-void enqueue_stage(int in, int out, int sn = -1, double wn = 0.0, double ws = 1.0, double *dbg = nullptr)
+// The dynamic shared memory of the TMA-staged CT kernel is above the 48 KB default: the attribute is
+// per device and per function, set at every pluto_init (the current device may have changed).
+int set_kernel_attributes()
 {
-    const Grid &g = C.g;
-    fill_ghosts(arr(in));
-    const bool two_d = !g.act[2];
-    const Combine cb = { sn >= 0 ? arr(sn) : nullptr, wn, ws };
-    if (g.limiter == 0)      { if (two_d) launch_sweeps<0, true>(arr(in), arr(out), cb);
-                               else       launch_sweeps<0, false>(arr(in), arr(out), cb); }
-    else if (g.limiter == 1) { if (two_d) launch_sweeps<1, true>(arr(in), arr(out), cb);
-                               else       launch_sweeps<1, false>(arr(in), arr(out), cb); }
-    else                     { if (two_d) launch_sweeps<2, true>(arr(in), arr(out), cb);
-                               else       launch_sweeps<2, false>(arr(in), arr(out), cb); }
-    const Combine cbf = { sn >= 0 ? arr(sn + S_B) : nullptr, wn, ws };
-    launch_ct(arr(in + S_B), arr(out + S_B), cbf, dbg);
+    CUDA_TRY(cudaFuncSetAttribute(k_ct_tma<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(k_ct_tma<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(k_ct_tma<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES));
+    CUDA_TRY(cudaFuncSetAttribute(k_ct_tma<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, CTM_SMEM_BYTES));
+    return PLUTO_OK;
+}
+
+// One Runge-Kutta stage over the slabs held here: Sout <- Euler(Sin), or with a combine
+// Sout <- wn * S^n + ws * Euler(Sin) (sn < 0: no combine; sn may equal out: in place).  Every slab's
+// ghost fill comes first: it reads the neighbours' interiors of `in`, which the compute kernels of this
+// stage never write (out != in).
+void enqueue_stage(int in, int out, int sn, double wn, double ws, bool last, double *dbg = nullptr)
+{
+    for (const Domain &d : C.dom) fill_ghosts(d, in);
+    for (const Domain &d : C.dom) {
+        const Grid &g = d.g;
+        const bool two_d = !g.act[2];
+        const Combine cb = { sn >= 0 ? arr(d, sn) : nullptr, wn, ws };
+        if (g.limiter == 0)      { if (two_d) launch_sweeps<0, true>(d, arr(d, in), arr(d, out), cb, last);
+                                   else       launch_sweeps<0, false>(d, arr(d, in), arr(d, out), cb, last); }
+        else if (g.limiter == 1) { if (two_d) launch_sweeps<1, true>(d, arr(d, in), arr(d, out), cb, last);
+                                   else       launch_sweeps<1, false>(d, arr(d, in), arr(d, out), cb, last); }
+        else                     { if (two_d) launch_sweeps<2, true>(d, arr(d, in), arr(d, out), cb, last);
+                                   else       launch_sweeps<2, false>(d, arr(d, in), arr(d, out), cb, last); }
+        const Combine cbf = { sn >= 0 ? arr(d, sn + S_B) : nullptr, wn, ws };
+        launch_ct(d, arr(d, in + S_B), arr(d, out + S_B), cbf, dbg);
+    }
+}
+
+// stage s of the step (0-based); SSP-RK2 (R3) or SSP-RK3 (Eq. 5; R17: the last stage carries 2 L**)
+void enqueue_rk_stage(int s)
+{
+    if (C.rk_order == 3) {
+        if (s == 0) enqueue_stage(A_SA, A_SB, -1, 0.0, 1.0, false);                    // S*   = S^n + L(S^n)
+        if (s == 1) enqueue_stage(A_SB, A_SC, A_SA, 0.75, 0.25, false);                // S**  = (3 S^n + S* + L(S*)) / 4
+        if (s == 2) enqueue_stage(A_SC, A_SA, A_SA, 1.0 / 3.0, 2.0 / 3.0, true);       // S^{n+1} = (S^n + 2 (S** + L(S**))) / 3
+    } else {
+        if (s == 0) enqueue_stage(A_SA, A_SB, -1, 0.0, 1.0, false);                    // S^1 = S^n + L(S^n)
+        if (s == 1) enqueue_stage(A_SB, A_SA, A_SA, 0.5, 0.5, true);                   // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
+    }
+}
+
+// exact max of the CFL candidates over the slabs held here (into P->smax_bits); the bound grid is spent
+void enqueue_dtmax(bool keep_bounds)
+{
+    for (const Domain &d : C.dom) {
+        const BoundGrid bg = final_bound_grid(d, true);
+        const double *bz_up = peer_arr(d.nb[1], A_SA + S_B + 2);
+        LAUNCH(K_DTMAX, launch_dtmax(d.g, arr(d, A_SA), bz_up, C.P, bg, C.sm_count * 8, C.stream));
+    }
+    if (!keep_bounds)
+        for (const Domain &d : C.dom) cudaMemsetAsync(d.bound, 0, bound_cells(d.g) * 8, C.stream);
+}
+
+// no bound known for the current state: every row is visited
+void reset_bounds()
+{
+    for (const Domain &d : C.dom) cudaMemsetAsync(d.bound, 0x7f, bound_cells(d.g) * 8, C.stream);
 }
 
 void enqueue_dt(int mode)
 {
-    if (mode != 1) LAUNCH(K_DTMAX, launch_dtmax(C.g, arr(A_SA), C.P, C.sm_count * 8, C.stream));
-    LAUNCH(K_SCALAR, launch_dtfinish(C.g, C.P, mode, C.stream));
+    if (mode != 1) enqueue_dtmax(mode == 2);
+    LAUNCH(K_SCALAR, launch_dtfinish(C.dom[0].g, C.P, mode, C.stream));
 }
 
 void enqueue_step(bool fixed)
 {
     enqueue_dt(fixed ? 1 : 0);
-    if (C.rk_order == 3) {
-        // SSP-RK3, Eq. 5 (R17: the last stage carries 2 L**)
-        enqueue_stage(A_SA, A_SB);                                  // S*   = S^n + L(S^n)
-        enqueue_stage(A_SB, A_SC, A_SA, 0.75, 0.25);                // S**  = (3 S^n + S* + L(S*)) / 4
-        enqueue_stage(A_SC, A_SA, A_SA, 1.0 / 3.0, 2.0 / 3.0);      // S^{n+1} = (S^n + 2 (S** + L(S**))) / 3
-    } else {
-        enqueue_stage(A_SA, A_SB);                                  // S^1 = S^n + L(S^n)
-        enqueue_stage(A_SB, A_SA, A_SA, 0.5, 0.5);                  // S^{n+1} = (S^n + S^1 + L(S^1)) / 2
-    }
+    for (int s = 0; s < C.rk_order; s++) enqueue_rk_stage(s);
     LAUNCH(K_SCALAR, launch_advance_time(C.P, C.stream));
 }
 
+int ensure_rk3_storage();
+
 int run_steps(int nsteps, bool fixed)
 {
+    if (!C.whole()) return fail(PLUTO_ESTATE, "this process holds %d of %d slabs: drive the step with pluto_step_begin / pluto_step_stage",
+                                (int)C.dom.size(), C.nslab);
+    if (int rc = ensure_rk3_storage()) return rc;
     const int gi = fixed ? 1 : 0;
     const bool graph = C.use_graph && !C.prof_on;
     if (graph && !C.graph[gi] && nsteps > 0) {
@@ -372,21 +499,181 @@ bool is_device_ptr(const void *p)
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-// extents of the caller's array for the face family d (d = -1: cell array)
-void api_extent(const Grid &g, int d, int m[3])
+// extents of the caller's array for the face family d (d = -1: cell array) over nz planes
+void api_extent(const Grid &g, int nz, int d, int m[3])
 {
-    for (int a = 0; a < 3; a++) m[a] = g.n[a] + (a == d ? 1 : 0);
+    m[0] = g.n[0] + (d == 0 ? 1 : 0);
+    m[1] = g.n[1] + (d == 1 ? 1 : 0);
+    m[2] = nz + (d == 2 ? 1 : 0);
 }
 
-size_t api_count(const Grid &g, int d)
+size_t api_count(const Grid &g, int nz, int d)
 {
     int m[3];
-    api_extent(g, d, m);
+    api_extent(g, nz, d, m);
     return (size_t)m[0] * m[1] * m[2];
 }
 
-// staging buffer: the CT work arrays are free outside a step (12 padded arrays > 11 interior arrays)
-double *staging() { return arr(A_CT); }
+// Host-copy staging: the CT work arrays of the slabs are free outside a step.  With one slab they hold
+// the whole caller's array (12 padded arrays > 11 interior arrays); with several slabs a temporary is used.
+struct Staging {
+    double *p = nullptr;
+    bool temp = false;
+    int get(size_t doubles)
+    {
+        const Domain &d0 = C.dom[0];
+        if (C.dom.size() == 1 && doubles <= (size_t)CT_COUNT * d0.g.sa) { p = arr(d0, A_CT); return PLUTO_OK; }
+        if (cudaMalloc((void **)&p, doubles * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+            return fail(PLUTO_ENOMEM, "cannot allocate %zu bytes of staging", doubles * sizeof(double));
+        }
+        temp = true;
+        return PLUTO_OK;
+    }
+    ~Staging() { if (temp && p) cudaFree(p); }
+};
+
+void free_domains()
+{
+    for (Domain &d : C.dom) {
+        for (Peer &p : d.nb)
+            if (p.ipc_mapping) { cudaIpcCloseMemHandle(p.ipc_mapping); p.ipc_mapping = nullptr; }
+        if (d.own_sc && d.sc) cudaFree(d.sc);
+        if (d.own_mem && d.base) cudaFree(d.base);
+    }
+    C.dom.clear();
+    C.P = nullptr;
+}
+
+// SSP-RK3 keeps a third state: allocated on first use when pluto_init ran with the RK2 layout
+int ensure_rk3_storage()
+{
+    if (C.rk_order != 3) return PLUTO_OK;
+    for (Domain &d : C.dom) {
+        if (d.narrays >= A_COUNT || d.sc) continue;
+        if (!C.whole()) return fail(PLUTO_ESTATE, "select SSP-RK3 before pluto_init_slabs (peers map one allocation per slab)");
+        const size_t bytes = (size_t)S_COUNT * d.g.sa * sizeof(double);
+        cudaError_t e = cudaMalloc((void **)&d.sc, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); d.sc = nullptr; return fail(PLUTO_ENOMEM, "cudaMalloc(%zu) for the RK3 stage state: %s", bytes, cudaGetErrorString(e)); }
+        d.own_sc = true;
+        CUDA_TRY(cudaMemsetAsync(d.sc, 0, bytes, C.stream));
+    }
+    // neighbours inside this process: their S^2 lives where arr() finds it
+    for (size_t s = 0; s < C.dom.size(); s++) {
+        Domain &d = C.dom[s];
+        if (C.whole()) {
+            d.nb[0].sc = C.dom[(s + C.dom.size() - 1) % C.dom.size()].sc;
+            d.nb[1].sc = C.dom[(s + 1) % C.dom.size()].sc;
+        }
+    }
+    destroy_graphs();
+    return PLUTO_OK;
+}
+
+// everything pluto_finalize does, except forgetting the registered workspace (pluto_init re-creates a live context)
+void release()
+{
+    if (C.init) {
+        cudaStreamSynchronize(C.stream);
+        destroy_graphs();
+    }
+    free_domains();
+    C.init = false; C.have_state = false; C.stepped = false;
+    C.nslab = 1; C.first = 0;
+}
+
+int init_common(int nslab, int first, int count, int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); ndev = 0; }
+    if (ndev < 1) return fail(PLUTO_ECUDA, "no CUDA device: this library has no CPU fallback");
+    release();
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!C.stream || (C.stream == C.own_stream && C.own_stream_dev != dev)) {
+        C.stream = nullptr;
+        int rc = pluto_set_stream(nullptr);
+        if (rc) return rc;
+    }
+    if (nslab < 1 || first < 0 || count < 1 || first + count > nslab) return fail(PLUTO_EINVAL, "bad slab range");
+    Grid gg;
+    if (!make_grid(gg, nx, ny, nz, ghost))
+        return fail(PLUTO_EINVAL, "need nx >= 2, ny >= 2, nz >= 1, 2 <= ghost <= %d, active extents >= ghost", XOFF);
+    if (!(gamma > 1.0) || !(cfl > 0.0) || limiter < PLUTO_MINMOD || limiter > PLUTO_WENOZ)
+        return fail(PLUTO_EINVAL, "need gamma > 1, cfl > 0, limiter in {0,1,2}");
+    if (limiter == PLUTO_WENOZ && ghost < 3)
+        return fail(PLUTO_EINVAL, "the WENO-Z stencil needs ghost >= 3");
+    if (nslab > 1 && (nz / nslab < ghost + 1))
+        return fail(PLUTO_EINVAL, "every z slab needs at least ghost + 1 = %d planes", ghost + 1);
+    const int narrays = C.rk_order == 3 ? A_COUNT : A_COUNT_RK2;
+    C.nslab = nslab; C.first = first; C.nzg = nz;
+    C.dom.resize(count);
+    int kbase = 0, dummy = 0;
+    slab_range(nz, nslab, first, kbase, dummy);
+    size_t total = 0;
+    for (int s = 0; s < count; s++) {
+        Domain &d = C.dom[s];
+        int k0 = 0, nzl = nz;
+        slab_range(nz, nslab, first + s, k0, nzl);
+        if (!make_grid(d.g, nx, ny, nzl, ghost)) { C.dom.clear(); return fail(PLUTO_EINVAL, "bad slab"); }
+        if ((long long)d.g.tot[2] * 8 > 65535 || d.g.tot[1] > 65535) { C.dom.clear(); return fail(PLUTO_EINVAL, "extent too large for the launch grid"); }
+        d.g.gamma = gamma; d.g.igm1 = 1.0 / (gamma - 1.0); d.g.cfl = cfl; d.g.limiter = limiter;
+        for (int a = 0; a < 3; a++) { d.g.dx[a] = 1.0 / nx; d.g.idx[a] = 1.0 / d.g.dx[a]; }   // R11: Lx = 1, cubic cells
+        d.kz0 = k0 - kbase;
+        d.narrays = narrays;
+        total += layout_bytes(d.g, narrays);
+    }
+    C.nzloc = C.dom.back().kz0 + C.dom.back().g.n[2];
+    // memory: the registered workspace (one piece per slab, in order) or our own allocations
+    if (C.ws) {
+        if (C.ws_bytes < total) { C.dom.clear(); return fail(PLUTO_ENOMEM, "workspace has %zu bytes, need %zu", C.ws_bytes, total); }
+        char *p = (char *)C.ws;
+        for (Domain &d : C.dom) { d.base = (double *)p; d.own_mem = false; p += layout_bytes(d.g, narrays); }
+    } else {
+        for (Domain &d : C.dom) {
+            const size_t bytes = layout_bytes(d.g, narrays);
+            cudaError_t e = cudaMalloc((void **)&d.base, bytes);
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                d.base = nullptr;
+                free_domains();
+                return fail(PLUTO_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e));
+            }
+            d.own_mem = true;
+        }
+    }
+    cudaDeviceGetAttribute(&C.sm_count, cudaDevAttrMultiProcessorCount, dev);
+    for (Domain &d : C.dom) {
+        cudaError_t e = cudaMemsetAsync(d.base, 0, layout_bytes(d.g, narrays), C.stream);
+        if (e != cudaSuccess) { free_domains(); return fail(PLUTO_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e)); }
+        d.bound = (unsigned long long *)((char *)d.base + (size_t)narrays * d.g.sa * sizeof(double) + 256);
+    }
+    C.P = (StepParams *)(C.dom[0].base + (long long)narrays * C.dom[0].g.sa);
+    // neighbours inside this process; the two outer ones are peers unless the whole box is here
+    for (int s = 0; s < count; s++) {
+        Domain &d = C.dom[s];
+        for (int side = 0; side < 2; side++) {
+            int t = s + (side ? 1 : -1);
+            if (C.whole()) t = (t + count) % count;
+            if (t < 0 || t >= count) continue;            // attached later with pluto_attach_peer
+            d.nb[side].base = C.dom[t].base; d.nb[side].sa = C.dom[t].g.sa; d.nb[side].n2 = C.dom[t].g.n[2];
+        }
+    }
+    if (cudaStreamSynchronize(C.stream) != cudaSuccess) { free_domains(); return fail(PLUTO_ECUDA, "device memset failed"); }
+    int rc = set_kernel_attributes();
+    for (Domain &d : C.dom) if (!rc) rc = make_ct_map(d);
+    if (rc) { free_domains(); return rc; }
+    C.init = true; C.have_state = false; C.stepped = false; C.launches = 0;
+    return PLUTO_OK;
+}
+
+bool peers_attached()
+{
+    for (const Domain &d : C.dom)
+        if (!d.nb[0].base || !d.nb[1].base) return false;
+    return true;
+}
 
 } // namespace
 
@@ -405,14 +692,27 @@ int pluto_device_count(void)
 
 size_t pluto_workspace_bytes(int nx, int ny, int nz, int ghost)
 {
-    Grid g;
-    if (!make_grid(g, nx, ny, nz, ghost)) return 0;
-    return layout_bytes(g);
+    return pluto_workspace_bytes_slabs(1, 0, 1, nx, ny, nz, ghost, 2);
+}
+
+size_t pluto_workspace_bytes_slabs(int nslab, int first, int count, int nx, int ny, int nz, int ghost, int rk_order)
+{
+    if (nslab < 1 || first < 0 || count < 1 || first + count > nslab || (rk_order != 2 && rk_order != 3)) return 0;
+    if (nslab > 1 && nz / nslab < ghost + 1) return 0;
+    size_t total = 0;
+    for (int s = first; s < first + count; s++) {
+        int k0, nzl;
+        slab_range(nz, nslab, s, k0, nzl);
+        Grid g;
+        if (!make_grid(g, nx, ny, nzl, ghost)) return 0;
+        total += layout_bytes(g, rk_order == 3 ? A_COUNT : A_COUNT_RK2);
+    }
+    return total;
 }
 
 int pluto_set_workspace(void *dev, size_t bytes)
 {
-    if (C.init && !C.own_mem) return fail(PLUTO_ESTATE, "workspace in use: call pluto_finalize first");
+    if (C.init && !C.dom.empty() && !C.dom[0].own_mem) return fail(PLUTO_ESTATE, "workspace in use: call pluto_finalize first");
     if (dev && !is_device_ptr(dev)) return fail(PLUTO_EINVAL, "workspace is not device memory");
     if (dev && ((size_t)dev & 255)) return fail(PLUTO_EINVAL, "workspace must be 256-byte aligned");
     C.ws = dev;
@@ -424,12 +724,17 @@ int pluto_set_stream(void *cuda_stream)
 {
     if (C.init) cudaStreamSynchronize(C.stream);
     if (!cuda_stream) {
-        // the legacy default stream cannot be captured into a graph: use a stream of our own
-        if (!C.own_stream && pluto_device_count() > 0)
+        // the legacy default stream cannot be captured into a graph: use a stream of our own, on the current device
+        int dev = 0;
+        if (pluto_device_count() > 0) cudaGetDevice(&dev);
+        if (C.own_stream && C.own_stream_dev != dev) { cudaStreamDestroy(C.own_stream); C.own_stream = nullptr; }
+        if (!C.own_stream && pluto_device_count() > 0) {
             if (cudaStreamCreateWithFlags(&C.own_stream, cudaStreamNonBlocking) != cudaSuccess) {
                 cudaGetLastError();
                 return fail(PLUTO_ECUDA, "cannot create a stream");
             }
+            C.own_stream_dev = dev;
+        }
         C.stream = C.own_stream;
     } else {
         C.stream = (cudaStream_t)cuda_stream;
@@ -440,51 +745,87 @@ int pluto_set_stream(void *cuda_stream)
 
 int pluto_finalize(void)
 {
-    if (C.init) {
-        cudaStreamSynchronize(C.stream);
-        destroy_graphs();
-        if (C.own_mem && C.base) cudaFree(C.base);
-    }
-    C.base = nullptr; C.P = nullptr; C.init = false; C.have_state = false; C.stepped = false; C.own_mem = false;
+    release();
+    // the registration of a workspace ends here (pluto.h: the caller keeps it alive until pluto_finalize)
+    C.ws = nullptr; C.ws_bytes = 0;
     return PLUTO_OK;
 }
 
 int pluto_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter)
 {
-    if (pluto_device_count() < 1) return fail(PLUTO_ECUDA, "no CUDA device: this library has no CPU fallback");
-    pluto_finalize();
-    if (!C.stream) { int rc = pluto_set_stream(nullptr); if (rc) return rc; }
-    Grid g;
-    if (!make_grid(g, nx, ny, nz, ghost))
-        return fail(PLUTO_EINVAL, "need nx >= 2, ny >= 2, nz >= 1, 2 <= ghost <= %d, active extents >= ghost", XOFF);
-    if (!(gamma > 1.0) || !(cfl > 0.0) || limiter < PLUTO_MINMOD || limiter > PLUTO_WENOZ)
-        return fail(PLUTO_EINVAL, "need gamma > 1, cfl > 0, limiter in {0,1,2}");
-    if (limiter == PLUTO_WENOZ && ghost < 3)
-        return fail(PLUTO_EINVAL, "the WENO-Z stencil needs ghost >= 3");
-    if ((long long)g.tot[2] * 8 > 65535 || g.tot[1] > 65535)
-        return fail(PLUTO_EINVAL, "extent too large for the launch grid");
-    g.gamma = gamma; g.igm1 = 1.0 / (gamma - 1.0); g.cfl = cfl; g.limiter = limiter;
-    for (int a = 0; a < 3; a++) { g.dx[a] = 1.0 / nx; g.idx[a] = 1.0 / g.dx[a]; }   // R11: Lx = 1, cubic cells
-    size_t bytes = layout_bytes(g);
-    if (C.ws) {
-        if (C.ws_bytes < bytes) return fail(PLUTO_ENOMEM, "workspace has %zu bytes, need %zu", C.ws_bytes, bytes);
-        C.base = (double *)C.ws;
-        C.own_mem = false;
-    } else {
-        cudaError_t e = cudaMalloc((void **)&C.base, bytes);
-        if (e != cudaSuccess) { cudaGetLastError(); C.base = nullptr; return fail(PLUTO_ENOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); }
-        C.own_mem = true;
+    return init_common(1, 0, 1, nx, ny, nz, ghost, gamma, cfl, limiter);
+}
+
+int pluto_init_slabs(int nslab, int first, int count, int nx, int ny, int nz, int ghost, double gamma, double cfl, int limiter)
+{
+    if (nz < 2) return fail(PLUTO_EINVAL, "the z-slab decomposition needs a 3D box");
+    return init_common(nslab, first, count, nx, ny, nz, ghost, gamma, cfl, limiter);
+}
+
+int pluto_slab_planes(int nz, int nslab, int slab, int *k0, int *planes)
+{
+    if (nz < 1 || nslab < 1 || slab < 0 || slab >= nslab) return fail(PLUTO_EINVAL, "bad slab");
+    int kb = 0, n = 0;
+    slab_range(nz, nslab, slab, kb, n);
+    if (k0) *k0 = kb;
+    if (planes) *planes = n;
+    return PLUTO_OK;
+}
+
+int pluto_local_planes(int *k0, int *nz_local)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    int kb = 0, n = 0;
+    slab_range(C.nzg, C.nslab, C.first, kb, n);
+    if (k0) *k0 = kb;
+    if (nz_local) *nz_local = C.nzloc;
+    return PLUTO_OK;
+}
+
+int pluto_export_slab(int side, void *ipc_handle64, void **device_ptr, long long *array_stride, int *planes)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    if (side != 0 && side != 1) return fail(PLUTO_EINVAL, "side must be 0 (lowest slab) or 1 (highest slab)");
+    const Domain &d = side ? C.dom.back() : C.dom.front();
+    if (ipc_handle64) {
+        if (!d.own_mem) return fail(PLUTO_ESTATE, "a slab inside a registered workspace cannot be exported by IPC handle");
+        cudaIpcMemHandle_t h;
+        CUDA_TRY(cudaIpcGetMemHandle(&h, d.base));
+        static_assert(sizeof(h) == 64, "cudaIpcMemHandle_t is 64 bytes");
+        memcpy(ipc_handle64, &h, 64);
     }
-    C.g = g;
-    C.P = (StepParams *)(C.base + (long long)A_COUNT * g.sa);
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&C.sm_count, cudaDevAttrMultiProcessorCount, dev);
-    CUDA_TRY(cudaMemsetAsync(C.base, 0, bytes, C.stream));
-    CUDA_TRY(cudaStreamSynchronize(C.stream));
-    C.init = true; C.have_state = false; C.stepped = false; C.launches = 0;
-    int rc = make_ct_map();
-    if (rc) { C.init = false; return rc; }
+    if (device_ptr) *device_ptr = d.base;
+    if (array_stride) *array_stride = d.g.sa;
+    if (planes) *planes = d.g.n[2];
+    return PLUTO_OK;
+}
+
+int pluto_attach_peer(int side, const void *ipc_handle64, void *device_ptr, long long array_stride, int planes)
+{
+    if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    if (side != 0 && side != 1) return fail(PLUTO_EINVAL, "side must be 0 (the slab below) or 1 (the slab above)");
+    if (C.whole()) return fail(PLUTO_ESTATE, "every slab is in this process: there is no peer");
+    if (planes < C.dom[0].g.ng + 1 || array_stride <= 0) return fail(PLUTO_EINVAL, "bad peer layout");
+    Domain &d = side ? C.dom.back() : C.dom.front();
+    Peer &p = d.nb[side];
+    Peer &other = (side ? C.dom.front() : C.dom.back()).nb[1 - side];
+    if (p.ipc_mapping) { cudaIpcCloseMemHandle(p.ipc_mapping); p.ipc_mapping = nullptr; }
+    void *ptr = device_ptr;
+    if (ipc_handle64) {
+        if (other.ipc_mapping && !memcmp(other.ipc_handle, ipc_handle64, 64)) {
+            // two processes: the slab below and the slab above are the same allocation, mapped once
+            ptr = other.ipc_mapping;
+            other.ipc_mapping = nullptr;          // this side closes it
+        } else {
+            cudaIpcMemHandle_t h;
+            memcpy(&h, ipc_handle64, 64);
+            CUDA_TRY(cudaIpcOpenMemHandle(&ptr, h, cudaIpcMemLazyEnablePeerAccess));
+        }
+        p.ipc_mapping = ptr;
+        memcpy(p.ipc_handle, ipc_handle64, 64);
+    }
+    if (!ptr) return fail(PLUTO_EINVAL, "need an IPC handle or a device pointer");
+    p.base = (double *)ptr; p.sa = array_stride; p.n2 = planes; p.sc = nullptr;
     return PLUTO_OK;
 }
 
@@ -492,8 +833,10 @@ int pluto_set_box(double Lx, double Ly, double Lz)
 {
     if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
     if (!(Lx > 0.0) || !(Ly > 0.0) || !(Lz > 0.0)) return fail(PLUTO_EINVAL, "box lengths must be positive");
-    double L[3] = { Lx, Ly, Lz };
-    for (int a = 0; a < 3; a++) { C.g.dx[a] = L[a] / C.g.n[a]; C.g.idx[a] = 1.0 / C.g.dx[a]; }
+    const int n[3] = { C.dom[0].g.n[0], C.dom[0].g.n[1], C.nzg };      // Lz is the length of the WHOLE box
+    const double L[3] = { Lx, Ly, Lz };
+    for (Domain &d : C.dom)
+        for (int a = 0; a < 3; a++) { d.g.dx[a] = L[a] / n[a]; d.g.idx[a] = 1.0 / d.g.dx[a]; }
     destroy_graphs();          // kernels take the grid by value: captured copies are stale
     return PLUTO_OK;
 }
@@ -527,82 +870,120 @@ int pluto_set_state(const double *U, const double *Bface)
 {
     if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
     if (!U || !Bface) return fail(PLUTO_EINVAL, "null pointer");
-    const Grid &g = C.g;
+    const Grid &g0 = C.dom[0].g;
+    const int ndim = g0.ndim, nzl = C.nzloc;
     cudaStream_t s = C.stream;
-    Box in = interior(g);
-    const size_t n = api_count(g, -1);
+    const size_t n = api_count(g0, nzl, -1);
     size_t nface = 0;
-    for (int d = 0; d < g.ndim; d++) nface += api_count(g, d);
-    // Host arrays are staged in the CT work arrays (free outside a step): U at offset 0, Bface behind it.
-    // U[4..6], the cell-centred B of the active dimensions, is never read (R7: it IS the face mean) and
-    // is not even copied; 2D: U[6] = B_z goes to the third magnetic array.
+    for (int d = 0; d < ndim; d++) nface += api_count(g0, nzl, d);
+    // Host arrays are staged on the device: U at offset 0, Bface behind it.  U[4..6], the cell-centred B of
+    // the active dimensions, is never read (R7: it IS the face mean) and is not even copied; 2D: U[6] = B_z
+    // goes to the third magnetic array.
     const double *dU = U, *dB = Bface;
+    Staging st;
+    if (!is_device_ptr(U) || !is_device_ptr(Bface)) {
+        if (int rc = st.get(8 * n + nface)) return rc;
+    }
     if (!is_device_ptr(U)) {
-        if ((8 * n + nface) * sizeof(double) > (size_t)CT_COUNT * g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
-        CUDA_TRY(cudaMemcpyAsync(staging(), U, 4 * n * sizeof(double), cudaMemcpyHostToDevice, s));
-        if (!g.act[2]) CUDA_TRY(cudaMemcpyAsync(staging() + 6 * n, U + 6 * n, n * sizeof(double), cudaMemcpyHostToDevice, s));
-        CUDA_TRY(cudaMemcpyAsync(staging() + 7 * n, U + 7 * n, n * sizeof(double), cudaMemcpyHostToDevice, s));
-        dU = staging();
+        CUDA_TRY(cudaMemcpyAsync(st.p, U, 4 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        if (ndim == 2) CUDA_TRY(cudaMemcpyAsync(st.p + 6 * n, U + 6 * n, n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaMemcpyAsync(st.p + 7 * n, U + 7 * n, n * sizeof(double), cudaMemcpyHostToDevice, s));
+        dU = st.p;
     }
     if (!is_device_ptr(Bface)) {
-        if ((8 * n + nface) * sizeof(double) > (size_t)CT_COUNT * g.sa * sizeof(double)) return fail(PLUTO_ENOMEM, "staging too small");
-        CUDA_TRY(cudaMemcpyAsync(staging() + 8 * n, Bface, nface * sizeof(double), cudaMemcpyHostToDevice, s));
-        dB = staging() + 8 * n;
+        CUDA_TRY(cudaMemcpyAsync(st.p + 8 * n, Bface, nface * sizeof(double), cudaMemcpyHostToDevice, s));
+        dB = st.p + 8 * n;
     }
     const int src_of[5] = { 0, 1, 2, 3, 7 };
-    for (int v = 0; v < 5; v++)
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + (size_t)src_of[v] * n, g.n[0], g.n[1], arr(A_SA + v));
-    if (!g.act[2])
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + 6 * n, g.n[0], g.n[1], arr(A_SA + S_B + 2));
-    const double *dev = dB;
-    size_t off = 0;
-    for (int d = 0; d < g.ndim; d++) {
-        int m[3];
-        api_extent(g, d, m);
-        k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dev + off, m[0], m[1], arr(A_SA + S_B + d));   // upper duplicate ignored
-        off += api_count(g, d);
+    for (const Domain &d : C.dom) {
+        const Grid &g = d.g;
+        Box in = interior(g);
+        for (int v = 0; v < 5; v++)
+            k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + (size_t)src_of[v] * n, g.n[0], g.n[1], d.kz0, arr(d, A_SA + v));
+        if (ndim == 2)
+            k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + 6 * n, g.n[0], g.n[1], 0, arr(d, A_SA + S_B + 2));
+        size_t off = 0;
+        for (int f = 0; f < ndim; f++) {
+            int m[3];
+            api_extent(g0, nzl, f, m);
+            k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dB + off, m[0], m[1], d.kz0, arr(d, A_SA + S_B + f));   // upper duplicates ignored
+            off += api_count(g0, nzl, f);
+        }
+        C.launches += 5 + ndim + (ndim == 2 ? 1 : 0);
     }
-    fill_ghosts(arr(A_SA), true);    // every ghost once (the per-stage fill may skip x: see fill_ghosts)
+    // every ghost once (the per-stage fill may skip x: see fill_ghosts); with peers the caller fills them
+    // after all processes have set their state (pluto_fill_ghosts)
+    if (peers_attached() && C.whole())
+        for (const Domain &d : C.dom) fill_ghosts(d, A_SA, true);
+    reset_bounds();
     StepParams p0;
     memset(&p0, 0, sizeof p0);
     CUDA_TRY(cudaMemcpyAsync(C.P, &p0, sizeof p0, cudaMemcpyHostToDevice, s));
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
-    C.launches += 6 + g.ndim;
     C.have_state = true; C.stepped = false;
+    return PLUTO_OK;
+}
+
+int pluto_fill_ghosts(void)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (!peers_attached()) return fail(PLUTO_ESTATE, "a neighbour slab is not attached (pluto_attach_peer)");
+    for (const Domain &d : C.dom) fill_ghosts(d, A_SA, true);
+    CUDA_TRY(cudaStreamSynchronize(C.stream));
+    CUDA_TRY(cudaGetLastError());
     return PLUTO_OK;
 }
 
 int pluto_get_state(double *U, double *Bface)
 {
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
-    const Grid &g = C.g;
+    if (!peers_attached()) return fail(PLUTO_ESTATE, "a neighbour slab is not attached (pluto_attach_peer)");
+    const Grid &g0 = C.dom[0].g;
+    const int ndim = g0.ndim, nzl = C.nzloc;
     cudaStream_t s = C.stream;
-    const size_t n = api_count(g, -1);
+    const size_t n = api_count(g0, nzl, -1);
+    size_t nface = 0;
+    for (int d = 0; d < ndim; d++) nface += api_count(g0, nzl, d);
+    Staging st;
+    const bool udev = U && is_device_ptr(U), bdev = Bface && is_device_ptr(Bface);
+    if ((U && !udev) || (Bface && !bdev)) {
+        if (int rc = st.get(8 * n + nface)) return rc;
+    }
     if (U) {
-        bool dev = is_device_ptr(U);
-        double *dst = dev ? U : staging();
-        Box in = interior(g);
+        double *dst = udev ? U : st.p;
         const int dst_of[5] = { 0, 1, 2, 3, 7 };
-        for (int v = 0; v < 5; v++)
-            k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SA + v), g.n[0], g.n[1], dst + (size_t)dst_of[v] * n);
-        k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SA + S_B), dst + 4 * n, (long long)n);
-        if (!dev) CUDA_TRY(cudaMemcpyAsync(U, dst, 8 * n * sizeof(double), cudaMemcpyDeviceToHost, s));
-        C.launches += 6;
+        for (const Domain &d : C.dom) {
+            const Grid &g = d.g;
+            Box in = interior(g);
+            for (int v = 0; v < 5; v++)
+                k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_SA + v), g.n[0], g.n[1], d.kz0, -1, dst + (size_t)dst_of[v] * n);
+            k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_SA + S_B), peer_arr(d.nb[1], A_SA + S_B + 2), dst + 4 * n, (long long)n, d.kz0);
+            C.launches += 6;
+        }
+        if (!udev) CUDA_TRY(cudaMemcpyAsync(U, dst, 8 * n * sizeof(double), cudaMemcpyDeviceToHost, s));
     }
     if (Bface) {
-        bool dev = is_device_ptr(Bface);
-        double *dst = dev ? Bface : staging() + 8 * n;      // behind U's staging: both copies overlap the packing
-        size_t off = 0;
-        for (int d = 0; d < g.ndim; d++) {
-            int m[3];
-            api_extent(g, d, m);
-            Box b = make_box(g, 0, m[0], 0, m[1], 0, m[2]);
-            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_SA + S_B + d), m[0], m[1], dst + off);
-            off += api_count(g, d);
+        double *dst = bdev ? Bface : st.p + 8 * n;      // behind U's staging: both copies overlap the packing
+        for (const Domain &d : C.dom) {
+            const Grid &g = d.g;
+            size_t off = 0;
+            for (int f = 0; f < ndim; f++) {
+                int m[3];
+                api_extent(g0, nzl, f, m);
+                Box b = make_box(g, 0, g.n[0] + (f == 0), 0, g.n[1] + (f == 1), 0, g.n[2]);
+                k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(d, A_SA + S_B + f), m[0], m[1], d.kz0, -1, dst + off);
+                if (f == 2 && &d == &C.dom.back()) {
+                    // the duplicate upper z face of this process's planes: face 0 of the slab above
+                    Box top = make_box(g, 0, g.n[0], 0, g.n[1], g.n[2], g.n[2] + 1);
+                    k_pack<<<grid_for(top), 128, 0, s>>>(g, top, peer_arr(d.nb[1], A_SA + S_B + 2), m[0], m[1], d.kz0, 0, dst + off);
+                    C.launches += 1;
+                }
+                off += api_count(g0, nzl, f);
+            }
+            C.launches += ndim;
         }
-        if (!dev) CUDA_TRY(cudaMemcpyAsync(Bface, dst, off * sizeof(double), cudaMemcpyDeviceToHost, s));
-        C.launches += g.ndim;
+        if (!bdev) CUDA_TRY(cudaMemcpyAsync(Bface, dst, nface * sizeof(double), cudaMemcpyDeviceToHost, s));
     }
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
@@ -638,11 +1019,45 @@ int pluto_step_fixed_dt(int nsteps, double dt)
     return rc ? rc : finish();
 }
 
+// ---- the step in phases, for a box whose slabs live in several processes (one per GPU)
+
+int pluto_step_begin(double fixed_dt)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (!peers_attached()) return fail(PLUTO_ESTATE, "a neighbour slab is not attached (pluto_attach_peer)");
+    if (int rc = ensure_rk3_storage()) return rc;
+    if (fixed_dt > 0.0) {
+        CUDA_TRY(cudaMemcpyAsync(&C.P->dt_fixed, &fixed_dt, sizeof fixed_dt, cudaMemcpyHostToDevice, C.stream));
+        CUDA_TRY(cudaStreamSynchronize(C.stream));
+    } else {
+        enqueue_dtmax(false);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return PLUTO_OK;
+}
+
+void *pluto_dt_max_bits(void) { return C.init ? (void *)&C.P->smax_bits : nullptr; }
+
+int pluto_step_stage(int stage, int fixed)
+{
+    if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (stage < 0 || stage >= C.rk_order) return fail(PLUTO_EINVAL, "stage out of range");
+    if (stage == 0) LAUNCH(K_SCALAR, launch_dtfinish(C.dom[0].g, C.P, fixed ? 1 : 0, C.stream));
+    enqueue_rk_stage(stage);
+    if (stage == C.rk_order - 1) {
+        LAUNCH(K_SCALAR, launch_advance_time(C.P, C.stream));
+        C.stepped = true;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return PLUTO_OK;
+}
+
 double pluto_get_dt(void)
 {
     if (!C.init || !C.have_state) return NAN;
     double dt = NAN;
     if (!C.stepped) {
+        if (!C.whole()) return NAN;             // the max over every process is the caller's (pluto_dt_max_bits)
         enqueue_dt(2);
         if (cudaMemcpyAsync(&dt, &C.P->dt_probe, sizeof dt, cudaMemcpyDeviceToHost, C.stream) != cudaSuccess) return NAN;
     } else {
@@ -708,8 +1123,10 @@ double pluto_probe_fp64_gflops(void)
 int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem, double *Eedge)
 {
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (C.dom.size() != 1 || !C.whole()) return fail(PLUTO_ESTATE, "pluto_debug_euler works on a single domain");
     if (!(dt > 0.0)) return fail(PLUTO_EINVAL, "dt must be positive");
-    const Grid &g = C.g;
+    const Domain &d = C.dom[0];
+    const Grid &g = d.g;
     cudaStream_t s = C.stream;
     CUDA_TRY(cudaMemcpyAsync(&C.P->dt_fixed, &dt, sizeof dt, cudaMemcpyHostToDevice, s));
     CUDA_TRY(cudaStreamSynchronize(s));
@@ -717,16 +1134,21 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     StepParams saved;
     CUDA_TRY(cudaMemcpy(&saved, C.P, sizeof saved, cudaMemcpyDeviceToHost));
     launch_dtfinish(g, C.P, 1, s);
-    double *dbgE = nullptr;                     // edge EMFs are never stored by the production path
-    CUDA_TRY(cudaMalloc((void **)&dbgE, 3 * (size_t)g.sa * sizeof(double)));
-    CUDA_TRY(cudaMemsetAsync(dbgE, 0, 3 * (size_t)g.sa * sizeof(double), s));
-    enqueue_stage(A_SA, A_SB, -1, 0.0, 1.0, dbgE);
+    // two library-owned temporaries, freed on every path: the edge EMFs (never stored by the production
+    // path) and a private staging area (the CT work arrays are being read)
+    struct DevBuf {
+        double *p = nullptr;
+        ~DevBuf() { if (p) cudaFree(p); }
+    } dbgE, tmpb;
+    CUDA_TRY(cudaMalloc((void **)&dbgE.p, 3 * (size_t)g.sa * sizeof(double)));
+    CUDA_TRY(cudaMemsetAsync(dbgE.p, 0, 3 * (size_t)g.sa * sizeof(double), s));
+    enqueue_stage(A_SA, A_SB, -1, 0.0, 1.0, false, dbgE.p);
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
-    const size_t n = api_count(g, -1);
-    double *tmp = nullptr;                      // private staging: the flux arrays are being read
+    const size_t n = api_count(g, g.n[2], -1);
     size_t maxcount = 8 * n + 3 * (n + (size_t)g.n[0] * g.n[1] + (size_t)g.n[1] * g.n[2] + (size_t)g.n[0] * g.n[2]);
-    CUDA_TRY(cudaMalloc((void **)&tmp, maxcount * sizeof(double)));
+    CUDA_TRY(cudaMalloc((void **)&tmpb.p, maxcount * sizeof(double)));
+    double *tmp = tmpb.p;
     Box in = interior(g);
     auto emit = [&](double *user, size_t count) -> int {
         if (is_device_ptr(user)) return cudaMemcpy(user, tmp, count * sizeof(double), cudaMemcpyDeviceToDevice) == cudaSuccess ? 0 : 1;
@@ -735,45 +1157,47 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     int bad = 0;
     if (U1) {
         const int dst_of[5] = { 0, 1, 2, 3, 7 };
-        for (int v = 0; v < 5; v++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SB + v), g.n[0], g.n[1], tmp + dst_of[v] * n);
-        k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_SB + S_B), tmp + 4 * n, (long long)n);
+        for (int v = 0; v < 5; v++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_SB + v), g.n[0], g.n[1], 0, -1, tmp + dst_of[v] * n);
+        k_pack_cellb<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_SB + S_B), arr(d, A_SB + S_B + 2), tmp + 4 * n, (long long)n, 0);
         cudaStreamSynchronize(s);
         bad |= emit(U1, 8 * n);
     }
     if (Bf1) {
         size_t off = 0;
-        for (int d = 0; d < g.ndim; d++) {
+        for (int f = 0; f < g.ndim; f++) {
             int m[3];
-            api_extent(g, d, m);
-            Box b = make_box(g, 0, m[0], 0, m[1], 0, m[2]);
-            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(A_SB + S_B + d), m[0], m[1], tmp + off);
-            off += api_count(g, d);
+            api_extent(g, g.n[2], f, m);
+            Box b = make_box(g, 0, m[0], 0, m[1], 0, g.n[2]);
+            k_pack<<<grid_for(b), 128, 0, s>>>(g, b, arr(d, A_SB + S_B + f), m[0], m[1], 0, -1, tmp + off);
+            if (f == 2) {
+                Box top = make_box(g, 0, g.n[0], 0, g.n[1], g.n[2], g.n[2] + 1);
+                k_pack<<<grid_for(top), 128, 0, s>>>(g, top, arr(d, A_SB + S_B + 2), m[0], m[1], 0, 0, tmp + off);
+            }
+            off += api_count(g, g.n[2], f);
         }
         cudaStreamSynchronize(s);
         bad |= emit(Bf1, off);
     }
     if (W) {
         cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
-        for (int d = 0; d < g.ndim; d++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT + CT_W + d), g.n[0], g.n[1], tmp + d * n);
+        for (int f = 0; f < g.ndim; f++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_CT + CT_W + f), g.n[0], g.n[1], 0, -1, tmp + f * n);
         cudaStreamSynchronize(s);
         bad |= emit(W, 3 * n);
     }
     if (Fem) {
         cudaMemsetAsync(tmp, 0, 6 * n * sizeof(double), s);
-        for (int d = 0; d < g.ndim; d++)
+        for (int f = 0; f < g.ndim; f++)
             for (int q = 0; q < 2; q++)
-                k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(A_CT + CT_FEM + 2 * d + q), g.n[0], g.n[1], tmp + (2 * d + q) * n);
+                k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_CT + CT_FEM + 2 * f + q), g.n[0], g.n[1], 0, -1, tmp + (2 * f + q) * n);
         cudaStreamSynchronize(s);
         bad |= emit(Fem, 6 * n);
     }
     if (Eedge) {
         cudaMemsetAsync(tmp, 0, 3 * n * sizeof(double), s);
-        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, dbgE + (size_t)e * g.sa, g.n[0], g.n[1], tmp + e * n);
+        for (int e = (g.act[2] ? 0 : 2); e < 3; e++) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, dbgE.p + (size_t)e * g.sa, g.n[0], g.n[1], 0, -1, tmp + e * n);
         cudaStreamSynchronize(s);
         bad |= emit(Eedge, 3 * n);
     }
-    cudaFree(dbgE);
-    cudaFree(tmp);
     int err = 0;
     CUDA_TRY(cudaMemcpy(&err, &C.P->err, sizeof(int), cudaMemcpyDeviceToHost));
     CUDA_TRY(cudaMemcpy(C.P, &saved, sizeof saved, cudaMemcpyHostToDevice));

@@ -14,37 +14,55 @@ TOL_1STEP_MAXREL = 1e-10
 TOL_100STEP_L1REL = 1e-8
 
 
-def _scales(b, reduce):
-    """reference magnitude per component (R15).  For the 8-component state the three momentum and the three
-    field components share the magnitude of their vector: a component that is tiny against its vector
-    (B_z ~ 1e-10 growing out of noise in the 3D Orszag-Tang vortex) carries the round-off of the
-    vector's arithmetic, not of its own size."""
-    ref = [reduce(np.abs(b[v])) for v in range(b.shape[0])]
-    if b.shape[0] == 8:
+ZERO_COMPONENT_ABS = 1e-14      # R15: a component that is identically 0 in the oracle
+
+
+def _component_errors(a, b, reduce, pooled=False):
+    """R15: per component  reduce|a - b| / reduce|b|  with reduce = max or sum; a component
+    that is identically zero in the oracle must be <= 1e-14 absolute (returned as the second list).
+
+    pooled=True is the explicitly named SECOND metric, used only by the 3D Orszag-Tang cases: the three
+    momentum and the three field components are divided by the largest magnitude of their vector.  There
+    B_z is not identically zero but ~1e-10 of |B| (it grows out of the seeded noise), so its own scale is
+    far below the round-off of the vector arithmetic that produces it (|B| eps ~ 1e-16 against 1e-10)."""
+    ref = [float(reduce(np.abs(b[v]))) for v in range(b.shape[0])]
+    if pooled and b.shape[0] == 8:
         for grp in ((1, 2, 3), (4, 5, 6)):
             m = max(ref[v] for v in grp)
             for v in grp:
                 ref[v] = m
-    return ref
+    rel, absolute = [], []
+    for v in range(a.shape[0]):
+        d = float(reduce(np.abs(a[v] - b[v])))
+        if ref[v] > 0:
+            rel.append(d / ref[v])
+        else:
+            absolute.append(float(np.abs(a[v] - b[v]).max()))
+    return rel, absolute
+
+
+def _norm(a, b, reduce, pooled=False):
+    rel, absolute = _component_errors(a, b, reduce, pooled)
+    assert all(d <= ZERO_COMPONENT_ABS for d in absolute), ("component identically zero in the oracle", absolute)
+    return max(rel) if rel else 0.0
 
 
 def maxrel(a, b):
-    """per component: max|a-b| / max|b| (R15); components identically zero in the oracle: absolute"""
-    ref = _scales(b, np.max)
-    out = []
-    for v in range(a.shape[0]):
-        d = np.abs(a[v] - b[v]).max()
-        out.append(d / ref[v] if ref[v] > 0 else d / 1.0)
-    return max(out)
+    """per component max|a-b| / max|b| (R15, strict: every component against its own magnitude)"""
+    return _norm(a, b, np.max)
 
 
 def l1rel(a, b):
-    ref = _scales(b, np.sum)
-    out = []
-    for v in range(a.shape[0]):
-        d = np.abs(a[v] - b[v]).sum()
-        out.append(d / ref[v] if ref[v] > 0 else d)
-    return max(out)
+    """per component sum|a-b| / sum|b| (R15, strict)"""
+    return _norm(a, b, np.sum)
+
+
+def maxrel_vector_scaled(a, b):
+    return _norm(a, b, np.max, pooled=True)
+
+
+def l1rel_vector_scaled(a, b):
+    return _norm(a, b, np.sum, pooled=True)
 
 
 def faces_as_components(Bf, w):
@@ -272,6 +290,59 @@ def test_config4_full_size_sampled(pluto, oracle):
     pluto.finalize()
 
 
+def _full_size_multi_step(pluto, oracle, w, nsteps):
+    """the oracle run at FULL size next to the CUDA path, same seeded input, every element compared:
+    max-rel <= 1e-10 after one step, L1-rel <= 1e-8 after `nsteps` (north_star), strict per-component R15 norm"""
+    pluto.load(w)
+    oracle.load(w)
+    try:
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(1)
+        assert oracle.step(1) == 0
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+        pluto.step(nsteps - 1)
+        assert oracle.step(nsteps - 1) == 0
+        e_l1 = compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+        e_max = compare_state(pluto, oracle, w, 1e-6, norm=maxrel)      # reported; loose sanity bound only
+        assert abs(pluto.get_time() - oracle.get_time()) <= 1e-10 * oracle.get_time()
+        assert abs(pluto.get_dt() - oracle.get_dt()) <= 1e-10 * oracle.get_dt()
+        print("\n%s: %d steps at full size: L1-rel (U, faces) = %.2e, %.2e; max-rel = %.2e, %.2e"
+              % (w.name, nsteps, e_l1[0], e_l1[1], e_max[0], e_max[1]))
+    finally:
+        oracle.finalize()
+
+
+def test_config2_full_size_100_steps(pluto, oracle):
+    """configs[2] (2D Orszag-Tang 2048^2): 100 of its 200 steps, element-wise against the oracle at full size"""
+    _full_size_multi_step(pluto, oracle, wl.config(2), 100)
+
+
+def test_config3_full_size_50_steps(pluto, oracle):
+    """configs[3] (3D blast 256^3): all 50 steps, element-wise against the oracle at full size (~10 GB host)"""
+    _full_size_multi_step(pluto, oracle, wl.config(3), 50)
+
+
+def test_config4_full_size_one_step_whole_domain(pluto, oracle):
+    """configs[4] (3D blast 512^3): one step, every element, when the host can hold the oracle at 512^3
+    (63 resident doubles per zone for RK2 = 68 GB, plus the 24 GB of input/output copies); otherwise
+    test_config4_full_size_sampled (sub-boxes, one step) is the full-size evidence and DESIGN.md says so"""
+    import psutil
+    avail = psutil.virtual_memory().available / 2 ** 30
+    if avail < 110:
+        pytest.skip("host has %.0f GiB available: the 512^3 oracle needs ~95 GiB" % avail)
+    w = wl.config(4)
+    pluto.load(w)
+    oracle.load(w)
+    try:
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(1)
+        assert oracle.step(1) == 0
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+    finally:
+        oracle.finalize()
+        pluto.finalize()
+
+
 @pytest.mark.parametrize("cfg", [2, 3])
 def test_dt_bit_exact_at_full_size(pluto, oracle, cfg):
     """the filtered CFL reduction returns the oracle's dt bit for bit on the full-size initial states"""
@@ -321,17 +392,21 @@ def test_wenoz_parity(pluto, oracle, name, make, rk):
         oracle.load(w)
         oracle.set_integrator(rk)
         assert pluto.get_dt() == oracle.get_dt()
+        # 3D Orszag-Tang: B_z is analytically zero (v_z depends on z only) and grows out of the seeded noise
+        # to ~1e-10 |B|; it is compared on the scale of its vector (the named second metric of
+        # _component_errors); every other case uses the strict per-component R15 norm
+        n1, nl = (maxrel_vector_scaled, l1rel_vector_scaled) if name.startswith("ot3d") else (maxrel, l1rel)
         g = pluto.debug_euler(oracle.get_dt())
         o = oracle.debug_euler(oracle.get_dt())
         assert g["rc"] == 0 and o["rc"] == 0
-        assert maxrel(g["U1"].reshape(8, -1), o["U1"].reshape(8, -1)) <= 1e-11
+        assert n1(g["U1"].reshape(8, -1), o["U1"].reshape(8, -1)) <= 1e-11
         assert maxrel(g["Bf1"][None], o["Bf1"][None]) <= 1e-11
         pluto.step(1)
         assert oracle.step(1) == 0
-        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL, norm=n1)
         pluto.step(19)
         assert oracle.step(19) == 0
-        compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+        compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=nl)
     finally:
         pluto.set_integrator(2)
         oracle.set_integrator(2)
@@ -353,12 +428,13 @@ def test_paper_orszag_tang_3d_rk3(pluto, oracle):
         oracle.load(w)
         oracle.set_integrator(3)
         assert pluto.get_dt() == oracle.get_dt()
+        # B_z of this problem is noise-grown (~1e-10 |B|): vector-scaled metric, see test_wenoz_parity
         pluto.step(1)
         assert oracle.step(1) == 0
-        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL, norm=maxrel_vector_scaled)
         pluto.step(29)
         assert oracle.step(29) == 0
-        compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+        compare_state(pluto, oracle, w, TOL_100STEP_L1REL, norm=l1rel_vector_scaled)
     finally:
         pluto.set_integrator(2)
         oracle.set_integrator(2)
@@ -663,3 +739,65 @@ def test_uniform_state_is_a_fixed_point(pluto):
     pluto.step(3)
     U1, Bf1 = pluto.get_state()
     assert np.abs(U1 - U).max() <= 1e-15 and np.abs(Bf1 - Bf).max() <= 1e-15
+
+
+# ---------------------------------------------------------------- z-slab domain decomposition
+
+SLAB_CASES = [
+    ("blast_32_chunk", lambda: wl.blast_3d(32), 2, 2),
+    ("smooth_wrap64_mc", lambda: wl.random_smooth(64, 20, 26, seed=61, limiter=1, box=(1.0, 0.4, 0.5)), 2, 2),
+    ("smooth_ragged_rk3", lambda: wl.random_smooth(37, 23, 19, seed=62, limiter=0), 3, 2),
+    ("ot3d_wenoz_rk3", lambda: _wz(wl.orszag_tang_3d(32, noise=1e-3)), 3, 3),
+]
+
+
+@pytest.mark.parametrize("nslab", [2, 4])
+@pytest.mark.parametrize("name,make,rk,ghost", SLAB_CASES, ids=[s[0] for s in SLAB_CASES])
+def test_slabs_match_the_single_domain_bit_for_bit(pluto, name, make, rk, ghost, nslab):
+    """the box cut into z slabs (ghost planes pulled from the neighbour slab, one max for dt: section 3.4,
+    PAPER.md:208-244) advances exactly like the periodic single domain: same bits after 4 steps, same dt"""
+    w = make()
+    if w.nz // nslab < ghost + 1:
+        pytest.skip("slab thinner than ghost + 1 planes")
+    pluto.set_integrator(rk)
+    try:
+        pluto.load(w, ghost=ghost)
+        dt0 = pluto.get_dt()
+        pluto.step(4)
+        ref = pluto.get_state()
+        ref_dt, ref_t = pluto.get_dt(), pluto.get_time()
+        pluto.load(w, ghost=ghost, nslab=nslab)
+        assert pluto.get_dt() == dt0
+        pluto.step(4)
+        out = pluto.get_state()
+        assert pluto.get_dt() == ref_dt and pluto.get_time() == ref_t
+        assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
+    finally:
+        pluto.set_integrator(2)
+
+
+def test_slabs_against_the_oracle(pluto, oracle):
+    """the decomposed step against the oracle directly (not only against the single-domain CUDA run)"""
+    w = wl.random_smooth(40, 24, 21, seed=63, limiter=1)
+    pluto.load(w, nslab=3)
+    oracle.load(w)
+    assert pluto.get_dt() == oracle.get_dt()
+    pluto.step(2)
+    assert oracle.step(2) == 0
+    compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+
+
+def test_slab_argument_checks(pluto):
+    from paper_2511_20337_b200 import binding
+    with pytest.raises(binding.PlutoError):
+        pluto.init(16, 16, 8, 2, nslab=4)            # 2 planes per slab < ghost + 1
+    with pytest.raises(binding.PlutoError):
+        pluto.init(16, 16, 1, 2, nslab=2)            # 2D box
+    pluto.init(16, 16, 12, 2, nslab=4)
+    k0, n = ctypes_int(), ctypes_int()
+    assert pluto.L.pluto_local_planes(k0, n) == 0 and (k0.value, n.value) == (0, 12)
+
+
+def ctypes_int():
+    import ctypes
+    return ctypes.c_int(0)
