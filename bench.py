@@ -12,8 +12,11 @@ Prints ONE JSON line (rank 0).  Timing: CUDA events on the library's stream, bar
 synchronize on both sides, max over ranks.  The state (>= 1 GB) is larger than L2 (126 MB), so no
 explicit flush is needed between steps.
 
-Multi-GPU (torchrun): the path has no exchange step on one GPU and the north_star names none, so
-ranks run independent replicas of the workload ("replicas only") and value is the sum.
+Multi-GPU (torchrun, N > 1): the domain-decomposed step of the paper's section 3.4 in
+its weak-scaling shape (a fixed mesh per GPU): the box grows along z with N, every rank
+holds one 256^3 slab (configs[3]'s zones per GPU, one blast per slab-sized section), the ghost planes
+are pulled from the neighbour GPUs' memory inside the ghost-fill kernel and dt is one MAX all-reduce.
+value = all zones of the box x steps / max-over-ranks time; "scaling": "weak".
 """
 from __future__ import annotations
 
@@ -34,24 +37,72 @@ import numpy as np  # noqa: E402
 METRIC = "zone-updates/sec (fp64 3D MHD step, 1 B200); achieved HBM GB/s vs peak"
 UNIT = "zone-updates/s"
 
-# Algorithmic traffic of the sweep kernels, doubles per zone and launch; a
-# state is 5 hydro arrays + 3 face arrays (cell-centred B is never stored):
-#   sweep_xy  : read S 8, write S' 5, write CT data 9 (4 induction fluxes, 2 weights, 3 cell EMFs) = 22;
-#               the combine stage also reads S^n 5 = 27; the two launches of a step average 24.5
-#   sweep_x   : read S 8, write S' 5, CT data 6 (2 fluxes, 1 weight, 3 cell EMFs)                  = 19
-#   sweep_y/z : read S 8, read + write S' 5 + 5, CT data 3                                           = 21
-#   ct        : read CT data 12 + faces 3, write faces 3 = 18; the combine stage also reads S^n faces 3 = 21;
-#               the two launches of a step average 19.5
-#   dt_max    : read S 8
-ALGO_DOUBLES = {"sweep_xy": 24.5, "sweep_x": 19, "sweep_y": 21, "sweep_z": 21, "ct": 19.5, "dt_max": 8}
+# Bytes per zone and launch, two accountings (a state is 5 hydro + 3 face arrays):
+#   METHOD  -- what the method itself must move through this kernel if every stage reads each state
+#              array once and writes it once (320 B per zone-update for the whole step);
+#              this is the `achieved` / `frac` of the roofline object;
+#   DESIGN  -- what this implementation's kernel is written to move (METHOD + the CT work arrays it
+#              exchanges with the other kernels through HBM + re-reads across kernels); reported as
+#              `design_*` next to it, so that wasted traffic is visible.
+# Keyed by kernel class; values = doubles per zone for (first stage, combine stage).
+def kernel_doubles(ndim, rk):
+    """(method, design) doubles per zone per launch, averaged over the stages of one step"""
+    nface = 3 if ndim == 3 else 2
+    nct_xy = 9 if ndim == 3 else 5            # x/y induction fluxes + weights + cell EMFs kept for CT
+    combine_stages = rk - 1                   # stages that also read S^n
+    def avg(first, comb):
+        return (first + combine_stages * comb) / rk
+    method = {
+        # the x+y sweep reads S (8 arrays) [+ S^n hydro 5 in a combine stage] and writes S' hydro (5)
+        "sweep_xy": avg(8 + 5, 8 + 5 + 5),
+        "sweep_x": avg(8 + 5, 8 + 5 + 5), "sweep_y": avg(8 + 5, 8 + 5), "sweep_z": avg(8 + 5, 8 + 5),
+        # CT reads the faces (nface) [+ S^n faces] and writes them
+        "ct": avg(2 * nface, 3 * nface),
+        "dt_max": 8.0,
+    }
+    design = {
+        "sweep_xy": avg(8 + 5 + nct_xy, 8 + 5 + 5 + nct_xy),
+        "sweep_x": avg(8 + 5 + 6, 8 + 5 + 5 + 6), "sweep_y": 8 + 5 + 5 + 3, "sweep_z": 8 + 5 + 5 + 3,
+        "ct": avg((12 if ndim == 3 else 5) + 2 * nface, (12 if ndim == 3 else 5) + 3 * nface),
+        "dt_max": 8.0,
+    }
+    return method, design
 
-# From the committed ncu capture of the same workload (profiles/, `ncu --set full`, per launch, mean of the
-# stage-1 and stage-2 launches of a step): DRAM bytes moved and fp64-pipe instructions executed per zone.
-NCU = {
-    "sweep_xy": {"dram_bytes_per_launch": 3.54e9, "fp64_instr_per_zone": 576, "profile": "profiles/r1c_step_kernels.md"},
-    "sweep_z": {"dram_bytes_per_launch": 2.88e9, "fp64_instr_per_zone": 285, "profile": "profiles/r1c_step_kernels.md"},
-    "ct": {"dram_bytes_per_launch": 2.89e9, "fp64_instr_per_zone": 117, "profile": "profiles/r1c_step_kernels.md"},
-}
+
+def ncu_table(ndim, rk, limiter, zones):
+    """per-kernel DRAM bytes per launch and fp64-pipe instructions per zone from the newest committed
+    `profiles/r*_step_kernels.md` (an `ncu --set full` capture of configs[3], RK2, minmod); None for any
+    other scheme: those numbers do not transfer"""
+    import glob
+    import re
+    if not (ndim == 3 and rk == 2 and limiter == 0):
+        return None, None
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_step_kernels.md")))
+    if not files:
+        return None, None
+    path = files[-1]
+    cls = {"k_sweep_xy": "sweep_xy", "k_sweep_march<2": "sweep_z", "k_sweep_march<1": "sweep_y", "k_sweep_x<": "sweep_x",
+           "k_ct_tma": "ct", "k_ct<": "ct", "k_dtmax": "dt_max"}
+    acc = {}
+    for line in open(path):
+        m = re.match(r"\|\s*(k_[^|]+?)\s*\|(.+)\|\s*$", line)
+        if not m:
+            continue
+        cells = [c.strip() for c in m.group(2).split("|")]
+        if len(cells) < 10:
+            continue
+        name = m.group(1)
+        key = next((v for k, v in cls.items() if name.startswith(k)), None)
+        if key is None:
+            continue
+        try:
+            rd, wr, dp = float(cells[1]), float(cells[2]), float(cells[9])
+        except ValueError:
+            continue
+        acc.setdefault(key, []).append(((rd + wr) * 1e9, dp))
+    out = {k: {"dram_bytes_per_launch": sum(x[0] for x in v) / len(v) * (zones / 256 ** 3),
+               "fp64_instr_per_zone": sum(x[1] for x in v) / len(v)} for k, v in acc.items()}
+    return out, os.path.relpath(path, ROOT)
 
 
 def max_over_ranks(value, dist, device="cpu"):
@@ -65,7 +116,8 @@ def max_over_ranks(value, dist, device="cpu"):
 
 
 def aggregate_throughput(zones_per_rank, steps, ms_max, world):
-    """whole-job zone-updates/s of `world` independent replicas (replicas only)"""
+    """whole-job zone-updates/s: every rank advances its slab of zones_per_rank zones, the job takes as
+    long as its slowest rank"""
     return world * zones_per_rank * steps / (ms_max * 1e-3)
 
 
@@ -129,67 +181,80 @@ class ClockSampler:
                 "power_w": statistics.median(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_throughput(workload_small, budget_s=12.0, threads=None, rk=2, max_steps=400):
-    """the oracle as it stands, timed on the host cores (zone-updates/s): whole steps until ~budget_s
-    seconds of CPU work are done"""
+def oracle_run(w, steps, threads=None, rk=2, warmup=1):
+    """the oracle as it stands on the host cores: `steps` whole steps of workload w; returns
+    (zone-updates/s, threads used, seconds, per-step seconds)"""
     from oracle import Oracle
     o = Oracle()
     if threads:
         o.set_threads(threads)
-    o.load(workload_small)
+    o.load(w)
     o.set_integrator(rk)
-    o.step(1)                                   # touch memory
-    t0 = time.perf_counter()
-    steps = 0
-    while steps < max_steps:
+    for _ in range(warmup):
+        assert o.step(1) == 0                   # touch memory
+    per = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
         assert o.step(1) == 0
-        steps += 1
-        dt = time.perf_counter() - t0
-        if dt >= budget_s:
-            break
+        per.append(time.perf_counter() - t0)
     cores = o.get_threads()
     o.finalize()
-    return workload_small.zones * steps / dt, cores, dt, steps
+    return w.zones * steps / sum(per), cores, sum(per), per
 
 
-def sample_workload(cfg):
-    """bounded sample of configs[cfg] for the CPU legs: the same generator at a size the oracle steps in seconds"""
+def small_sample(cfg):
+    """a smaller instance of configs[cfg] from the same generator, for the single-thread figure"""
     from paper_2511_20337_b200 import workloads as wl
     if cfg == 5:
-        return wl.orszag_tang_3d(128, noise=1e-3), "orszag_tang_3d 128^3 (1/8 of the zones of the 256^3 run)"
+        return wl.orszag_tang_3d(96, noise=1e-3), "orszag_tang_3d 96^3"
     if cfg in (3, 4):
-        return wl.blast_3d(128, name="blast_3d_128 (1/8 of the zones of configs[3])"), "blast_3d 128^3, same recipe and seed as configs[3]"
+        return wl.blast_3d(96, name="blast_3d_96"), "blast_3d 96^3, same recipe and seed as configs[3]"
     if cfg == 2:
-        return wl.orszag_tang_2d(1024), "orszag_tang_2d 1024^2 (1/4 of the zones of configs[2])"
+        return wl.orszag_tang_2d(768), "orszag_tang_2d 768^2"
     return wl.config(cfg), f"configs[{cfg}] at full size"
 
 
+def cpu_workload(cfg):
+    """what the CPU legs step: the bench workload itself, except configs[4] (512^3: the oracle needs
+    ~70 GB and 25 s per step), which is represented by configs[3] -- same recipe, 1/8 of the zones"""
+    from paper_2511_20337_b200 import workloads as wl
+    if cfg == 4:
+        return wl.config(3), "configs[3] (256^3) standing in for configs[4]: same recipe and seed"
+    return wl.config(cfg), "the bench workload itself, full size"
+
+
+def scheme_of(w, rk):
+    return "recon(%s)+HLLD+RK%d+CT, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], rk, w.cfl)
+
+
+def config_of(args, w, world):
+    name = (f"configs[{args.config}] {w.name}" if args.config < 5
+            else f"paper section 4.1 workload (not a BASELINE config) {w.name}")
+    return {"workload": name, "grid": [w.nx, w.ny, w.nz], "zones": w.zones, "scheme": scheme_of(w, args.rk),
+            "l2": "inputs larger than L2 (state %.2f GB)" % (11 * w.zones * 8 / 1e9) if w.zones * 88 > 126e6
+                  else "L2 flushed between timed repeats (a 256 MB buffer is rewritten); the state fits in L2",
+            "parallelism": "single GPU" if world == 1 else "z-slab domain decomposition, one slab per GPU"}
+
+
 def run_reference(args):
-    """--impl reference: the oracle on the host cores, same metric/config keys (rank 0 only)"""
+    """--impl reference: the oracle on the host cores, same metric / config keys (rank 0 only).  Each step
+    is one whole oracle step of the bench workload (configs[3]: 256^3, ~3 s per step on 16 threads)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    w, what = sample_workload(args.config)
+    w, what = cpu_workload(args.config)
     if args.wenoz:
         w.limiter = 2
-    from oracle import Oracle
-    o = Oracle()
-    o.load(w)
-    o.set_integrator(args.rk)
-    for _ in range(args.warmup):
-        o.step(1)
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        assert o.step(1) == 0
-    dt = time.perf_counter() - t0
-    val = w.zones * args.steps / dt
-    cores = o.get_threads()
+    val, cores, secs, per = oracle_run(w, args.steps, rk=args.rk, warmup=max(1, min(args.warmup, 2)))
+    from paper_2511_20337_b200 import workloads as wl
+    wcfg = wl.config(args.config) if args.config != 4 else w
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD_NAMES.get(args.config, f"configs[{args.config}]"), "sample": what,
-                   "scheme": "recon(%s)+HLLD+RK%d+CT, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], args.rk, w.cfl)},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": f"{what}, {args.steps} steps"},
+        "config": config_of(args, wcfg, 1),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{what}, {args.steps} steps, {secs:.1f} s; warm-up capped at 2 steps",
+                         "best_step_s": min(per), "median_step_s": statistics.median(per)},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line))
@@ -206,6 +271,7 @@ def main():
     ap.add_argument("--rk", type=int, default=2, help="2: SSP-RK2 (the north_star's step, default); 3: SSP-RK3 of Eq. 5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--repeats", type=int, default=3, help="timed repeats of the K steps (median and best reported)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -219,14 +285,8 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
-    dist = None
     if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
+        return main_slabs(args, rank, world, local)
 
     w = wl.config(args.config)
     if args.wenoz:
@@ -236,28 +296,32 @@ def main():
     sim.load(w)
     K, W = args.steps, max(args.warmup, 3)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    small = w.zones * 88 <= 126e6                 # the state fits in L2: flush it between repeats
+    flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=sim.device) if small else None
 
-    # ---------------- device-resident timing: K steps, state already in HBM
+    # ---------------- device-resident timing: K steps, state already in HBM; >= 3 repeats
     sim.step(W)
-    launches0 = sim.launch_count()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.3)
-    barrier()
-    torch.cuda.synchronize()
+    times, launches = [], 0
     t0 = time.time()
-    e0.record(sim.stream)
-    sim.step_async(K)
-    e1.record(sim.stream)
-    sim.sync()
-    torch.cuda.synchronize()
-    barrier()
+    for rep_i in range(max(args.repeats, 1)):
+        if flush is not None:
+            flush.fill_(rep_i)
+        torch.cuda.synchronize()
+        l0 = sim.launch_count()
+        e0.record(sim.stream)
+        sim.step_async(K)
+        e1.record(sim.stream)
+        sim.sync()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+        launches = sim.launch_count() - l0
     t1 = time.time()
-    ms = e0.elapsed_time(e1)
     clocks = sampler.stop(t0, t1)
-    launches = sim.launch_count() - launches0
-    ms = max_over_ranks(ms, dist, "cuda")
-    value = aggregate_throughput(w.zones, K, ms, world)
+    ms = statistics.median(times)
+    value = w.zones * K / (ms * 1e-3)
 
     # ---------------- per-kernel timing of the same K steps (events around every launch)
     sim.profile(True)
@@ -273,85 +337,185 @@ def main():
     dom = max(rep, key=lambda k: rep[k][0])
     dom_ms, dom_cnt = rep[dom]
     hbm_peak, peak_src = peaks()
-    # units one launch of the dominant kernel processes
-    units = w.zones
-    algo_bytes = ALGO_DOUBLES.get(dom, 0) * 8 * units
+    units = w.zones                              # zones one launch of the dominant kernel processes
+    method, design = kernel_doubles(w.ndim, args.rk)
+    ncu, ncu_src = ncu_table(w.ndim, args.rk, w.limiter, units)
     dur = dom_ms * 1e-3 / max(dom_cnt, 1)
-    achieved = algo_bytes / dur * 1e-9 if dur > 0 else 0.0
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src,
-                "avg_launch_ms": dur * 1e3, "launches": dom_cnt, "share_of_step": dom_ms / total_kernel_ms,
-                "algorithmic_bytes_per_launch": algo_bytes,
-                "kernels_ms_per_step": {k: v[0] / K for k, v in rep.items() if v[1]},
-                "profiled_ms_per_step": ms_prof / K}
-    # the same HBM view for every kernel of the step (algorithmic bytes / live launch time / HBM peak)
-    roofline["all_kernels_hbm_frac"] = {
-        k: round(ALGO_DOUBLES[k] * 8 * units / (v[0] * 1e-3 / v[1]) * 1e-9 / hbm_peak, 4)
-        for k, v in rep.items() if v[1] and k in ALGO_DOUBLES}
-    if dom in NCU:
-        roofline["traffic"] = NCU[dom]["dram_bytes_per_launch"] * (units / 256 ** 3)   # scaled from the 256^3 capture
-        roofline["traffic_source"] = NCU[dom]["profile"]
-        # the same kernel against the fp64 pipe: instructions executed per second vs the probed DFMA rate
-        fp64_peak = sim.probe_fp64_gflops() * 0.5e9            # DFMA/s (2 flops each)
-        rate = NCU[dom]["fp64_instr_per_zone"] * units / dur if dur > 0 else 0.0
-        roofline["alu"] = {"bound": "alu", "achieved": rate * 1e-12, "peak": fp64_peak * 1e-12, "unit": "T fp64-instr/s",
-                           "frac": rate / fp64_peak, "peak_source": "pluto_probe_fp64_gflops (register-resident DFMA loop, this run)",
-                           "fp64_instr_per_zone": NCU[dom]["fp64_instr_per_zone"]}
-    # whole-step view: minimum traffic 320 B per zone-update
-    roofline["step_hbm_frac_at_320B"] = value / world * 320.0 / (hbm_peak * 1e9)
+    method_bytes = method.get(dom, 0) * 8 * units
+    design_bytes = design.get(dom, 0) * 8 * units
+    hbm_achieved = method_bytes / dur * 1e-9 if dur > 0 else 0.0
+    hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_achieved / hbm_peak,
+           "algorithmic_bytes_per_launch": method_bytes, "algorithmic_doubles_per_zone": method.get(dom),
+           "design_bytes_per_launch": design_bytes, "design_doubles_per_zone": design.get(dom),
+           "design_frac": design_bytes / dur * 1e-9 / hbm_peak if dur > 0 else 0.0,
+           "peak_source": peak_src}
+    fp64_peak = sim.probe_fp64_gflops() * 0.5e9   # DFMA/s (2 flops each), register-resident loop, this run
+    alu = None
+    if ncu and dom in ncu:
+        rate = ncu[dom]["fp64_instr_per_zone"] * units / dur if dur > 0 else 0.0
+        alu = {"bound": "alu", "achieved": rate * 1e-12, "peak": fp64_peak * 1e-12, "unit": "T fp64-instr/s",
+               "frac": rate / fp64_peak, "fp64_instr_per_zone": ncu[dom]["fp64_instr_per_zone"],
+               "peak_source": "pluto_probe_fp64_gflops (register-resident DFMA loop, this run); "
+                              "nominal 148 SM x 64 lanes x 1.965 GHz = 18.6 T/s"}
+    # the roofline that binds the dominant kernel is the one it is closer to
+    primary = alu if (alu and alu["frac"] > hbm["frac"]) else hbm
+    roofline = dict(primary)
+    roofline.update({"kernel": dom, "traffic": ncu[dom]["dram_bytes_per_launch"] if ncu and dom in ncu else None,
+                     "traffic_source": ncu_src if ncu and dom in ncu else "no ncu capture of this scheme is committed",
+                     "avg_launch_ms": dur * 1e3, "launches": dom_cnt, "share_of_step": dom_ms / total_kernel_ms,
+                     "hbm": hbm, "alu": alu,
+                     "kernels_ms_per_step": {k: v[0] / K for k, v in rep.items() if v[1]},
+                     "profiled_ms_per_step": ms_prof / K})
+    # the same two views for every kernel of the step
+    roofline["all_kernels"] = {
+        k: {"hbm_frac": round(method[k] * 8 * units / (v[0] * 1e-3 / v[1]) * 1e-9 / hbm_peak, 4),
+            "design_hbm_frac": round(design[k] * 8 * units / (v[0] * 1e-3 / v[1]) * 1e-9 / hbm_peak, 4),
+            "alu_frac": round(ncu[k]["fp64_instr_per_zone"] * units / (v[0] * 1e-3 / v[1]) / fp64_peak, 4) if ncu and k in ncu else None}
+        for k, v in rep.items() if v[1] and k in method}
+    # whole-step view: 320 B per zone-update against the HBM peak, and the step's fp64-pipe
+    # instructions against the probed fp64 peak
+    roofline["step_hbm_frac_at_320B"] = value * 320.0 / (hbm_peak * 1e9)
+    if ncu:
+        per_zu = sum(ncu[k]["fp64_instr_per_zone"] * (rep[k][1] / K) for k in ncu if k in rep and rep[k][1])
+        roofline["step_fp64_instr_per_zone_update"] = per_zu
+        roofline["step_alu_frac"] = value * per_zu / fp64_peak
+        roofline["step_dram_bytes_per_zone_update"] = sum(ncu[k]["dram_bytes_per_launch"] * (rep[k][1] / K)
+                                                          for k in ncu if k in rep and rep[k][1]) / units
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": (f"configs[{args.config}] {w.name}" if args.config < 5 else f"paper section 4.1 workload (not a BASELINE config) {w.name}"), "grid": [w.nx, w.ny, w.nz], "zones": w.zones,
-                   "scheme": "recon(%s)+HLLD+RK%d+CT, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], args.rk, w.cfl),
-                   "l2": "inputs larger than L2 (state %.2f GB)" % (11 * w.zones * 8 / 1e9),
-                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "dtype": "f64", "data": "synthetic", "config": config_of(args, w, world),
+        "timing": {"repeats": len(times), "median_ms_per_step": ms / K, "best_ms_per_step": min(times) / K,
+                   "all_ms_per_step": [t / K for t in times]},
         "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline,
     }
 
     # ---------------- end to end through the C ABI with HOST buffers
-    if rank == 0 or world > 1:
-        Uh = torch.from_numpy(w.U).pin_memory()
-        Bh = torch.from_numpy(w.Bface).pin_memory()
-        Uo = torch.empty_like(Uh).pin_memory()
-        Bo = torch.empty_like(Bh).pin_memory()
-        Un, Bn, Uon, Bon = Uh.numpy(), Bh.numpy(), Uo.numpy(), Bo.numpy()
-        sim.set_state(Un, Bn)
+    Uh = torch.from_numpy(w.U).pin_memory()
+    Bh = torch.from_numpy(w.Bface).pin_memory()
+    Uo = torch.empty_like(Uh).pin_memory()
+    Bo = torch.empty_like(Bh).pin_memory()
+    Un, Bn, Uon, Bon = Uh.numpy(), Bh.numpy(), Uo.numpy(), Bo.numpy()
+    sim.set_state(Un, Bn)
+    sim.step(1)
+    sim.get_state(Uon, Bon)
+    torch.cuda.synchronize()
+    tw0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        sim.set_state(Un, Bn)               # host -> device inside the timed region
         sim.step(1)
-        sim.get_state(Uon, Bon)
-        barrier()
-        torch.cuda.synchronize()
-        tw0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            sim.set_state(Un, Bn)               # host -> device inside the timed region
-            sim.step(1)
-            sim.get_state(Uon, Bon)             # device -> host read of the step's result
-        torch.cuda.synchronize()
-        te = (time.perf_counter() - tw0) / args.e2e_steps
-        te = max_over_ranks(te, dist, "cuda")
-        nbytes = (Uh.numel() + Bh.numel()) * 8
-        # pluto_set_state does not copy U[4..6] of the active dimensions (the cell-centred B is the face mean)
-        h2d = (Uh.numel() // 8 * (5 if w.nz > 1 else 6) + Bh.numel()) * 8
-        line["e2e"] = {"value": world * w.zones / te, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                       "d2h_bytes_per_step": nbytes, "ms_per_step": te * 1e3, "steps": args.e2e_steps}
+        sim.get_state(Uon, Bon)             # device -> host read of the step's result
+    torch.cuda.synchronize()
+    te = (time.perf_counter() - tw0) / args.e2e_steps
+    nbytes = (Uh.numel() + Bh.numel()) * 8
+    # pluto_set_state does not copy U[4..6] of the active dimensions (the cell-centred B is the face mean)
+    h2d = (Uh.numel() // 8 * (5 if w.nz > 1 else 6) + Bh.numel()) * 8
+    line["e2e"] = {"value": w.zones / te, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": nbytes, "ms_per_step": te * 1e3, "steps": args.e2e_steps}
+    sim.finalize()
 
-    # ---------------- the oracle timed beside it (rank 0, N = 1 only)
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        ws, what = sample_workload(args.config)
+    # ---------------- the oracle timed beside it (N = 1 only): the bench workload itself on every host
+    # thread (3 steps), and a single-thread figure on a smaller instance of the same generator
+    if not args.no_cpu_baseline:
+        wc, what = cpu_workload(args.config)
+        if args.wenoz:
+            wc.limiter = 2
+        v, cores, secs, per = oracle_run(wc, 3, rk=args.rk)
+        ws, what1 = small_sample(args.config)
         if args.wenoz:
             ws.limiter = 2
-        v, cores, secs, steps = oracle_throughput(ws, rk=args.rk)
+        v1, _, secs1, _ = oracle_run(ws, 1, threads=1, rk=args.rk, warmup=0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{what}, {steps} steps, {secs:.1f} s"}
+                                "sample": f"{what}, 3 steps, {secs:.1f} s",
+                                "best_step_s": min(per), "median_step_s": statistics.median(per),
+                                "single_thread": {"value": v1, "cores": 1, "sample": f"{what1}, 1 step, {secs1:.1f} s"}}
     else:
         line["cpu_baseline"] = None
+    print(json.dumps(line))
 
+
+def main_slabs(args, rank, world, local):
+    """N > 1: one z slab per rank (paper_2511_20337_b200.distributed.SlabPluto), weak scaling"""
+    import torch
+    import torch.distributed as dist
+    from paper_2511_20337_b200 import workloads as wl
+    from paper_2511_20337_b200.distributed import SlabPluto
+
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    base = wl.config(args.config)                    # scheme parameters and the per-GPU mesh
+    if base.nz < 2:
+        raise SystemExit("the z-slab decomposition needs a 3D config")
+    nx, ny, nzl = base.nx, base.ny, base.nz
+    nz = nzl * world
+    sim = SlabPluto(dist, device=local)
+    sim.set_integrator(args.rk)
+    limiter = 2 if args.wenoz else base.limiter
+    ghost = 3 if args.wenoz else 2
+    U, Bl, box = wl.blast_3d_planes(nx, ny, nz, rank * nzl, nzl, nblast=world, gamma=base.gamma)
+    sim.init(nx, ny, nz, ghost, base.gamma, base.cfl, limiter, box=box)
+    assert (sim.k0, sim.nzl) == (rank * nzl, nzl)
+    Uh, Bh = torch.from_numpy(U).pin_memory(), torch.from_numpy(Bl).pin_memory()
+    sim.set_state(Uh.numpy(), Bh.numpy())
+    K, W = args.steps, max(args.warmup, 3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.step(W)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    times = []
+    t0 = time.time()
+    for _ in range(max(args.repeats, 1)):
+        dist.barrier()
+        torch.cuda.synchronize()
+        l0 = sim.launch_count()
+        e0.record(sim.stream)
+        sim.step_async(K)
+        e1.record(sim.stream)
+        sim.sync()
+        torch.cuda.synchronize()
+        dist.barrier()
+        times.append(max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
+        launches = sim.launch_count() - l0
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms = statistics.median(times)
+    zones = nx * ny * nzl
+    value = aggregate_throughput(zones, K, ms, world)
+    hbm_peak, peak_src = peaks()
+    # end to end: every rank's planes from pinned host memory and back, every step
+    tw0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        sim.set_state(Uh.numpy(), Bh.numpy())
+        sim.step(1)
+        sim.get_state()
+    torch.cuda.synchronize()
+    te = max_over_ranks((time.perf_counter() - tw0) / args.e2e_steps, dist, "cuda")
+    h2d = (U.size // 8 * 5 + Bl.size) * 8
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[%d] %s per GPU, box %dx%dx%d cut into %d z slabs (one blast per slab-sized section)"
+                               % (args.config, base.name, nx, ny, nz, world),
+                   "grid": [nx, ny, nz], "zones": zones * world, "zones_per_gpu": zones,
+                   "scheme": scheme_of(base, args.rk) if not args.wenoz else scheme_of(base, args.rk).replace("minmod", "WENOZ").replace("MC", "WENOZ"),
+                   "l2": "inputs larger than L2 (state %.2f GB per GPU)" % (11 * zones * 8 / 1e9),
+                   "parallelism": "z-slab domain decomposition, one slab per GPU; ghost planes pulled from peer memory "
+                                  "(CUDA IPC over NVLink) inside the ghost-fill kernel; 1 MAX all-reduce + %d barriers per step" % (args.rk - 1)},
+        "timing": {"repeats": len(times), "median_ms_per_step": ms / K, "best_ms_per_step": min(times) / K},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "achieved": value / world * 320.0 * 1e-9, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": value / world * 320.0 / (hbm_peak * 1e9), "traffic": None, "peak_source": peak_src,
+                     "note": "per-GPU whole-step view at the method's 320 B per zone-update; the per-kernel rooflines are those of the N = 1 line"},
+        "e2e": {"value": world * zones / te, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": (U.size + Bl.size) * 8,
+                "ms_per_step": te * 1e3, "steps": args.e2e_steps},
+        "cpu_baseline": None,
+    }
+    sim.finalize()
     if rank == 0:
         print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    dist.destroy_process_group()
 
 
 if __name__ == "__main__":

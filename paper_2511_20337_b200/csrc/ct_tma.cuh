@@ -162,8 +162,8 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
             const double ezx = e[1], ezy = e[CT_TX];
             const long long c = (long long)zc(k) * st2 + oc;
             if (TWO_D) {
-                const double bxn = pbx - dtdy * (ezy - ez);
-                const double byn = pby + dtdx * (ezx - ez);
+                const double bxn = fma(-dtdy, ezy - ez, pbx);
+                const double byn = fma(dtdx, ezx - ez, pby);
                 const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                 bout[c] = bxo;
                 if (i == 0) bout[c + g.n[0]] = bxo;       // periodic copy: x-face n0 is face 0
@@ -172,8 +172,8 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
             } else {
                 if (k > k0) {                    // b_x, b_y of plane k-1
                     const long long cm = (long long)zc(k - 1) * st2 + oc;
-                    const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
-                    const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
+                    const double bxn = fma(-dtdy, dEzy, fma(dtdz, eyN - eyP, pbx));
+                    const double byn = fma(-dtdz, exN - exP, fma(dtdx, dEzx, pby));
                     const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                     bout[cm] = bxo;
                     if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
@@ -181,7 +181,7 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
                 }
                 if (k < k1) {                    // b_z on the lower face of plane k
                     const double eyx = e[2 * CT_TX * CT_TY + 1], exy = e[CT_TX * CT_TY + CT_TX];
-                    const double bzn = pbz - (dtdx * (eyx - eyN) - dtdy * (exy - exN));
+                    const double bzn = fma(-dtdx, eyx - eyN, fma(dtdy, exy - exN, pbz));
                     bout[2 * sa + c] = COMBINE ? fma(cb.wn, qbz, cb.ws * bzn) : bzn;
                     if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
                     // operands of the next iteration: b_x, b_y of this plane, b_z of the next

@@ -77,70 +77,108 @@ k_dtmax(Grid g, const double *__restrict__ U, const double *__restrict__ bz_up, 
     const long long sa = g.sa;
     const double *__restrict__ b = U + S_B * sa;
     const double gm1 = g.gamma - 1.0;
+    __shared__ double sbound[256];                       // filter 0: the bounds of the block's next 256 rows
+    __shared__ double swmax[8];
+    __shared__ int swarg[8];
     double smax = 0.0, published = 0.0, seen = 0.0;      // published, seen: uniform across the warp
-    int nrow = 0;                                        // rows this block has visited
+    int nrow = 0;                                        // rows this warp has visited
     int bad = 0;
-    for (int row = blockIdx.x; row < nrows; row += gridDim.x) {
-        const int k = row / g.n[1], j = row - k * g.n[1];
-        // the global running maximum is re-read on each of a block's first eight visited rows, while it is
-        // still rising fast, then every eighth row
-        if (nrow < 8 || (nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
-        if (bg.b) {                                                              // filter 0 (warp uniform)
-            const double bound = __longlong_as_double((long long)bg.b[(long long)(k / bg.bk) * bg.nbj + j / bg.bj]);
-            if (bound < fmax(seen, published)) continue;
-        }
-        const long long r0 = g.at(0, j, k);
-        const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
-        const bool top = g.act[2] && k + 1 == g.n[2];
-        const double *__restrict__ bzu = top ? bz_up + g.at(0, j, 0) : b + 2 * sa + r0 + g.st[2];
-        double thr = fmax(smax, fmax(seen, published));
-        for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
-            const long long c = r0 + i;
-            const double rho = U[c], mx = U[sa + c], my = U[2 * sa + c], mz = U[3 * sa + c], E = U[4 * sa + c];
-            // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
-            const double B[3] = { 0.5 * (b[c] + b[r0 + (i + 1 == g.n[0] ? 0 : i + 1)]),
-                                  0.5 * (b[sa + c] + b[sa + c + upj]),
-                                  g.act[2] ? 0.5 * (b[2 * sa + c] + bzu[i]) : b[2 * sa + c] };
-            const double ir = rcp_nr(rho);
-            const double B2 = fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2]));
-            const double vx = mx * ir, vy = my * ir, vz = mz * ir;
-            const double pf = gm1 * (E - 0.5 * fma(mx, vx, fma(my, vy, mz * vz)) - 0.5 * B2);
-            const double a2 = g.gamma * pf * ir;
-            // rho <= 0, p <= 0, NaN or inf: flag, and let the exact path decide what enters the maximum
-            const bool odd = (unsigned)(__double2hiint(rho) - 0x00100000) >= 0x7fe00000u ||
-                             (unsigned)(__double2hiint(pf) - 0x00100000) >= 0x7fe00000u;
-            if (!odd) {
-                const double cb = sqrt_nr(fma(B2, ir, a2));
-                double ub = 0.0;
-                if (g.act[0]) ub = fmax(ub, (fabs(vx) + cb) * g.idx[0]);
-                if (g.act[1]) ub = fmax(ub, (fabs(vy) + cb) * g.idx[1]);
-                if (g.act[2]) ub = fmax(ub, (fabs(vz) + cb) * g.idx[2]);
-                if (ub * (1.0 + 1e-9) < thr) continue;                       // filter 1
-                const double v[3] = { vx, vy, vz };
-                const double s = fma(B2, ir, a2);
-                double est = 0.0;
-#pragma unroll
-                for (int d = 0; d < 3; d++) {
-                    if (!g.act[d]) continue;
-                    const double disc = fma(s, s, -4.0 * a2 * (B[d] * B[d] * ir));
-                    const double cf = sqrt_nr(0.5 * (s + sqrt_nr(fmax(disc, 1e-300))));
-                    est = fmax(est, (fabs(v[d]) + cf) * g.idx[d]);
-                }
-                if (est * (1.0 + 1e-7) < thr) continue;                      // filter 2
+    // the block's rows are blockIdx.x + n * gridDim.x; they are taken 256 at a time: every thread fetches
+    // the bound of one of them (one memory round trip per 256 rows instead of one per row)
+    for (int chunk = blockIdx.x; chunk < nrows; chunk += 256 * gridDim.x) {
+        {
+            const long long myrow = chunk + (long long)threadIdx.x * gridDim.x;
+            double bd = 1e300;
+            if (bg.b && myrow < nrows) {
+                const int k = (int)(myrow / g.n[1]), j = (int)(myrow - (long long)k * g.n[1]);
+                bd = __longlong_as_double((long long)bg.b[(long long)(k / bg.bk) * bg.nbj + j / bg.bj]);
             }
-            const double sig = zone_sigma_exact(g, rho, mx, my, mz, E, B, bad);
-            if (sig > smax) smax = sig;
-            if (sig > thr) thr = sig;
+            // the row with the largest bound is visited first: its exact candidates raise the running maximum
+            // at once, and most other rows are then skipped unread
+            double wb = myrow < nrows ? bd : -1.0;
+            int wa = threadIdx.x;
+            for (int o = 16; o > 0; o >>= 1) {
+                const double ob = __shfl_xor_sync(0xffffffffu, wb, o);
+                const int oa = __shfl_xor_sync(0xffffffffu, wa, o);
+                if (ob > wb || (ob == wb && oa < wa)) { wb = ob; wa = oa; }
+            }
+            __syncthreads();                             // the previous chunk's bounds are no longer read
+            sbound[threadIdx.x] = bd;
+            if ((threadIdx.x & 31) == 0) { swmax[threadIdx.x >> 5] = wb; swarg[threadIdx.x >> 5] = wa; }
+            __syncthreads();
         }
-        // publish the warp's maximum when it raises the global one (rare after the first rows)
-        if (nrow < 8 || (nrow & 7) == 7) {
-            double wm = smax;
-            for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
-            if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published))
-                atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
-            published = fmax(published, wm);
+        int first = 0;
+        {
+            double fb = -2.0;
+            for (int w = 0; w < (int)(blockDim.x >> 5); w++)
+                if (swmax[w] > fb) { fb = swmax[w]; first = swarg[w]; }
         }
-        nrow++;
+        seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
+        for (int it = 0; it < 257; it++) {
+            // visiting order: the row with the largest bound, then the others in order
+            const int n = it == 0 ? first : it - 1;
+            if (it > 0 && n == first) continue;
+            const long long row64 = chunk + (long long)n * gridDim.x;
+            if (row64 >= nrows) { if (it == 0) continue; else break; }
+            if (sbound[n] < fmax(seen, published)) continue;                     // filter 0 (warp uniform)
+            const int row = (int)row64;
+            const int k = row / g.n[1], j = row - k * g.n[1];
+            // the global running maximum is re-read on each of a warp's first eight visited rows, while it is
+            // still rising fast, then every eighth row
+            if (nrow < 8 || (nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
+            const long long r0 = g.at(0, j, k);
+            const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
+            const bool top = g.act[2] && k + 1 == g.n[2];
+            const double *__restrict__ bzu = top ? bz_up + g.at(0, j, 0) : b + 2 * sa + r0 + g.st[2];
+            double thr = fmax(smax, fmax(seen, published));
+            for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
+                const long long c = r0 + i;
+                const double rho = U[c], mx = U[sa + c], my = U[2 * sa + c], mz = U[3 * sa + c], E = U[4 * sa + c];
+                // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
+                const double B[3] = { 0.5 * (b[c] + b[r0 + (i + 1 == g.n[0] ? 0 : i + 1)]),
+                                      0.5 * (b[sa + c] + b[sa + c + upj]),
+                                      g.act[2] ? 0.5 * (b[2 * sa + c] + bzu[i]) : b[2 * sa + c] };
+                const double ir = rcp_nr(rho);
+                const double B2 = fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2]));
+                const double vx = mx * ir, vy = my * ir, vz = mz * ir;
+                const double pf = gm1 * (E - 0.5 * fma(mx, vx, fma(my, vy, mz * vz)) - 0.5 * B2);
+                const double a2 = g.gamma * pf * ir;
+                // rho <= 0, p <= 0, NaN or inf: flag, and let the exact path decide what enters the maximum
+                const bool odd = (unsigned)(__double2hiint(rho) - 0x00100000) >= 0x7fe00000u ||
+                                 (unsigned)(__double2hiint(pf) - 0x00100000) >= 0x7fe00000u;
+                if (!odd) {
+                    const double cb = sqrt_nr(fma(B2, ir, a2));
+                    double ub = 0.0;
+                    if (g.act[0]) ub = fmax(ub, (fabs(vx) + cb) * g.idx[0]);
+                    if (g.act[1]) ub = fmax(ub, (fabs(vy) + cb) * g.idx[1]);
+                    if (g.act[2]) ub = fmax(ub, (fabs(vz) + cb) * g.idx[2]);
+                    if (ub * (1.0 + 1e-9) < thr) continue;                       // filter 1
+                    const double v[3] = { vx, vy, vz };
+                    const double s = fma(B2, ir, a2);
+                    double est = 0.0;
+#pragma unroll
+                    for (int d = 0; d < 3; d++) {
+                        if (!g.act[d]) continue;
+                        const double disc = fma(s, s, -4.0 * a2 * (B[d] * B[d] * ir));
+                        const double cf = sqrt_nr(0.5 * (s + sqrt_nr(fmax(disc, 1e-300))));
+                        est = fmax(est, (fabs(v[d]) + cf) * g.idx[d]);
+                    }
+                    if (est * (1.0 + 1e-7) < thr) continue;                      // filter 2
+                }
+                const double sig = zone_sigma_exact(g, rho, mx, my, mz, E, B, bad);
+                if (sig > smax) smax = sig;
+                if (sig > thr) thr = sig;
+            }
+            // publish the warp's maximum when it raises the global one (rare after the first rows)
+            if (nrow < 8 || (nrow & 7) == 7) {
+                double wm = smax;
+                for (int o = 16; o > 0; o >>= 1) wm = fmax(wm, __shfl_xor_sync(0xffffffffu, wm, o));
+                if ((threadIdx.x & 31) == 0 && wm > fmax(seen, published))
+                    atomicMax(&P->smax_bits, (unsigned long long)__double_as_longlong(wm));
+                published = fmax(published, wm);
+            }
+            nrow++;
+        }
     }
     {
         double wm = smax;

@@ -201,25 +201,42 @@ __device__ __forceinline__ void cell_b(const Grid &g, const double *__restrict__
 }
 
 // ---------------------------------------------------------------- CFL pre-filter written by the last stage (a8)
-// The kernel that writes the final hydro variables of a step also leaves, per cell of a coarse "bound
-// grid" (one cell = the part of a row-march segment a thread covers: bj rows x bk planes), an UPPER BOUND
-// of every CFL candidate (|v_d| + c_f,d)/dx_d of the zones in it.  The exact reduction of the next step
+// In 3D the z sweep, which writes the final hydro variables of a step, also leaves, per cell of a coarse
+// "bound grid" (grid.h BoundGrid; one cell = the zones one thread finishes: a row of a z segment), an UPPER BOUND of
+// every CFL candidate (|v_d| + c_f,d)/dx_d of the zones in it.  The exact reduction of the next step
 // (dt_kernel.cu) then only visits rows whose bound can still hold the maximum; the dt stays bit-exact
 // because a skipped row provably cannot raise it.  The bound needs no magnetic field (the final faces are
-// written later by the CT kernel):  c_f,d^2 <= (gamma p + B^2)/rho  and, with p >= 0,
-// B^2 <= 2 (E - K), K = |m|^2/(2 rho), so  gamma p + B^2 <= max(gamma (gamma-1), 2) (E - K).
-__device__ __forceinline__ double sigma_bound(const Grid &g, double cfac, double rho, double mx, double my, double mz, double En)
-{
-    const double ir = rcp_fast(rho);
-    const double eint = En - 0.5 * ir * fma(mx, mx, fma(my, my, mz * mz));
-    if (unphysical(rho) || unphysical(eint)) return __longlong_as_double(0x7fe0000000000000ll);   // visit it
-    const double cs = sqrt_fast(cfac * eint * ir);
-    double b = 0.0;
-    if (g.act[0]) b = fmax(b, fma(fabs(mx), ir, cs) * g.idx[0]);
-    if (g.act[1]) b = fmax(b, fma(fabs(my), ir, cs) * g.idx[1]);
-    if (g.act[2]) b = fmax(b, fma(fabs(mz), ir, cs) * g.idx[2]);
-    return b * (1.0 + 1e-9);
-}
+// written later by the CT kernel) and no division per zone:
+//     c_f,d^2 <= (gamma p + B^2)/rho,   p >= 0  =>  B^2 <= 2 (E - K) <= 2 E,
+//     gamma p + B^2 <= max(gamma (gamma - 1), 2) E   (linear in B^2 on [0, 2E]),
+// so with the minimum density, the maximum energy and the maximum of |m_d|/dx_d over the thread's zones
+//     (|v_d| + c_f,d)/dx_d <= ( max|m_d|/dx_d + sqrt(cfac E_max rho_min) max(1/dx_d) ) / rho_min.
+// The three running values live in shared memory (slot[0], slot[stride], slot[2 stride] of the thread):
+// the marching kernels have no registers to spare.
+struct SigmaBound {
+    double *slot;
+    int stride;
+    __device__ __forceinline__ void init(double *p, int st) { slot = p; stride = st; p[0] = 1e300; p[st] = 0.0; p[2 * st] = 0.0; }
+    __device__ __forceinline__ void add(const Grid &g, double rho, double mx, double my, double mz, double En)
+    {
+        slot[0] = fmin(slot[0], rho);
+        slot[stride] = fmax(slot[stride], En);
+        double m = fabs(mx) * g.idx[0];
+        if (g.act[1]) m = fmax(m, fabs(my) * g.idx[1]);
+        if (g.act[2]) m = fmax(m, fabs(mz) * g.idx[2]);
+        slot[2 * stride] = fmax(slot[2 * stride], m);
+    }
+    // (a NaN never enters fmin / fmax; such a zone is reported by the sweeps' own check)
+    __device__ __forceinline__ double value(const Grid &g, double cfac) const
+    {
+        const double rho_min = slot[0], e_max = slot[stride], m_max = slot[2 * stride];
+        double imax = g.idx[0];
+        if (g.act[1]) imax = fmax(imax, g.idx[1]);
+        if (g.act[2]) imax = fmax(imax, g.idx[2]);
+        const double b = (m_max + sqrt(cfac * e_max * rho_min) * imax) / rho_min * (1.0 + 1e-9);
+        return (rho_min > 0.0 && b >= 0.0 && b < 1e300) ? b : 1e300;          // unknown: visit the row
+    }
+};
 
 __device__ __forceinline__ void bound_publish(const BoundGrid &bg, int j, int k, double b)
 {
@@ -274,9 +291,10 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
             if (TWO_D) o7 = Sn[7 * sa + c];
         }
         double ir = rcp_fast(rho);
-        q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = Bc[1]; q[5] = Bc[2];
-        q[6] = (g.gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3])
-                                     - 0.5 * (Bc[0] * Bc[0] + Bc[1] * Bc[1] + Bc[2] * Bc[2]));
+        q[0] = rho; q[1] = __dmul_rn(mx, ir); q[2] = __dmul_rn(my, ir); q[3] = __dmul_rn(mz, ir);      // see prim_rot
+        q[4] = Bc[1]; q[5] = Bc[2];
+        q[6] = __dmul_rn(g.gamma - 1.0, fma(-0.5, fma(Bc[0], Bc[0], fma(Bc[1], Bc[1], Bc[2] * Bc[2])),
+                                            fma(-0.5, fma(mx, q[1], fma(my, q[2], mz * q[3])), En)));
         if (f >= 0 && f < nx && (unphysical(rho) || unphysical(q[6]))) P->err = 1;
     }
 #pragma unroll
@@ -312,18 +330,18 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     // cell f in [0, nx): flux difference with the right neighbour's face, CT data of the own face
     if (face && f < nx && t <= SX_NT - H - 1) {
         const double dtdx = P->dtdx[0];
-        double r0 = rho - dtdx * (sP[0][t + 1] - F[0]);
-        double r1 = mx - dtdx * (sP[1][t + 1] - F[1]);
-        double r2 = my - dtdx * (sP[2][t + 1] - F[2]);
-        double r3 = mz - dtdx * (sP[3][t + 1] - F[3]);
-        double r4 = En - dtdx * (sP[4][t + 1] - F[6]);
+        double r0 = fma(-dtdx, sP[0][t + 1] - F[0], rho);
+        double r1 = fma(-dtdx, sP[1][t + 1] - F[1], mx);
+        double r2 = fma(-dtdx, sP[2][t + 1] - F[2], my);
+        double r3 = fma(-dtdx, sP[3][t + 1] - F[3], mz);
+        double r4 = fma(-dtdx, sP[4][t + 1] - F[6], En);
         if (cb.Sn) {
             r0 = fma(cb.wn, o0, cb.ws * r0); r1 = fma(cb.wn, o1, cb.ws * r1); r2 = fma(cb.wn, o2, cb.ws * r2);
             r3 = fma(cb.wn, o3, cb.ws * r3); r4 = fma(cb.wn, o4, cb.ws * r4);
         }
         Sout[c] = r0; Sout[sa + c] = r1; Sout[2 * sa + c] = r2; Sout[3 * sa + c] = r3; Sout[4 * sa + c] = r4;
         if (TWO_D) {   // B_z has no faces in 2D: cell centred, flux updated
-            double r7 = Bc[2] - dtdx * (sP[5][t + 1] - F[5]);
+            double r7 = fma(-dtdx, sP[5][t + 1] - F[5], Bc[2]);
             Sout[7 * sa + c] = cb.Sn ? fma(cb.wn, o7, cb.ws * r7) : r7;
         }
         // cell-centred EMF  E^c = -(v x B)
@@ -363,9 +381,12 @@ __device__ __forceinline__ void prim_rot(double rho, const double m[3], const do
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     double ir = rcp_fast(rho);
-    double v[3] = { m[0] * ir, m[1] * ir, m[2] * ir };
-    double p = (gamma - 1.0) * (En - 0.5 * (m[0] * v[0] + m[1] * v[1] + m[2] * v[2])
-                                   - 0.5 * (B[0] * B[0] + B[1] * B[1] + B[2] * B[2]));
+    // the velocities and the pressure are rounded products (__dmul_rn is never contracted into the
+    // consumer's add): a zone's primitives are then the same bits wherever they are formed -- the first
+    // cells of a march segment or the running loop -- and a run does not depend on how the marches are cut
+    double v[3] = { __dmul_rn(m[0], ir), __dmul_rn(m[1], ir), __dmul_rn(m[2], ir) };
+    double p = __dmul_rn(gamma - 1.0, fma(-0.5, fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2])),
+                                          fma(-0.5, fma(m[0], v[0], fma(m[1], v[1], m[2] * v[2])), En)));
     q[0] = rho; q[1] = v[DIR]; q[2] = v[T1]; q[3] = v[T2]; q[4] = B[T1]; q[5] = B[T2]; q[6] = p;
     bad = unphysical(rho) || unphysical(p);
 }
@@ -396,7 +417,7 @@ constexpr int MARCH_PF = 16;     // doubles per thread and iteration: U(s+1) 5, 
 // three blocks of 128 threads per SM: 168 registers per thread hold the running state without
 // spilling (measured: 4 blocks at 128 registers spill ~40 values per interface and run 20% slower)
 constexpr int MARCH_MINB = 3;
-template <int DIR, int LIM, bool TWO_D>
+template <int DIR, int LIM, bool TWO_D, bool BOUND>
 __global__ void __launch_bounds__(MARCH_NT, MARCH_MINB)
 k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
               double scale, int seglen, int tr0, BoundGrid bg)
@@ -404,6 +425,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
     __shared__ double pf[2][MARCH_PF][MARCH_NT];
+    __shared__ double sbnd[BOUND ? 3 : 1][MARCH_NT];
     const int t = threadIdx.x;
     const int i = blockIdx.x * blockDim.x + t;
     if (i >= g.n[0]) return;
@@ -414,9 +436,8 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     const int tr = (DIR == 1 ? blockIdx.z : blockIdx.y) + tr0;
     const int s0 = seg * seglen;
     const int s1 = min(s0 + seglen, g.n[DIR]);
-    // the z sweep also leaves the CT data of the upper boundary face n (a periodic single domain gets
+    // (the z sweep also leaves the CT data of the upper boundary face n: a periodic single domain gets
     // the same bits as on face 0; a z slab gets the face it shares with the slab above)
-    const int sct = (DIR == 2 && s1 == g.n[2]) ? s1 + 1 : s1;
     const long long sa = g.sa, st = g.st[DIR];
     long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
     const double gamma = g.gamma, igm1 = g.igm1;
@@ -426,7 +447,8 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     const double *__restrict__ b2 = Sin + (S_B + T2) * sa;
     const long long st1 = g.st[T1], st2 = g.st[T2];
     bool bad, anybad = false;
-    double bmax = 0.0;                                   // dt bound of the zones this thread finishes (last stage)
+    SigmaBound sb;                                       // dt bound of the zones this thread finishes (last stage)
+    if (BOUND) sb.init(&sbnd[0][t], MARCH_NT);
 
     // what iteration s consumes: U of cell s+1 and the faces around it, U' of cell s-1
     auto prefetch = [&](int slot, long long cs) {
@@ -504,20 +526,20 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
             double m[3];
-            const double r0 = pf[slot][10][t] - fac * (F[0] - Fp[0]);
-            m[DIR] = pf[slot][11][t] - fac * (F[1] - Fp[1]);
-            m[T1] = pf[slot][12][t] - fac * (F[2] - Fp[2]);
-            m[T2] = pf[slot][13][t] - fac * (F[3] - Fp[3]);
-            const double r4 = pf[slot][14][t] - fac * (F[6] - Fp[4]);
+            const double r0 = fma(-fac, F[0] - Fp[0], pf[slot][10][t]);
+            m[DIR] = fma(-fac, F[1] - Fp[1], pf[slot][11][t]);
+            m[T1] = fma(-fac, F[2] - Fp[2], pf[slot][12][t]);
+            m[T2] = fma(-fac, F[3] - Fp[3], pf[slot][13][t]);
+            const double r4 = fma(-fac, F[6] - Fp[4], pf[slot][14][t]);
             Sout[cm] = r0;
             Sout[(1 + DIR) * sa + cm] = m[DIR];
             Sout[(1 + T1) * sa + cm] = m[T1];
             Sout[(1 + T2) * sa + cm] = m[T2];
             Sout[4 * sa + cm] = r4;
-            if (BZ2D) Sout[7 * sa + cm] = pf[slot][15][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
-            if (bg.b) bmax = fmax(bmax, sigma_bound(g, bg.cfac, r0, m[0], m[1], m[2], r4));
+            if (BZ2D) Sout[7 * sa + cm] = fma(-fac, F[4] - Fp[5], pf[slot][15][t]);   // F_y[B_z]
+            if (BOUND) sb.add(g, r0, m[0], m[1], m[2], r4);
         }
-        if (s < sct) {
+        if (s < s1 || (DIR == 2 && s == g.n[2])) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;
@@ -539,7 +561,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
     }
     if (s <= s1) iteration(0, s);
     if (anybad) P->err = 1;
-    if (bg.b) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, bmax);
+    if (BOUND) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, sb.value(g, bg.cfac));
 }
 
 // ---------------------------------------------------------------- y / z sweep with the five-cell WENO-Z stencil
@@ -549,7 +571,7 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
 // finishes cell s-1.  First version: operands are loaded directly (no prefetch ring).
 constexpr int WZ_PF = 17;        // doubles per thread and iteration: U(s+3) 5, faces 6, U'(s) 6
 
-template <int DIR, bool TWO_D>
+template <int DIR, bool TWO_D, bool BOUND>
 __global__ void __launch_bounds__(MARCH_NT, 3)
 k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
                  double scale, int seglen, int tr0, BoundGrid bg)
@@ -559,6 +581,7 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     extern __shared__ double wz_smem[];
     double (*ring)[7][MARCH_NT] = reinterpret_cast<double (*)[7][MARCH_NT]>(wz_smem);                    // [5]
     double (*pf)[WZ_PF][MARCH_NT] = reinterpret_cast<double (*)[WZ_PF][MARCH_NT]>(wz_smem + 5 * 7 * MARCH_NT);   // [2]
+    __shared__ double sbnd[BOUND ? 3 : 1][MARCH_NT];
     const int t = threadIdx.x;
     const int i = blockIdx.x * blockDim.x + t;
     if (i >= g.n[0]) return;
@@ -566,7 +589,6 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     const int tr = (DIR == 1 ? blockIdx.z : blockIdx.y) + tr0;    // see k_sweep_march
     const int s0 = seg * seglen;
     const int s1 = min(s0 + seglen, g.n[DIR]);
-    const int sct = (DIR == 2 && s1 == g.n[2]) ? s1 + 1 : s1;     // CT data of the upper boundary face too
     const long long sa = g.sa, st = g.st[DIR];
     long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);   // cell s0 of the segment
     const double gamma = g.gamma, igm1 = g.igm1;
@@ -577,7 +599,8 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
     const long long st1 = g.st[T1], st2 = g.st[T2];
     const int xdup = ct_xdup(i, g.n[0]);
     bool bad, anybad = false;
-    double bmax = 0.0;
+    SigmaBound sb;
+    if (BOUND) sb.init(&sbnd[0][t], MARCH_NT);
     auto slot = [](int m) { return ((m % 5) + 5) % 5; };
 
     // what iteration s consumes: U of cell s+2 and the faces around it, U' of cell s-1 (cs = cell s)
@@ -655,20 +678,20 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
             double m[3];
-            const double r0 = pf[ps][11][t] - fac * (F[0] - Fp[0]);
-            m[DIR] = pf[ps][12][t] - fac * (F[1] - Fp[1]);
-            m[T1] = pf[ps][13][t] - fac * (F[2] - Fp[2]);
-            m[T2] = pf[ps][14][t] - fac * (F[3] - Fp[3]);
-            const double r4 = pf[ps][15][t] - fac * (F[6] - Fp[4]);
+            const double r0 = fma(-fac, F[0] - Fp[0], pf[ps][11][t]);
+            m[DIR] = fma(-fac, F[1] - Fp[1], pf[ps][12][t]);
+            m[T1] = fma(-fac, F[2] - Fp[2], pf[ps][13][t]);
+            m[T2] = fma(-fac, F[3] - Fp[3], pf[ps][14][t]);
+            const double r4 = fma(-fac, F[6] - Fp[4], pf[ps][15][t]);
             Sout[cm] = r0;
             Sout[(1 + DIR) * sa + cm] = m[DIR];
             Sout[(1 + T1) * sa + cm] = m[T1];
             Sout[(1 + T2) * sa + cm] = m[T2];
             Sout[4 * sa + cm] = r4;
-            if (BZ2D) Sout[7 * sa + cm] = pf[ps][16][t] - fac * (F[4] - Fp[5]);   // F_y[B_z]
-            if (bg.b) bmax = fmax(bmax, sigma_bound(g, bg.cfac, r0, m[0], m[1], m[2], r4));
+            if (BZ2D) Sout[7 * sa + cm] = fma(-fac, F[4] - Fp[5], pf[ps][16][t]);   // F_y[B_z]
+            if (BOUND) sb.add(g, r0, m[0], m[1], m[2], r4);
         }
-        if (s < sct) {
+        if (s < s1 || (DIR == 2 && s == g.n[2])) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;
@@ -681,7 +704,7 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
         Fp[0] = F[0]; Fp[1] = F[1]; Fp[2] = F[2]; Fp[3] = F[3]; Fp[4] = F[6]; Fp[5] = F[4];
     }
     if (anybad) P->err = 1;
-    if (bg.b) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, bmax);
+    if (BOUND) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, sb.value(g, bg.cfac));
 }
 constexpr int WZ_SMEM_BYTES = (5 * 7 + 2 * WZ_PF) * MARCH_NT * 8;
 
@@ -709,7 +732,7 @@ constexpr int XY128_MINB = 3;
 template <int LIM, bool TWO_D, bool WRAP, int NT>
 __global__ void __launch_bounds__(NT, NT == 128 ? XY128_MINB : 512 / NT)
 k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-           Combine cb, int seglen, int kz0, BoundGrid bg)
+           Combine cb, int seglen, int kz0)
 {
     extern __shared__ __align__(128) double xy_smem[];
     const int t = threadIdx.x;
@@ -749,7 +772,6 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const double *__restrict__ bz = Sin + (S_B + 2) * sa;
     long long c = g.at(valid ? i : 0, s0, k);                       // cell (i, s0, k)
     bool anybad = false;
-    double bmax = 0.0;
 
     // TMA row copies, issued by thread 0: the block's x range [i0, i0 + NT) of one row of each array
     const long long row0 = g.at(WRAP ? 0 : (int)blockIdx.x * (NT - 4) - 2, s0, k);    // first cell of row s0
@@ -785,8 +807,10 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     auto to_prim = [&](double rho, double mx, double my, double mz, double En, double B0, double B1, double B2,
                        double q[8], bool &bad) {
         double ir = rcp_fast(rho);
-        q[0] = rho; q[1] = mx * ir; q[2] = my * ir; q[3] = mz * ir; q[4] = B0; q[5] = B1; q[6] = B2;
-        q[7] = (gamma - 1.0) * (En - 0.5 * (mx * q[1] + my * q[2] + mz * q[3]) - 0.5 * (B0 * B0 + B1 * B1 + B2 * B2));
+        q[0] = rho; q[1] = __dmul_rn(mx, ir); q[2] = __dmul_rn(my, ir); q[3] = __dmul_rn(mz, ir);      // see prim_rot
+        q[4] = B0; q[5] = B1; q[6] = B2;
+        q[7] = __dmul_rn(gamma - 1.0, fma(-0.5, fma(B0, B0, fma(B1, B1, B2 * B2)),
+                                          fma(-0.5, fma(mx, q[1], fma(my, q[2], mz * q[3])), En)));
         bad = unphysical(rho) || unphysical(q[7]);
     };
     auto load_prim = [&](long long cc, double q[8], double &bxf, bool &bad) {
@@ -947,11 +971,11 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         if (s > s0 && cell && kin) {
             const long long cm = c - st;
             // S of row s-1 minus the x flux difference (own lower face, right neighbour's lower face)
-            double r0v = pff[t] - dtdx * (sQ[tr] - sQ[t]);
-            double r1v = pff[NT + t] - dtdx * (sQ[NT + tr] - sQ[NT + t]);
-            double r2v = pff[2 * NT + t] - dtdx * (sQ[2 * NT + tr] - sQ[2 * NT + t]);
-            double r3v = pff[3 * NT + t] - dtdx * (sQ[3 * NT + tr] - sQ[3 * NT + t]);
-            double r4v = pff[4 * NT + t] - dtdx * (sQ[4 * NT + tr] - sQ[4 * NT + t]);
+            double r0v = fma(-dtdx, sQ[tr] - sQ[t], pff[t]);
+            double r1v = fma(-dtdx, sQ[NT + tr] - sQ[NT + t], pff[NT + t]);
+            double r2v = fma(-dtdx, sQ[2 * NT + tr] - sQ[2 * NT + t], pff[2 * NT + t]);
+            double r3v = fma(-dtdx, sQ[3 * NT + tr] - sQ[3 * NT + t], pff[3 * NT + t]);
+            double r4v = fma(-dtdx, sQ[4 * NT + tr] - sQ[4 * NT + t], pff[4 * NT + t]);
             if (combine) {
                 r0v = fma(cb.wn, pff[5 * NT + t], cb.ws * r0v); r1v = fma(cb.wn, pff[6 * NT + t], cb.ws * r1v);
                 r2v = fma(cb.wn, pff[7 * NT + t], cb.ws * r2v); r3v = fma(cb.wn, pff[8 * NT + t], cb.ws * r3v);
@@ -960,22 +984,20 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             // y-rotated flux: (rho, m_y, m_z, m_x, B_z, B_x, E)
 #pragma unroll
             for (int n = 0; n < NFPS; n++) Fpy[n] = *fpy[n];
-            r0v -= facy * (Fy[0] - Fpy[0]);
-            r2v -= facy * (Fy[1] - Fpy[1]);
-            r3v -= facy * (Fy[2] - Fpy[2]);
-            r1v -= facy * (Fy[3] - Fpy[3]);
-            r4v -= facy * (Fy[6] - Fpy[4]);
+            r0v = fma(-facy, Fy[0] - Fpy[0], r0v);
+            r2v = fma(-facy, Fy[1] - Fpy[1], r2v);
+            r3v = fma(-facy, Fy[2] - Fpy[2], r3v);
+            r1v = fma(-facy, Fy[3] - Fpy[3], r1v);
+            r4v = fma(-facy, Fy[6] - Fpy[4], r4v);
             Sout[cm] = r0v;
             Sout[2 * sa + cm] = r2v;
             Sout[3 * sa + cm] = r3v;
             Sout[sa + cm] = r1v;
             Sout[4 * sa + cm] = r4v;
             if (TWO_D) {
-                double r7v = rm[6 * NT] - dtdx * (sQ[5 * NT + tr] - sQ[5 * NT + t]);
+                double r7v = fma(-dtdx, sQ[5 * NT + tr] - sQ[5 * NT + t], rm[6 * NT]);
                 if (combine) r7v = fma(cb.wn, pff[10 * NT + t], cb.ws * r7v);
-                Sout[7 * sa + cm] = r7v - facy * (Fy[4] - Fpy[5]);
-                // 2D: this kernel writes the final hydro variables of the step
-                if (bg.b) bmax = fmax(bmax, sigma_bound(g, bg.cfac, r0v, r1v, r2v, r3v, r4v));
+                Sout[7 * sa + cm] = fma(-facy, Fy[4] - Fpy[5], r7v);
             }
         }
         if (cell && s < s1) {
@@ -997,7 +1019,6 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         double *rt = rm; rm = r0; r0 = rn; rn = rt;
     }
     if (anybad && kin) P->err = 1;
-    if (TWO_D && bg.b && cell) bound_publish(bg, s0, 0, bmax);
 }
 
 // ---------------------------------------------------------------- CT (a6, R6) [+ RK2 combine of the faces (a7)]
@@ -1114,8 +1135,8 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
             const double ezx = sE[buf][0][ty][tx + 1], ezy = sE[buf][0][ty + 1][tx];
             const long long c = plane(k) + oc;
             if (TWO_D) {
-                const double bxn = pbx - dtdy * (ezy - ez);
-                const double byn = pby + dtdx * (ezx - ez);
+                const double bxn = fma(-dtdy, ezy - ez, pbx);
+                const double byn = fma(dtdx, ezx - ez, pby);
                 const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                 bout[c] = bxo;
                 if (i == 0) bout[c + g.n[0]] = bxo;       // periodic copy: x-face n0 is face 0
@@ -1124,8 +1145,8 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
             } else {
                 if (k > k0) {                                 // b_x, b_y of plane k-1
                     const long long cm = plane(k - 1) + oc;
-                    const double bxn = pbx - (dtdy * dEzy - dtdz * (eyN - eyP));
-                    const double byn = pby - (dtdz * (exN - exP) - dtdx * dEzx);
+                    const double bxn = fma(-dtdy, dEzy, fma(dtdz, eyN - eyP, pbx));
+                    const double byn = fma(-dtdz, exN - exP, fma(dtdx, dEzx, pby));
                     const double bxo = COMBINE ? fma(cb.wn, qbx, cb.ws * bxn) : bxn;
                     bout[cm] = bxo;
                     if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
@@ -1133,7 +1154,7 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
                 }
                 if (k < k1) {                                 // b_z on the lower face of plane k
                     const double eyx = sE[buf][2][ty][tx + 1], exy = sE[buf][1][ty + 1][tx];
-                    const double bzn = pbz - (dtdx * (eyx - eyN) - dtdy * (exy - exN));
+                    const double bzn = fma(-dtdx, eyx - eyN, fma(dtdy, exy - exN, pbz));
                     bout[2 * sa + c] = COMBINE ? fma(cb.wn, qbz, cb.ws * bzn) : bzn;
                     if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
                     // operands of the next iteration: b_x, b_y of this plane, b_z of the next

@@ -4,6 +4,13 @@
 //   plm_slope      : limited slope for Eq. 6, minmod / MC (reading R4)
 //   hlld           : HLLD flux in the rotated frame (Eq. 8; [56] PAPER.md:649; R5)
 //                    + the continuous upwind weight used by CT (R6)
+//
+// Rounding discipline.  These functions are inlined at several sites (the first cells of a march segment
+// and its running loop, the two unrolled copies of a loop body), and the compiler is free to contract
+// a * b + c into an FMA differently at each site.  Wherever a product feeds an addition the choice is
+// therefore written out -- fma() or __dmul_rn() (which is never contracted) -- so that a flux is the same
+// bits wherever it is evaluated and a run does not depend on how the marches are cut into segments or the
+// box into slabs.  Products that only feed other products, selects or comparisons are left plain.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -82,31 +89,32 @@ __device__ __forceinline__ void plm_faces(double q, double dm, double dp, double
 // tau5 are unchanged, so the indicators and the three quotients are formed once for both faces.
 __device__ __forceinline__ void wenoz_faces(double a, double b, double c, double d, double e, double &lo, double &hi)
 {
-    const double a0 = a - 2.0 * b + c, b0 = a - 4.0 * b + 3.0 * c;
+    // (multiples by 2 and 4 are exact; every other product that feeds a sum is an explicit fma / __dmul_rn)
+    const double a0 = a - 2.0 * b + c, b0 = fma(3.0, c, a - 4.0 * b);
     const double a1 = b - 2.0 * c + d, b1 = b - d;
-    const double a2 = c - 2.0 * d + e, b2 = 3.0 * c - 4.0 * d + e;
+    const double a2 = c - 2.0 * d + e, b2 = fma(3.0, c, e - 4.0 * d);
     const double be0 = fma(13.0 / 12.0 * a0, a0, 0.25 * b0 * b0);
     const double be1 = fma(13.0 / 12.0 * a1, a1, 0.25 * b1 * b1);
     const double be2 = fma(13.0 / 12.0 * a2, a2, 0.25 * b2 * b2);
     const double tau = fabs(be0 - be2);
     const double r0 = fma(tau, rcp_fast(be0 + 1e-40), 1.0);
-    const double r1 = 0.6 * fma(tau, rcp_fast(be1 + 1e-40), 1.0);
+    const double r1 = __dmul_rn(0.6, fma(tau, rcp_fast(be1 + 1e-40), 1.0));
     const double r2 = fma(tau, rcp_fast(be2 + 1e-40), 1.0);
     // upper face: stencils (a,b,c), (b,c,d), (c,d,e) with d = (0.1, 0.6, 0.3)
     {
-        const double q0 = (2.0 * a - 7.0 * b + 11.0 * c) * (1.0 / 6.0);
-        const double q1 = (-b + 5.0 * c + 2.0 * d) * (1.0 / 6.0);
-        const double q2 = (2.0 * c + 5.0 * d - e) * (1.0 / 6.0);
-        const double al0 = 0.1 * r0, al2 = 0.3 * r2;
-        hi = fma(al0, q0, fma(r1, q1, al2 * q2)) * rcp_fast(al0 + r1 + al2);
+        const double q0 = fma(11.0, c, fma(-7.0, b, 2.0 * a)) * (1.0 / 6.0);
+        const double q1 = fma(5.0, c, 2.0 * d - b) * (1.0 / 6.0);
+        const double q2 = fma(5.0, d, 2.0 * c - e) * (1.0 / 6.0);
+        const double al0 = __dmul_rn(0.1, r0), al2 = __dmul_rn(0.3, r2);
+        hi = __dmul_rn(fma(al0, q0, fma(r1, q1, al2 * q2)), rcp_fast(al0 + r1 + al2));
     }
     // lower face: the mirrored stencils (e,d,c), (d,c,b), (c,b,a)
     {
-        const double q0 = (2.0 * e - 7.0 * d + 11.0 * c) * (1.0 / 6.0);
-        const double q1 = (-d + 5.0 * c + 2.0 * b) * (1.0 / 6.0);
-        const double q2 = (2.0 * c + 5.0 * b - a) * (1.0 / 6.0);
-        const double al0 = 0.1 * r2, al2 = 0.3 * r0;
-        lo = fma(al0, q0, fma(r1, q1, al2 * q2)) * rcp_fast(al0 + r1 + al2);
+        const double q0 = fma(11.0, c, fma(-7.0, d, 2.0 * e)) * (1.0 / 6.0);
+        const double q1 = fma(5.0, c, 2.0 * b - d) * (1.0 / 6.0);
+        const double q2 = fma(5.0, b, 2.0 * c - a) * (1.0 / 6.0);
+        const double al0 = __dmul_rn(0.1, r2), al2 = __dmul_rn(0.3, r0);
+        lo = __dmul_rn(fma(al0, q0, fma(r1, q1, al2 * q2)), rcp_fast(al0 + r1 + al2));
     }
 }
 
@@ -152,7 +160,7 @@ struct Side {
 __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, double gamma, double igm1,
                                      double f[7], double &wgt)
 {
-    const double Bx2 = Bx * Bx;
+    const double Bx2 = __dmul_rn(Bx, Bx);
     const double B2L = Bx2 + fma(L.By, L.By, L.Bz * L.Bz), B2R = Bx2 + fma(R.By, R.By, R.Bz * R.Bz);
     const double pTL = fma(0.5, B2L, L.p), pTR = fma(0.5, B2R, R.p);
 
@@ -160,10 +168,10 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
                                        fast_speed2(R.rho, gamma * R.p, Bx2, B2R)));
     const double SL = fmin(L.u, R.u) - cmax, SR = fmax(L.u, R.u) + cmax;
     const double dL = SL - L.u, dR = SR - R.u;              // S_a - u_a
-    const double aL = L.rho * dL, aR = R.rho * dR;
+    const double aL = __dmul_rn(L.rho, dL), aR = __dmul_rn(R.rho, dR);
     const double idenom = rcp_fast(aR - aL);
-    const double SM  = (aR * R.u - aL * L.u - pTR + pTL) * idenom;
-    const double pTs = (aR * pTL - aL * pTR + aL * aR * (R.u - L.u)) * idenom;
+    const double SM  = __dmul_rn(fma(aR, R.u, fma(-aL, L.u, pTL - pTR)), idenom);
+    const double pTs = __dmul_rn(fma(aR, pTL, fma(-aL, pTR, aL * aR * (R.u - L.u))), idenom);
     const double guard = kDegen * pTs;
 
     // star states: density and the transverse velocity / field of both sides
@@ -172,7 +180,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     {
         const double dS = SL - SM, D = fma(aL, dS, -Bx2);
         idSL = rcp_fast(dS);
-        rsL = aL * idSL;
+        rsL = __dmul_rn(aL, idSL);
         // (S_M - u)/D, zero in the guarded degenerate case: then v* = v, B_t* = B_t (R5)
         const double m = fabs(D) <= guard ? 0.0 : (dL - dS) * rcp_fast(D);
         const double cv = Bx * m, cb = aL * m;                      // B_t*/B_t = 1 + a (S_M - u)/D
@@ -182,7 +190,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     {
         const double dS = SR - SM, D = fma(aR, dS, -Bx2);
         idSR = rcp_fast(dS);
-        rsR = aR * idSR;
+        rsR = __dmul_rn(aR, idSR);
         const double m = fabs(D) <= guard ? 0.0 : (dR - dS) * rcp_fast(D);
         const double cv = Bx * m, cb = aR * m;
         vsR = fma(-cv, R.By, R.v); wsR = fma(-cv, R.Bz, R.w);
@@ -195,11 +203,11 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     const double sig = copysign(1.0, Bx);
     const double iR = rcp_fast(rL + rR);
     const double srr = sig * rL * rR;
-    const double vss  = (fma(rL, vsL, rR * vsR) + sig * (BysR - BysL)) * iR;
-    const double wss  = (fma(rL, wsL, rR * wsR) + sig * (BzsR - BzsL)) * iR;
-    const double Byss = (fma(rL, BysR, rR * BysL) + srr * (vsR - vsL)) * iR;
-    const double Bzss = (fma(rL, BzsR, rR * BzsL) + srr * (wsR - wsL)) * iR;
-    const double SMBx = SM * Bx;
+    const double vss  = fma(sig, BysR - BysL, fma(rL, vsL, rR * vsR)) * iR;
+    const double wss  = fma(sig, BzsR - BzsL, fma(rL, wsL, rR * wsR)) * iR;
+    const double Byss = fma(srr, vsR - vsL, fma(rL, BysR, rR * BysL)) * iR;
+    const double Bzss = fma(srr, wsR - wsL, fma(rL, BzsR, rR * BzsL)) * iR;
+    const double SMBx = __dmul_rn(SM, Bx);
     const double vBss = fma(vss, Byss, fma(wss, Bzss, SMBx));
 
     // the side the interface lies in (test order of R5: ..., S*_L >= 0, S_M >= 0, S*_R > 0), and
@@ -216,7 +224,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     const double E  = fma(p, igm1, 0.5 * fma(rho, fma(u, u, fma(v, v, w * w)), B2));
     const double vB = fma(u, Bx, fma(v, By, w * Bz));
     const double vBs = fma(vs, Bys, fma(ws, Bzs, SMBx));
-    const double Es = (fma(d, E, -pT * u) + fma(pTs, SM, Bx * (vB - vBs))) * idS;
+    const double Es = __dmul_rn(fma(d, E, -pT * u) + fma(pTs, SM, Bx * (vB - vBs)), idS);
     const double sr = left ? -sig * r : sig * r;
     const double Ess = fma(sr, vBs - vBss, Es);
 
@@ -233,7 +241,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
         }
         vBf = fma(uf, Bx, fma(vf, Byf, wf * Bzf));
     }
-    const double F0 = rho_f * uf;
+    const double F0 = __dmul_rn(rho_f, uf);      // a rounded product: the same bits for both cells sharing the face
     f[0] = F0;
     f[1] = fma(F0, uf, pf - Bx2);
     f[2] = fma(F0, vf, -Bx * Byf);

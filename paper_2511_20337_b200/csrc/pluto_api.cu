@@ -13,6 +13,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 namespace pluto {
@@ -261,8 +262,8 @@ int march_seglen(int n, long long columns)
     return len;
 }
 
-// The sweep that writes the final hydro variables of a stage is the z sweep (3D) or the y part of the
-// x+y sweep (2D); in the last stage of a step it also fills the dt bound grid (kernels.cuh sigma_bound).
+// In 3D the z sweep writes the final hydro variables of a stage; in the last stage of a step it also fills
+// the dt bound grid (kernels.cuh SigmaBound).
 BoundGrid bound_grid(const Domain &d, bool last, int bj, int bk)
 {
     BoundGrid bg;
@@ -277,10 +278,10 @@ BoundGrid bound_grid(const Domain &d, bool last, int bj, int bk)
 int seglen_y(const Grid &g) { return march_seglen(g.n[1], (long long)g.n[0] * g.n[2]); }
 int seglen_z(const Grid &g) { return march_seglen(g.n[2], (long long)g.n[0] * g.n[1]); }
 
-// the bound grid of the slab: one cell per (row, z segment) in 3D, per y segment in 2D
+// the bound grid of the slab: one cell per (row, z segment); 2D runs keep none (the dt kernel reads every row)
 BoundGrid final_bound_grid(const Domain &d, bool last)
 {
-    return d.g.act[2] ? bound_grid(d, last, 1, seglen_z(d.g)) : bound_grid(d, last, seglen_y(d.g), 1);
+    return bound_grid(d, last && d.g.act[2], 1, d.g.act[2] ? seglen_z(d.g) : 1);
 }
 
 template <int LIM, bool TWO_D>
@@ -306,18 +307,18 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         const int len = seglen_y(g);
         dim3 grid(chunks, (g.n[1] + len - 1) / len, nplanes);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
-        void (*k)(Grid, const double *, double *, double *, StepParams *, Combine, int, int, BoundGrid) =
+        void (*k)(Grid, const double *, double *, double *, StepParams *, Combine, int, int) =
             wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
                     : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
                  : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        const BoundGrid bg = TWO_D ? final_bound_grid(d, last) : none;
-        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len, kz0, bg));
+        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len, kz0));
     }
     if (!fused) {
         if constexpr (LIM == 2) {
-            cudaFuncSetAttribute(k_sweep_march_wz<1, TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
-            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<1, TWO_D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D, !TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
         }
         const long long nitems = (long long)(g.n[0] + 2 * sx_halo(LIM)) * g.n[1] * nplanes;
         LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + sx_out(LIM) - 1) / sx_out(LIM)), SX_NT, 0, s>>>(
@@ -325,17 +326,21 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = seglen_y(g);
         dim3 grid(bx, (g.n[1] + len - 1) / len, nplanes);
-        const BoundGrid bg = TWO_D ? final_bound_grid(d, last) : none;
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, bg));
-        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, bg));
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, none));
+        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, none));
     }
     if (!TWO_D) {
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = seglen_z(g);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
         const BoundGrid bg = final_bound_grid(d, last);
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
-        else LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+        if constexpr (LIM == 2) {
+            if (last) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, !TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+            else      LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+        } else {
+            if (last) LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, !TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+            else      LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+        }
     }
 }
 

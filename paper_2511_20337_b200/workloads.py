@@ -21,12 +21,12 @@ import numpy as np
 _M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
 
 
-def counter_noise(seed: int, n: int) -> np.ndarray:
-    """u[c] in [0,1) for linear cell index c = 0..n-1: a 64-bit integer mixer keyed by (seed, c).
+def counter_noise(seed: int, n: int, start: int = 0) -> np.ndarray:
+    """u[c] in [0,1) for linear cell index c = start..start+n-1: a 64-bit integer mixer keyed by (seed, c).
 
     Stateless (counter based), so any sub-range can be regenerated independently."""
     with np.errstate(over="ignore"):
-        z = np.arange(n, dtype=np.uint64) + np.uint64(seed) * np.uint64(0x9E3779B97F4A7C15)
+        z = np.arange(start, start + n, dtype=np.uint64) + np.uint64(seed) * np.uint64(0x9E3779B97F4A7C15)
         z = z + np.uint64(0x9E3779B97F4A7C15)
         z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
         z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
@@ -266,6 +266,30 @@ def blast_3d(n=256, nsteps=50, seed=511, noise=1e-3, gamma=5.0 / 3.0, cfl=0.3, l
     U = conserved_from_fields(rho, [zero, zero, zero], Bc, p, gamma)
     return Workload(name or f"blast_3d_{nx}x{ny}x{nz}", nx, ny, nz, L, gamma, cfl, limiter, nsteps, U,
                     join_faces(faces, nx, ny, nz), seed=seed)
+
+
+def blast_3d_planes(nx, ny, nz, k0, nzl, nblast=1, seed=511, noise=1e-3, gamma=5.0 / 3.0, p_in=10.0):
+    """Planes [k0, k0 + nzl) of a blast problem in an nx x ny x nz box with cubic cells (Lx = 1), in the
+    local layouts of a z slab (U[8][nzl][ny][nx]; bx, by with nzl planes, bz with nzl + 1): the weak-scaling
+    workload of bench.py --gpus N, where the box grows along z with the number of GPUs and carries one
+    blast of configs[3]'s recipe per slab-sized section (nblast of them, centred in their sections).  The
+    noise is keyed by the GLOBAL linear cell index, so every rank generates exactly its part of one state."""
+    L = (1.0, ny / nx, nz / nx)
+    shp = (nzl, ny, nx)
+    xc, yc = cell_centres(nx, L[0]), cell_centres(ny, L[1])
+    zc = (np.arange(k0, k0 + nzl) + 0.5) * (L[2] / nz)
+    sec = L[2] / nblast
+    zrel = zc - (np.floor(zc / sec) + 0.5) * sec            # distance to the centre of the section
+    r2 = (xc[None, None, :] - 0.5 * L[0]) ** 2 + (yc[None, :, None] - 0.5 * L[1]) ** 2 + zrel[:, None, None] ** 2
+    p = np.where(r2 < 0.1 ** 2, p_in, 0.1)
+    u = counter_noise(seed, nx * ny * nzl, start=k0 * nx * ny).reshape(shp)
+    rho = 1.0 + noise * (2.0 * u - 1.0)
+    b0 = 1.0 / np.sqrt(3.0)
+    Bc = [np.full(shp, b0)] * 3
+    zero = np.zeros(shp)
+    U = conserved_from_fields(rho, [zero, zero, zero], Bc, p, gamma)
+    Bl = np.full(nzl * ny * (nx + 1) + nzl * (ny + 1) * nx + (nzl + 1) * ny * nx, b0)
+    return U, Bl, L
 
 
 # --------------------------------------------------------------------------- generic small test problems
