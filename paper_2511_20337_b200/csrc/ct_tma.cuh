@@ -179,15 +179,20 @@ k_ct_tma(Grid g, const __grid_constant__ CUtensorMap tmap, const double *__restr
                     if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
                     bout[sa + cm] = COMBINE ? fma(cb.wn, qby, cb.ws * byn) : byn;
                 }
-                if (k < k1) {                    // b_z on the lower face of plane k
+                // b_z on the lower face of plane k.  The last segment also writes face nz, into the ghost plane:
+                // the same bits as face 0 of the slab above (of this domain, if periodic), so the dt kernel
+                // finds the upper face of the top cells in its own array
+                if (k < k1 || k1 == g.n[2]) {
                     const double eyx = e[2 * CT_TX * CT_TY + 1], exy = e[CT_TX * CT_TY + CT_TX];
                     const double bzn = fma(-dtdx, eyx - eyN, fma(dtdy, exy - exN, pbz));
                     bout[2 * sa + c] = COMBINE ? fma(cb.wn, qbz, cb.ws * bzn) : bzn;
+                }
+                if (k < k1) {
                     if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
                     // operands of the next iteration: b_x, b_y of this plane, b_z of the next
                     pbx = bin[c]; pby = bin[sa + c];
                     if (COMBINE) { qbx = cb.Sn[c]; qby = cb.Sn[sa + c]; }
-                    if (k + 1 < k1) {
+                    if (k + 1 < k1 || k1 == g.n[2]) {
                         pbz = bin[2 * sa + c + st2];
                         if (COMBINE) qbz = cb.Sn[2 * sa + c + st2];
                     }

@@ -68,10 +68,10 @@ __device__ __forceinline__ double sqrt_nr(double x)      // x > 0
 //   filter 2:  the candidates themselves in fast arithmetic (relative error <= 1e-8 even where the
 //              discriminant cancels), with a 1e-7 margin
 // One block walks whole rows (x contiguous); the running global maximum is re-read once per row.
-// bz_up: the b_z array holding the upper face of the last plane in its plane 0 (the slab above in a
-// z-slab decomposition; the state itself in a periodic single domain).
+// The upper z face of the top plane is read from the ghost plane nz of the state itself: the CT kernel
+// leaves the final value there (ct_tma.cuh), so a z slab never reads its neighbour's memory here.
 __global__ void __launch_bounds__(256)
-k_dtmax(Grid g, const double *__restrict__ U, const double *__restrict__ bz_up, StepParams *P, BoundGrid bg)
+k_dtmax(Grid g, const double *__restrict__ U, StepParams *P, BoundGrid bg)
 {
     const int nrows = g.n[1] * g.n[2];
     const long long sa = g.sa;
@@ -128,8 +128,7 @@ k_dtmax(Grid g, const double *__restrict__ U, const double *__restrict__ bz_up, 
             if (nrow < 8 || (nrow & 7) == 0) seen = __longlong_as_double((long long)*(volatile unsigned long long *)&P->smax_bits);
             const long long r0 = g.at(0, j, k);
             const long long upj = g.at(0, j + 1 == g.n[1] ? 0 : j + 1, k) - r0;
-            const bool top = g.act[2] && k + 1 == g.n[2];
-            const double *__restrict__ bzu = top ? bz_up + g.at(0, j, 0) : b + 2 * sa + r0 + g.st[2];
+            const double *__restrict__ bzu = b + 2 * sa + r0 + g.st[2];
             double thr = fmax(smax, fmax(seen, published));
             for (int i = threadIdx.x; i < g.n[0]; i += blockDim.x) {
                 const long long c = r0 + i;
@@ -202,9 +201,9 @@ __global__ void k_dtfinish(Grid g, StepParams *P, int mode)
 
 __global__ void k_advance_time(StepParams *P) { P->time += P->dt; }
 
-void launch_dtmax(const Grid &g, const double *U, const double *bz_up, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s)
+void launch_dtmax(const Grid &g, const double *U, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s)
 {
-    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, bz_up, P, bg);
+    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, P, bg);
 }
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s)
 {

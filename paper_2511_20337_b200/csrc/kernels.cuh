@@ -369,8 +369,11 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
 // Thread = one column (fixed i and transverse index), marching along DIR over `seglen` cells.  It
 // keeps the running q^L, the last two primitive states (as state + difference) and the previous
 // flux in registers, so every cell is loaded and converted once and every flux is computed once per
-// segment (+1 at the segment end).  Sout already holds the x-sweep result and is updated in place:
-//     Sout -= scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (Euler stage) or the combine weight ws.
+// segment (+1 at the segment end).  The update is
+//     Sout = base - scale * dt/dx_d * (F_d(+) - F_d(-)),  scale = 1 (Euler stage) or the combine weight ws,
+// with base = Sout when the x+y sweep has already left its result there (update in place), or base = Sin
+// when this sweep runs FIRST in a plain Euler stage and the x+y sweep then finishes the zone from Sout
+// (the read-modify-write of S' moves from this HBM-bound kernel to the ALU-bound one).
 // The operands of iteration s+1 travel global -> shared by 8-byte cp.async while interface s is
 // being solved (two slots per thread, no block synchronisation: a thread only reads what it copied).
 
@@ -419,8 +422,8 @@ constexpr int MARCH_PF = 16;     // doubles per thread and iteration: U(s+1) 5, 
 constexpr int MARCH_MINB = 3;
 template <int DIR, int LIM, bool TWO_D, bool BOUND>
 __global__ void __launch_bounds__(MARCH_NT, MARCH_MINB)
-k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-              double scale, int seglen, int tr0, BoundGrid bg)
+k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, const double *base, double *__restrict__ ct,
+              StepParams *P, double scale, int seglen, int tr0, BoundGrid bg)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
@@ -461,12 +464,12 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, double *__re
         cp_async8(&pf[slot][8][t], b2 + cn);
         if (!(TWO_D && T2 == 2)) cp_async8(&pf[slot][9][t], b2 + cn + st2);
         const long long cm = cs - st;
-        cp_async8(&pf[slot][10][t], Sout + cm);
-        cp_async8(&pf[slot][11][t], Sout + (1 + DIR) * sa + cm);
-        cp_async8(&pf[slot][12][t], Sout + (1 + T1) * sa + cm);
-        cp_async8(&pf[slot][13][t], Sout + (1 + T2) * sa + cm);
-        cp_async8(&pf[slot][14][t], Sout + 4 * sa + cm);
-        if (BZ2D) cp_async8(&pf[slot][15][t], Sout + 7 * sa + cm);
+        cp_async8(&pf[slot][10][t], base + cm);
+        cp_async8(&pf[slot][11][t], base + (1 + DIR) * sa + cm);
+        cp_async8(&pf[slot][12][t], base + (1 + T1) * sa + cm);
+        cp_async8(&pf[slot][13][t], base + (1 + T2) * sa + cm);
+        cp_async8(&pf[slot][14][t], base + 4 * sa + cm);
+        if (BZ2D) cp_async8(&pf[slot][15][t], base + 7 * sa + cm);
         cp_async_commit();
     };
     prefetch(0, c);
@@ -720,6 +723,8 @@ constexpr int WZ_SMEM_BYTES = (5 * 7 + 2 * WZ_PF) * MARCH_NT * 8;
 // Operands travel global -> shared as whole row segments by TMA bulk copies (cp.async.bulk + mbarrier)
 // issued by one thread: group A, the row that arrives next, one iteration ahead; group F, S and S^n of
 // the row that is finished in this iteration.  They bypass L1 and cost the other threads no instruction.
+// fin: the state the finished row starts from -- Sin, or Sout when the z sweep has already run in this
+// stage and left S - dt/dz (Fz(+) - Fz(-)) there (see k_sweep_march).
 constexpr int XY_RING = 9;       // rho, vx, vy, vz, Bx, By, Bz, p (cell centred), b_x on the lower x-face
 constexpr int XY_PFA = 10;       // arriving row: U 5, (rows 5, 6: carried y flux, see fpy), by upper 7, bz 8, bz upper 9
 constexpr int XY_PFF = 11;       // finishing row: U 5, S^n 6
@@ -731,8 +736,8 @@ constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 32; }   /
 constexpr int XY128_MINB = 3;
 template <int LIM, bool TWO_D, bool WRAP, int NT>
 __global__ void __launch_bounds__(NT, NT == 128 ? XY128_MINB : 512 / NT)
-k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-           Combine cb, int seglen, int kz0)
+k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, const double *fin, double *__restrict__ ct,
+           StepParams *P, Combine cb, int seglen, int kz0)
 {
     extern __shared__ __align__(128) double xy_smem[];
     const int t = threadIdx.x;
@@ -756,11 +761,14 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     const bool xface = WRAP || (has_slope && t >= 2 && i <= nx);
     const bool cell = WRAP || (xface && t <= NT - 3 && i < nx);     // this thread owns an interior cell
     const int xdup = cell ? ct_xdup(i, nx) : 0;
+    // only the warps holding the first / last cell of the row write periodic copies: a warp-uniform branch
+    // spares the other warps the predicated stores
+    const bool wdup = __any_sync(0xffffffffu, xdup != 0);
     // 3D: kz0 = -1 and the grid covers planes -1 .. nz: the CT kernel reads the x- and y-face data one plane
-    // beyond the interior (no z wrap: a z slab's neighbour planes are not its own); only the CT data of
-    // those two planes is kept, their hydro update is not stored
+    // beyond the interior (no z wrap: a z slab's neighbour planes are not its own).  Only the CT data of
+    // those two planes is used; their hydro update lands in ghost planes of Sout, which nothing reads
+    // before the next ghost fill overwrites them.
     const int k = (int)blockIdx.z + kz0;
-    const bool kin = TWO_D || (k >= 0 && k < g.n[2]);
     const int s0 = blockIdx.y * seglen, s1 = min(s0 + seglen, g.n[1]);
     const long long sa = g.sa, st = g.st[1], stz = g.st[2];
     const double gamma = g.gamma;
@@ -788,7 +796,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
     auto issue_finish = [&](long long cf) {                         // cf = first cell of the row finished next
         mbar_expect_tx(bars + 1, (5 + (combine ? (TWO_D ? 6 : 5) : 0)) * ROWB);
 #pragma unroll
-        for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + v * NT, Sin + v * sa + cf, ROWB, bars + 1);
+        for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + v * NT, fin + v * sa + cf, ROWB, bars + 1);
         if (combine) {
 #pragma unroll
             for (int v = 0; v < 5; v++) tma_bulk_g2s(pff + (5 + v) * NT, cb.Sn + v * sa + cf, ROWB, bars + 1);
@@ -926,7 +934,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
                 ct[(CT_EC + 0) * sa + cm] = e0;
                 ct[(CT_EC + 1) * sa + cm] = e1;
                 ct[(CT_EC + 2) * sa + cm] = e2;
-                if (xdup) {
+                if (wdup && xdup) {
                     const long long cd = cm + xdup;
                     ct[(CT_FEM + 0) * sa + cd] = F[4];
                     ct[(CT_FEM + 1) * sa + cd] = F[5];
@@ -968,7 +976,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             mbar_wait(bars + 2, (s - s0 - 1) & 1);   // all x fluxes of row s-1 are in shared memory
             mbar_wait(bars + 1, (s - s0 - 1) & 1);   // group F(s) has landed
         }
-        if (s > s0 && cell && kin) {
+        if (s > s0 && cell) {
             const long long cm = c - st;
             // S of row s-1 minus the x flux difference (own lower face, right neighbour's lower face)
             double r0v = fma(-dtdx, sQ[tr] - sQ[t], pff[t]);
@@ -1004,7 +1012,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
             ct[(CT_FEM + 2) * sa + c] = Fy[4];
             ct[(CT_FEM + 3) * sa + c] = Fy[5];
             ct[(CT_W + 1) * sa + c] = wy;
-            if (xdup) {
+            if (wdup && xdup) {
                 ct[(CT_FEM + 2) * sa + c + xdup] = Fy[4];
                 ct[(CT_FEM + 3) * sa + c + xdup] = Fy[5];
                 ct[(CT_W + 1) * sa + c + xdup] = wy;
@@ -1018,7 +1026,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, double *__restr
         bface = bnext; bnext = byu;
         double *rt = rm; rm = r0; r0 = rn; rn = rt;
     }
-    if (anybad && kin) P->err = 1;
+    if (anybad) P->err = 1;
 }
 
 // ---------------------------------------------------------------- CT (a6, R6) [+ RK2 combine of the faces (a7)]
@@ -1152,15 +1160,19 @@ k_ct(Grid g, const double *__restrict__ ct, const double *__restrict__ bin, doub
                     if (i == 0) bout[cm + g.n[0]] = bxo;  // periodic copy: x-face n0 is face 0
                     bout[sa + cm] = COMBINE ? fma(cb.wn, qby, cb.ws * byn) : byn;
                 }
-                if (k < k1) {                                 // b_z on the lower face of plane k
+                // b_z on the lower face of plane k (the last segment also writes face nz into the ghost
+                // plane: see k_ct_tma)
+                if (k < k1 || k1 == g.n[2]) {
                     const double eyx = sE[buf][2][ty][tx + 1], exy = sE[buf][1][ty + 1][tx];
                     const double bzn = fma(-dtdx, eyx - eyN, fma(dtdy, exy - exN, pbz));
                     bout[2 * sa + c] = COMBINE ? fma(cb.wn, qbz, cb.ws * bzn) : bzn;
+                }
+                if (k < k1) {
                     if (dbg) { dbg[c] = exN; dbg[sa + c] = eyN; dbg[2 * sa + c] = ez; }
                     // operands of the next iteration: b_x, b_y of this plane, b_z of the next
                     pbx = bin[c]; pby = bin[sa + c];
                     if (COMBINE) { qbx = cb.Sn[c]; qby = cb.Sn[sa + c]; }
-                    if (k + 1 < k1) {
+                    if (k + 1 < k1 || k1 == g.n[2]) {
                         pbz = bin[2 * sa + c + st2];
                         if (COMBINE) qbz = cb.Sn[2 * sa + c + st2];
                     }

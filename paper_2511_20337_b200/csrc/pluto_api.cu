@@ -17,7 +17,7 @@
 #include <vector>
 
 namespace pluto {
-void launch_dtmax(const Grid &g, const double *U, const double *bz_up, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s);
+void launch_dtmax(const Grid &g, const double *U, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s);
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s);
 void launch_advance_time(StepParams *P, cudaStream_t s);
 double probe_fp64_gflops(cudaStream_t s);
@@ -295,6 +295,26 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
     const int nplanes = TWO_D ? 1 : g.n[2] + 2;
     const BoundGrid none = bound_grid(d, false, 1, 1);
     bool fused = false;
+    // In a plain Euler stage of a 3D run the z sweep goes FIRST and writes S - dt/dz dFz; the fused x+y
+    // sweep then finishes the zones from there.  The read-modify-write of S' (5 + 5 doubles per zone) thereby
+    // moves from the HBM-bound z sweep to the ALU-bound x+y sweep.  Combine stages keep the x+y sweep first
+    // (S^n has to be read either way, and the last writer of the step fills the dt bound grid: the z sweep).
+    bool zfirst = false;
+    if constexpr (LIM != 2 && !TWO_D) zfirst = C.fuse_xy && !cb.Sn;
+    auto z_sweep = [&](const double *base) {
+        const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
+        const int len = seglen_z(g);
+        dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
+        const BoundGrid bg = final_bound_grid(d, last);
+        if constexpr (LIM == 2) {
+            if (last) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, !TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+            else      LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+        } else {
+            if (last) LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, !TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, base, ct, C.P, scale, len, 0, bg));
+            else      LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, base, ct, C.P, scale, len, 0, bg));
+        }
+    };
+    if (zfirst) z_sweep(Sin);
     if constexpr (LIM != 2) if (C.fuse_xy) {
         fused = true;
         // fused x + y sweep: one block per x-row chunk and y-segment.  The block width is a template
@@ -307,12 +327,12 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         const int len = seglen_y(g);
         dim3 grid(chunks, (g.n[1] + len - 1) / len, nplanes);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
-        void (*k)(Grid, const double *, double *, double *, StepParams *, Combine, int, int) =
+        void (*k)(Grid, const double *, double *, const double *, double *, StepParams *, Combine, int, int) =
             wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
                     : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
                  : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, ct, C.P, cb, len, kz0));
+        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, zfirst ? Sout : Sin, ct, C.P, cb, len, kz0));
     }
     if (!fused) {
         if constexpr (LIM == 2) {
@@ -327,21 +347,9 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         const int len = seglen_y(g);
         dim3 grid(bx, (g.n[1] + len - 1) / len, nplanes);
         if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, none));
-        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, none));
+        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, Sout, ct, C.P, scale, len, kz0, none));
     }
-    if (!TWO_D) {
-        const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
-        const int len = seglen_z(g);
-        dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
-        const BoundGrid bg = final_bound_grid(d, last);
-        if constexpr (LIM == 2) {
-            if (last) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, !TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
-            else      LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
-        } else {
-            if (last) LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, !TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
-            else      LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
-        }
-    }
+    if (!TWO_D && !zfirst) z_sweep(Sout);
 }
 
 // CT: edge EMFs + face update (+ combine) in one kernel; dbg (debug only) receives the edge EMFs
@@ -427,8 +435,7 @@ void enqueue_dtmax(bool keep_bounds)
 {
     for (const Domain &d : C.dom) {
         const BoundGrid bg = final_bound_grid(d, true);
-        const double *bz_up = peer_arr(d.nb[1], A_SA + S_B + 2);
-        LAUNCH(K_DTMAX, launch_dtmax(d.g, arr(d, A_SA), bz_up, C.P, bg, C.sm_count * 8, C.stream));
+        LAUNCH(K_DTMAX, launch_dtmax(d.g, arr(d, A_SA), C.P, bg, C.sm_count * 8, C.stream));
     }
     if (!keep_bounds)
         for (const Domain &d : C.dom) cudaMemsetAsync(d.bound, 0, bound_cells(d.g) * 8, C.stream);
