@@ -61,6 +61,11 @@ class Oracle:
         L.oracle_physical_flux.restype = None
         L.oracle_hlld.argtypes = [_dp, _dp, C.c_double, C.c_double, _dp, _dp, _dp]
         L.oracle_debug_euler.argtypes = [C.c_double, _dp, _dp, _dp, _dp, _dp]
+        L.oracle_set_divb.argtypes = [C.c_int]
+        L.oracle_set_psi.argtypes = [_dp]
+        L.oracle_get_psi.argtypes = [_dp]
+        L.oracle_glm_interface.argtypes = [C.c_double] * 5 + [_dp, _dp]
+        L.oracle_glm_interface.restype = None
         self.L = L
         self.shape = None
 
@@ -81,14 +86,17 @@ class Oracle:
 
     def set_state(self, U, Bface):
         U = np.ascontiguousarray(U, dtype=np.float64)
+        assert U.size == 8 * np.prod(self.shape)
+        if Bface is None:                        # GLM variant: no face fields
+            return self.L.oracle_set_state(_ptr(U), None)
         Bface = np.ascontiguousarray(Bface, dtype=np.float64)
-        assert U.size == 8 * np.prod(self.shape) and Bface.size == self.nface()
+        assert Bface.size == self.nface()
         return self.L.oracle_set_state(_ptr(U), _ptr(Bface))
 
-    def get_state(self):
+    def get_state(self, faces=True):
         nx, ny, nz = self.shape
         U = np.empty((8, nz, ny, nx))
-        Bf = np.empty(self.nface())
+        Bf = np.empty(self.nface()) if faces else None
         rc = self.L.oracle_get_state(_ptr(U), _ptr(Bf))
         assert rc == 0
         return U, Bf
@@ -116,6 +124,35 @@ class Oracle:
 
     def finalize(self):
         return self.L.oracle_finalize()
+
+    # ---- GLM divergence cleaning (R20)
+    def set_divb(self, mode):
+        return self.L.oracle_set_divb(mode)
+
+    def set_psi(self, psi):
+        psi = np.ascontiguousarray(psi, dtype=np.float64)
+        return self.L.oracle_set_psi(_ptr(psi))
+
+    def get_psi(self):
+        nx, ny, nz = self.shape
+        psi = np.empty((nz, ny, nx))
+        assert self.L.oracle_get_psi(_ptr(psi)) == 0
+        return psi
+
+    def glm_interface(self, BnL, BnR, psiL, psiR, ch):
+        out = np.empty(2)
+        self.L.oracle_glm_interface(BnL, BnR, psiL, psiR, ch, _ptr(out[0:1]), _ptr(out[1:2]))
+        return float(out[0]), float(out[1])
+
+    def load_glm(self, w, threads=None):
+        """init + set_box + GLM mode + set_state (cell-centred B of w.U, psi = 0)"""
+        if threads is not None:
+            self.set_threads(threads)
+        assert self.init(w.nx, w.ny, w.nz, 2, w.gamma, w.cfl, w.limiter) == 0
+        assert self.set_box(*w.box) == 0
+        assert self.set_divb(1) == 0
+        assert self.set_state(w.U, None) == 0
+        return self
 
     def load(self, w, threads=None):
         """init + set_box + set_state from a workloads.Workload"""

@@ -47,6 +47,10 @@ typedef struct {
     int rk_order;          /* 2 (or 0: default) = SSP-RK2, 3 = SSP-RK3 */
     int err;
     int threads;
+    /* divergence control: 0 = constrained transport (default), 1 = GLM divergence cleaning (R20) */
+    int divb;
+    double *psi, *psi1, *psi2;   /* the cleaning scalar of the GLM variant, [N] each */
+    double *Fpsi;                /* its flux through the lower d-face, [3][N] */
 } ctx_t;
 
 static ctx_t g;
@@ -307,6 +311,7 @@ static void free_all(void)
     free(g.U); free(g.U1); free(g.U2);
     for (d = 0; d < 3; d++) { free(g.b[d]); free(g.b1[d]); free(g.b2[d]); }
     free(g.V); free(g.F); free(g.W); free(g.Eg); free(g.Ec);
+    free(g.psi); free(g.psi1); free(g.psi2); free(g.Fpsi);
     memset(&g, 0, sizeof g);
 }
 
@@ -345,7 +350,10 @@ int oracle_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int
     g.W  = calloc(3 * N, sizeof(double));
     g.Eg = calloc(3 * N, sizeof(double));
     g.Ec = calloc(3 * N, sizeof(double));
+    g.psi = calloc(N, sizeof(double)); g.psi1 = calloc(N, sizeof(double)); g.psi2 = calloc(N, sizeof(double));
+    g.Fpsi = calloc(3 * N, sizeof(double));
     if (!g.U || !g.U1 || !g.U2 || !g.V || !g.F || !g.W || !g.Eg || !g.Ec) { free_all(); return ORACLE_ENOMEM; }
+    if (!g.psi || !g.psi1 || !g.psi2 || !g.Fpsi) { free_all(); return ORACLE_ENOMEM; }
     for (d = 0; d < 3; d++) if (!g.b[d] || !g.b1[d] || !g.b2[d]) { free_all(); return ORACLE_ENOMEM; }
     g.init = 1;
     g.time = 0.0; g.dt_last = 0.0; g.stepped = 0; g.err = 0;
@@ -411,6 +419,11 @@ int oracle_set_state(const double *U, const double *Bface)
     if (!g.init) return ORACLE_ESTATE;
     if (!U) return ORACLE_EINVAL;
     memcpy(g.U, U, 8 * g.N * sizeof(double));
+    if (g.divb == 1) {       /* GLM: the cell-centred B of U is the field; no faces; psi starts at zero */
+        memset(g.psi, 0, g.N * sizeof(double));
+        g.time = 0.0; g.stepped = 0; g.err = 0; g.dt_last = 0.0;
+        return ORACLE_OK;
+    }
     for (d = 0; d < 3; d++) {
         int i, j, k, m[3];
         if (!g.act[d]) continue;
@@ -436,7 +449,7 @@ int oracle_get_state(double *U, double *Bface)
     for (d = 0; d < 3; d++) {
         int i, j, k, m[3];
         if (!g.act[d]) continue;
-        if (!Bface) break;
+        if (!Bface || g.divb == 1) break;
         m[0] = g.n[0]; m[1] = g.n[1]; m[2] = g.n[2]; m[d] += 1;
         for (k = 0; k < m[2]; k++)
             for (j = 0; j < m[1]; j++)
@@ -623,10 +636,164 @@ static void euler(const double *Uin, double *const bin[3], double dt, double *Uo
     cell_b_from_faces(Uout, bout);
 }
 
+
+/* ------------------------------------------------------------------ GLM divergence cleaning (R20)
+ * The paper's other divergence control ("divergence cleaning [43, 44]", used in its strong-scaling
+ * runs) is named, not printed.  Reading R20 restates the mixed hyperbolic / parabolic GLM-MHD
+ * scheme of Dedner et al. 2002 [43] in its conservative form:
+ *     dB/dt + div(v B - B v) + grad psi = 0,      dpsi/dt + c_h^2 div B = -(c_h^2 / c_p^2) psi,
+ * cell-centred B, one extra scalar psi, no face fields, no CT.  Per interface, the (B_n, psi) pair obeys a
+ * linear 2x2 system with the waves -c_h, +c_h whatever the fluid does; its Riemann problem is solved exactly,
+ *     B_m   = (B_nL + B_nR)/2 - (psi_R - psi_L)/(2 c_h),      psi_m = (psi_L + psi_R)/2 - c_h (B_nR - B_nL)/2,
+ * the flux of B_n is psi_m and the flux of psi is c_h^2 B_m, and the other seven fluxes are the HLLD fluxes
+ * with the normal field B_m on both sides.  c_h = cfl * min_d(dx_d) / dt (the fastest speed the time step
+ * allows); after every full step psi is damped exactly, psi *= exp(-dt c_h / c_r), with the constant
+ * c_r = c_p^2 / c_h = 0.18 that [43] recommends.  The energy equation is unchanged (total energy conserved). */
+#define GLM_CR 0.18
+
+void oracle_glm_interface(double BnL, double BnR, double psiL, double psiR, double ch, double *Bm, double *psim)
+{
+    *Bm = 0.5 * (BnL + BnR) - 0.5 * (psiR - psiL) / ch;
+    *psim = 0.5 * (psiL + psiR) - 0.5 * ch * (BnR - BnL);
+}
+
+static double glm_ch(double dt)
+{
+    int d; double h = 0.0;
+    for (d = 0; d < 3; d++) if (g.act[d] && (h == 0.0 || g.dx[d] < h)) h = g.dx[d];
+    return g.cfl * h / dt;
+}
+
+/* Euler(S, dt) of the GLM variant: (Uin, psin) -> (Uout, psout); fills g.V, g.F, g.Fpsi */
+static void euler_glm(const double *Uin, const double *psin, double dt, double ch, double *Uout, double *psout)
+{
+    const size_t N = g.N;
+    int d;
+    long c;
+    if (all_prims(Uin, g.V)) g.err = 1;
+    memset(g.F, 0, 24 * N * sizeof(double));
+    memset(g.Fpsi, 0, 3 * N * sizeof(double));
+    for (d = 0; d < 3; d++) {
+        const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+        /* the 7 HLLD primitives in rotated order, then the normal field and psi */
+        const int qv[8] = { 0, 1 + d, 1 + t1, 1 + t2, 4 + t1, 4 + t2, 7, 4 + d };
+        double *Fd = g.F + (size_t)d * 8 * N;
+        double *Fp = g.Fpsi + (size_t)d * N;
+        if (!g.act[d]) continue;
+#pragma omp parallel for
+        for (c = 0; c < (long)N; c++) {
+            int i, j, k, q;
+            size_t cm3, cm2, cm1, c0, cp1, cp2;
+            double VL[9], VR[9], Fr[8], w, Bm, psim;
+            c2ijk((size_t)c, &i, &j, &k);
+            cm2 = shift(i, j, k, d, -2); cm1 = shift(i, j, k, d, -1);
+            c0 = (size_t)c;              cp1 = shift(i, j, k, d, +1);
+            cm3 = shift(i, j, k, d, -3); cp2 = shift(i, j, k, d, +2);
+            for (q = 0; q < 9; q++) {
+                const double *Q = q < 8 ? g.V + (size_t)qv[q] * N : psin;
+                if (g.limiter == 2) {
+                    double sl[5] = { Q[cm3], Q[cm2], Q[cm1], Q[c0], Q[cp1] };
+                    double sr[5] = { Q[cp2], Q[cp1], Q[c0], Q[cm1], Q[cm2] };
+                    VL[q] = oracle_wenoz(sl);
+                    VR[q] = oracle_wenoz(sr);
+                } else {
+                    double sm = oracle_plm_slope(Q[cm1] - Q[cm2], Q[c0] - Q[cm1], g.limiter);
+                    double s0 = oracle_plm_slope(Q[c0] - Q[cm1], Q[cp1] - Q[c0], g.limiter);
+                    VL[q] = Q[cm1] + 0.5 * sm;
+                    VR[q] = Q[c0] - 0.5 * s0;
+                }
+            }
+            /* interface c-1/2: exact (B_n, psi) state, then HLLD with that normal field on both sides */
+            oracle_glm_interface(VL[7], VR[7], VL[8], VR[8], ch, &Bm, &psim);
+            oracle_hlld(VL, VR, Bm, g.gamma, Fr, &w, NULL);
+            Fd[0 * N + c0] = Fr[0];
+            Fd[(1 + d) * N + c0] = Fr[1]; Fd[(1 + t1) * N + c0] = Fr[2]; Fd[(1 + t2) * N + c0] = Fr[3];
+            Fd[(4 + d) * N + c0] = psim;  Fd[(4 + t1) * N + c0] = Fr[5]; Fd[(4 + t2) * N + c0] = Fr[6];
+            Fd[7 * N + c0] = Fr[7];
+            Fp[c0] = ch * ch * Bm;
+        }
+    }
+    memcpy(Uout, Uin, 8 * N * sizeof(double));
+    memcpy(psout, psin, N * sizeof(double));
+    for (d = 0; d < 3; d++) {
+        const double *Fd = g.F + (size_t)d * 8 * N;
+        const double *Fp = g.Fpsi + (size_t)d * N;
+        double dtdx;
+        if (!g.act[d]) continue;
+        dtdx = dt / g.dx[d];
+#pragma omp parallel for
+        for (c = 0; c < (long)N; c++) {
+            int i, j, k, v; size_t cp1;
+            c2ijk((size_t)c, &i, &j, &k);
+            cp1 = shift(i, j, k, d, +1);
+            for (v = 0; v < 8; v++)
+                Uout[v * N + c] -= dtdx * (Fd[v * N + cp1] - Fd[v * N + c]);
+            psout[c] -= dtdx * (Fp[cp1] - Fp[c]);
+        }
+    }
+}
+
+static void one_step_glm(double dt)
+{
+    const size_t N = g.N;
+    const double ch = glm_ch(dt);
+    const double damp = exp(-dt * ch / GLM_CR);
+    long c;
+    if (g.rk_order == 3) {      /* Eq. 5 (R17), as in one_step */
+        euler_glm(g.U, g.psi, dt, ch, g.U1, g.psi1);
+        euler_glm(g.U1, g.psi1, dt, ch, g.U2, g.psi2);
+#pragma omp parallel for
+        for (c = 0; c < (long)(8 * N); c++) g.U2[c] = (3.0 * g.U[c] + g.U2[c]) / 4.0;
+#pragma omp parallel for
+        for (c = 0; c < (long)N; c++) g.psi2[c] = (3.0 * g.psi[c] + g.psi2[c]) / 4.0;
+        euler_glm(g.U2, g.psi2, dt, ch, g.U1, g.psi1);
+#pragma omp parallel for
+        for (c = 0; c < (long)(8 * N); c++) g.U[c] = (g.U[c] + 2.0 * g.U1[c]) / 3.0;
+#pragma omp parallel for
+        for (c = 0; c < (long)N; c++) g.psi[c] = (g.psi[c] + 2.0 * g.psi1[c]) / 3.0;
+    } else {                    /* R3 */
+        euler_glm(g.U, g.psi, dt, ch, g.U1, g.psi1);
+        euler_glm(g.U1, g.psi1, dt, ch, g.U2, g.psi2);
+#pragma omp parallel for
+        for (c = 0; c < (long)(8 * N); c++) g.U[c] = 0.5 * (g.U[c] + g.U2[c]);
+#pragma omp parallel for
+        for (c = 0; c < (long)N; c++) g.psi[c] = 0.5 * (g.psi[c] + g.psi2[c]);
+    }
+    /* the parabolic part of the psi equation, integrated exactly over the step */
+#pragma omp parallel for
+    for (c = 0; c < (long)N; c++) g.psi[c] *= damp;
+    g.time += dt;
+    g.dt_last = dt;
+    g.stepped = 1;
+}
+
+int oracle_set_divb(int mode)
+{
+    if (!g.init) return ORACLE_ESTATE;
+    if (mode != 0 && mode != 1) return ORACLE_EINVAL;
+    g.divb = mode;
+    return ORACLE_OK;
+}
+
+int oracle_set_psi(const double *psi)
+{
+    if (!g.init || g.divb != 1) return ORACLE_ESTATE;
+    memcpy(g.psi, psi, g.N * sizeof(double));
+    return ORACLE_OK;
+}
+
+int oracle_get_psi(double *psi)
+{
+    if (!g.init || g.divb != 1) return ORACLE_ESTATE;
+    memcpy(psi, g.psi, g.N * sizeof(double));
+    return ORACLE_OK;
+}
+
 static void one_step(double dt)
 {
     const size_t N = g.N;
     long c; int d;
+    if (g.divb == 1) { one_step_glm(dt); return; }
     if (g.rk_order == 3) {
         /* Eq. 5, SSP-RK3 in Shu-Osher form; reading R17: the last stage carries 2 L**
            (as printed, "+ L**", the weights of L do not sum to one):

@@ -42,6 +42,15 @@ int    oracle_set_integrator(int order); /* after oracle_init: 2 = SSP-RK2 (defa
 int    oracle_set_threads(int n);      /* OpenMP threads (results do not depend on it) */
 int    oracle_get_threads(void);
 
+/* ---- GLM divergence cleaning ([43] PAPER.md:636; reading R20 in oracle.c) ----
+ * oracle_set_divb(1) after oracle_init switches to the cell-centred-B variant: U[4..6] is the field, Bface is
+ * ignored (may be NULL), psi starts at zero (oracle_set_psi overrides it).  0 = constrained transport (default). */
+int    oracle_set_divb(int mode);
+int    oracle_set_psi(const double *psi);       /* [nz][ny][nx] */
+int    oracle_get_psi(double *psi);
+/* exact interface state of the (B_n, psi) subsystem with the waves -c_h, +c_h */
+void   oracle_glm_interface(double BnL, double BnR, double psiL, double psiR, double ch, double *Bm, double *psim);
+
 /* ---- pieces, exposed so that tests can pin each one separately ---- */
 
 /* Eq. 7: U[8] -> V[8] = (rho, vx, vy, vz, Bx, By, Bz, p). returns 0, or ORACLE_EPHYS */
