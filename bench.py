@@ -45,8 +45,13 @@ UNIT = "zone-updates/s"
 #              exchanges with the other kernels through HBM + re-reads across kernels); reported as
 #              `design_*` next to it, so that wasted traffic is visible.
 # Keyed by kernel class; values = doubles per zone for (first stage, combine stage).
-def kernel_doubles(ndim, rk):
+def kernel_doubles(ndim, rk, glm=False):
     """(method, design) doubles per zone per launch, averaged over the stages of one step"""
+    if glm:
+        # GLM variant (first version, one kernel per direction; a state is 9 arrays): the x sweep reads S and
+        # writes S', the y and z sweeps read S and read-modify-write S'
+        m = {"sweep_x": 18.0, "sweep_y": 27.0, "sweep_z": 27.0, "dt_max": 8.0}
+        return m, dict(m)
     nface = 3 if ndim == 3 else 2
     nct_xy = 9 if ndim == 3 else 5            # x/y induction fluxes + weights + cell EMFs kept for CT
     combine_stages = rk - 1                   # stages that also read S^n
@@ -181,14 +186,17 @@ class ClockSampler:
                 "power_w": statistics.median(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_run(w, steps, threads=None, rk=2, warmup=1):
+def oracle_run(w, steps, threads=None, rk=2, warmup=1, glm=False):
     """the oracle as it stands on the host cores: `steps` whole steps of workload w; returns
     (zone-updates/s, threads used, seconds, per-step seconds)"""
     from oracle import Oracle
     o = Oracle()
     if threads:
         o.set_threads(threads)
-    o.load(w)
+    if glm:
+        o.load_glm(w)
+    else:
+        o.load(w)
     o.set_integrator(rk)
     for _ in range(warmup):
         assert o.step(1) == 0                   # touch memory
@@ -223,14 +231,14 @@ def cpu_workload(cfg):
     return wl.config(cfg), "the bench workload itself, full size"
 
 
-def scheme_of(w, rk):
-    return "recon(%s)+HLLD+RK%d+CT, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], rk, w.cfl)
+def scheme_of(w, rk, glm=False):
+    return "recon(%s)+HLLD+RK%d+%s, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], rk, "GLM" if glm else "CT", w.cfl)
 
 
 def config_of(args, w, world):
     name = (f"configs[{args.config}] {w.name}" if args.config < 5
             else f"paper section 4.1 workload (not a BASELINE config) {w.name}")
-    return {"workload": name, "grid": [w.nx, w.ny, w.nz], "zones": w.zones, "scheme": scheme_of(w, args.rk),
+    return {"workload": name, "grid": [w.nx, w.ny, w.nz], "zones": w.zones, "scheme": scheme_of(w, args.rk, args.glm),
             "l2": "inputs larger than L2 (state %.2f GB)" % (11 * w.zones * 8 / 1e9) if w.zones * 88 > 126e6
                   else "L2 flushed between timed repeats (a 256 MB buffer is rewritten); the state fits in L2",
             "parallelism": "single GPU" if world == 1 else "z-slab domain decomposition, one slab per GPU"}
@@ -244,7 +252,7 @@ def run_reference(args):
     w, what = cpu_workload(args.config)
     if args.wenoz:
         w.limiter = 2
-    val, cores, secs, per = oracle_run(w, args.steps, rk=args.rk, warmup=max(1, min(args.warmup, 2)))
+    val, cores, secs, per = oracle_run(w, args.steps, rk=args.rk, warmup=max(1, min(args.warmup, 2)), glm=args.glm)
     from paper_2511_20337_b200 import workloads as wl
     wcfg = wl.config(args.config) if args.config != 4 else w
     line = {
@@ -269,6 +277,7 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--wenoz", action="store_true", help="WENO-Z reconstruction instead of the config's PLM limiter")
     ap.add_argument("--rk", type=int, default=2, help="2: SSP-RK2 (the north_star's step, default); 3: SSP-RK3 of Eq. 5")
+    ap.add_argument("--glm", action="store_true", help="GLM divergence cleaning (cell-centred B) instead of constrained transport")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--repeats", type=int, default=3, help="timed repeats of the K steps (median and best reported)")
@@ -293,7 +302,10 @@ def main():
         w.limiter = 2
     sim = Pluto(device=local)
     sim.set_integrator(args.rk)
-    sim.load(w)
+    if args.glm:
+        sim.load_glm(w)
+    else:
+        sim.load(w)
     K, W = args.steps, max(args.warmup, 3)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     small = w.zones * 88 <= 126e6                 # the state fits in L2: flush it between repeats
@@ -338,8 +350,8 @@ def main():
     dom_ms, dom_cnt = rep[dom]
     hbm_peak, peak_src = peaks()
     units = w.zones                              # zones one launch of the dominant kernel processes
-    method, design = kernel_doubles(w.ndim, args.rk)
-    ncu, ncu_src = ncu_table(w.ndim, args.rk, w.limiter, units)
+    method, design = kernel_doubles(w.ndim, args.rk, args.glm)
+    ncu, ncu_src = ncu_table(w.ndim, args.rk, w.limiter, units) if not args.glm else (None, None)
     dur = dom_ms * 1e-3 / max(dom_cnt, 1)
     method_bytes = method.get(dom, 0) * 8 * units
     design_bytes = design.get(dom, 0) * 8 * units
@@ -421,11 +433,11 @@ def main():
         wc, what = cpu_workload(args.config)
         if args.wenoz:
             wc.limiter = 2
-        v, cores, secs, per = oracle_run(wc, 3, rk=args.rk)
+        v, cores, secs, per = oracle_run(wc, 3, rk=args.rk, glm=args.glm)
         ws, what1 = small_sample(args.config)
         if args.wenoz:
             ws.limiter = 2
-        v1, _, secs1, _ = oracle_run(ws, 1, threads=1, rk=args.rk, warmup=0)
+        v1, _, secs1, _ = oracle_run(ws, 1, threads=1, rk=args.rk, warmup=0, glm=args.glm)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{what}, 3 steps, {secs:.1f} s",
                                 "best_step_s": min(per), "median_step_s": statistics.median(per),

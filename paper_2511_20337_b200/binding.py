@@ -20,6 +20,8 @@ OPT_GRAPH = 1
 OPT_FUSE_XY = 2
 OPT_CT_TMA = 3
 OPT_RK_ORDER = 4
+OPT_DIVB = 5
+DIVB_CT, DIVB_GLM = 0, 1
 
 # every symbol include/pluto.h declares
 SYMBOLS = [
@@ -30,7 +32,7 @@ SYMBOLS = [
     "pluto_set_option", "pluto_debug_euler", "pluto_profile", "pluto_profile_get", "pluto_kernel_name",
     "pluto_probe_fp64_gflops",
     "pluto_init_slabs", "pluto_workspace_bytes_slabs", "pluto_local_planes", "pluto_export_slab",
-    "pluto_attach_peer", "pluto_fill_ghosts", "pluto_slab_planes", "pluto_step_begin", "pluto_dt_max_bits", "pluto_step_stage",
+    "pluto_attach_peer", "pluto_fill_ghosts", "pluto_slab_planes", "pluto_set_psi", "pluto_get_psi", "pluto_step_begin", "pluto_dt_max_bits", "pluto_step_stage",
 ]
 
 
@@ -81,6 +83,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pluto_step_begin.argtypes = [dbl]
     L.pluto_dt_max_bits.restype = vp
     L.pluto_step_stage.argtypes = [i32, i32]
+    L.pluto_set_psi.argtypes = [vp]
+    L.pluto_get_psi.argtypes = [vp]
     return L
 
 
@@ -218,6 +222,41 @@ class Pluto:
 
     def finalize(self):
         return self.L.pluto_finalize()
+
+    # ---- GLM divergence cleaning (PLUTO_OPT_DIVB; reading R20)
+    def set_divb(self, mode):
+        """divergence control of the NEXT init: DIVB_CT (default) or DIVB_GLM"""
+        old = self.L.pluto_set_option(OPT_DIVB, mode)
+        if old < 0:
+            raise PlutoError(old, self.L.pluto_last_error().decode())
+        return old
+
+    def load_glm(self, w, ghost=2):
+        """init (GLM variant) + set_box + set_state from a workloads.Workload: cell-centred B of w.U, psi = 0"""
+        self.set_divb(DIVB_GLM)
+        try:
+            self.init(w.nx, w.ny, w.nz, ghost, w.gamma, w.cfl, w.limiter)
+        finally:
+            self.set_divb(DIVB_CT)
+        self.set_box(*w.box)
+        U = np.ascontiguousarray(w.U, dtype=np.float64)
+        return self._check(self.L.pluto_set_state(_addr(U), None))
+
+    def get_state_glm(self):
+        nx, ny, nz = self.shape
+        U = np.empty((8, nz, ny, nx))
+        self._check(self.L.pluto_get_state(_addr(U), None))
+        return U
+
+    def set_psi(self, psi):
+        psi = np.ascontiguousarray(psi, dtype=np.float64)
+        return self._check(self.L.pluto_set_psi(_addr(psi)))
+
+    def get_psi(self):
+        nx, ny, nz = self.shape
+        psi = np.empty((nz, ny, nx))
+        self._check(self.L.pluto_get_psi(_addr(psi)))
+        return psi
 
     def load(self, w, ghost=None, nslab=1):
         """init + set_box + set_state from a workloads.Workload (host arrays)"""

@@ -71,7 +71,7 @@ __device__ __forceinline__ double sqrt_nr(double x)      // x > 0
 // The upper z face of the top plane is read from the ghost plane nz of the state itself: the CT kernel
 // leaves the final value there (ct_tma.cuh), so a z slab never reads its neighbour's memory here.
 __global__ void __launch_bounds__(256)
-k_dtmax(Grid g, const double *__restrict__ U, StepParams *P, BoundGrid bg)
+k_dtmax(Grid g, const double *__restrict__ U, StepParams *P, BoundGrid bg, int cell_b)
 {
     const int nrows = g.n[1] * g.n[2];
     const long long sa = g.sa;
@@ -134,9 +134,10 @@ k_dtmax(Grid g, const double *__restrict__ U, StepParams *P, BoundGrid bg)
                 const long long c = r0 + i;
                 const double rho = U[c], mx = U[sa + c], my = U[2 * sa + c], mz = U[3 * sa + c], E = U[4 * sa + c];
                 // cell-centred B = mean of the two faces (R7); 2D: the third magnetic array is the cell B_z
-                const double B[3] = { 0.5 * (b[c] + b[r0 + (i + 1 == g.n[0] ? 0 : i + 1)]),
-                                      0.5 * (b[sa + c] + b[sa + c + upj]),
-                                      g.act[2] ? 0.5 * (b[2 * sa + c] + bzu[i]) : b[2 * sa + c] };
+                // (cell_b: the GLM variant keeps cell-centred B in the three magnetic arrays)
+                const double B[3] = { cell_b ? b[c] : 0.5 * (b[c] + b[r0 + (i + 1 == g.n[0] ? 0 : i + 1)]),
+                                      cell_b ? b[sa + c] : 0.5 * (b[sa + c] + b[sa + c + upj]),
+                                      (g.act[2] && !cell_b) ? 0.5 * (b[2 * sa + c] + bzu[i]) : b[2 * sa + c] };
                 const double ir = rcp_nr(rho);
                 const double B2 = fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2]));
                 const double vx = mx * ir, vy = my * ir, vz = mz * ir;
@@ -197,13 +198,18 @@ __global__ void k_dtfinish(Grid g, StepParams *P, int mode)
     if (mode == 2) { P->dt_probe = dt; return; }
     P->dt = dt;
     for (int d = 0; d < 3; d++) P->dtdx[d] = dt / g.dx[d];
+    // GLM variant (glm.cuh, reading R20): c_h = cfl min_d(dx_d) / dt, damping factor of psi over the step
+    double h = 0.0;
+    for (int d = 0; d < 3; d++) if (g.act[d] && (h == 0.0 || g.dx[d] < h)) h = g.dx[d];
+    P->glm_ch = g.cfl * h / dt;
+    P->glm_damp = exp(-dt * P->glm_ch / 0.18);
 }
 
 __global__ void k_advance_time(StepParams *P) { P->time += P->dt; }
 
-void launch_dtmax(const Grid &g, const double *U, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s)
+void launch_dtmax(const Grid &g, const double *U, StepParams *P, BoundGrid bg, int cell_b, int nblocks, cudaStream_t s)
 {
-    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, P, bg);
+    k_dtmax<<<nblocks, 256, 0, s>>>(g, U, P, bg, cell_b);
 }
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s)
 {

@@ -43,6 +43,8 @@ struct StepParams {
     unsigned long long smax_bits;   // running max of (|v_d| + c_f,d)/dx_d as an IEEE bit pattern
     int err;                        // sticky: unphysical zone met
     int pad;
+    double glm_ch;                  // GLM variant (glm.cuh): c_h = cfl min(dx) / dt of the step being taken
+    double glm_damp;                // exp(-dt c_h / c_r)
 };
 
 // Coarse grid of CFL upper bounds left by the kernel that writes the final hydro variables of a step

@@ -8,6 +8,7 @@
 #include "../../include/pluto.h"
 #include "kernels.cuh"
 #include "ct_tma.cuh"
+#include "glm.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -17,7 +18,7 @@
 #include <vector>
 
 namespace pluto {
-void launch_dtmax(const Grid &g, const double *U, StepParams *P, BoundGrid bg, int nblocks, cudaStream_t s);
+void launch_dtmax(const Grid &g, const double *U, StepParams *P, BoundGrid bg, int cell_b, int nblocks, cudaStream_t s);
 void launch_dtfinish(const Grid &g, StepParams *P, int mode, cudaStream_t s);
 void launch_advance_time(StepParams *P, cudaStream_t s);
 double probe_fp64_gflops(cudaStream_t s);
@@ -73,6 +74,8 @@ struct Context {
     int fuse_xy = 1;
     int ct_tma = 1;
     int rk_order = 2;                // 2: SSP-RK2 (R3), 3: SSP-RK3 (Eq. 5)
+    int divb = 0;                    // PLUTO_OPT_DIVB of the next pluto_init: 0 constrained transport, 1 GLM cleaning
+    bool glm = false;                // the live context runs the GLM variant (glm.cuh)
     cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step (of the current rk_order)
     int sm_count = 148;
     char err[512] = "";
@@ -399,8 +402,41 @@ int set_kernel_attributes()
 // Sout <- wn * S^n + ws * Euler(Sin) (sn < 0: no combine; sn may equal out: in place).  Every slab's
 // ghost fill comes first: it reads the neighbours' interiors of `in`, which the compute kernels of this
 // stage never write (out != in).
+// ---- the GLM variant (glm.cuh): cell-centred B in the three magnetic arrays of a state, psi and the scratch
+// state of the combine stages in the (otherwise unused) CT work arrays
+int glm_psi(int state) { return A_CT + (state == A_SA ? 0 : state == A_SB ? 1 : 2); }
+constexpr int GLM_TMP = A_CT + 3, GLM_TMP_PSI = A_CT + 11;
+
+template <int LIM>
+void enqueue_stage_glm(int in, int out, int sn, double wn, double ws, bool last)
+{
+    const Domain &d = C.dom[0];
+    const Grid &g = d.g;
+    cudaStream_t s = C.stream;
+    ZSrc zs = zsrc(d, in);
+    LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 8, 256, 0, s>>>(g, arr(d, in), S_COUNT, zs));
+    double *psin = arr(d, glm_psi(in));
+    ZSrc zp = zs;
+    zp.lo = zp.hi = psin;
+    LAUNCH(K_GHOST, k_ghost<<<C.sm_count * 2, 256, 0, s>>>(g, psin, 1, zp));
+    // a combine stage computes Euler(S) into scratch arrays first (out may be S^n itself)
+    double *So = arr(d, sn >= 0 ? GLM_TMP : out), *po = arr(d, sn >= 0 ? GLM_TMP_PSI : glm_psi(out));
+    const dim3 grid((g.n[0] + 127) / 128, g.n[1], g.n[2]);
+    LAUNCH(K_FLUX_X, k_glm_sweep<0, LIM, true><<<grid, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
+    LAUNCH(K_FLUX_Y, k_glm_sweep<1, LIM, false><<<grid, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
+    if (g.act[2]) LAUNCH(K_FLUX_Z, k_glm_sweep<2, LIM, false><<<grid, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
+    if (sn >= 0)
+        LAUNCH(K_SCALAR, k_glm_combine<<<grid, 128, 0, s>>>(g, arr(d, out), arr(d, glm_psi(out)), arr(d, sn), arr(d, glm_psi(sn)),
+                                                          So, po, wn, ws, last ? 1 : 0, C.P));
+}
+
 void enqueue_stage(int in, int out, int sn, double wn, double ws, bool last, double *dbg = nullptr)
 {
+    if (C.glm) {
+        if (C.dom[0].g.limiter == 0) enqueue_stage_glm<0>(in, out, sn, wn, ws, last);
+        else                         enqueue_stage_glm<1>(in, out, sn, wn, ws, last);
+        return;
+    }
     for (const Domain &d : C.dom) fill_ghosts(d, in);
     for (const Domain &d : C.dom) {
         const Grid &g = d.g;
@@ -434,8 +470,9 @@ void enqueue_rk_stage(int s)
 void enqueue_dtmax(bool keep_bounds)
 {
     for (const Domain &d : C.dom) {
-        const BoundGrid bg = final_bound_grid(d, true);
-        LAUNCH(K_DTMAX, launch_dtmax(d.g, arr(d, A_SA), C.P, bg, C.sm_count * 8, C.stream));
+        BoundGrid bg = final_bound_grid(d, true);
+        if (C.glm) bg.b = nullptr;               // the GLM sweeps leave no bound grid
+        LAUNCH(K_DTMAX, launch_dtmax(d.g, arr(d, A_SA), C.P, bg, C.glm ? 1 : 0, C.sm_count * 8, C.stream));
     }
     if (!keep_bounds)
         for (const Domain &d : C.dom) cudaMemsetAsync(d.bound, 0, bound_cells(d.g) * 8, C.stream);
@@ -534,7 +571,7 @@ struct Staging {
     int get(size_t doubles)
     {
         const Domain &d0 = C.dom[0];
-        if (C.dom.size() == 1 && doubles <= (size_t)CT_COUNT * d0.g.sa) { p = arr(d0, A_CT); return PLUTO_OK; }
+        if (C.dom.size() == 1 && !C.glm && doubles <= (size_t)CT_COUNT * d0.g.sa) { p = arr(d0, A_CT); return PLUTO_OK; }
         if (cudaMalloc((void **)&p, doubles * sizeof(double)) != cudaSuccess) {
             cudaGetLastError();
             p = nullptr;
@@ -618,6 +655,9 @@ int init_common(int nslab, int first, int count, int nx, int ny, int nz, int gho
         return fail(PLUTO_EINVAL, "the WENO-Z stencil needs ghost >= 3");
     if (nslab > 1 && (nz / nslab < ghost + 1))
         return fail(PLUTO_EINVAL, "every z slab needs at least ghost + 1 = %d planes", ghost + 1);
+    if (C.divb == 1 && (nslab != 1 || limiter == PLUTO_WENOZ))
+        return fail(PLUTO_EINVAL, "the GLM variant runs PLM on a single domain");
+    C.glm = C.divb == 1;
     const int narrays = C.rk_order == 3 ? A_COUNT : A_COUNT_RK2;
     C.nslab = nslab; C.first = first; C.nzg = nz;
     C.dom.resize(count);
@@ -685,6 +725,58 @@ bool peers_attached()
     for (const Domain &d : C.dom)
         if (!d.nb[0].base || !d.nb[1].base) return false;
     return true;
+}
+
+// GLM variant: the caller's U[8] (cell-centred B in U[4..6]) and psi <-> the padded arrays.  to_device: U
+// in (psi untouched unless given); otherwise out.  Host pointers go through a temporary device buffer.
+int copy_state_glm(double *U, double *psi, bool to_device)
+{
+    const Domain &d = C.dom[0];
+    const Grid &g = d.g;
+    cudaStream_t s = C.stream;
+    const size_t n = api_count(g, g.n[2], -1);
+    Box in = interior(g);
+    const int arr_of[8] = { 0, 1, 2, 3, 5, 6, 7, 4 };          // U component -> state array (E is array 4)
+    Staging st;
+    double *dU = U, *dpsi = psi;
+    const bool uhost = U && !is_device_ptr(U), phost = psi && !is_device_ptr(psi);
+    if (uhost || phost) {
+        if (int rc = st.get(9 * n)) return rc;
+        if (uhost) dU = st.p;
+        if (phost) dpsi = st.p + 8 * n;
+    }
+    if (to_device) {
+        if (uhost) CUDA_TRY(cudaMemcpyAsync(dU, U, 8 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        if (phost) CUDA_TRY(cudaMemcpyAsync(dpsi, psi, n * sizeof(double), cudaMemcpyHostToDevice, s));
+        if (U) for (int v = 0; v < 8; v++)
+            k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dU + (size_t)v * n, g.n[0], g.n[1], 0, arr(d, A_SA + arr_of[v]));
+        if (psi) k_unpack<<<grid_for(in), 128, 0, s>>>(g, in, dpsi, g.n[0], g.n[1], 0, arr(d, glm_psi(A_SA)));
+    } else {
+        if (U) for (int v = 0; v < 8; v++)
+            k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, A_SA + arr_of[v]), g.n[0], g.n[1], 0, -1, dU + (size_t)v * n);
+        if (psi) k_pack<<<grid_for(in), 128, 0, s>>>(g, in, arr(d, glm_psi(A_SA)), g.n[0], g.n[1], 0, -1, dpsi);
+        if (uhost) CUDA_TRY(cudaMemcpyAsync(U, dU, 8 * n * sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (phost) CUDA_TRY(cudaMemcpyAsync(psi, dpsi, n * sizeof(double), cudaMemcpyDeviceToHost, s));
+    }
+    C.launches += (U ? 8 : 0) + (psi ? 1 : 0);
+    CUDA_TRY(cudaStreamSynchronize(s));
+    CUDA_TRY(cudaGetLastError());
+    return PLUTO_OK;
+}
+
+int set_state_glm(const double *U)
+{
+    if (!U) return fail(PLUTO_EINVAL, "null pointer");
+    const Domain &d = C.dom[0];
+    CUDA_TRY(cudaMemsetAsync(arr(d, glm_psi(A_SA)), 0, (size_t)d.g.sa * sizeof(double), C.stream));     // psi = 0
+    if (int rc = copy_state_glm(const_cast<double *>(U), nullptr, true)) return rc;
+    reset_bounds();
+    StepParams p0;
+    memset(&p0, 0, sizeof p0);
+    CUDA_TRY(cudaMemcpyAsync(C.P, &p0, sizeof p0, cudaMemcpyHostToDevice, C.stream));
+    CUDA_TRY(cudaStreamSynchronize(C.stream));
+    C.have_state = true; C.stepped = false;
+    return PLUTO_OK;
 }
 
 } // namespace
@@ -869,6 +961,12 @@ int pluto_set_option(int opt, int value)
         destroy_graphs();
         return old;
     }
+    if (opt == PLUTO_OPT_DIVB) {
+        if (value != PLUTO_DIVB_CT && value != PLUTO_DIVB_GLM) return fail(PLUTO_EINVAL, "divergence control must be PLUTO_DIVB_CT or PLUTO_DIVB_GLM");
+        int old = C.divb;
+        C.divb = value;                          // takes effect at the next pluto_init
+        return old;
+    }
     if (opt == PLUTO_OPT_FUSE_XY) {
         int old = C.fuse_xy;
         C.fuse_xy = value ? 1 : 0;
@@ -881,6 +979,7 @@ int pluto_set_option(int opt, int value)
 int pluto_set_state(const double *U, const double *Bface)
 {
     if (!C.init) return fail(PLUTO_ESTATE, "not initialised");
+    if (C.glm) return set_state_glm(U);
     if (!U || !Bface) return fail(PLUTO_EINVAL, "null pointer");
     const Grid &g0 = C.dom[0].g;
     const int ndim = g0.ndim, nzl = C.nzloc;
@@ -950,6 +1049,7 @@ int pluto_fill_ghosts(void)
 int pluto_get_state(double *U, double *Bface)
 {
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
+    if (C.glm) return copy_state_glm(U, nullptr, false);
     if (!peers_attached()) return fail(PLUTO_ESTATE, "a neighbour slab is not attached (pluto_attach_peer)");
     const Grid &g0 = C.dom[0].g;
     const int ndim = g0.ndim, nzl = C.nzloc;
@@ -1000,6 +1100,20 @@ int pluto_get_state(double *U, double *Bface)
     CUDA_TRY(cudaStreamSynchronize(s));
     CUDA_TRY(cudaGetLastError());
     return PLUTO_OK;
+}
+
+int pluto_set_psi(const double *psi)
+{
+    if (!C.init || !C.have_state || !C.glm) return fail(PLUTO_ESTATE, "needs a state of the GLM variant");
+    if (!psi) return fail(PLUTO_EINVAL, "null pointer");
+    return copy_state_glm(nullptr, const_cast<double *>(psi), true);
+}
+
+int pluto_get_psi(double *psi)
+{
+    if (!C.init || !C.have_state || !C.glm) return fail(PLUTO_ESTATE, "needs a state of the GLM variant");
+    if (!psi) return fail(PLUTO_EINVAL, "null pointer");
+    return copy_state_glm(nullptr, psi, false);
 }
 
 int pluto_step_async(int nsteps)
@@ -1135,7 +1249,7 @@ double pluto_probe_fp64_gflops(void)
 int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem, double *Eedge)
 {
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
-    if (C.dom.size() != 1 || !C.whole()) return fail(PLUTO_ESTATE, "pluto_debug_euler works on a single domain");
+    if (C.dom.size() != 1 || !C.whole() || C.glm) return fail(PLUTO_ESTATE, "pluto_debug_euler works on a single domain of the CT scheme");
     if (!(dt > 0.0)) return fail(PLUTO_EINVAL, "dt must be positive");
     const Domain &d = C.dom[0];
     const Grid &g = d.g;

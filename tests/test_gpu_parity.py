@@ -902,3 +902,96 @@ def test_repeated_runs_give_identical_bits(pluto, name, make, rk, ghost, nslab):
     finally:
         pluto.set_option(OPT_GRAPH, 1)
         pluto.set_integrator(2)
+
+
+# ---------------------------------------------------------------- GLM divergence cleaning (reading R20)
+
+GLM_CASES = [
+    ("2d_ragged_minmod", lambda: wl.random_smooth(37, 23, 1, seed=91, limiter=0, box=(1.0, 0.7, 1.0)), 2),
+    ("2d_wide_mc_rk3", lambda: wl.random_smooth(150, 21, 1, seed=92, limiter=1), 3),
+    ("3d_ragged_mc", lambda: wl.random_smooth(19, 13, 11, seed=93, limiter=1, box=(1.0, 0.8, 1.1)), 2),
+    ("3d_minmod_rk3", lambda: wl.random_smooth(40, 12, 10, seed=94, limiter=0), 3),
+    ("ot_48", lambda: wl.orszag_tang_2d(48), 2),
+    ("blast_24", lambda: wl.blast_3d(24), 2),
+]
+
+
+def _glm_compare(pluto, oracle, tol, norm):
+    Ug = pluto.get_state_glm()
+    Uo, _ = oracle.get_state(faces=False)
+    e_u = norm(Ug.reshape(8, -1), Uo.reshape(8, -1))
+    pg, po = pluto.get_psi(), oracle.get_psi()
+    e_p = norm(pg.reshape(1, -1), po.reshape(1, -1))
+    assert e_u <= tol and e_p <= tol, (e_u, e_p)
+
+
+@pytest.mark.parametrize("name,make,rk", GLM_CASES, ids=[c[0] for c in GLM_CASES])
+def test_glm_parity(pluto, oracle, name, make, rk):
+    """the GLM variant (cell-centred B + psi, [43]) against the oracle's: dt bit-exact, one step max-rel <= 1e-10,
+    20 steps L1-rel <= 1e-8, strict per-component norms, psi included"""
+    w = make()
+    pluto.set_integrator(rk)
+    try:
+        pluto.load_glm(w)
+        oracle.load_glm(w)
+        oracle.set_integrator(rk)
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(1)
+        assert oracle.step(1) == 0
+        assert pluto.get_dt() == oracle.get_dt()
+        _glm_compare(pluto, oracle, TOL_1STEP_MAXREL, maxrel)
+        pluto.step(19)
+        assert oracle.step(19) == 0
+        _glm_compare(pluto, oracle, TOL_100STEP_L1REL, l1rel)
+        assert abs(pluto.get_time() - oracle.get_time()) <= 1e-12
+    finally:
+        pluto.set_integrator(2)
+        oracle.set_integrator(2)
+
+
+def test_glm_conserves_and_cleans(pluto, oracle):
+    """on the GPU itself: mass, momentum, energy and the cell-centred field are conserved; a divergence bump on a
+    uniform magnetised fluid at rest is radiated away and damped (as in the oracle's pin)"""
+    w = wl.random_smooth(32, 20, 12, seed=95, limiter=1)
+    pluto.load_glm(w)
+    pluto.step(30)
+    U = pluto.get_state_glm()
+    for v in range(8):
+        ref = np.abs(w.U[1:4]).sum() if 1 <= v <= 3 else (np.abs(w.U[4:7]).sum() if 4 <= v <= 6 else abs(math.fsum(w.U[v].ravel())))
+        assert abs(math.fsum(U[v].ravel()) - math.fsum(w.U[v].ravel())) <= 1e-12 * ref, v
+    n = 64
+    U0 = np.zeros((8, 1, n, n))
+    X, Y = np.meshgrid((np.arange(n) + 0.5) / n, (np.arange(n) + 0.5) / n)
+    U0[0] = 1.0
+    U0[4, 0] = 0.3 + 1e-3 * np.exp(-((X - 0.5) ** 2 + (Y - 0.5) ** 2) / 0.06 ** 2)
+    U0[5, 0] = 0.2
+    U0[7] = 1.0 / (5.0 / 3.0 - 1.0) + 0.5 * (U0[4] ** 2 + U0[5] ** 2)
+    wb = wl.orszag_tang_2d(n)
+    wb.U, wb.limiter, wb.cfl = U0, 1, 0.4
+
+    def div(V):
+        bx, by = V[4, 0], V[5, 0]
+        return (np.roll(bx, -1, 1) - np.roll(bx, 1, 1)) * n / 2 + (np.roll(by, -1, 0) - np.roll(by, 1, 0)) * n / 2
+
+    pluto.load_glm(wb)
+    pluto.step(100)
+    U1 = pluto.get_state_glm()
+    assert math.sqrt((div(U1) ** 2).mean()) < 0.15 * math.sqrt((div(U0) ** 2).mean())
+    psi = pluto.get_psi()
+    pluto.set_psi(2.0 * psi)
+    assert np.array_equal(pluto.get_psi(), 2.0 * psi)
+
+
+def test_glm_argument_checks(pluto):
+    from paper_2511_20337_b200 import binding
+    pluto.set_divb(binding.DIVB_GLM)
+    try:
+        with pytest.raises(binding.PlutoError):
+            pluto.init(16, 16, 16, 3, 5.0 / 3.0, 0.3, binding.WENOZ)       # PLM only
+        with pytest.raises(binding.PlutoError):
+            pluto.init(16, 16, 16, 2, nslab=2)                             # one domain
+    finally:
+        pluto.set_divb(binding.DIVB_CT)
+    pluto.init(16, 16, 1, 2)
+    with pytest.raises(binding.PlutoError):
+        pluto.get_psi()                                                    # CT context has no psi
