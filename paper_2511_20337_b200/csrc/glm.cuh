@@ -11,9 +11,9 @@
 // flux(B_n) = psi_m, flux(psi) = c_h^2 B_m, and the other seven fluxes are HLLD's with the normal field B_m.
 // c_h = cfl min_d(dx_d) / dt; after a full step psi *= exp(-dt c_h / c_r), c_r = 0.18 ([43]'s recommendation).
 //
-// First version of this path: one thread per zone and direction, both faces of the zone solved by the
-// thread itself (every interface is solved twice; loads are x-contiguous in every direction), one launch per
-// direction, an elementwise combine.  It is correct and measured, not yet fused like the CT path.
+// One launch per direction and an elementwise combine (not fused like the CT path): along x a block works on a
+// row segment in shared memory (k_glm_sweep_x), along y and z a thread marches up its column (k_glm_march);
+// every interface is solved once.
 #pragma once
 #include "kernels.cuh"
 
@@ -21,23 +21,39 @@ namespace pluto {
 
 constexpr double kGlmCr = 0.18;      // c_p^2 / c_h of [43]
 
+// the nine stored values of one zone: rho, m_x, m_y, m_z, E, B_x, B_y, B_z, psi
+__device__ __forceinline__ void glm_load(const Grid &g, const double *__restrict__ S, const double *__restrict__ psi,
+                                         long long c, double u[9])
+{
+#pragma unroll
+    for (int v = 0; v < 8; v++) u[v] = S[v * g.sa + c];
+    u[8] = psi[c];
+}
+
 // rotated primitives of one zone for a sweep along DIR: rho, u, v, w, B_t1, B_t2, p, B_n, psi
 template <int DIR>
-__device__ __forceinline__ void glm_prims(const Grid &g, const double *__restrict__ S, const double *__restrict__ psi,
-                                          long long c, double q[9], bool &bad)
+__device__ __forceinline__ void glm_convert(const Grid &g, const double u[9], double q[9], bool &bad)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
-    const long long sa = g.sa;
-    const double rho = S[c], En = S[4 * sa + c];
-    const double m[3] = { S[sa + c], S[2 * sa + c], S[3 * sa + c] };
-    const double B[3] = { S[5 * sa + c], S[6 * sa + c], S[7 * sa + c] };
+    const double rho = u[0], En = u[4];
+    const double m[3] = { u[1], u[2], u[3] };
+    const double B[3] = { u[5], u[6], u[7] };
     const double ir = rcp_fast(rho);
     const double v[3] = { __dmul_rn(m[0], ir), __dmul_rn(m[1], ir), __dmul_rn(m[2], ir) };
     const double p = __dmul_rn(g.gamma - 1.0, fma(-0.5, fma(B[0], B[0], fma(B[1], B[1], B[2] * B[2])),
                                                   fma(-0.5, fma(m[0], v[0], fma(m[1], v[1], m[2] * v[2])), En)));
     q[0] = rho; q[1] = v[DIR]; q[2] = v[T1]; q[3] = v[T2]; q[4] = B[T1]; q[5] = B[T2]; q[6] = p; q[7] = B[DIR];
-    q[8] = psi[c];
+    q[8] = u[8];
     bad = unphysical(rho) || unphysical(p);
+}
+
+template <int DIR>
+__device__ __forceinline__ void glm_prims(const Grid &g, const double *__restrict__ S, const double *__restrict__ psi,
+                                          long long c, double q[9], bool &bad)
+{
+    double u[9];
+    glm_load(g, S, psi, c, u);
+    glm_convert<DIR>(g, u, q, bad);
 }
 
 // flux of the nine variables through one interface from the reconstructed states (rotated frame):
@@ -56,48 +72,151 @@ __device__ __forceinline__ void glm_face_flux(const double L[9], const double R[
 }
 
 // One direction of one Euler stage: out = (FIRST ? in : out) - dt/dx_DIR (F(+) - F(-)) for the nine variables.
+
+// The x direction: a block takes GLMX_NT consecutive zones of one row (blocks overlap by four zones), every
+// thread converts its zone once, limits its own slopes from its two neighbours' primitives in shared memory,
+// solves the interface on its lower face with its left neighbour's upper-face value, and differences its flux
+// with its right neighbour's: every interface once, three block barriers.
+constexpr int GLMX_NT = 128;
+
+template <int LIM, bool FIRST>
+__global__ void __launch_bounds__(GLMX_NT, 4)
+k_glm_sweep_x(Grid g, const double *__restrict__ Sin, const double *__restrict__ psin, double *Sout, double *psout,
+              StepParams *P)
+{
+    __shared__ double sq[9][GLMX_NT];      // primitives, then the fluxes
+    __shared__ double sh[9][GLMX_NT];      // upper-face values
+    const int t = threadIdx.x, nx = g.n[0];
+    const int i = (int)blockIdx.x * (GLMX_NT - 4) - 2 + t, j = blockIdx.y, k = blockIdx.z;
+    const bool valid = i < nx + 2;
+    const long long sa = g.sa, c = g.at(valid ? i : 0, j, k);
+    const double ch = P->glm_ch, dtdx = P->dtdx[0];
+    double u[9], q[9];
+    bool bad;
+    glm_load(g, Sin, psin, c, u);
+    glm_convert<0>(g, u, q, bad);
+    if (valid && i >= 0 && i < nx && bad) P->err = 1;
+#pragma unroll
+    for (int v = 0; v < 9; v++) sq[v][t] = q[v];
+    __syncthreads();
+    const bool has_nb = valid && t >= 1 && t <= GLMX_NT - 2 && i + 1 < nx + 2;
+    double R[9];
+    if (has_nb) {
+#pragma unroll
+        for (int v = 0; v < 9; v++) {
+            double hi;
+            plm_faces<LIM>(q[v], q[v] - sq[v][t - 1], sq[v][t + 1] - q[v], R[v], hi);
+            sh[v][t] = hi;
+        }
+    }
+    __syncthreads();
+    const bool face = has_nb && t >= 2 && i >= 0;
+    double F[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };
+    if (face) {
+        const double L[9] = { sh[0][t - 1], sh[1][t - 1], sh[2][t - 1], sh[3][t - 1], sh[4][t - 1],
+                              sh[5][t - 1], sh[6][t - 1], sh[7][t - 1], sh[8][t - 1] };
+        glm_face_flux(L, R, ch, g.gamma, g.igm1, F);
+#pragma unroll
+        for (int v = 0; v < 9; v++) sq[v][t] = F[v];
+    }
+    __syncthreads();
+    if (face && i < nx && t <= GLMX_NT - 3) {
+        // rotated flux along x: (rho, m_x, m_y, m_z, B_y, B_z, E, B_x, psi); base = the zone's own stored values
+        double b[9];
+#pragma unroll
+        for (int v = 0; v < 9; v++) b[v] = u[v];
+        if (!FIRST) glm_load(g, Sout, psout, c, b);
+        Sout[c] = fma(-dtdx, sq[0][t + 1] - F[0], b[0]);
+        Sout[sa + c] = fma(-dtdx, sq[1][t + 1] - F[1], b[1]);
+        Sout[2 * sa + c] = fma(-dtdx, sq[2][t + 1] - F[2], b[2]);
+        Sout[3 * sa + c] = fma(-dtdx, sq[3][t + 1] - F[3], b[3]);
+        Sout[4 * sa + c] = fma(-dtdx, sq[6][t + 1] - F[6], b[4]);
+        Sout[5 * sa + c] = fma(-dtdx, sq[7][t + 1] - F[7], b[5]);
+        Sout[6 * sa + c] = fma(-dtdx, sq[4][t + 1] - F[4], b[6]);
+        Sout[7 * sa + c] = fma(-dtdx, sq[5][t + 1] - F[5], b[7]);
+        psout[c] = fma(-dtdx, sq[8][t + 1] - F[8], b[8]);
+    }
+}
+
+// The same update along y or z (DIR = 1, 2) by marching: thread = one column, the running PLM state of the
+// nine primitives in registers, every interface solved once per segment (+1 at the segment end), every zone
+// loaded and converted once -- the scheme of k_sweep_march (kernels.cuh) for the cell-centred variant.
+// DIR = 1: grid.y = segment, grid.z = k;  DIR = 2: grid.y = j, grid.z = segment.
 template <int DIR, int LIM, bool FIRST>
-__global__ void __launch_bounds__(128)
-k_glm_sweep(Grid g, const double *__restrict__ Sin, const double *__restrict__ psin, double *Sout, double *psout,
-            StepParams *P)
+__global__ void __launch_bounds__(128, 2)
+k_glm_march(Grid g, const double *__restrict__ Sin, const double *__restrict__ psin, double *Sout, double *psout,
+            StepParams *P, int seglen)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.n[0]) return;
-    const long long sa = g.sa, st = g.st[DIR], c = g.at(i, j, k);
+    const int seg = DIR == 1 ? blockIdx.y : blockIdx.z;
+    const int tr = DIR == 1 ? blockIdx.z : blockIdx.y;
+    const int s0 = seg * seglen, s1 = min(s0 + seglen, g.n[DIR]);
+    const long long sa = g.sa, st = g.st[DIR];
+    long long c = DIR == 1 ? g.at(i, s0, tr) : g.at(i, tr, s0);
     const double ch = P->glm_ch, dtdx = P->dtdx[DIR];
-    double q[5][9];
-    bool bad, mybad = false;
-#pragma unroll
-    for (int m = 0; m < 5; m++) {
-        glm_prims<DIR>(g, Sin, psin, c + (m - 2) * st, q[m], bad);
-        if (m == 2) mybad = bad;
-    }
-    if (mybad) P->err = 1;
-    // faces of the cells c-1, c, c+1 (Eq. 6; R4): lo on the lower face, hi on the upper face
-    double Ll[9], Rl[9], Lu[9], Ru[9];
-#pragma unroll
-    for (int v = 0; v < 9; v++) {
-        double lo, hi;
-        plm_faces<LIM>(q[1][v], q[1][v] - q[0][v], q[2][v] - q[1][v], lo, Ll[v]);      // cell c-1: its upper face value
-        plm_faces<LIM>(q[2][v], q[2][v] - q[1][v], q[3][v] - q[2][v], Rl[v], Lu[v]);   // cell c
-        plm_faces<LIM>(q[3][v], q[3][v] - q[2][v], q[4][v] - q[3][v], Ru[v], hi);      // cell c+1: its lower face value
-    }
-    double fl[9], fu[9];
-    glm_face_flux(Ll, Rl, ch, g.gamma, g.igm1, fl);
-    glm_face_flux(Lu, Ru, ch, g.gamma, g.igm1, fu);
-    // rotated flux (rho, m_n, m_t1, m_t2, B_t1, B_t2, E, B_n, psi) -> state arrays
     const double *base = FIRST ? Sin : Sout;
     const double *pbase = FIRST ? psin : psout;
-    Sout[c] = fma(-dtdx, fu[0] - fl[0], base[c]);
-    Sout[(1 + DIR) * sa + c] = fma(-dtdx, fu[1] - fl[1], base[(1 + DIR) * sa + c]);
-    Sout[(1 + T1) * sa + c] = fma(-dtdx, fu[2] - fl[2], base[(1 + T1) * sa + c]);
-    Sout[(1 + T2) * sa + c] = fma(-dtdx, fu[3] - fl[3], base[(1 + T2) * sa + c]);
-    Sout[4 * sa + c] = fma(-dtdx, fu[6] - fl[6], base[4 * sa + c]);
-    Sout[(5 + DIR) * sa + c] = fma(-dtdx, fu[7] - fl[7], base[(5 + DIR) * sa + c]);
-    Sout[(5 + T1) * sa + c] = fma(-dtdx, fu[4] - fl[4], base[(5 + T1) * sa + c]);
-    Sout[(5 + T2) * sa + c] = fma(-dtdx, fu[5] - fl[5], base[(5 + T2) * sa + c]);
-    psout[c] = fma(-dtdx, fu[8] - fl[8], pbase[c]);
+    bool bad, anybad = false;
+    double q0[9], d0[9], qL[9];
+    {
+        double qm[9];
+        glm_prims<DIR>(g, Sin, psin, c - 2 * st, qm, bad);
+        glm_prims<DIR>(g, Sin, psin, c - st, q0, bad);
+#pragma unroll
+        for (int v = 0; v < 9; v++) d0[v] = q0[v] - qm[v];
+        glm_prims<DIR>(g, Sin, psin, c, qm, bad);
+        anybad |= bad;
+#pragma unroll
+        for (int v = 0; v < 9; v++) {
+            double d1 = qm[v] - q0[v], lo;
+            plm_faces<LIM>(q0[v], d0[v], d1, lo, qL[v]);
+            q0[v] = qm[v];
+            d0[v] = d1;
+        }
+    }
+    double Fp[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };
+    // software pipeline: the stored values of zone s+1 (and the update base of zone s-1) are loaded one
+    // iteration before they are used, so the march does not stall on memory
+    double un[9], ub[9];
+    glm_load(g, Sin, psin, c + st, un);
+    glm_load(g, base, pbase, c - st, ub);
+    for (int s = s0; s <= s1; s++, c += st) {
+        double q1[9], qR[9], F[9], uc[9], bc[9];
+#pragma unroll
+        for (int v = 0; v < 9; v++) { uc[v] = un[v]; bc[v] = ub[v]; }
+        if (s < s1) {
+            glm_load(g, Sin, psin, c + 2 * st, un);
+            glm_load(g, base, pbase, c, ub);
+        }
+        glm_convert<DIR>(g, uc, q1, bad);
+        if (s + 1 < s1) anybad |= bad;
+        const double L9[9] = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6], qL[7], qL[8] };
+#pragma unroll
+        for (int v = 0; v < 9; v++) {
+            double d1 = q1[v] - q0[v];
+            plm_faces<LIM>(q0[v], d0[v], d1, qR[v], qL[v]);
+            q0[v] = q1[v];
+            d0[v] = d1;
+        }
+        glm_face_flux(L9, qR, ch, g.gamma, g.igm1, F);
+        if (s > s0) {
+            const long long cm = c - st;
+            Sout[cm] = fma(-dtdx, F[0] - Fp[0], bc[0]);
+            Sout[(1 + DIR) * sa + cm] = fma(-dtdx, F[1] - Fp[1], bc[1 + DIR]);
+            Sout[(1 + T1) * sa + cm] = fma(-dtdx, F[2] - Fp[2], bc[1 + T1]);
+            Sout[(1 + T2) * sa + cm] = fma(-dtdx, F[3] - Fp[3], bc[1 + T2]);
+            Sout[4 * sa + cm] = fma(-dtdx, F[6] - Fp[6], bc[4]);
+            Sout[(5 + DIR) * sa + cm] = fma(-dtdx, F[7] - Fp[7], bc[5 + DIR]);
+            Sout[(5 + T1) * sa + cm] = fma(-dtdx, F[4] - Fp[4], bc[5 + T1]);
+            Sout[(5 + T2) * sa + cm] = fma(-dtdx, F[5] - Fp[5], bc[5 + T2]);
+            psout[cm] = fma(-dtdx, F[8] - Fp[8], bc[8]);
+        }
+#pragma unroll
+        for (int v = 0; v < 9; v++) Fp[v] = F[v];
+    }
+    if (anybad) P->err = 1;
 }
 
 // Runge-Kutta combine of the nine arrays (a7), out <- wn * S^n + ws * S~ with S~ = Euler(S) in scratch arrays

@@ -422,9 +422,18 @@ void enqueue_stage_glm(int in, int out, int sn, double wn, double ws, bool last)
     // a combine stage computes Euler(S) into scratch arrays first (out may be S^n itself)
     double *So = arr(d, sn >= 0 ? GLM_TMP : out), *po = arr(d, sn >= 0 ? GLM_TMP_PSI : glm_psi(out));
     const dim3 grid((g.n[0] + 127) / 128, g.n[1], g.n[2]);
-    LAUNCH(K_FLUX_X, k_glm_sweep<0, LIM, true><<<grid, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
-    LAUNCH(K_FLUX_Y, k_glm_sweep<1, LIM, false><<<grid, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
-    if (g.act[2]) LAUNCH(K_FLUX_Z, k_glm_sweep<2, LIM, false><<<grid, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
+    const dim3 gx((g.n[0] + GLMX_NT - 5) / (GLMX_NT - 4), g.n[1], g.n[2]);
+    LAUNCH(K_FLUX_X, k_glm_sweep_x<LIM, true><<<gx, GLMX_NT, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
+    {
+        const int len = seglen_y(g);
+        const dim3 gy((g.n[0] + 127) / 128, (g.n[1] + len - 1) / len, g.n[2]);
+        LAUNCH(K_FLUX_Y, k_glm_march<1, LIM, false><<<gy, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len));
+    }
+    if (g.act[2]) {
+        const int len = seglen_z(g);
+        const dim3 gz((g.n[0] + 127) / 128, g.n[1], (g.n[2] + len - 1) / len);
+        LAUNCH(K_FLUX_Z, k_glm_march<2, LIM, false><<<gz, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len));
+    }
     if (sn >= 0)
         LAUNCH(K_SCALAR, k_glm_combine<<<grid, 128, 0, s>>>(g, arr(d, out), arr(d, glm_psi(out)), arr(d, sn), arr(d, glm_psi(sn)),
                                                           So, po, wn, ws, last ? 1 : 0, C.P));
