@@ -995,3 +995,27 @@ def test_glm_argument_checks(pluto):
     pluto.init(16, 16, 1, 2)
     with pytest.raises(binding.PlutoError):
         pluto.get_psi()                                                    # CT context has no psi
+
+
+@pytest.mark.parametrize("rk", [2, 3])
+def test_glm_poisoned_workspace_and_repeatability(pluto, rk):
+    """the memory-safety checks of the CT path, for the GLM kernels: NaN-poisoned workspace, repeated runs"""
+    from paper_2511_20337_b200 import binding
+    w = wl.random_smooth(40, 13, 9, seed=96, limiter=1)
+    pluto.set_integrator(rk)
+    try:
+        pluto.load_glm(w)
+        pluto.step(4)
+        ref, ref_psi = pluto.get_state_glm(), pluto.get_psi()
+        for rep in range(3):
+            pluto.set_divb(binding.DIVB_GLM)
+            pluto.init(w.nx, w.ny, w.nz, 2, w.gamma, w.cfl, w.limiter)
+            pluto.set_divb(binding.DIVB_CT)
+            pluto.workspace.fill_(0xFF)
+            pluto.torch.cuda.synchronize()
+            pluto.set_box(*w.box)
+            pluto._check(pluto.L.pluto_set_state(w.U.ctypes.data, None))
+            pluto.step(4)
+            assert np.array_equal(pluto.get_state_glm(), ref) and np.array_equal(pluto.get_psi(), ref_psi)
+    finally:
+        pluto.set_integrator(2)
