@@ -455,9 +455,9 @@ def main_slabs(args, rank, world, local):
     from paper_2511_20337_b200.distributed import SlabPluto
 
     dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.config not in (3, 4):
+        raise SystemExit("--gpus N > 1 times the weak-scaling blast: per-GPU mesh and scheme of configs[3] (default) or configs[4]")
     base = wl.config(args.config)                    # scheme parameters and the per-GPU mesh
-    if base.nz < 2:
-        raise SystemExit("the z-slab decomposition needs a 3D config")
     nx, ny, nzl = base.nx, base.ny, base.nz
     nz = nzl * world
     sim = SlabPluto(dist, device=local)
