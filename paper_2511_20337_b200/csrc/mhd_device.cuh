@@ -21,11 +21,12 @@ constexpr double kDegen = 1e-8;   // R5: guard of the star-state denominator
 
 // ---------------------------------------------------------------- fp64 reciprocal / square root
 // IEEE division and sqrt cost ~9 fp64-pipe instructions each plus range checks and a slow-path call;
-// HLLD needs 9 reciprocals and 6 square roots per interface, about half of its arithmetic.  These
+// HLLD needs 9 reciprocals and 5 square roots per interface, about a third of its arithmetic.  These
 // versions start from the hardware seed (MUFU.RCP64H / MUFU.RSQ64H, relative error <= 2^-22) and
-// refine it with a third-order / two second-order steps: results are within ~1 ulp of the IEEE
-// value for normal, finite, positive-range arguments, which is all this path produces (the error
-// flag catches non-positive density / pressure).  No denormal, zero or infinity handling.
+// refine it with a third-order step / a second-order step plus a residual correction: results are
+// within ~1 ulp of the IEEE value for normal, finite, positive-range arguments, which is all this path
+// produces (the error flag catches non-positive density / pressure).  No denormal, zero or infinity
+// handling.
 __device__ __forceinline__ double rcp_fast(double x)
 {
     double y;
@@ -35,17 +36,24 @@ __device__ __forceinline__ double rcp_fast(double x)
     return fma(y, e, y);                 // y (1 + e + e^2): error ~ e^3
 }
 
-// sqrt(x), x > 0: two coupled Newton steps on (g, h) -> (sqrt x, 1 / (2 sqrt x))
+// sqrt(x), x > 0: one coupled Newton step on (g, h) -> (sqrt x, 1 / (2 sqrt x)) takes the seed's relative
+// error d to g (1 - 3/2 d^2); the exact residual x - g^2 (one fma) times the unrefined h then cancels
+// the d^2 term: g (1 + 3/2 d^3), below half an ulp before the final rounding.  Six fp64-pipe instructions.
 __device__ __forceinline__ double sqrt_fast(double x)
 {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     double g = x * y, h = 0.5 * y;
-    double e = fma(-g, h, 0.5);
-    g = fma(g, e, g); h = fma(h, e, h);
-    e = fma(-g, h, 0.5);
-    return fma(g, e, g);
+    const double e = fma(-g, h, 0.5);
+    g = fma(g, e, g);
+    return fma(fma(-g, g, x), h, g);
 }
+
+// max / min of two numbers by one comparison and a select.  fmax() / fmin() also quiet NaNs (seven
+// instructions for the IEEE rule); no NaN reaches these on a physical state, and an unphysical one is
+// reported by the sweeps' own check.  A NaN in `a` returns b.
+__device__ __forceinline__ double max_sel(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double min_sel(double a, double b) { return a < b ? a : b; }
 
 // Limited slope (R4).  The sign test dm * dp > 0 is taken on the sign bits (integer pipe) instead
 // of a DMUL + DSETP: identical unless dm * dp underflows, where the slope is < 1e-154 anyway.
@@ -58,7 +66,7 @@ __device__ __forceinline__ double plm_slope(double dm, double dp)
         return same ? s : 0.0;
     } else {
         double sum = dm + dp;
-        double mag = fmin(2.0 * fmin(fabs(dm), fabs(dp)), 0.5 * fabs(sum));
+        double mag = min_sel(2.0 * min_sel(fabs(dm), fabs(dp)), 0.5 * fabs(sum));
         return same ? copysign(mag, dm) : 0.0;        // same sign: sign(dm + dp) = sign(dm)
     }
 }
@@ -76,7 +84,7 @@ __device__ __forceinline__ void plm_faces(double q, double dm, double dp, double
         s = fabs(dm) < fabs(dp) ? dm : dp;
     } else {
         double sum = dm + dp;
-        s = copysign(fmin(2.0 * fmin(fabs(dm), fabs(dp)), 0.5 * fabs(sum)), dm);
+        s = copysign(min_sel(2.0 * min_sel(fabs(dm), fabs(dp)), 0.5 * fabs(sum)), dm);
     }
     lo = fma(-h, s, q);
     hi = fma(h, s, q);
@@ -134,14 +142,16 @@ __device__ __forceinline__ bool unphysical(double x)
     return (unsigned)(__double2hiint(x) - 0x00100000) >= 0x7fe00000u;
 }
 
-// square of the fast magnetosonic speed from gp = gamma * p, B-normal^2 and |B|^2
+// square of the fast magnetosonic speed from gp = gamma * p, B-normal^2 and |B|^2:
+// c_f^2 = s/2 + sqrt((s/2)^2 - a^2 b_n^2 / rho),  s = a^2 + B^2 / rho  (the halved form of
+// (s + sqrt(s^2 - 4 a^2 b_n^2/rho)) / 2: scaling by two is exact, so the roundings are the same)
 __device__ __forceinline__ double fast_speed2(double rho, double gp, double bn2, double b2)
 {
-    double ir  = rcp_fast(rho);
-    double a2  = gp * ir;
-    double s   = fma(b2, ir, a2);
-    double disc = fma(s, s, -4.0 * a2 * (bn2 * ir));
-    return 0.5 * (s + sqrt_fast(fmax(disc, 1e-300)));   // max(0, disc) of R5 up to 1e-150
+    const double ir = rcp_fast(rho);
+    const double a2 = gp * ir;
+    const double h  = 0.5 * fma(b2, ir, a2);
+    const double disc = fma(h, h, -(a2 * (bn2 * ir)));
+    return h + sqrt_fast(max_sel(disc, 1e-300));        // max(0, disc) of R5 up to 1e-150
 }
 
 // One side of the Riemann fan in the rotated frame.
@@ -164,9 +174,9 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     const double B2L = Bx2 + fma(L.By, L.By, L.Bz * L.Bz), B2R = Bx2 + fma(R.By, R.By, R.Bz * R.Bz);
     const double pTL = fma(0.5, B2L, L.p), pTR = fma(0.5, B2R, R.p);
 
-    const double cmax = sqrt_fast(fmax(fast_speed2(L.rho, gamma * L.p, Bx2, B2L),
-                                       fast_speed2(R.rho, gamma * R.p, Bx2, B2R)));
-    const double SL = fmin(L.u, R.u) - cmax, SR = fmax(L.u, R.u) + cmax;
+    const double cmax = sqrt_fast(max_sel(fast_speed2(L.rho, gamma * L.p, Bx2, B2L),
+                                          fast_speed2(R.rho, gamma * R.p, Bx2, B2R)));
+    const double SL = min_sel(L.u, R.u) - cmax, SR = max_sel(L.u, R.u) + cmax;
     const double dL = SL - L.u, dR = SR - R.u;              // S_a - u_a
     const double aL = __dmul_rn(L.rho, dL), aR = __dmul_rn(R.rho, dR);
     const double idenom = rcp_fast(aR - aL);
@@ -252,7 +262,7 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
 
     // R6: w = clamp(1/2 + F[rho] / (2 theta f_ref)), f_ref = (rho_L + rho_R)(S_R - S_L) / 4
     const double wv = fma(F0, rcp_fast((0.5 * kTheta) * ((L.rho + R.rho) * (SR - SL))), 0.5);
-    wgt = fmin(fmax(wv, 0.0), 1.0);
+    wgt = min_sel(max_sel(wv, 0.0), 1.0);
 }
 
 } // namespace pluto
