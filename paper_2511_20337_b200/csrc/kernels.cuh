@@ -249,7 +249,7 @@ __device__ __forceinline__ void bound_publish(const BoundGrid &bg, int j, int k,
 // shared memory, limits its own slopes from its two list neighbours, solves the Riemann problem on
 // its lower face with its left neighbour's q^L, and differences its flux with its right neighbour's.
 // Consecutive blocks overlap by 4 items, so no flux is computed twice inside a block and rows of any
-// length pack without a ragged tail.
+// length pack without a ragged tail.  The halo cells of a row are its own periodic images.
 constexpr int SX_NT = 128;
 // halo cells on each side of a block's output range: 2 for PLM, 3 for the five-cell WENO-Z stencil
 __host__ __device__ constexpr int sx_halo(int lim) { return lim == 2 ? 3 : 2; }
@@ -280,7 +280,9 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
         long long row = item / M;
         f = (int)(item - row * M) - H;
         int j = (int)(row % g.n[1]), k = (int)(row / g.n[1]) + kz0;
-        c = g.at(f, j, k);
+        // halo cells are read from their periodic image (x-face nx is kept equal to face 0 by the CT kernel):
+        // no kernel of this path reads an x ghost of the state
+        c = g.at(((f % nx) + nx) % nx, j, k);
         rho = Sin[c]; mx = Sin[sa + c]; my = Sin[2 * sa + c]; mz = Sin[3 * sa + c];
         En = Sin[4 * sa + c];
         bxf = Sin[S_B * sa + c];

@@ -238,7 +238,10 @@ void fill_ghosts(const Domain &d, int state, bool all = false)
 {
     const Grid &g = d.g;
     const ZSrc zs = zsrc(d, state);
-    if (!all && C.fuse_xy && g.limiter != 2 && row_wraps(g.n[0])) {
+    // only the chunked form of the fused x+y sweep reads x ghosts (k_sweep_x reads periodic images, the row-wide
+    // x+y sweep wraps inside shared memory, the marching kernels stay inside the row)
+    const bool chunked_xy = C.fuse_xy && g.limiter != 2 && !row_wraps(g.n[0]);
+    if (!all && !chunked_xy) {
         const int ngh = 2 * g.ng + 1;
         const int rows = (g.act[2] ? ngh * (g.n[1] + ngh) : 0) + g.n[2] * ngh;
         LAUNCH(K_GHOST, k_ghost_yz<<<dim3(rows, S_COUNT), 128, 0, C.stream>>>(g, arr(d, state), zs));
