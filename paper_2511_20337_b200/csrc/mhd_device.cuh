@@ -49,11 +49,22 @@ __device__ __forceinline__ double sqrt_fast(double x)
     return fma(fma(-g, g, x), h, g);
 }
 
-// max / min of two numbers by one comparison and a select.  fmax() / fmin() also quiet NaNs (seven
-// instructions for the IEEE rule); no NaN reaches these on a physical state, and an unphysical one is
-// reported by the sweeps' own check.  A NaN in `a` returns b.
-__device__ __forceinline__ double max_sel(double a, double b) { return a > b ? a : b; }
-__device__ __forceinline__ double min_sel(double a, double b) { return a < b ? a : b; }
+// max / min of two numbers by one comparison and a select (three instructions).  fmax() / fmin() also
+// quiet NaNs, seven instructions for the IEEE rule, and the compiler turns a > b ? a : b back into them when
+// b is a constant: hence PTX.  No NaN reaches these on a physical state, and an unphysical one is reported
+// by the sweeps' own check.  A NaN in `a` returns b.
+__device__ __forceinline__ double max_sel(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.gt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
+__device__ __forceinline__ double min_sel(double a, double b)
+{
+    double r;
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f64 p, %1, %2;\n\tselp.f64 %0, %1, %2, p;\n\t}" : "=d"(r) : "d"(a), "d"(b));
+    return r;
+}
 
 // Limited slope (R4).  The sign test dm * dp > 0 is taken on the sign bits (integer pipe) instead
 // of a DMUL + DSETP: identical unless dm * dp underflows, where the slope is < 1e-154 anyway.
