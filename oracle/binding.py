@@ -62,6 +62,8 @@ class Oracle:
         L.oracle_hlld.argtypes = [_dp, _dp, C.c_double, C.c_double, _dp, _dp, _dp]
         L.oracle_debug_euler.argtypes = [C.c_double, _dp, _dp, _dp, _dp, _dp]
         L.oracle_set_divb.argtypes = [C.c_int]
+        L.oracle_set_emf.argtypes = [C.c_int]
+        L.oracle_hlld_uct.argtypes = [_dp, _dp, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
         L.oracle_set_psi.argtypes = [_dp]
         L.oracle_get_psi.argtypes = [_dp]
         L.oracle_glm_interface.argtypes = [C.c_double] * 5 + [_dp, _dp]
@@ -124,6 +126,10 @@ class Oracle:
 
     def finalize(self):
         return self.L.oracle_finalize()
+
+    # ---- EMF average of the CT step: 0 = contact-mode upwinding with the continuous weight (R6), 1 = UCT-HLLD (R19)
+    def set_emf(self, mode):
+        return self.L.oracle_set_emf(mode)
 
     # ---- GLM divergence cleaning (R20)
     def set_divb(self, mode):
@@ -198,6 +204,18 @@ class Oracle:
         rc = self.L.oracle_hlld(_ptr(VL), _ptr(VR), Bn, gamma, _ptr(F), C.byref(w), _ptr(dbg))
         assert rc == 0
         return (F, w.value, dbg) if debug else (F, w.value)
+
+    def hlld_uct(self, VL, VR, Bn, gamma):
+        """flux, and uct = (a^L, d^L, d^R, vbar_t1, vbar_t2) of the UCT-HLLD average (R19)"""
+        VL = np.ascontiguousarray(VL, dtype=np.float64)
+        VR = np.ascontiguousarray(VR, dtype=np.float64)
+        F = np.empty(8)
+        uct = np.empty(5)
+        w = C.c_double(0.0)
+        dbg = np.zeros(72)
+        rc = self.L.oracle_hlld_uct(_ptr(VL), _ptr(VR), Bn, gamma, _ptr(F), C.byref(w), _ptr(dbg), _ptr(uct))
+        assert rc == 0
+        return F, uct, dbg
 
     def debug_euler(self, dt, want=("U1", "Bf1", "F", "W", "E")):
         nx, ny, nz = self.shape

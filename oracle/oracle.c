@@ -42,6 +42,10 @@ typedef struct {
     double *U1, *U2, *b1[3], *b2[3];
     /* work */
     double *V, *F, *W, *Eg, *Ec;
+    /* EMF average: 0 = upwind by the contact mode with the continuous weight (R6, default),
+       1 = UCT-HLLD (R19); its face data [3][5][N]: a^L, d^L, d^R, transverse velocities t1, t2 */
+    int emf;
+    double *Uct;
     double time, dt_last;
     int stepped;
     int rk_order;          /* 2 (or 0: default) = SSP-RK2, 3 = SSP-RK3 */
@@ -182,6 +186,30 @@ void oracle_physical_flux(const double V[7], double Bn, double gamma, double F[8
 int oracle_hlld(const double VL[7], const double VR[7], double Bn, double gamma,
                 double F[8], double *wout, double *dbg)
 {
+    return oracle_hlld_uct(VL, VR, Bn, gamma, F, wout, dbg, NULL);
+}
+
+/* The same solver, also returning (uct != NULL) what the UCT-HLLD EMF average of [47] (named at PAPER.md:271,
+   reference entry :640; reading R19) takes from every interface.  For fixed wave speeds the HLLD flux of a
+   transverse field component B_t is LINEAR in (v_t^L, v_t^R, B_t^L, B_t^R); writing it as
+
+       F[B_t] = a^L (u B_t)^L + a^R (u B_t)^R - (d^R B_t^R - d^L B_t^L) - B_n (a^L v_t^L + a^R v_t^R)
+
+   fixes the four coefficients uniquely (a^L + a^R = 1).  With lambda^L = S_L, lambda^R = S_R, the Alfven speeds
+   lambda^*L = S*_L, lambda^*R = S*_R and lambda_c = S_M:
+
+       chi^s = (u^s - lambda_c)(lambda^s - lambda_c) / (lambda^*s + lambda^s - 2 lambda_c)
+       nu^s  = (lambda^*s + lambda^s) / (|lambda^*s| + |lambda^s|)
+       nu^*  = (lambda^*R + lambda^*L) / (|lambda^*R| + |lambda^*L|)      (0 when both Alfven speeds vanish)
+       a^L = (1 + nu^*)/2,  a^R = (1 - nu^*)/2
+       d^s = (nu^s - nu^*) chi^s / 2 + (|lambda^*s| - nu^* lambda^*s) / 2
+
+   (one-sided fans: a = 1 on the upwind side, d^L = d^R = 0).  tests/test_oracle_uct.py checks the identity above
+   against the flux this routine returns, region by region.
+   uct[5] = a^L, d^L, d^R, a^L v^L + a^R v^R (first transverse velocity), a^L w^L + a^R w^R (second). */
+int oracle_hlld_uct(const double VL[7], const double VR[7], double Bn, double gamma,
+                    double F[8], double *wout, double *dbg, double *uct)
+{
     const double *Va[2] = { VL, VR };
     double U[2][8], Fp[2][8], pT[2], vB[2], cf[2], S[2];
     double Us[2][8], Uss[2][8], vBs[2], Sa[2];
@@ -215,9 +243,11 @@ int oracle_hlld(const double VL[7], const double VR[7], double Bn, double gamma,
     if (S[0] >= 0.0) {
         for (v = 0; v < 8; v++) F[v] = Fp[0][v];
         region = 0;
+        if (uct) { uct[0] = 1.0; uct[1] = 0.0; uct[2] = 0.0; uct[3] = VL[2]; uct[4] = VL[3]; }
     } else if (S[1] <= 0.0) {
         for (v = 0; v < 8; v++) F[v] = Fp[1][v];
         region = 5;
+        if (uct) { uct[0] = 0.0; uct[1] = 0.0; uct[2] = 0.0; uct[3] = VR[2]; uct[4] = VR[3]; }
     } else {
         double aL = VL[0] * (S[0] - VL[1]);
         double aR = VR[0] * (S[1] - VR[1]);
@@ -285,6 +315,21 @@ int oracle_hlld(const double VL[7], const double VR[7], double Bn, double gamma,
             region = 4;
         }
         F[4] = 0.0;   /* the normal-field component carries no flux */
+        if (uct) {   /* R19 */
+            double chi[2], nu[2], nus, den, al, ar;
+            for (a = 0; a < 2; a++) {
+                chi[a] = (Va[a][1] - SM) * (S[a] - SM) / (Sa[a] + S[a] - 2.0 * SM);
+                nu[a]  = (Sa[a] + S[a]) / (fabs(Sa[a]) + fabs(S[a]));
+            }
+            den = fabs(Sa[1]) + fabs(Sa[0]);
+            nus = den > 0.0 ? (Sa[1] + Sa[0]) / den : 0.0;
+            al = 0.5 * (1.0 + nus); ar = 0.5 * (1.0 - nus);
+            uct[0] = al;
+            uct[1] = 0.5 * (nu[0] - nus) * chi[0] + 0.5 * (fabs(Sa[0]) - nus * Sa[0]);
+            uct[2] = 0.5 * (nu[1] - nus) * chi[1] + 0.5 * (fabs(Sa[1]) - nus * Sa[1]);
+            uct[3] = al * VL[2] + ar * VR[2];
+            uct[4] = al * VL[3] + ar * VR[3];
+        }
         if (dbg) {
             dbg[2] = SM; dbg[3] = pTs; dbg[4] = Sa[0]; dbg[5] = Sa[1];
             for (v = 0; v < 8; v++) {
@@ -310,7 +355,7 @@ static void free_all(void)
     int d;
     free(g.U); free(g.U1); free(g.U2);
     for (d = 0; d < 3; d++) { free(g.b[d]); free(g.b1[d]); free(g.b2[d]); }
-    free(g.V); free(g.F); free(g.W); free(g.Eg); free(g.Ec);
+    free(g.V); free(g.F); free(g.W); free(g.Eg); free(g.Ec); free(g.Uct);
     free(g.psi); free(g.psi1); free(g.psi2); free(g.Fpsi);
     memset(&g, 0, sizeof g);
 }
@@ -350,9 +395,10 @@ int oracle_init(int nx, int ny, int nz, int ghost, double gamma, double cfl, int
     g.W  = calloc(3 * N, sizeof(double));
     g.Eg = calloc(3 * N, sizeof(double));
     g.Ec = calloc(3 * N, sizeof(double));
+    g.Uct = calloc(15 * N, sizeof(double));
     g.psi = calloc(N, sizeof(double)); g.psi1 = calloc(N, sizeof(double)); g.psi2 = calloc(N, sizeof(double));
     g.Fpsi = calloc(3 * N, sizeof(double));
-    if (!g.U || !g.U1 || !g.U2 || !g.V || !g.F || !g.W || !g.Eg || !g.Ec) { free_all(); return ORACLE_ENOMEM; }
+    if (!g.U || !g.U1 || !g.U2 || !g.V || !g.F || !g.W || !g.Eg || !g.Ec || !g.Uct) { free_all(); return ORACLE_ENOMEM; }
     if (!g.psi || !g.psi1 || !g.psi2 || !g.Fpsi) { free_all(); return ORACLE_ENOMEM; }
     for (d = 0; d < 3; d++) if (!g.b[d] || !g.b1[d] || !g.b2[d]) { free_all(); return ORACLE_ENOMEM; }
     g.init = 1;
@@ -499,6 +545,78 @@ static double cfl_dt(const double *U)
     return g.cfl / smax;
 }
 
+/* values at the edge between positions m1 and p0 of a quantity Q on a line of positions (m3, m2, m1 | p0, p1, p2):
+   from below (the upper-face value of m1) and from above (the lower-face value of p0), with the reconstruction
+   of the run: PLM (R4) or WENO-Z (R18) */
+static void edge_values(const double *Q, size_t m3, size_t m2, size_t m1, size_t p0, size_t p1, size_t p2,
+                        double *below, double *above)
+{
+    if (g.limiter == 2) {
+        double sl[5] = { Q[m3], Q[m2], Q[m1], Q[p0], Q[p1] };
+        double sr[5] = { Q[p2], Q[p1], Q[p0], Q[m1], Q[m2] };
+        *below = oracle_wenoz(sl);
+        *above = oracle_wenoz(sr);
+    } else {
+        *below = Q[m1] + 0.5 * oracle_plm_slope(Q[m1] - Q[m2], Q[p0] - Q[m1], g.limiter);
+        *above = Q[p0] - 0.5 * oracle_plm_slope(Q[p0] - Q[m1], Q[p1] - Q[p0], g.limiter);
+    }
+}
+
+/* UCT-HLLD edge EMF (reading R19; [47] named at PAPER.md:271, reference entry :640).  Component e at the edge
+   (a-1/2, b-1/2) of cell c, (e,a,b) cyclic, E_e = v_b B_a - v_a B_b.  In the notation of the general upwind
+   constrained-transport composition (W/E = below/above the edge along a, S/N = below/above it along b):
+
+       E_e = -[ a_a^W (vbar_a B_b)^W + a_a^E (vbar_a B_b)^E ] + [ a_b^S (vbar_b B_a)^S + a_b^N (vbar_b B_a)^N ]
+             + (d_a^E B_b^E - d_a^W B_b^W) - (d_b^N B_a^N - d_b^S B_a^S)
+
+   - B_b^{W,E}: the staggered field b_b on the two b-faces that meet at the edge, reconstructed along a up to the
+     edge from below (W) and from above (E); vbar_a^{W,E}: the transverse velocity a^L v_a^L + a^R v_a^R of the
+     Riemann problems on those same b-faces, reconstructed the same way.  Likewise B_a, vbar_b on the two a-faces
+     along b.  Reconstruction: the operator of the run (PLM with its limiter, or WENO-Z), as for the cell
+     states -- with any other operator a grid-aligned run would not reproduce the 1D solution.
+   - a_a^{W,E}, d_a^{W,E}: the coefficients a^L, a^R, d^L, d^R of the two a-interfaces that meet at the edge,
+     arithmetic mean of the two; likewise for b.
+   For data that does not vary along b this is the 1D formula of oracle_hlld_uct, i.e. -F_a[B_b] of HLLD. */
+static void uct_edge_emf(int e, double *const bin[3])
+{
+    const size_t N = g.N;
+    const int a = (e + 1) % 3, b = (e + 2) % 3;
+    /* face data of direction d: [d][0] a^L, [1] d^L, [2] d^R, [3] vbar_t1, [4] vbar_t2 with (t1,t2) = (d+1,d+2):
+       on a-faces vbar_b is t1 of a; on b-faces vbar_a is t2 of b */
+    const double *aLa = g.Uct + ((size_t)a * 5 + 0) * N, *dLa = g.Uct + ((size_t)a * 5 + 1) * N, *dRa = g.Uct + ((size_t)a * 5 + 2) * N;
+    const double *aLb = g.Uct + ((size_t)b * 5 + 0) * N, *dLb = g.Uct + ((size_t)b * 5 + 1) * N, *dRb = g.Uct + ((size_t)b * 5 + 2) * N;
+    const double *vb_on_a = g.Uct + ((size_t)a * 5 + 3) * N;
+    const double *va_on_b = g.Uct + ((size_t)b * 5 + 4) * N;
+    const double *Ba = bin[a], *Bb = bin[b];
+    double *Ee = g.Eg + (size_t)e * N;
+    long c;
+#pragma omp parallel for
+    for (c = 0; c < (long)N; c++) {
+        int i, j, k;
+        size_t c11, c01, c10, am2, ap1, bm2, bp1, am3, ap2, bm3, bp2;
+        double aW, aE, dW, dE, aS, aN, dS, dN;
+        double BbW, BbE, vaW, vaE, BaS, BaN, vbS, vbN;
+        c2ijk((size_t)c, &i, &j, &k);
+        c11 = (size_t)c;
+        c01 = shift(i, j, k, a, -1); am2 = shift(i, j, k, a, -2); ap1 = shift(i, j, k, a, +1);
+        c10 = shift(i, j, k, b, -1); bm2 = shift(i, j, k, b, -2); bp1 = shift(i, j, k, b, +1);
+        am3 = shift(i, j, k, a, -3); ap2 = shift(i, j, k, a, +2);
+        bm3 = shift(i, j, k, b, -3); bp2 = shift(i, j, k, b, +2);
+        /* a-interfaces below (c10) and above (c11) the edge along b; b-interfaces below (c01) / above (c11) along a */
+        aW = 0.5 * (aLa[c10] + aLa[c11]); aE = 0.5 * ((1.0 - aLa[c10]) + (1.0 - aLa[c11]));
+        dW = 0.5 * (dLa[c10] + dLa[c11]); dE = 0.5 * (dRa[c10] + dRa[c11]);
+        aS = 0.5 * (aLb[c01] + aLb[c11]); aN = 0.5 * ((1.0 - aLb[c01]) + (1.0 - aLb[c11]));
+        dS = 0.5 * (dLb[c01] + dLb[c11]); dN = 0.5 * (dRb[c01] + dRb[c11]);
+        /* b-face quantities along a (cells am3, am2, c01 | edge | c11, ap1, ap2), a-face quantities along b */
+        edge_values(Bb, am3, am2, c01, c11, ap1, ap2, &BbW, &BbE);
+        edge_values(va_on_b, am3, am2, c01, c11, ap1, ap2, &vaW, &vaE);
+        edge_values(Ba, bm3, bm2, c10, c11, bp1, bp2, &BaS, &BaN);
+        edge_values(vb_on_a, bm3, bm2, c10, c11, bp1, bp2, &vbS, &vbN);
+        Ee[c] = -(aW * vaW * BbW + aE * vaE * BbE) + (aS * vbS * BaS + aN * vbN * BaN)
+                + (dE * BbE - dW * BbW) - (dN * BaN - dS * BaS);
+    }
+}
+
 /* Euler(S, dt): (Uin, bin) -> (Uout, bout); fills g.V, g.F, g.W, g.Eg, g.Ec */
 static void euler(const double *Uin, double *const bin[3], double dt, double *Uout, double *const bout[3])
 {
@@ -545,6 +663,11 @@ static void euler(const double *Uin, double *const bin[3], double dt, double *Uo
                 VR[q] = Q[c0] - 0.5 * s0;      /* q^R at c-1/2 */
             }
             /* interface c-1/2: normal field is the face value on both sides (R7) */
+            if (g.emf == 1) {
+                double uct[5]; int m;
+                oracle_hlld_uct(VL, VR, bin[d][c0], g.gamma, Fr, &w, NULL, uct);
+                for (m = 0; m < 5; m++) g.Uct[((size_t)d * 5 + m) * N + c0] = uct[m];
+            } else
             oracle_hlld(VL, VR, bin[d][c0], g.gamma, Fr, &w, NULL);
             /* rotate back to lab components */
             Fd[0 * N + c0] = Fr[0];
@@ -592,6 +715,7 @@ static void euler(const double *Uin, double *const bin[3], double dt, double *Uo
         const double *Ec = g.Ec + (size_t)e * N;
         double *Ee = g.Eg + (size_t)e * N;
         if (!(g.act[a] && g.act[b])) continue;
+        if (g.emf == 1) { uct_edge_emf(e, bin); continue; }
 #pragma omp parallel for
         for (c = 0; c < (long)N; c++) {
             int i, j, k, q[3];
@@ -765,6 +889,14 @@ static void one_step_glm(double dt)
     g.time += dt;
     g.dt_last = dt;
     g.stepped = 1;
+}
+
+int oracle_set_emf(int mode)
+{
+    if (!g.init) return ORACLE_ESTATE;
+    if (mode != 0 && mode != 1) return ORACLE_EINVAL;
+    g.emf = mode;
+    return ORACLE_OK;
 }
 
 int oracle_set_divb(int mode)

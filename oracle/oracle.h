@@ -75,6 +75,14 @@ void   oracle_physical_flux(const double V[7], double Bn, double gamma, double F
 int    oracle_hlld(const double VL[7], const double VR[7], double Bn, double gamma,
                    double F[8], double *w, double *dbg);
 
+/* the same, also returning uct[5] = a^L, d^L, d^R and the two transverse velocities a^L v_t^L + a^R v_t^R of the
+   UCT-HLLD EMF average ([47] named at PAPER.md:271; reading R19, formulas in oracle.c) */
+int    oracle_hlld_uct(const double VL[7], const double VR[7], double Bn, double gamma,
+                       double F[8], double *w, double *dbg, double *uct);
+/* after oracle_init: EMF average of the constrained-transport step: 0 = upwind by the contact mode with the
+   continuous weight (R6, default), 1 = UCT-HLLD (R19) */
+int    oracle_set_emf(int mode);
+
 /* One Euler stage S -> S + L(S) (R1, Eq. 4) from the CURRENT state with the given
    dt; the state is not modified.  Any output pointer may be NULL.
      U1, Bf1 : same layouts as U / Bface
