@@ -182,13 +182,22 @@ enum {
     PLUTO_OPT_FUSE_XY = 2, /* 1 (default): x and y sweeps fused in one kernel; 0: one kernel per direction */
     PLUTO_OPT_CT_TMA = 3,  /* 1 (default): CT operands staged by TMA (cp.async.bulk.tensor); 0: per-thread loads */
     PLUTO_OPT_RK_ORDER = 4,/* 2 (default): SSP-RK2 (north star, reading R3); 3: SSP-RK3 of Eq. 5 (R17) */
-    PLUTO_OPT_DIVB = 5     /* divergence control of the NEXT pluto_init: PLUTO_DIVB_CT (default) or PLUTO_DIVB_GLM */
+    PLUTO_OPT_DIVB = 5,    /* divergence control of the NEXT pluto_init: PLUTO_DIVB_CT (default) or PLUTO_DIVB_GLM */
+    PLUTO_OPT_EMF = 6      /* EMF average of the constrained-transport step: PLUTO_EMF_CONTACT (default) or PLUTO_EMF_UCT_HLLD */
 };
 /* Divergence control: constrained transport (the north-star path), or the GLM
  * divergence cleaning of [43] (reading R20 in DESIGN.md): cell-centred B, one more scalar
  * psi, no face fields.  With PLUTO_DIVB_GLM: PLM only, one domain; pluto_set_state reads the cell-centred field
  * from U[4..6] and ignores Bface (may be NULL), psi starts at zero; pluto_get_state writes U only. */
 enum { PLUTO_DIVB_CT = 0, PLUTO_DIVB_GLM = 1 };
+/* EMF average of the constrained-transport step: PLUTO_EMF_CONTACT, the upwind-by-contact-mode
+ * rule with the continuous weight (reading R6; the north-star path, fused x+y sweep, TMA-staged CT kernel), or
+ * PLUTO_EMF_UCT_HLLD, the UCT-HLLD average of [47] that the paper's runs use (reference entry :640;
+ * reading R19 in DESIGN.md: the interface coefficients are the linear decomposition of the HLLD induction flux,
+ * the edge value is composed from them with the run's reconstruction).  May be switched at any time outside a
+ * step; the first step in UCT-HLLD mode allocates six more work arrays per slab with cudaMalloc (freed by
+ * pluto_finalize); its sweeps run one kernel per direction.  Ignored by the GLM variant. */
+enum { PLUTO_EMF_CONTACT = 0, PLUTO_EMF_UCT_HLLD = 1 };
 int    pluto_set_psi(const double *psi);      /* [nz][ny][nx], host or device; GLM variant only */
 int    pluto_get_psi(double *psi);
 int    pluto_set_option(int opt, int value);

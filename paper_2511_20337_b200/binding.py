@@ -22,6 +22,8 @@ OPT_CT_TMA = 3
 OPT_RK_ORDER = 4
 OPT_DIVB = 5
 DIVB_CT, DIVB_GLM = 0, 1
+OPT_EMF = 6
+EMF_CONTACT, EMF_UCT_HLLD = 0, 1
 
 # every symbol include/pluto.h declares
 SYMBOLS = [
@@ -222,6 +224,13 @@ class Pluto:
 
     def finalize(self):
         return self.L.pluto_finalize()
+
+    def set_emf(self, mode):
+        """EMF average of the CT step: EMF_CONTACT (default, reading R6) or EMF_UCT_HLLD (reading R19)"""
+        old = self.L.pluto_set_option(OPT_EMF, mode)
+        if old < 0:
+            raise ValueError(self.last_error())
+        return old
 
     # ---- GLM divergence cleaning (PLUTO_OPT_DIVB; reading R20)
     def set_divb(self, mode):

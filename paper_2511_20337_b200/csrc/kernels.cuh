@@ -186,6 +186,12 @@ __global__ void __launch_bounds__(128) k_ghost_yz(Grid g, double *__restrict__ b
 // ct + CT_EC + e        : cell-centred EMF component e, E^c = -(v x B)
 enum { CT_FEM = 0, CT_W = 6, CT_EC = 9, CT_COUNT = 12 };
 
+// UCT-HLLD mode (reading R19): instead of the two induction fluxes and the weight, a sweep along d leaves on the
+// lower d-face of every cell the five numbers of hlld_t<true>: a^L, d^L, d^R and the two transverse velocities
+// (t1, t2) = (d+1, d+2).  No periodic x copies: k_uct_halo fills the halos of these arrays.
+struct UctOut { double *p[5]; };
+constexpr int UCT_FACE = 15, UCT_COUNT = 18;      // 3 x 5 face arrays, then the three edge EMFs
+
 // The CT kernel reads the CT arrays one position beyond the interior in x (i = -1 and i = nx hold the
 // periodic copies of cells nx-1 and 0).  The sweep kernels write those copies with the value itself:
 // offset of the copy for cell i, or 0.
@@ -255,9 +261,12 @@ constexpr int SX_NT = 128;
 __host__ __device__ constexpr int sx_halo(int lim) { return lim == 2 ? 3 : 2; }
 __host__ __device__ constexpr int sx_out(int lim) { return SX_NT - 2 * sx_halo(lim); }
 
-template <int LIM, bool TWO_D>
+// hz: planes beyond the interior on each side of a 3D slab whose face data the CT step reads (1; UCT-HLLD: the
+// reach of the reconstruction).  UCT: leave the UCT-HLLD face data in uo instead of the CT arrays.
+template <int LIM, bool TWO_D, bool UCT>
 __global__ void __launch_bounds__(SX_NT, 4)
-k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P, Combine cb)
+k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P, Combine cb,
+          int hz, UctOut uo)
 {
     __shared__ double sP[8][SX_NT];     // primitives; rows 0..5 are reused for the fluxes
     __shared__ double sQ[7][SX_NT];     // q^L = q + slope/2 of each cell
@@ -265,8 +274,8 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
     constexpr int H = sx_halo(LIM);
     const int nx = g.n[0], M = nx + 2 * H;
     const long long sa = g.sa;
-    // 3D: planes -1 .. nz -- the CT kernel reads the x-face data one plane beyond the interior (no z wrap)
-    const int nzp = TWO_D ? 1 : g.n[2] + 2, kz0 = TWO_D ? 0 : -1;
+    // 3D: planes -hz .. nz + hz - 1 -- the CT kernel reads the x-face data beyond the interior (no z wrap)
+    const int nzp = TWO_D ? 1 : g.n[2] + 2 * hz, kz0 = TWO_D ? 0 : -hz;
     const long long nitems = (long long)M * g.n[1] * nzp;
     const long long item = (long long)blockIdx.x * sx_out(LIM) - H + t;
     const bool valid = item >= 0 && item < nitems;
@@ -319,11 +328,11 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
 
     // Riemann problem on the lower face of cell f (faces 0 .. nx)
     const bool face = has_nb && t >= H && f >= 0;
-    double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5;
+    double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5, uct[5];
     if (face) {
         Side L = { sQ[0][t - 1], sQ[1][t - 1], sQ[2][t - 1], sQ[3][t - 1], sQ[4][t - 1], sQ[5][t - 1], sQ[6][t - 1] };
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-        hlld(L, R, bxf, g.gamma, g.igm1, F, w);
+        hlld_t<UCT>(L, R, bxf, g.gamma, g.igm1, F, w, uct);
         sP[0][t] = F[0]; sP[1][t] = F[1]; sP[2][t] = F[2]; sP[3][t] = F[3]; sP[4][t] = F[6];
         if (TWO_D) sP[5][t] = F[5];
     }
@@ -345,6 +354,11 @@ k_sweep_x(Grid g, const double *__restrict__ Sin, double *Sout, double *__restri
         if (TWO_D) {   // B_z has no faces in 2D: cell centred, flux updated
             double r7 = fma(-dtdx, sP[5][t + 1] - F[5], Bc[2]);
             Sout[7 * sa + c] = cb.Sn ? fma(cb.wn, o7, cb.ws * r7) : r7;
+        }
+        if (UCT) {
+#pragma unroll
+            for (int m = 0; m < 5; m++) uo.p[m][c] = uct[m];
+            return;
         }
         // cell-centred EMF  E^c = -(v x B)
         const double e0 = q[3] * q[4] - q[2] * q[5], e1 = q[1] * q[5] - q[3] * Bc[0], e2 = q[2] * Bc[0] - q[1] * q[4];
@@ -422,10 +436,10 @@ constexpr int MARCH_PF = 16;     // doubles per thread and iteration: U(s+1) 5, 
 // three blocks of 128 threads per SM: 168 registers per thread hold the running state without
 // spilling (measured: 4 blocks at 128 registers spill ~40 values per interface and run 20% slower)
 constexpr int MARCH_MINB = 3;
-template <int DIR, int LIM, bool TWO_D, bool BOUND>
+template <int DIR, int LIM, bool TWO_D, bool BOUND, bool UCT>
 __global__ void __launch_bounds__(MARCH_NT, MARCH_MINB)
 k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, const double *base, double *__restrict__ ct,
-              StepParams *P, double scale, int seglen, int tr0, BoundGrid bg)
+              StepParams *P, double scale, int seglen, int tr0, BoundGrid bg, UctOut uo)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
@@ -525,8 +539,8 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, const double
             d0[v] = d1;
         }
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-        double F[7], w;
-        hlld(L, R, bface, gamma, igm1, F, w);
+        double F[7], w, uct[5];
+        hlld_t<UCT>(L, R, bface, gamma, igm1, F, w, uct);
         bface = bnext; bnext = bup;
         if (s > s0) {
             const long long cm = c - st;                  // cell s-1
@@ -544,7 +558,12 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, const double
             if (BZ2D) Sout[7 * sa + cm] = fma(-fac, F[4] - Fp[5], pf[slot][15][t]);   // F_y[B_z]
             if (BOUND) sb.add(g, r0, m[0], m[1], m[2], r4);
         }
-        if (s < s1 || (DIR == 2 && s == g.n[2])) {
+        if (UCT) {
+            if (s < s1 || (DIR == 2 && s == g.n[2])) {
+#pragma unroll
+                for (int m = 0; m < 5; m++) uo.p[m][c] = uct[m];
+            }
+        } else if (s < s1 || (DIR == 2 && s == g.n[2])) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;
@@ -576,10 +595,10 @@ k_sweep_march(Grid g, const double *__restrict__ Sin, double *Sout, const double
 // finishes cell s-1.  First version: operands are loaded directly (no prefetch ring).
 constexpr int WZ_PF = 17;        // doubles per thread and iteration: U(s+3) 5, faces 6, U'(s) 6
 
-template <int DIR, bool TWO_D, bool BOUND>
+template <int DIR, bool TWO_D, bool BOUND, bool UCT>
 __global__ void __launch_bounds__(MARCH_NT, 3)
 k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *__restrict__ ct, StepParams *P,
-                 double scale, int seglen, int tr0, BoundGrid bg)
+                 double scale, int seglen, int tr0, BoundGrid bg, UctOut uo)
 {
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     constexpr bool BZ2D = TWO_D && DIR == 1;           // F_y[B_z] updates the cell-centred B_z in 2D
@@ -676,8 +695,8 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
             recon_faces<2>(ring[m2][v][t], ring[m1][v][t], ring[c0][v][t], ring[p1][v][t], ring[p2][v][t], qR[v], qLn[v]);
         Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
         Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-        double F[7], w;
-        hlld(L, R, bn[c], gamma, igm1, F, w);
+        double F[7], w, uct[5];
+        hlld_t<UCT>(L, R, bn[c], gamma, igm1, F, w, uct);
 #pragma unroll
         for (int v = 0; v < 7; v++) qL[v] = qLn[v];
         if (s > s0) {
@@ -696,7 +715,12 @@ k_sweep_march_wz(Grid g, const double *__restrict__ Sin, double *Sout, double *_
             if (BZ2D) Sout[7 * sa + cm] = fma(-fac, F[4] - Fp[5], pf[ps][16][t]);   // F_y[B_z]
             if (BOUND) sb.add(g, r0, m[0], m[1], m[2], r4);
         }
-        if (s < s1 || (DIR == 2 && s == g.n[2])) {
+        if (UCT) {
+            if (s < s1 || (DIR == 2 && s == g.n[2])) {
+#pragma unroll
+                for (int m = 0; m < 5; m++) uo.p[m][c] = uct[m];
+            }
+        } else if (s < s1 || (DIR == 2 && s == g.n[2])) {
             ct[(CT_FEM + 2 * DIR) * sa + c] = F[4];
             ct[(CT_FEM + 2 * DIR + 1) * sa + c] = F[5];
             ct[(CT_W + DIR) * sa + c] = w;

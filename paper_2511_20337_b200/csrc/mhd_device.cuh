@@ -77,7 +77,7 @@ __device__ __forceinline__ double plm_slope(double dm, double dp)
         return same ? s : 0.0;
     } else {
         double sum = dm + dp;
-        double mag = min_sel(2.0 * min_sel(fabs(dm), fabs(dp)), 0.5 * fabs(sum));
+        double mag = fmin(2.0 * fmin(fabs(dm), fabs(dp)), 0.5 * fabs(sum));
         return same ? copysign(mag, dm) : 0.0;        // same sign: sign(dm + dp) = sign(dm)
     }
 }
@@ -95,7 +95,7 @@ __device__ __forceinline__ void plm_faces(double q, double dm, double dp, double
         s = fabs(dm) < fabs(dp) ? dm : dp;
     } else {
         double sum = dm + dp;
-        s = copysign(min_sel(2.0 * min_sel(fabs(dm), fabs(dp)), 0.5 * fabs(sum)), dm);
+        s = copysign(fmin(2.0 * fmin(fabs(dm), fabs(dp)), 0.5 * fabs(sum)), dm);
     }
     lo = fma(-h, s, q);
     hi = fma(h, s, q);
@@ -182,8 +182,17 @@ struct Side {
 // jump form F_K + S_K (U* - U_K) [+ S* (U** - U*)] of the HLLD paper up to rounding (in the guarded
 // degenerate case the two differ by < 1e-8 pT* B_t |S_M - u|, second order small).  Only the chosen
 // side's energy chain is computed.  Supersonic fans take the rarely executed branch at the end.
-__device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, double gamma, double igm1,
-                                     double f[7], double &wgt)
+//
+// UCT = true also returns what the UCT-HLLD EMF average ([47] named at PAPER.md:271; reading R19) takes from the
+// interface: uct[5] = a^L, d^L, d^R and the transverse velocities a^L v^L + a^R v^R, a^L w^L + a^R w^R, where
+//     F[B_t] = a^L (u B_t)^L + a^R (u B_t)^R - (d^R B_t^R - d^L B_t^L) - B_n (a^L v_t^L + a^R v_t^R)
+// is the (unique) decomposition of the HLLD induction flux that is linear in the four transverse inputs:
+//     chi^s = (u^s - S_M)(S_s - S_M) / (S*_s + S_s - 2 S_M),   nu^s = (S*_s + S_s) / (|S*_s| + |S_s|),
+//     nu* = (S*_R + S*_L) / (|S*_R| + |S*_L|)  (0 when both Alfven speeds vanish),
+//     a^L = (1 + nu*)/2,  d^s = (nu^s - nu*) chi^s / 2 + (|S*_s| - nu* S*_s) / 2.
+template <bool UCT>
+__device__ __forceinline__ void hlld_t(const Side &L, const Side &R, double Bx, double gamma, double igm1,
+                                       double f[7], double &wgt, double uct[5])
 {
     const double Bx2 = __dmul_rn(Bx, Bx);
     const double B2L = Bx2 + fma(L.By, L.By, L.Bz * L.Bz), B2R = Bx2 + fma(R.By, R.By, R.Bz * R.Bz);
@@ -256,8 +265,25 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     double rho_f = rs, uf = SM, pf = pTs;
     double vf = outer ? vs : vss, wf = outer ? ws : wss, Byf = outer ? Bys : Byss, Bzf = outer ? Bzs : Bzss;
     double Ef = outer ? Es : Ess, vBf = outer ? vBs : vBss;
+    if (UCT) {
+        const double aBx = fabs(Bx);
+        const double SaL = fma(-aBx, rcp_fast(rL), SM), SaR = fma(aBx, rcp_fast(rR), SM);     // Alfven speeds S*_L, S*_R
+        const double chiL = (L.u - SM) * (SL - SM) * rcp_fast((SaL + SL) - 2.0 * SM);
+        const double chiR = (R.u - SM) * (SR - SM) * rcp_fast((SaR + SR) - 2.0 * SM);
+        const double nuL = (SaL + SL) * rcp_fast(fabs(SaL) + fabs(SL));
+        const double nuR = (SaR + SR) * rcp_fast(fabs(SaR) + fabs(SR));
+        const double den = fabs(SaR) + fabs(SaL);
+        const double nus = den > 0.0 ? (SaR + SaL) * rcp_fast(den) : 0.0;
+        const double al = fma(0.5, nus, 0.5), ar = fma(-0.5, nus, 0.5);
+        uct[0] = al;
+        uct[1] = fma(0.5 * (nuL - nus), chiL, 0.5 * fma(-nus, SaL, fabs(SaL)));
+        uct[2] = fma(0.5 * (nuR - nus), chiR, 0.5 * fma(-nus, SaR, fabs(SaR)));
+        uct[3] = fma(al, L.v, ar * R.v);
+        uct[4] = fma(al, L.w, ar * R.w);
+    }
     if (__builtin_expect(SL >= 0.0 || SR <= 0.0, 0)) {          // one-sided fan: the upwind physical flux (Eq. 2)
         const bool sl = SL >= 0.0;
+        if (UCT) { uct[0] = sl ? 1.0 : 0.0; uct[1] = 0.0; uct[2] = 0.0; uct[3] = sl ? L.v : R.v; uct[4] = sl ? L.w : R.w; }
         rho_f = sl ? L.rho : R.rho; uf = sl ? L.u : R.u; vf = sl ? L.v : R.v; wf = sl ? L.w : R.w;
         Byf = sl ? L.By : R.By; Bzf = sl ? L.Bz : R.Bz; pf = sl ? pTL : pTR;
         {
@@ -278,6 +304,13 @@ __device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, do
     // R6: w = clamp(1/2 + F[rho] / (2 theta f_ref)), f_ref = (rho_L + rho_R)(S_R - S_L) / 4
     const double wv = fma(F0, rcp_fast((0.5 * kTheta) * ((L.rho + R.rho) * (SR - SL))), 0.5);
     wgt = min_sel(max_sel(wv, 0.0), 1.0);
+}
+
+__device__ __forceinline__ void hlld(const Side &L, const Side &R, double Bx, double gamma, double igm1,
+                                     double f[7], double &wgt)
+{
+    double none[5];
+    hlld_t<false>(L, R, Bx, gamma, igm1, f, wgt, none);
 }
 
 } // namespace pluto

@@ -9,6 +9,7 @@
 #include "kernels.cuh"
 #include "ct_tma.cuh"
 #include "glm.cuh"
+#include "uct.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -48,6 +49,7 @@ struct Domain {
     double *base = nullptr;          // A_COUNT_RK2 (or A_COUNT) arrays, then the scalars / bound grid of slab 0
     double *sc = nullptr;            // S^2 (8 arrays) when it was allocated after pluto_init
     bool own_mem = false, own_sc = false;
+    double *uct = nullptr;           // UCT-HLLD mode: the six work arrays beyond the twelve CT arrays (allocated on first use)
     int narrays = A_COUNT_RK2;
     unsigned long long *bound = nullptr;     // dt bound grid: n1 * n2 cells at most
     CUtensorMap ct_map{};
@@ -74,6 +76,7 @@ struct Context {
     int fuse_xy = 1;
     int ct_tma = 1;
     int rk_order = 2;                // 2: SSP-RK2 (R3), 3: SSP-RK3 (Eq. 5)
+    int emf = 0;                     // PLUTO_OPT_EMF: 0 contact-mode upwinding (R6), 1 UCT-HLLD (R19)
     int divb = 0;                    // PLUTO_OPT_DIVB of the next pluto_init: 0 constrained transport, 1 GLM cleaning
     bool glm = false;                // the live context runs the GLM variant (glm.cuh)
     cudaGraphExec_t graph[2] = { nullptr, nullptr };   // [0] CFL dt step, [1] fixed dt step (of the current rk_order)
@@ -241,7 +244,7 @@ void fill_ghosts(const Domain &d, int state, bool all = false)
     // only the chunked form of the fused x+y sweep reads x ghosts (k_sweep_x reads periodic images, the row-wide
     // x+y sweep wraps inside shared memory, the marching kernels stay inside the row)
     const bool chunked_xy = C.fuse_xy && g.limiter != 2 && !row_wraps(g.n[0]);
-    if (!all && !chunked_xy) {
+    if (!all && !chunked_xy && C.emf != 1) {      // (the UCT-HLLD edge kernel reconstructs the face fields across x too)
         const int ngh = 2 * g.ng + 1;
         const int rows = (g.act[2] ? ngh * (g.n[1] + ngh) : 0) + g.n[2] * ngh;
         LAUNCH(K_GHOST, k_ghost_yz<<<dim3(rows, S_COUNT), 128, 0, C.stream>>>(g, arr(d, state), zs));
@@ -290,15 +293,37 @@ BoundGrid final_bound_grid(const Domain &d, bool last)
     return bound_grid(d, last && d.g.act[2], 1, d.g.act[2] ? seglen_z(d.g) : 1);
 }
 
-template <int LIM, bool TWO_D>
+// UCT-HLLD work arrays of a slab: the twelve CT arrays first, then the six of d.uct
+UctArrays uct_arrays(const Domain &d)
+{
+    UctArrays A;
+    for (int n = 0; n < UCT_COUNT; n++)
+        A.p[n] = n < CT_COUNT ? arr(d, A_CT + n) : d.uct + (long long)(n - CT_COUNT) * d.g.sa;
+    return A;
+}
+
+UctOut uct_out(const Domain &d, int dir)
+{
+    UctOut o;
+    const UctArrays A = uct_arrays(d);
+    for (int m = 0; m < 5; m++) o.p[m] = A.p[dir * 5 + m];
+    return o;
+}
+
+template <int LIM, bool TWO_D, bool UCT>
 void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb, bool last)
 {
     const Grid &g = d.g;
     cudaStream_t s = C.stream;
     double *ct = arr(d, A_CT);
     const double scale = cb.Sn ? cb.ws : 1.0;
-    const int kz0 = TWO_D ? 0 : -1;                      // 3D: the x and y sweeps cover planes -1 .. nz
-    const int nplanes = TWO_D ? 1 : g.n[2] + 2;
+    // 3D: the x and y sweeps cover hz planes beyond the slab on each side (the CT step reads their face data there:
+    // one plane for the contact-mode rule, the reach of the transverse reconstruction for UCT-HLLD)
+    const int hz = TWO_D ? 0 : (UCT ? sx_halo(LIM) : 1);
+    const int kz0 = -hz;
+    const int nplanes = g.n[2] + 2 * hz;
+    UctOut ux{}, uy{}, uz{};
+    if constexpr (UCT) { ux = uct_out(d, 0); uy = uct_out(d, 1); uz = uct_out(d, 2); }
     const BoundGrid none = bound_grid(d, false, 1, 1);
     bool fused = false;
     // In a plain Euler stage of a 3D run the z sweep goes FIRST and writes S - dt/dz dFz; the fused x+y
@@ -306,22 +331,22 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
     // moves from the HBM-bound z sweep to the ALU-bound x+y sweep.  Combine stages keep the x+y sweep first
     // (S^n has to be read either way, and the last writer of the step fills the dt bound grid: the z sweep).
     bool zfirst = false;
-    if constexpr (LIM != 2 && !TWO_D) zfirst = C.fuse_xy && !cb.Sn;
+    if constexpr (LIM != 2 && !TWO_D && !UCT) zfirst = C.fuse_xy && !cb.Sn;
     auto z_sweep = [&](const double *base) {
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = seglen_z(g);
         dim3 grid(bx, g.n[1], (g.n[2] + len - 1) / len);
         const BoundGrid bg = final_bound_grid(d, last);
         if constexpr (LIM == 2) {
-            if (last) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, !TWO_D><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
-            else      LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg));
+            if (last) LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, !TWO_D, UCT><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg, uz));
+            else      LAUNCH(K_FLUX_Z, k_sweep_march_wz<2, TWO_D, false, UCT><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, 0, bg, uz));
         } else {
-            if (last) LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, !TWO_D><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, base, ct, C.P, scale, len, 0, bg));
-            else      LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, base, ct, C.P, scale, len, 0, bg));
+            if (last) LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, !TWO_D, UCT><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, base, ct, C.P, scale, len, 0, bg, uz));
+            else      LAUNCH(K_FLUX_Z, k_sweep_march<2, LIM, TWO_D, false, UCT><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, base, ct, C.P, scale, len, 0, bg, uz));
         }
     };
     if (zfirst) z_sweep(Sin);
-    if constexpr (LIM != 2) if (C.fuse_xy) {
+    if constexpr (LIM != 2 && !UCT) if (C.fuse_xy) {
         fused = true;
         // fused x + y sweep: one block per x-row chunk and y-segment.  The block width is a template
         // parameter (shared-memory offsets become immediates): a whole periodic row when nx is one of
@@ -342,18 +367,18 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
     }
     if (!fused) {
         if constexpr (LIM == 2) {
-            cudaFuncSetAttribute(k_sweep_march_wz<1, TWO_D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
-            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
-            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D, !TWO_D>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<1, TWO_D, false, UCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D, false, UCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
+            cudaFuncSetAttribute(k_sweep_march_wz<2, TWO_D, !TWO_D, UCT>, cudaFuncAttributeMaxDynamicSharedMemorySize, WZ_SMEM_BYTES);
         }
         const long long nitems = (long long)(g.n[0] + 2 * sx_halo(LIM)) * g.n[1] * nplanes;
-        LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D><<<(unsigned)((nitems + sx_out(LIM) - 1) / sx_out(LIM)), SX_NT, 0, s>>>(
-                             g, Sin, Sout, ct, C.P, cb));
+        LAUNCH(K_FLUX_X, k_sweep_x<LIM, TWO_D, UCT><<<(unsigned)((nitems + sx_out(LIM) - 1) / sx_out(LIM)), SX_NT, 0, s>>>(
+                             g, Sin, Sout, ct, C.P, cb, hz, ux));
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = seglen_y(g);
         dim3 grid(bx, (g.n[1] + len - 1) / len, nplanes);
-        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D, false><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, none));
-        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D, false><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, Sout, ct, C.P, scale, len, kz0, none));
+        if constexpr (LIM == 2) LAUNCH(K_FLUX_Y, k_sweep_march_wz<1, TWO_D, false, UCT><<<grid, MARCH_NT, WZ_SMEM_BYTES, s>>>(g, Sin, Sout, ct, C.P, scale, len, kz0, none, uy));
+        else LAUNCH(K_FLUX_Y, k_sweep_march<1, LIM, TWO_D, false, UCT><<<grid, MARCH_NT, 0, s>>>(g, Sin, Sout, Sout, ct, C.P, scale, len, kz0, none, uy));
     }
     if (!TWO_D && !zfirst) z_sweep(Sout);
 }
@@ -364,6 +389,33 @@ void launch_ct(const Domain &d, const double *bin, double *bout, Combine cb, dou
     const bool combine = cb.Sn != nullptr;
     const Grid &g = d.g;
     cudaStream_t s = C.stream;
+    if (C.emf == 1) {
+        // UCT-HLLD (R19, uct.cuh): halos of the face data, edge EMFs, face update
+        const bool two_d = !g.act[2];
+        const int h = sx_halo(g.limiter), hz = two_d ? 0 : h;
+        const UctArrays A = uct_arrays(d);
+        LAUNCH(K_CT_HALO, k_uct_halo<<<dim3(g.n[1] + 2 * h, g.n[2] + 2 * hz, UCT_FACE), 128, 0, s>>>(g, A, h, hz));
+        const dim3 ge((g.n[0] + 1 + 127) / 128, g.n[1] + 1, two_d ? 1 : g.n[2] + 1);
+        if (two_d) {
+            if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, true><<<ge, 128, 0, s>>>(g, A, bin));
+            else if (g.limiter == 1) LAUNCH(K_CT, k_emf_uct<1, true><<<ge, 128, 0, s>>>(g, A, bin));
+            else                     LAUNCH(K_CT, k_emf_uct<2, true><<<ge, 128, 0, s>>>(g, A, bin));
+        } else {
+            if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, false><<<ge, 128, 0, s>>>(g, A, bin));
+            else if (g.limiter == 1) LAUNCH(K_CT, k_emf_uct<1, false><<<ge, 128, 0, s>>>(g, A, bin));
+            else                     LAUNCH(K_CT, k_emf_uct<2, false><<<ge, 128, 0, s>>>(g, A, bin));
+        }
+        const dim3 gu((g.n[0] + 127) / 128, g.n[1], two_d ? 1 : g.n[2] + 1);
+        if (two_d) {
+            if (combine) LAUNCH(K_CT, k_ct_update<true, true><<<gu, 128, 0, s>>>(g, A, bin, bout, C.P, cb));
+            else         LAUNCH(K_CT, k_ct_update<false, true><<<gu, 128, 0, s>>>(g, A, bin, bout, C.P, cb));
+        } else {
+            if (combine) LAUNCH(K_CT, k_ct_update<true, false><<<gu, 128, 0, s>>>(g, A, bin, bout, C.P, cb));
+            else         LAUNCH(K_CT, k_ct_update<false, false><<<gu, 128, 0, s>>>(g, A, bin, bout, C.P, cb));
+        }
+        if (dbg) cudaMemcpyAsync(dbg, A.p[UCT_FACE], 3 * g.sa * sizeof(double), cudaMemcpyDeviceToDevice, s);
+        return;
+    }
     const int tiles_x = (g.n[0] + CT_TX - 2) / (CT_TX - 1), tiles_y = (g.n[1] + CT_TY - 2) / (CT_TY - 1);
     const int len = march_seglen(g.n[2], (long long)tiles_x * tiles_y * CT_TX * CT_TY);
     dim3 grid(tiles_x, tiles_y, (g.n[2] + len - 1) / len), block(CT_TX, CT_TY);
@@ -454,12 +506,16 @@ void enqueue_stage(int in, int out, int sn, double wn, double ws, bool last, dou
         const Grid &g = d.g;
         const bool two_d = !g.act[2];
         const Combine cb = { sn >= 0 ? arr(d, sn) : nullptr, wn, ws };
-        if (g.limiter == 0)      { if (two_d) launch_sweeps<0, true>(d, arr(d, in), arr(d, out), cb, last);
-                                   else       launch_sweeps<0, false>(d, arr(d, in), arr(d, out), cb, last); }
-        else if (g.limiter == 1) { if (two_d) launch_sweeps<1, true>(d, arr(d, in), arr(d, out), cb, last);
-                                   else       launch_sweeps<1, false>(d, arr(d, in), arr(d, out), cb, last); }
-        else                     { if (two_d) launch_sweeps<2, true>(d, arr(d, in), arr(d, out), cb, last);
-                                   else       launch_sweeps<2, false>(d, arr(d, in), arr(d, out), cb, last); }
+        auto sweeps = [&](auto lim, auto twod) {
+            constexpr int L = decltype(lim)::value;
+            constexpr bool T = decltype(twod)::value;
+            if (C.emf == 1) launch_sweeps<L, T, true>(d, arr(d, in), arr(d, out), cb, last);
+            else            launch_sweeps<L, T, false>(d, arr(d, in), arr(d, out), cb, last);
+        };
+        using I0 = std::integral_constant<int, 0>; using I1 = std::integral_constant<int, 1>; using I2 = std::integral_constant<int, 2>;
+        if (g.limiter == 0)      { if (two_d) sweeps(I0{}, std::true_type{}); else sweeps(I0{}, std::false_type{}); }
+        else if (g.limiter == 1) { if (two_d) sweeps(I1{}, std::true_type{}); else sweeps(I1{}, std::false_type{}); }
+        else                     { if (two_d) sweeps(I2{}, std::true_type{}); else sweeps(I2{}, std::false_type{}); }
         const Combine cbf = { sn >= 0 ? arr(d, sn + S_B) : nullptr, wn, ws };
         launch_ct(d, arr(d, in + S_B), arr(d, out + S_B), cbf, dbg);
     }
@@ -510,12 +566,14 @@ void enqueue_step(bool fixed)
 }
 
 int ensure_rk3_storage();
+int ensure_uct_storage();
 
 int run_steps(int nsteps, bool fixed)
 {
     if (!C.whole()) return fail(PLUTO_ESTATE, "this process holds %d of %d slabs: drive the step with pluto_step_begin / pluto_step_stage",
                                 (int)C.dom.size(), C.nslab);
     if (int rc = ensure_rk3_storage()) return rc;
+    if (int rc = ensure_uct_storage()) return rc;
     const int gi = fixed ? 1 : 0;
     const bool graph = C.use_graph && !C.prof_on;
     if (graph && !C.graph[gi] && nsteps > 0) {
@@ -601,6 +659,7 @@ void free_domains()
         for (Peer &p : d.nb)
             if (p.ipc_mapping) { cudaIpcCloseMemHandle(p.ipc_mapping); p.ipc_mapping = nullptr; }
         if (d.own_sc && d.sc) cudaFree(d.sc);
+        if (d.uct) cudaFree(d.uct);
         if (d.own_mem && d.base) cudaFree(d.base);
     }
     C.dom.clear();
@@ -629,6 +688,22 @@ int ensure_rk3_storage()
         }
     }
     destroy_graphs();
+    return PLUTO_OK;
+}
+
+// UCT-HLLD mode needs 18 work arrays (15 of face data, 3 edge EMFs): the twelve CT arrays and six more
+int ensure_uct_storage()
+{
+    if (C.emf != 1 || C.glm) return PLUTO_OK;
+    for (Domain &d : C.dom) {
+        if (d.uct) continue;
+        const size_t bytes = (size_t)(UCT_COUNT - CT_COUNT) * d.g.sa * sizeof(double);
+        cudaError_t e = cudaMalloc((void **)&d.uct, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); d.uct = nullptr; return fail(PLUTO_ENOMEM, "cudaMalloc(%zu) for the UCT-HLLD work arrays: %s", bytes, cudaGetErrorString(e)); }
+        // NaN patterns: a kernel that used a location no kernel had written would carry a NaN into the state
+        CUDA_TRY(cudaMemsetAsync(d.uct, 0xFF, bytes, C.stream));
+        destroy_graphs();
+    }
     return PLUTO_OK;
 }
 
@@ -973,6 +1048,13 @@ int pluto_set_option(int opt, int value)
         destroy_graphs();
         return old;
     }
+    if (opt == PLUTO_OPT_EMF) {
+        if (value != PLUTO_EMF_CONTACT && value != PLUTO_EMF_UCT_HLLD) return fail(PLUTO_EINVAL, "EMF average must be PLUTO_EMF_CONTACT or PLUTO_EMF_UCT_HLLD");
+        int old = C.emf;
+        C.emf = value;
+        destroy_graphs();
+        return old;
+    }
     if (opt == PLUTO_OPT_DIVB) {
         if (value != PLUTO_DIVB_CT && value != PLUTO_DIVB_GLM) return fail(PLUTO_EINVAL, "divergence control must be PLUTO_DIVB_CT or PLUTO_DIVB_GLM");
         int old = C.divb;
@@ -1164,6 +1246,7 @@ int pluto_step_begin(double fixed_dt)
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
     if (!peers_attached()) return fail(PLUTO_ESTATE, "a neighbour slab is not attached (pluto_attach_peer)");
     if (int rc = ensure_rk3_storage()) return rc;
+    if (int rc = ensure_uct_storage()) return rc;
     if (fixed_dt > 0.0) {
         CUDA_TRY(cudaMemcpyAsync(&C.P->dt_fixed, &fixed_dt, sizeof fixed_dt, cudaMemcpyHostToDevice, C.stream));
         CUDA_TRY(cudaStreamSynchronize(C.stream));
@@ -1263,6 +1346,7 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
     if (C.dom.size() != 1 || !C.whole() || C.glm) return fail(PLUTO_ESTATE, "pluto_debug_euler works on a single domain of the CT scheme");
     if (!(dt > 0.0)) return fail(PLUTO_EINVAL, "dt must be positive");
+    if (int rc = ensure_uct_storage()) return rc;
     const Domain &d = C.dom[0];
     const Grid &g = d.g;
     cudaStream_t s = C.stream;

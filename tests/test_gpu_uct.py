@@ -1,0 +1,156 @@
+"""GPU parity of the UCT-HLLD EMF average (PLUTO_OPT_EMF = PLUTO_EMF_UCT_HLLD; reading R19, [47] named at
+PAPER.md:271) against the oracle, element by element, through the C ABI: edge EMFs of one Euler stage, one step
+(max-rel 1e-10), 20 steps (L1-rel 1e-8), dt bit-exact; 2D / 3D, minmod / MC / WENO-Z, RK2 / RK3, row widths that
+wrap and that do not, ragged shapes, z slabs (bit-identical to the single domain), and that leaving the mode
+restores the default path bit for bit."""
+import numpy as np
+import pytest
+
+from paper_2511_20337_b200 import workloads as wl
+from paper_2511_20337_b200.binding import EMF_CONTACT, EMF_UCT_HLLD
+from test_gpu_parity import (TOL_1STEP_MAXREL, TOL_100STEP_L1REL, compare_state, l1rel, l1rel_vector_scaled, maxrel,
+                             maxrel_vector_scaled)
+
+pytestmark = pytest.mark.gpu
+
+
+def _wz(w):
+    w.limiter = 2
+    return w
+
+
+CASES = [
+    ("ot2d_48_minmod", lambda: wl.orszag_tang_2d(48), 2, 2),
+    ("ot2d_64_mc_rk3", lambda: wl.orszag_tang_2d(64, limiter=1), 3, 2),
+    ("smooth3d_mc", lambda: wl.random_smooth(24, 20, 18, seed=91, limiter=1, box=(1.0, 0.9, 0.8)), 2, 2),
+    ("smooth3d_ragged_rk3", lambda: wl.random_smooth(37, 23, 9, seed=92, limiter=0), 3, 2),
+    ("blast_24", lambda: wl.blast_3d(24), 2, 2),
+    ("blast_wrap64", lambda: wl.blast_3d(64), 2, 2),
+    ("cp_alfven_3d", lambda: wl.cp_alfven_3d(32), 2, 3),
+    ("wenoz_2d_rk3", lambda: _wz(wl.orszag_tang_2d(48)), 3, 3),
+    ("wenoz_3d_rk3", lambda: _wz(wl.random_smooth(20, 18, 16, seed=93)), 3, 3),
+    ("ot3d_32_wenoz_rk3", lambda: _wz(wl.orszag_tang_3d(32, noise=1e-3)), 3, 3),
+]
+
+
+@pytest.fixture()
+def uct(pluto, oracle):
+    pluto.set_emf(EMF_UCT_HLLD)
+    yield pluto
+    pluto.set_emf(EMF_CONTACT)
+    pluto.set_integrator(2)
+    oracle.set_integrator(2)
+
+
+@pytest.mark.parametrize("name,make,rk,ghost", CASES, ids=[c[0] for c in CASES])
+def test_uct_parity(uct, oracle, name, make, rk, ghost):
+    w = make()
+    uct.set_integrator(rk)
+    uct.load(w, ghost=ghost)
+    oracle.load(w)
+    assert oracle.set_emf(1) == 0
+    oracle.set_integrator(rk)
+    dt = oracle.get_dt()
+    assert uct.get_dt() == dt
+    n1, nl = (maxrel_vector_scaled, l1rel_vector_scaled) if name.startswith("ot3d") else (maxrel, l1rel)
+    g = uct.debug_euler(dt)
+    o = oracle.debug_euler(dt)
+    assert g["rc"] == 0 and o["rc"] == 0
+    escale = max(np.abs(o["E"]).max(), 1e-300)
+    for e in range(3):
+        assert np.abs(g["E"][e] - o["E"][e]).max() <= 1e-12 * escale, e
+    assert n1(g["U1"].reshape(8, -1), o["U1"].reshape(8, -1)) <= 1e-11
+    assert maxrel(g["Bf1"][None], o["Bf1"][None]) <= 1e-11
+    uct.step(1)
+    assert oracle.step(1) == 0
+    compare_state(uct, oracle, w, TOL_1STEP_MAXREL, norm=n1)
+    uct.step(19)
+    assert oracle.step(19) == 0
+    compare_state(uct, oracle, w, TOL_100STEP_L1REL, norm=nl)
+    # the two rules are different schemes: the comparison above is not vacuous
+    oracle.load(w)
+    oracle.set_integrator(rk)
+    assert oracle.step(20) == 0
+    Uc, _ = oracle.get_state()
+    Uu, _ = uct.get_state()
+    assert np.abs(Uu - Uc).max() > 1e-9 * np.abs(Uc).max()
+
+
+def test_uct_invariants_on_the_gpu(uct):
+    """div B, conserved sums and the periodic duplicates after 30 steps of the 3D blast in UCT-HLLD mode"""
+    import math
+    w = wl.blast_3d(32)
+    uct.load(w)
+    uct.step(30)
+    U, Bf = uct.get_state()
+    for v in (0, 7):
+        s0, s1 = math.fsum(w.U[v].ravel()), math.fsum(U[v].ravel())
+        assert abs(s1 - s0) <= 1e-12 * abs(s0)
+    f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+    div = ((f["bx"][:, :, 1:] - f["bx"][:, :, :-1]) + (f["by"][:, 1:, :] - f["by"][:, :-1, :])
+           + (f["bz"][1:, :, :] - f["bz"][:-1, :, :]))
+    assert np.abs(div).max() <= 1e-12 * np.abs(Bf).max()
+    assert np.array_equal(f["bx"][:, :, 0], f["bx"][:, :, -1])
+    assert np.array_equal(f["by"][:, 0, :], f["by"][:, -1, :])
+    assert np.array_equal(f["bz"][0], f["bz"][-1])
+
+
+@pytest.mark.parametrize("nslab", [2, 3])
+def test_uct_slabs_match_the_single_domain_bit_for_bit(uct, nslab):
+    for make, rk, ghost in ((lambda: wl.random_smooth(40, 14, 18, seed=94, limiter=1), 2, 2),
+                            (lambda: _wz(wl.random_smooth(24, 12, 16, seed=95)), 3, 3)):
+        w = make()
+        uct.set_integrator(rk)
+        uct.load(w, ghost=ghost)
+        uct.step(3)
+        ref = uct.get_state()
+        ref_dt = uct.get_dt()
+        uct.load(w, ghost=ghost, nslab=nslab)
+        uct.step(3)
+        out = uct.get_state()
+        assert uct.get_dt() == ref_dt
+        assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
+
+
+def test_leaving_the_mode_restores_the_default_path(pluto):
+    w = wl.blast_3d(32)
+    pluto.load(w)
+    pluto.step(3)
+    ref = pluto.get_state()
+    pluto.set_emf(EMF_UCT_HLLD)
+    try:
+        pluto.load(w)
+        pluto.step(3)
+        mid = pluto.get_state()
+    finally:
+        pluto.set_emf(EMF_CONTACT)
+    pluto.load(w)
+    pluto.step(3)
+    out = pluto.get_state()
+    assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
+    assert not np.array_equal(mid[1], ref[1])
+
+
+def test_uct_poisoned_workspace_and_repeatability(uct):
+    """the memory-safety substitutes of test_gpu_parity for the UCT-HLLD kernels: a workspace full of NaN patterns
+    between init and set_state gives the same bits; repeated runs (graph replay and plain launches) agree"""
+    from paper_2511_20337_b200.binding import OPT_GRAPH
+    for make, rk, ghost in ((lambda: wl.random_smooth(37, 13, 11, seed=96, limiter=1), 3, 2),
+                            (lambda: wl.orszag_tang_2d(40), 2, 2),
+                            (lambda: _wz(wl.random_smooth(20, 9, 8, seed=97)), 2, 3)):
+        w = make()
+        uct.set_integrator(rk)
+        uct.load(w, ghost=ghost)
+        uct.step(3)
+        ref = uct.get_state()
+        for n in range(3):
+            uct.set_option(OPT_GRAPH, n % 2)
+            uct.init(w.nx, w.ny, w.nz, ghost, w.gamma, w.cfl, w.limiter)
+            uct.workspace.fill_(0xFF)
+            uct.torch.cuda.synchronize()
+            uct.set_box(*w.box)
+            uct.set_state(w.U, w.Bface)
+            uct.step(3)
+            out = uct.get_state()
+            assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
+        uct.set_option(OPT_GRAPH, 1)
