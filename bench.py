@@ -186,7 +186,7 @@ class ClockSampler:
                 "power_w": statistics.median(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_run(w, steps, threads=None, rk=2, warmup=1, glm=False):
+def oracle_run(w, steps, threads=None, rk=2, warmup=1, glm=False, uct=False):
     """the oracle as it stands on the host cores: `steps` whole steps of workload w; returns
     (zone-updates/s, threads used, seconds, per-step seconds)"""
     from oracle import Oracle
@@ -197,6 +197,8 @@ def oracle_run(w, steps, threads=None, rk=2, warmup=1, glm=False):
         o.load_glm(w)
     else:
         o.load(w)
+        if uct:
+            assert o.set_emf(1) == 0
     o.set_integrator(rk)
     for _ in range(warmup):
         assert o.step(1) == 0                   # touch memory
@@ -231,14 +233,15 @@ def cpu_workload(cfg):
     return wl.config(cfg), "the bench workload itself, full size"
 
 
-def scheme_of(w, rk, glm=False):
-    return "recon(%s)+HLLD+RK%d+%s, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], rk, "GLM" if glm else "CT", w.cfl)
+def scheme_of(w, rk, glm=False, uct=False):
+    return "recon(%s)+HLLD+RK%d+%s, CFL %.2g" % (("minmod", "MC", "WENOZ")[w.limiter], rk,
+                                                 "GLM" if glm else ("CT(UCT-HLLD)" if uct else "CT"), w.cfl)
 
 
 def config_of(args, w, world):
     name = (f"configs[{args.config}] {w.name}" if args.config < 5
             else f"paper section 4.1 workload (not a BASELINE config) {w.name}")
-    return {"workload": name, "grid": [w.nx, w.ny, w.nz], "zones": w.zones, "scheme": scheme_of(w, args.rk, args.glm),
+    return {"workload": name, "grid": [w.nx, w.ny, w.nz], "zones": w.zones, "scheme": scheme_of(w, args.rk, args.glm, args.uct),
             "l2": "inputs larger than L2 (state %.2f GB)" % (11 * w.zones * 8 / 1e9) if w.zones * 88 > 126e6
                   else "L2 flushed between timed repeats (a 256 MB buffer is rewritten); the state fits in L2",
             "parallelism": "single GPU" if world == 1 else "z-slab domain decomposition, one slab per GPU"}
@@ -252,7 +255,7 @@ def run_reference(args):
     w, what = cpu_workload(args.config)
     if args.wenoz:
         w.limiter = 2
-    val, cores, secs, per = oracle_run(w, args.steps, rk=args.rk, warmup=max(1, min(args.warmup, 2)), glm=args.glm)
+    val, cores, secs, per = oracle_run(w, args.steps, rk=args.rk, warmup=max(1, min(args.warmup, 2)), glm=args.glm, uct=args.uct)
     from paper_2511_20337_b200 import workloads as wl
     wcfg = wl.config(args.config) if args.config != 4 else w
     line = {
@@ -278,6 +281,7 @@ def main():
     ap.add_argument("--wenoz", action="store_true", help="WENO-Z reconstruction instead of the config's PLM limiter")
     ap.add_argument("--rk", type=int, default=2, help="2: SSP-RK2 (the north_star's step, default); 3: SSP-RK3 of Eq. 5")
     ap.add_argument("--glm", action="store_true", help="GLM divergence cleaning (cell-centred B) instead of constrained transport")
+    ap.add_argument("--uct", action="store_true", help="UCT-HLLD EMF average (reading R19) instead of the contact-mode rule (R6)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--repeats", type=int, default=3, help="timed repeats of the K steps (median and best reported)")
@@ -302,6 +306,8 @@ def main():
         w.limiter = 2
     sim = Pluto(device=local)
     sim.set_integrator(args.rk)
+    if args.uct:
+        sim.set_emf(1)
     if args.glm:
         sim.load_glm(w)
     else:
@@ -351,7 +357,7 @@ def main():
     hbm_peak, peak_src = peaks()
     units = w.zones                              # zones one launch of the dominant kernel processes
     method, design = kernel_doubles(w.ndim, args.rk, args.glm)
-    ncu, ncu_src = ncu_table(w.ndim, args.rk, w.limiter, units) if not args.glm else (None, None)
+    ncu, ncu_src = ncu_table(w.ndim, args.rk, w.limiter, units) if not (args.glm or args.uct) else (None, None)
     dur = dom_ms * 1e-3 / max(dom_cnt, 1)
     method_bytes = method.get(dom, 0) * 8 * units
     design_bytes = design.get(dom, 0) * 8 * units
@@ -433,11 +439,11 @@ def main():
         wc, what = cpu_workload(args.config)
         if args.wenoz:
             wc.limiter = 2
-        v, cores, secs, per = oracle_run(wc, 3, rk=args.rk, glm=args.glm)
+        v, cores, secs, per = oracle_run(wc, 3, rk=args.rk, glm=args.glm, uct=args.uct)
         ws, what1 = small_sample(args.config)
         if args.wenoz:
             ws.limiter = 2
-        v1, _, secs1, _ = oracle_run(ws, 1, threads=1, rk=args.rk, warmup=0, glm=args.glm)
+        v1, _, secs1, _ = oracle_run(ws, 1, threads=1, rk=args.rk, warmup=0, glm=args.glm, uct=args.uct)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{what}, 3 steps, {secs:.1f} s",
                                 "best_step_s": min(per), "median_step_s": statistics.median(per),

@@ -14,6 +14,7 @@
  * Beyond the north-star step: SSP-RK3 (Eq. 5 itself; PLUTO_OPT_RK_ORDER, reading R17) and WENO-Z
  * reconstruction ([51] named at PAPER.md:100,260; limiter PLUTO_WENOZ, reading R18).
  *
+ * The EMF average of the paper's own runs, UCT-HLLD ([47] named at PAPER.md:271; reading R19): PLUTO_OPT_EMF.
  * The paper's other divergence control, GLM divergence cleaning ([43] named at PAPER.md:47,306,369; reading R20):
  * PLUTO_OPT_DIVB.
  * Beyond one GPU: the box cut into z slabs, one or more per process, with the ghost planes pulled out of

@@ -394,7 +394,7 @@ void launch_ct(const Domain &d, const double *bin, double *bout, Combine cb, dou
         const bool two_d = !g.act[2];
         const int h = sx_halo(g.limiter), hz = two_d ? 0 : h;
         const UctArrays A = uct_arrays(d);
-        LAUNCH(K_CT_HALO, k_uct_halo<<<dim3(g.n[1] + 2 * h, g.n[2] + 2 * hz, UCT_FACE), 128, 0, s>>>(g, A, h, hz));
+        LAUNCH(K_CT_HALO, k_uct_halo<<<dim3((g.n[1] + 2 * h + UCT_HALO_ROWS - 1) / UCT_HALO_ROWS, g.n[2] + 2 * hz, UCT_FACE), 256, 0, s>>>(g, A, h, hz));
         const dim3 ge((g.n[0] + 1 + 127) / 128, g.n[1] + 1, two_d ? 1 : g.n[2] + 1);
         if (two_d) {
             if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, true><<<ge, 128, 0, s>>>(g, A, bin));

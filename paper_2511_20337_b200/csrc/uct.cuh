@@ -13,19 +13,34 @@ namespace pluto {
 // the 15 face arrays [direction d][a^L, d^L, d^R, vbar_t1, vbar_t2] and the edge EMFs E_x, E_y, E_z
 struct UctArrays { double *p[UCT_COUNT]; };
 
-// grid.x = padded row (j = -h .. n1 + h - 1), grid.y = plane (k = -hz .. n2 + hz - 1), grid.z = array.
-// Every halo position (i or j outside the interior, within h) receives its periodic image; sources are interior.
-__global__ void __launch_bounds__(128) k_uct_halo(Grid g, UctArrays A, int h, int hz)
+// Every halo position (i or j outside the interior, within h) of the 15 face arrays receives its periodic image;
+// sources are interior positions, so there is no ordering between copies.  grid.x = chunk of UCT_HALO_ROWS padded
+// rows (j = -h .. n1 + h - 1), grid.y = plane (k = -hz .. n2 + hz - 1), grid.z = array.  Halo rows are copied whole,
+// interior rows contribute their 2h end positions (walked as one flat list so that no thread idles).
+constexpr int UCT_HALO_ROWS = 32;
+__global__ void __launch_bounds__(256) k_uct_halo(Grid g, UctArrays A, int h, int hz)
 {
     const int n0 = g.n[0], n1 = g.n[1];
-    const int j = (int)blockIdx.x - h, k = (int)blockIdx.y - hz;
+    const int j0 = (int)blockIdx.x * UCT_HALO_ROWS - h, j1 = min(j0 + UCT_HALO_ROWS, n1 + h);
+    const int k = (int)blockIdx.y - hz;
     double *arr = A.p[blockIdx.z];
-    const int sj = ((j % n1) + n1) % n1;
-    const bool halo_row = j != sj;
-    for (int e = threadIdx.x; e < (halo_row ? n0 + 2 * h : 2 * h); e += blockDim.x) {
-        const int i = halo_row ? e - h : (e < h ? e - h : n0 + (e - h));
-        const int si = ((i % n0) + n0) % n0;
-        arr[g.at(i, j, k)] = arr[g.at(si, sj, k)];
+    // whole halo rows of this chunk
+    for (int j = j0; j < j1; j++) {
+        if (j >= 0 && j < n1) continue;
+        const int sj = ((j % n1) + n1) % n1;
+        double *dst = arr + g.at(-h, j, k);
+        const double *src = arr + g.at(0, sj, k);
+        for (int e = threadIdx.x; e < n0 + 2 * h; e += blockDim.x) {
+            const int i = e - h;
+            dst[e] = src[((i % n0) + n0) % n0];
+        }
+    }
+    // x ends of the interior rows of this chunk
+    const int i0 = max(j0, 0), i1 = min(j1, n1);
+    for (int t = threadIdx.x; t < (i1 - i0) * 2 * h; t += blockDim.x) {
+        const int j = i0 + t / (2 * h), e = t % (2 * h);
+        const int i = e < h ? e - h : n0 + (e - h);
+        arr[g.at(i, j, k)] = arr[g.at(((i % n0) + n0) % n0, j, k)];
     }
 }
 
