@@ -141,6 +141,24 @@ __device__ __forceinline__ void wenoz_faces(double a, double b, double c, double
     }
 }
 
+// The upper-face value alone (the lower-face value of a cell is this on the mirrored stencil): same arithmetic
+// as the upper face of wenoz_faces, 49 fp64 instructions.  Used where the two faces of a cell are wanted by
+// different threads (the edge reconstruction of uct.cuh).
+__device__ __forceinline__ double wenoz_upper(double a, double b, double c, double d, double e)
+{
+    const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+    const double a0 = d2 - d1, b0 = fma(3.0, d2, -d1);
+    const double a1 = d3 - d2, b1 = d2 + d3;
+    const double a2 = d4 - d3, b2 = fma(-3.0, d3, d4);
+    const double P0 = fma(13.0 / 3.0 * a0, a0, __dmul_rn(b0, b0)) + 4e-40;
+    const double P1 = fma(13.0 / 3.0 * a1, a1, __dmul_rn(b1, b1)) + 4e-40;
+    const double P2 = fma(13.0 / 3.0 * a2, a2, __dmul_rn(b2, b2)) + 4e-40;
+    const double tau = fabs(P0 - P2);
+    const double al0 = 0.1 * ((P0 + tau) * (P1 * P2)), m1 = 0.6 * ((P1 + tau) * (P0 * P2)), al2 = 0.3 * ((P2 + tau) * (P0 * P1));
+    const double num = fma(al0, fma(5.0, d2, -2.0 * d1), fma(m1, fma(2.0, d3, d2), __dmul_rn(al2, fma(4.0, d3, -d4))));
+    return fma(num, rcp_fast(6.0 * (al0 + m1 + al2)), c);
+}
+
 // Interface values of the centre cell from its five-cell stencil: LIM 0/1 = PLM with minmod / MC
 // (uses the inner three cells), LIM 2 = WENO-Z.  lo on the lower face, hi on the upper face.
 template <int LIM>

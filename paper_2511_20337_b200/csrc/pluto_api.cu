@@ -395,15 +395,15 @@ void launch_ct(const Domain &d, const double *bin, double *bout, Combine cb, dou
         const int h = sx_halo(g.limiter), hz = two_d ? 0 : h;
         const UctArrays A = uct_arrays(d);
         LAUNCH(K_CT_HALO, k_uct_halo<<<dim3((g.n[1] + 2 * h + UCT_HALO_ROWS - 1) / UCT_HALO_ROWS, g.n[2] + 2 * hz, UCT_FACE), 256, 0, s>>>(g, A, h, hz));
-        const dim3 ge((g.n[0] + 1 + 127) / 128, g.n[1] + 1, two_d ? 1 : g.n[2] + 1);
+        const dim3 ge((g.n[0] + UCT_TX) / UCT_TX, (g.n[1] + UCT_TY) / UCT_TY, two_d ? 1 : g.n[2] + 1), be(UCT_TX, UCT_TY);
         if (two_d) {
-            if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, true><<<ge, 128, 0, s>>>(g, A, bin));
-            else if (g.limiter == 1) LAUNCH(K_CT, k_emf_uct<1, true><<<ge, 128, 0, s>>>(g, A, bin));
-            else                     LAUNCH(K_CT, k_emf_uct<2, true><<<ge, 128, 0, s>>>(g, A, bin));
+            if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, true><<<ge, be, 0, s>>>(g, A, bin));
+            else if (g.limiter == 1) LAUNCH(K_CT, k_emf_uct<1, true><<<ge, be, 0, s>>>(g, A, bin));
+            else                     LAUNCH(K_CT, k_emf_uct<2, true><<<ge, be, 0, s>>>(g, A, bin));
         } else {
-            if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, false><<<ge, 128, 0, s>>>(g, A, bin));
-            else if (g.limiter == 1) LAUNCH(K_CT, k_emf_uct<1, false><<<ge, 128, 0, s>>>(g, A, bin));
-            else                     LAUNCH(K_CT, k_emf_uct<2, false><<<ge, 128, 0, s>>>(g, A, bin));
+            if (g.limiter == 0)      LAUNCH(K_CT, k_emf_uct<0, false><<<ge, be, 0, s>>>(g, A, bin));
+            else if (g.limiter == 1) LAUNCH(K_CT, k_emf_uct<1, false><<<ge, be, 0, s>>>(g, A, bin));
+            else                     LAUNCH(K_CT, k_emf_uct<2, false><<<ge, be, 0, s>>>(g, A, bin));
         }
         const dim3 gu((g.n[0] + 127) / 128, g.n[1], two_d ? 1 : g.n[2] + 1);
         if (two_d) {

@@ -50,12 +50,12 @@ template <int LIM>
 __device__ __forceinline__ void edge_values(const double *__restrict__ q, long long st, double &below, double &above)
 {
     const double m2 = q[-2 * st], m1 = q[-st], p0 = q[0], p1 = q[st];
-    double lo, hi;
     if (LIM == 2) {
         const double m3 = q[-3 * st], p2 = q[2 * st];
-        recon_faces<2>(m3, m2, m1, p0, p1, lo, below);
-        recon_faces<2>(m2, m1, p0, p1, p2, above, hi);
+        below = wenoz_upper(m3, m2, m1, p0, p1);
+        above = wenoz_upper(p2, p1, p0, m1, m2);
     } else {
+        double lo, hi;
         plm_faces<LIM == 2 ? 0 : LIM>(m1, m1 - m2, p0 - m1, lo, below);
         plm_faces<LIM == 2 ? 0 : LIM>(p0, p0 - m1, p1 - p0, above, hi);
     }
@@ -89,12 +89,14 @@ __device__ __forceinline__ double uct_edge(const UctArrays &A, const double *__r
            + fma(dE, BbE, -dW * BbW) - fma(dN, BaN, -dS * BaS);
 }
 
-// one thread per cell (i, j, k) of [0, n0] x [0, n1] x [0, n2]: the EMFs on its three lower edges
+// one thread per cell (i, j, k) of [0, n0] x [0, n1] x [0, n2]: the EMFs on its three lower edges.  Blocks are
+// UCT_TX x UCT_TY tiles of one plane: the stencils of neighbouring rows meet in L1.
+constexpr int UCT_TX = 32, UCT_TY = 4;
 template <int LIM, bool TWO_D>
-__global__ void __launch_bounds__(128) k_emf_uct(Grid g, UctArrays A, const double *__restrict__ bfaces)
+__global__ void __launch_bounds__(UCT_TX * UCT_TY) k_emf_uct(Grid g, UctArrays A, const double *__restrict__ bfaces)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-    if (i > g.n[0]) return;
+    const int i = blockIdx.x * UCT_TX + threadIdx.x, j = blockIdx.y * UCT_TY + threadIdx.y, k = blockIdx.z;
+    if (i > g.n[0] || j > g.n[1]) return;
     const long long c = g.at(i, j, k), sa = g.sa;
     A.p[UCT_FACE + 2][c] = uct_edge<LIM>(A, bfaces, sa, c, 0, 1, 1, g.st[1]);                 // E_z: a = x, b = y
     if (!TWO_D) {
