@@ -232,9 +232,10 @@ int make_ct_map(Domain &d)
 
 // ---------------------------------------------------------------- launch sequences
 
-// The fused x+y sweep spans a whole periodic row when nx is one of the instantiated block widths: no
-// kernel then reads an x ghost other than the x-face n0 (kept equal to face 0 by the CT kernel).
-bool row_wraps(int nx) { return nx == 64 || nx == 128 || nx == 256 || nx == 512; }
+// The fused x+y sweep spans a whole periodic row when nx is one of the instantiated block widths (every multiple of
+// 32 from 64 to 256, and 512; wider rows do not fit the registers of one block): no kernel then reads an x ghost
+// other than the x-face n0 (kept equal to face 0 by the CT kernel).
+bool row_wraps(int nx) { return (nx % 32 == 0 && nx >= 64 && nx <= 256) || nx == 512; }
 
 // ghost layers of the 8 arrays of one state of one slab, one launch (z planes from the neighbour slabs)
 void fill_ghosts(const Domain &d, int state, bool all = false)
@@ -359,7 +360,9 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         dim3 grid(chunks, (g.n[1] + len - 1) / len, nplanes);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
         void (*k)(Grid, const double *, double *, const double *, double *, StepParams *, Combine, int, int) =
-            wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128>
+            wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 96 ? k_sweep_xy<LIM, TWO_D, true, 96>
+                    : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128> : nt == 160 ? k_sweep_xy<LIM, TWO_D, true, 160>
+                    : nt == 192 ? k_sweep_xy<LIM, TWO_D, true, 192> : nt == 224 ? k_sweep_xy<LIM, TWO_D, true, 224>
                     : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
                  : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

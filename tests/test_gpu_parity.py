@@ -633,7 +633,7 @@ def test_device_pointers_and_graph_equivalence(pluto, oracle):
     assert pluto.launch_count() > 0
 
 
-@pytest.mark.parametrize("shape", [(40, 24, 12), (64, 20, 1), (37, 23, 9), (300, 9, 1)])
+@pytest.mark.parametrize("shape", [(40, 24, 12), (64, 20, 1), (37, 23, 9), (300, 9, 1), (96, 10, 6), (160, 7, 1), (192, 6, 5), (224, 5, 1)])
 def test_fused_and_per_direction_sweeps_agree(pluto, shape):
     """the fused x+y sweep (wrap and chunk modes) against one kernel per direction"""
     from paper_2511_20337_b200 import binding
@@ -650,6 +650,28 @@ def test_fused_and_per_direction_sweeps_agree(pluto, shape):
         pluto.set_option(binding.OPT_FUSE_XY, old)
     assert maxrel(Ua.reshape(8, -1), Ub.reshape(8, -1)) <= 1e-13
     assert maxrel(Ba[None], Bb[None]) <= 1e-13
+
+
+@pytest.mark.parametrize("nx,ny,nz,lim,rk", [(96, 12, 7, 0, 2), (160, 9, 1, 1, 3), (192, 8, 6, 1, 2), (224, 6, 5, 0, 3)])
+def test_row_wrapping_widths_against_the_oracle(pluto, oracle, nx, ny, nz, lim, rk):
+    """every multiple of 32 from 64 to 256 is an instantiated row-wide block of the fused x+y sweep (64, 128, 256
+    run in the configs): the widths in between, element by element against the oracle"""
+    w = wl.random_smooth(nx, ny, nz, seed=100 + nx, limiter=lim)
+    pluto.set_integrator(rk)
+    try:
+        pluto.load(w)
+        oracle.load(w)
+        oracle.set_integrator(rk)
+        assert pluto.get_dt() == oracle.get_dt()
+        pluto.step(1)
+        assert oracle.step(1) == 0
+        compare_state(pluto, oracle, w, TOL_1STEP_MAXREL)
+        pluto.step(9)
+        assert oracle.step(9) == 0
+        compare_state(pluto, oracle, w, TOL_100STEP_L1REL)
+    finally:
+        pluto.set_integrator(2)
+        oracle.set_integrator(2)
 
 
 def test_ghost_layers_do_not_change_the_result(pluto):
@@ -815,6 +837,8 @@ def _variant_cases():
     return [
         ("3d_wrap64_minmod", lambda: wl.random_smooth(64, 10, 9, seed=81, limiter=0), 2, 2, 1),
         ("3d_wrap128_mc", lambda: wl.random_smooth(128, 6, 5, seed=82, limiter=1), 2, 2, 1),
+        ("3d_wrap96_rk3", lambda: wl.random_smooth(96, 7, 6, seed=89, limiter=0), 3, 2, 1),
+        ("2d_wrap192", lambda: wl.random_smooth(192, 9, 1, seed=90, limiter=1), 2, 2, 1),
         ("3d_chunk_ragged", lambda: wl.random_smooth(37, 13, 11, seed=83, limiter=1), 3, 2, 1),
         ("3d_two_chunks", lambda: wl.random_smooth(300, 5, 4, seed=84, limiter=0), 2, 2, 1),
         ("2d_wrap64", lambda: wl.random_smooth(64, 20, 1, seed=85, limiter=1), 2, 2, 1),
