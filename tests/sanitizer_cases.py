@@ -8,7 +8,7 @@ Every kernel variant of the library runs at least once on a grid of a few thousa
 sweep with a whole row per block (widths 64 and 128) and in chunk mode (128- and 256-thread blocks), 2D and
 3D, both limiters, the per-direction sweeps, WENO-Z, the TMA-staged and the per-thread CT kernel, RK2 and
 RK3, CUDA-graph replay and plain launches, the general and the row-only ghost fill, z slabs, host and
-device copies, the dt reduction with and without a bound grid.  No oracle, no comparison: the summaries
+device copies, the dt reduction with and without a bound grid, the UCT-HLLD kernels.  No oracle, no comparison: the summaries
 the tool prints are kept under profiles/.
 """
 import os
@@ -64,6 +64,16 @@ def main():
         run(sim, w)
     sim.set_integrator(2)
     print("ok: RK3, WENO-Z", flush=True)
+    # UCT-HLLD EMF average (reading R19): per-direction sweeps with hlld_t<true>, k_uct_halo, k_emf_uct, k_ct_update
+    sim.set_emf(1)
+    run(sim, wl.random_smooth(40, 9, 6, seed=13, limiter=1))
+    run(sim, wl.random_smooth(36, 11, 1, seed=14, limiter=0))
+    w = wl.random_smooth(24, 9, 8, seed=15)
+    w.limiter = 2
+    run(sim, w)
+    run(sim, wl.random_smooth(32, 8, 12, seed=16, limiter=1), nslab=2)
+    sim.set_emf(0)
+    print("ok: UCT-HLLD", flush=True)
     # device-pointer copies
     w = wl.random_smooth(64, 6, 5, seed=12)
     sim.load(w)
