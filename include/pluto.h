@@ -10,7 +10,7 @@
  *   flux-difference update     (Eq. 4; Fig. 2)
  *   constrained transport: upwind edge EMFs + face-B curl update (reading R6)
  * and once per step the RK2 combine (Eq. 5's increment form; reading R3) and the
- * CFL max-signal-speed reduction for dt (reading R8).  Readings R1..R18 are listed in DESIGN.md.
+ * CFL max-signal-speed reduction for dt (reading R8).  Readings R1..R20 are listed in DESIGN.md.
  * Beyond the north-star step: SSP-RK3 (Eq. 5 itself; PLUTO_OPT_RK_ORDER, reading R17) and WENO-Z
  * reconstruction ([51] named at PAPER.md:100,260; limiter PLUTO_WENOZ, reading R18).
  *
