@@ -154,3 +154,23 @@ def test_uct_poisoned_workspace_and_repeatability(uct):
             out = uct.get_state()
             assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
         uct.set_option(OPT_GRAPH, 1)
+
+
+def test_uct_config3_full_size_6_steps(uct, oracle):
+    """configs[3] (3D blast 256^3) in UCT-HLLD mode, in the launch configuration `bench.py --uct` times: six steps,
+    every element against the oracle at full size (~12 GB host)"""
+    w = wl.config(3)
+    uct.load(w)
+    oracle.load(w)
+    try:
+        assert oracle.set_emf(1) == 0
+        assert uct.get_dt() == oracle.get_dt()
+        uct.step(1)
+        assert oracle.step(1) == 0
+        compare_state(uct, oracle, w, TOL_1STEP_MAXREL)
+        uct.step(5)
+        assert oracle.step(5) == 0
+        compare_state(uct, oracle, w, TOL_100STEP_L1REL, norm=l1rel)
+        assert abs(uct.get_time() - oracle.get_time()) <= 1e-10 * oracle.get_time()
+    finally:
+        oracle.finalize()
