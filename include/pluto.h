@@ -197,7 +197,7 @@ enum { PLUTO_DIVB_CT = 0, PLUTO_DIVB_GLM = 1 };
  * reading R19 in DESIGN.md: the interface coefficients are the linear decomposition of the HLLD induction flux,
  * the edge value is composed from them with the run's reconstruction).  May be switched at any time outside a
  * step; the first step in UCT-HLLD mode allocates six more work arrays per slab with cudaMalloc (freed by
- * pluto_finalize); its sweeps run one kernel per direction.  Ignored by the GLM variant. */
+ * pluto_finalize).  Ignored by the GLM variant. */
 enum { PLUTO_EMF_CONTACT = 0, PLUTO_EMF_UCT_HLLD = 1 };
 int    pluto_set_psi(const double *psi);      /* [nz][ny][nx], host or device; GLM variant only */
 int    pluto_get_psi(double *psi);

@@ -760,10 +760,11 @@ constexpr int XY_SMEM_EXTRA(int nt) { return (nt + XY_BXROW_PAD) * 8 + 32; }   /
 
 // 128-thread blocks run three per SM at 168 registers (measured 17% faster than four at 128)
 constexpr int XY128_MINB = 3;
-template <int LIM, bool TWO_D, bool WRAP, int NT>
+// UCT: UCT-HLLD mode (R19): the five face numbers of hlld_t<true> go to ux / uy instead of the CT arrays.
+template <int LIM, bool TWO_D, bool WRAP, int NT, bool UCT>
 __global__ void __launch_bounds__(NT, NT == 128 ? XY128_MINB : 512 / NT)
 k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, const double *fin, double *__restrict__ ct,
-           StepParams *P, Combine cb, int seglen, int kz0)
+           StepParams *P, Combine cb, int seglen, int kz0, UctOut ux, UctOut uy)
 {
     extern __shared__ __align__(128) double xy_smem[];
     const int t = threadIdx.x;
@@ -942,14 +943,20 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, const double *f
                 }
             }
             Side L = { qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6] };
-            double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5;
+            double F[7] = { 0, 0, 0, 0, 0, 0, 0 }, w = 0.5, uctx[5] = { 0.5, 0, 0, 0, 0 };
             if (xface) {
                 Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-                hlld(L, R, rm[8 * NT], gamma, g.igm1, F, w);
+                hlld_t<UCT>(L, R, rm[8 * NT], gamma, g.igm1, F, w, uctx);
                 sQ[t] = F[0]; sQ[NT + t] = F[1]; sQ[2 * NT + t] = F[2]; sQ[3 * NT + t] = F[3]; sQ[4 * NT + t] = F[6];
                 if (TWO_D) sQ[5 * NT + t] = F[5];
             }
-            if (cell) {
+            if (UCT) {
+                if (cell) {
+                    const long long cm = c - st;
+#pragma unroll
+                    for (int m = 0; m < 5; m++) ux.p[m][cm] = uctx[m];
+                }
+            } else if (cell) {
                 const long long cm = c - st;
                 // cell-centred EMF  E^c = -(v x B)
                 const double e0 = qo[3] * qo[5] - qo[2] * qo[6], e1 = qo[1] * qo[6] - qo[3] * qo[4],
@@ -991,7 +998,12 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, const double *f
             if (cell) {
                 Side L = { qLy[0], qLy[1], qLy[2], qLy[3], qLy[4], qLy[5], qLy[6] };
                 Side R = { qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6] };
-                hlld(L, R, bface, gamma, g.igm1, Fy, wy);
+                double ucty[5];
+                hlld_t<UCT>(L, R, bface, gamma, g.igm1, Fy, wy, ucty);
+                if (UCT && s < s1) {
+#pragma unroll
+                    for (int m = 0; m < 5; m++) uy.p[m][c] = ucty[m];
+                }
             }
 #pragma unroll
             for (int v = 0; v < 7; v++) qLy[v] = nl[v];
@@ -1034,7 +1046,7 @@ k_sweep_xy(Grid g, const double *__restrict__ Sin, double *Sout, const double *f
                 Sout[7 * sa + cm] = fma(-facy, Fy[4] - Fpy[5], r7v);
             }
         }
-        if (cell && s < s1) {
+        if (!UCT && cell && s < s1) {
             ct[(CT_FEM + 2) * sa + c] = Fy[4];
             ct[(CT_FEM + 3) * sa + c] = Fy[5];
             ct[(CT_W + 1) * sa + c] = wy;

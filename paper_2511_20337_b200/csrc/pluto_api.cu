@@ -332,7 +332,7 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
     // moves from the HBM-bound z sweep to the ALU-bound x+y sweep.  Combine stages keep the x+y sweep first
     // (S^n has to be read either way, and the last writer of the step fills the dt bound grid: the z sweep).
     bool zfirst = false;
-    if constexpr (LIM != 2 && !TWO_D && !UCT) zfirst = C.fuse_xy && !cb.Sn;
+    if constexpr (LIM != 2 && !TWO_D) zfirst = C.fuse_xy && !cb.Sn;
     auto z_sweep = [&](const double *base) {
         const int bx = (g.n[0] + MARCH_NT - 1) / MARCH_NT;
         const int len = seglen_z(g);
@@ -347,7 +347,7 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         }
     };
     if (zfirst) z_sweep(Sin);
-    if constexpr (LIM != 2 && !UCT) if (C.fuse_xy) {
+    if constexpr (LIM != 2) if (C.fuse_xy) {
         fused = true;
         // fused x + y sweep: one block per x-row chunk and y-segment.  The block width is a template
         // parameter (shared-memory offsets become immediates): a whole periodic row when nx is one of
@@ -359,14 +359,14 @@ void launch_sweeps(const Domain &d, const double *Sin, double *Sout, Combine cb,
         const int len = seglen_y(g);
         dim3 grid(chunks, (g.n[1] + len - 1) / len, nplanes);
         const size_t smem = (size_t)XY_DOUBLES_PER_THREAD * nt * sizeof(double) + XY_SMEM_EXTRA(nt);
-        void (*k)(Grid, const double *, double *, const double *, double *, StepParams *, Combine, int, int) =
-            wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64> : nt == 96 ? k_sweep_xy<LIM, TWO_D, true, 96>
-                    : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128> : nt == 160 ? k_sweep_xy<LIM, TWO_D, true, 160>
-                    : nt == 192 ? k_sweep_xy<LIM, TWO_D, true, 192> : nt == 224 ? k_sweep_xy<LIM, TWO_D, true, 224>
-                    : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256> : k_sweep_xy<LIM, TWO_D, true, 512>)
-                 : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128> : k_sweep_xy<LIM, TWO_D, false, 256>);
+        void (*k)(Grid, const double *, double *, const double *, double *, StepParams *, Combine, int, int, UctOut, UctOut) =
+            wrap ? (nt == 64 ? k_sweep_xy<LIM, TWO_D, true, 64, UCT> : nt == 96 ? k_sweep_xy<LIM, TWO_D, true, 96, UCT>
+                    : nt == 128 ? k_sweep_xy<LIM, TWO_D, true, 128, UCT> : nt == 160 ? k_sweep_xy<LIM, TWO_D, true, 160, UCT>
+                    : nt == 192 ? k_sweep_xy<LIM, TWO_D, true, 192, UCT> : nt == 224 ? k_sweep_xy<LIM, TWO_D, true, 224, UCT>
+                    : nt == 256 ? k_sweep_xy<LIM, TWO_D, true, 256, UCT> : k_sweep_xy<LIM, TWO_D, true, 512, UCT>)
+                 : (nt == 128 ? k_sweep_xy<LIM, TWO_D, false, 128, UCT> : k_sweep_xy<LIM, TWO_D, false, 256, UCT>);
         cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, zfirst ? Sout : Sin, ct, C.P, cb, len, kz0));
+        LAUNCH(K_FLUX_XY, k<<<grid, nt, smem, s>>>(g, Sin, Sout, zfirst ? Sout : Sin, ct, C.P, cb, len, kz0, ux, uy));
     }
     if (!fused) {
         if constexpr (LIM == 2) {

@@ -1,6 +1,6 @@
 // uct.cuh -- constrained transport with the UCT-HLLD EMF average ([47] named at PAPER.md:271, reference entry
-// :640; reading R19 in DESIGN.md).  First version: the sweeps run one kernel per direction (hlld_t<true> leaves
-// a^L, d^L, d^R and the two transverse velocities on every face), then
+// :640; reading R19 in DESIGN.md).  The sweeps (fused x+y with PLM, one kernel per direction with WENO-Z) call
+// hlld_t<true>, which leaves a^L, d^L, d^R and the two transverse velocities on every face; then
 //   k_uct_halo   periodic x / y halos of the 15 face arrays (the reconstruction along a transverse direction
 //                reaches 2 cells with PLM, 3 with WENO-Z),
 //   k_emf_uct    the three edge EMFs, one thread per edge triple, into three work arrays,

@@ -112,6 +112,25 @@ def test_uct_slabs_match_the_single_domain_bit_for_bit(uct, nslab):
         assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
 
 
+@pytest.mark.parametrize("shape", [(64, 12, 9), (37, 13, 7), (96, 10, 1)])
+def test_uct_fused_and_per_direction_sweeps_agree(uct, shape):
+    """UCT-HLLD mode with the fused x+y sweep (PLM) against one kernel per direction"""
+    from paper_2511_20337_b200.binding import OPT_FUSE_XY
+    w = wl.random_smooth(*shape, seed=98, limiter=1)
+    uct.load(w)
+    uct.step(2)
+    Ua, Ba = uct.get_state()
+    old = uct.set_option(OPT_FUSE_XY, 0)
+    try:
+        uct.load(w)
+        uct.step(2)
+        Ub, Bb = uct.get_state()
+    finally:
+        uct.set_option(OPT_FUSE_XY, old)
+    assert maxrel(Ua.reshape(8, -1), Ub.reshape(8, -1)) <= 1e-13
+    assert maxrel(Ba[None], Bb[None]) <= 1e-13
+
+
 def test_leaving_the_mode_restores_the_default_path(pluto):
     w = wl.blast_3d(32)
     pluto.load(w)
