@@ -11,9 +11,10 @@
 // flux(B_n) = psi_m, flux(psi) = c_h^2 B_m, and the other seven fluxes are HLLD's with the normal field B_m.
 // c_h = cfl min_d(dx_d) / dt; after a full step psi *= exp(-dt c_h / c_r), c_r = 0.18 ([43]'s recommendation).
 //
-// One launch per direction and an elementwise combine (not fused like the CT path): along x a block works on a
-// row segment in shared memory (k_glm_sweep_x), along y and z a thread marches up its column (k_glm_march);
-// every interface is solved once.
+// One launch per direction (not fused like the CT path): along x a block works on a row segment in shared memory
+// (k_glm_sweep_x), along y and z a thread marches up its column (k_glm_march); every interface is solved once.  The
+// last sweep of a combine stage applies the Runge-Kutta combine (a7) and the damping of psi itself and, at the end
+// of a step, leaves the dt bound grid.
 #pragma once
 #include "kernels.cuh"
 
@@ -142,11 +143,18 @@ k_glm_sweep_x(Grid g, const double *__restrict__ Sin, const double *__restrict__
 // nine primitives in registers, every interface solved once per segment (+1 at the segment end), every zone
 // loaded and converted once -- the scheme of k_sweep_march (kernels.cuh) for the cell-centred variant.
 // DIR = 1: grid.y = segment, grid.z = k;  DIR = 2: grid.y = j, grid.z = segment.
-template <int DIR, int LIM, bool FIRST>
+// COMB: this is the last sweep of a combine stage: the zone's result wn * S^n + ws * (base - dt/dx dF) goes to
+// the stage's output arrays Fout / fpsout (which may be S^n itself: each value is read before the same thread
+// overwrites it), psi also takes the damping factor at the end of a step; no separate combine pass.  BOUND (z march
+// of the last stage): the dt upper bound of the zones a thread finishes, as in k_sweep_march.
+struct GlmCombine { double *Fout, *fpsout; const double *Sn, *psn; double wn, ws; int do_damp; };
+
+template <int DIR, int LIM, bool FIRST, bool COMB, bool BOUND>
 __global__ void __launch_bounds__(128, 2)
 k_glm_march(Grid g, const double *__restrict__ Sin, const double *__restrict__ psin, double *Sout, double *psout,
-            StepParams *P, int seglen)
+            StepParams *P, int seglen, GlmCombine cbg, BoundGrid bg)
 {
+    __shared__ double sbnd[BOUND ? 3 : 1][128];
     constexpr int T1 = (DIR + 1) % 3, T2 = (DIR + 2) % 3;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.n[0]) return;
@@ -159,6 +167,9 @@ k_glm_march(Grid g, const double *__restrict__ Sin, const double *__restrict__ p
     const double *base = FIRST ? Sin : Sout;
     const double *pbase = FIRST ? psin : psout;
     bool bad, anybad = false;
+    SigmaBound sb;
+    if (BOUND) sb.init(&sbnd[0][threadIdx.x], 128);
+    const double damp = (COMB && cbg.do_damp) ? P->glm_damp : 1.0;
     double q0[9], d0[9], qL[9];
     {
         double qm[9];
@@ -179,16 +190,18 @@ k_glm_march(Grid g, const double *__restrict__ Sin, const double *__restrict__ p
     double Fp[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };
     // software pipeline: the stored values of zone s+1 (and the update base of zone s-1) are loaded one
     // iteration before they are used, so the march does not stall on memory
-    double un[9], ub[9];
+    double un[9], ub[9], us[9];
     glm_load(g, Sin, psin, c + st, un);
     glm_load(g, base, pbase, c - st, ub);
+    if (COMB) glm_load(g, cbg.Sn, cbg.psn, c - st, us);
     for (int s = s0; s <= s1; s++, c += st) {
-        double q1[9], qR[9], F[9], uc[9], bc[9];
+        double q1[9], qR[9], F[9], uc[9], bc[9], sc[9];
 #pragma unroll
-        for (int v = 0; v < 9; v++) { uc[v] = un[v]; bc[v] = ub[v]; }
+        for (int v = 0; v < 9; v++) { uc[v] = un[v]; bc[v] = ub[v]; if (COMB) sc[v] = us[v]; }
         if (s < s1) {
             glm_load(g, Sin, psin, c + 2 * st, un);
             glm_load(g, base, pbase, c, ub);
+            if (COMB) glm_load(g, cbg.Sn, cbg.psn, c, us);
         }
         glm_convert<DIR>(g, uc, q1, bad);
         if (s + 1 < s1) anybad |= bad;
@@ -203,38 +216,36 @@ k_glm_march(Grid g, const double *__restrict__ Sin, const double *__restrict__ p
         glm_face_flux(L9, qR, ch, g.gamma, g.igm1, F);
         if (s > s0) {
             const long long cm = c - st;
-            Sout[cm] = fma(-dtdx, F[0] - Fp[0], bc[0]);
-            Sout[(1 + DIR) * sa + cm] = fma(-dtdx, F[1] - Fp[1], bc[1 + DIR]);
-            Sout[(1 + T1) * sa + cm] = fma(-dtdx, F[2] - Fp[2], bc[1 + T1]);
-            Sout[(1 + T2) * sa + cm] = fma(-dtdx, F[3] - Fp[3], bc[1 + T2]);
-            Sout[4 * sa + cm] = fma(-dtdx, F[6] - Fp[6], bc[4]);
-            Sout[(5 + DIR) * sa + cm] = fma(-dtdx, F[7] - Fp[7], bc[5 + DIR]);
-            Sout[(5 + T1) * sa + cm] = fma(-dtdx, F[4] - Fp[4], bc[5 + T1]);
-            Sout[(5 + T2) * sa + cm] = fma(-dtdx, F[5] - Fp[5], bc[5 + T2]);
-            psout[cm] = fma(-dtdx, F[8] - Fp[8], bc[8]);
+            // stored order: rho, m_x, m_y, m_z, E, B_x, B_y, B_z, psi; rotated flux: (rho, m_n, m_t1, m_t2, B_t1, B_t2, E, B_n, psi)
+            double r[9];
+            r[0] = fma(-dtdx, F[0] - Fp[0], bc[0]);
+            r[1 + DIR] = fma(-dtdx, F[1] - Fp[1], bc[1 + DIR]);
+            r[1 + T1] = fma(-dtdx, F[2] - Fp[2], bc[1 + T1]);
+            r[1 + T2] = fma(-dtdx, F[3] - Fp[3], bc[1 + T2]);
+            r[4] = fma(-dtdx, F[6] - Fp[6], bc[4]);
+            r[5 + DIR] = fma(-dtdx, F[7] - Fp[7], bc[5 + DIR]);
+            r[5 + T1] = fma(-dtdx, F[4] - Fp[4], bc[5 + T1]);
+            r[5 + T2] = fma(-dtdx, F[5] - Fp[5], bc[5 + T2]);
+            r[8] = fma(-dtdx, F[8] - Fp[8], bc[8]);
+            if (COMB) {
+#pragma unroll
+                for (int v = 0; v < 9; v++) r[v] = fma(cbg.wn, sc[v], cbg.ws * r[v]);
+                if (cbg.do_damp) r[8] *= damp;
+#pragma unroll
+                for (int v = 0; v < 8; v++) cbg.Fout[v * sa + cm] = r[v];
+                cbg.fpsout[cm] = r[8];
+            } else {
+#pragma unroll
+                for (int v = 0; v < 8; v++) Sout[v * sa + cm] = r[v];
+                psout[cm] = r[8];
+            }
+            if (BOUND) sb.add(g, r[0], r[1], r[2], r[3], r[4]);
         }
 #pragma unroll
         for (int v = 0; v < 9; v++) Fp[v] = F[v];
     }
     if (anybad) P->err = 1;
-}
-
-// Runge-Kutta combine of the nine arrays (a7), out <- wn * S^n + ws * S~ with S~ = Euler(S) in scratch arrays
-// (out may be S^n itself: in place), and, at the end of a step, the exact damping of psi
-// (glm_damp = exp(-dt c_h / c_r) from the device scalars)
-__global__ void __launch_bounds__(128)
-k_glm_combine(Grid g, double *Sout, double *psout, const double *Sn, const double *psn,
-              const double *__restrict__ St, const double *__restrict__ pst,
-              double wn, double ws, int do_damp, const StepParams *__restrict__ P)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-    if (i >= g.n[0]) return;
-    const long long sa = g.sa, c = g.at(i, j, k);
-#pragma unroll
-    for (int v = 0; v < 8; v++) Sout[v * sa + c] = fma(wn, Sn[v * sa + c], ws * St[v * sa + c]);
-    double ps = fma(wn, psn[c], ws * pst[c]);
-    if (do_damp) ps *= P->glm_damp;
-    psout[c] = ps;
+    if (BOUND) bound_publish(bg, DIR == 1 ? s0 : tr, DIR == 1 ? tr : s0, sb.value(g, bg.cfac));
 }
 
 } // namespace pluto

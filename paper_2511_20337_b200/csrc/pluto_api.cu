@@ -482,19 +482,26 @@ void enqueue_stage_glm(int in, int out, int sn, double wn, double ws, bool last)
     const dim3 grid((g.n[0] + 127) / 128, g.n[1], g.n[2]);
     const dim3 gx((g.n[0] + GLMX_NT - 5) / (GLMX_NT - 4), g.n[1], g.n[2]);
     LAUNCH(K_FLUX_X, k_glm_sweep_x<LIM, true><<<gx, GLMX_NT, 0, s>>>(g, arr(d, in), psin, So, po, C.P));
+    // the last sweep of a combine stage writes wn * S^n + ws * Euler(S) (and damps psi at the end of a step) itself;
+    // the z march of the last stage also leaves the dt bound grid
+    const bool comb = sn >= 0, three_d = g.act[2] != 0;
+    GlmCombine cg{};
+    if (comb) cg = GlmCombine{ arr(d, out), arr(d, glm_psi(out)), arr(d, sn), arr(d, glm_psi(sn)), wn, ws, last ? 1 : 0 };
+    const BoundGrid none = bound_grid(d, false, 1, 1);
     {
         const int len = seglen_y(g);
         const dim3 gy((g.n[0] + 127) / 128, (g.n[1] + len - 1) / len, g.n[2]);
-        LAUNCH(K_FLUX_Y, k_glm_march<1, LIM, false><<<gy, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len));
+        if (comb && !three_d) LAUNCH(K_FLUX_Y, k_glm_march<1, LIM, false, true, false><<<gy, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len, cg, none));
+        else                  LAUNCH(K_FLUX_Y, k_glm_march<1, LIM, false, false, false><<<gy, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len, cg, none));
     }
-    if (g.act[2]) {
+    if (three_d) {
         const int len = seglen_z(g);
         const dim3 gz((g.n[0] + 127) / 128, g.n[1], (g.n[2] + len - 1) / len);
-        LAUNCH(K_FLUX_Z, k_glm_march<2, LIM, false><<<gz, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len));
+        const BoundGrid bg = final_bound_grid(d, last);
+        if (comb && last) LAUNCH(K_FLUX_Z, k_glm_march<2, LIM, false, true, true><<<gz, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len, cg, bg));
+        else if (comb)    LAUNCH(K_FLUX_Z, k_glm_march<2, LIM, false, true, false><<<gz, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len, cg, none));
+        else              LAUNCH(K_FLUX_Z, k_glm_march<2, LIM, false, false, false><<<gz, 128, 0, s>>>(g, arr(d, in), psin, So, po, C.P, len, cg, none));
     }
-    if (sn >= 0)
-        LAUNCH(K_SCALAR, k_glm_combine<<<grid, 128, 0, s>>>(g, arr(d, out), arr(d, glm_psi(out)), arr(d, sn), arr(d, glm_psi(sn)),
-                                                          So, po, wn, ws, last ? 1 : 0, C.P));
 }
 
 void enqueue_stage(int in, int out, int sn, double wn, double ws, bool last, double *dbg = nullptr)
@@ -542,7 +549,6 @@ void enqueue_dtmax(bool keep_bounds)
 {
     for (const Domain &d : C.dom) {
         BoundGrid bg = final_bound_grid(d, true);
-        if (C.glm) bg.b = nullptr;               // the GLM sweeps leave no bound grid
         LAUNCH(K_DTMAX, launch_dtmax(d.g, arr(d, A_SA), C.P, bg, C.glm ? 1 : 0, C.sm_count * 8, C.stream));
     }
     if (!keep_bounds)
