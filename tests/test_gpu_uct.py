@@ -30,6 +30,9 @@ CASES = [
     ("wenoz_2d_rk3", lambda: _wz(wl.orszag_tang_2d(48)), 3, 3),
     ("wenoz_3d_rk3", lambda: _wz(wl.random_smooth(20, 18, 16, seed=93)), 3, 3),
     ("ot3d_32_wenoz_rk3", lambda: _wz(wl.orszag_tang_3d(32, noise=1e-3)), 3, 3),
+    ("tiny_3d", lambda: wl.random_smooth(4, 3, 2, seed=99, limiter=1), 2, 2),
+    ("tiny_2d_ghost4", lambda: wl.random_smooth(5, 4, 1, seed=101, limiter=0), 3, 4),
+    ("tiny_wenoz", lambda: _wz(wl.random_smooth(6, 3, 3, seed=102)), 2, 3),
 ]
 
 
