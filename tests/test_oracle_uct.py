@@ -247,3 +247,52 @@ def test_blast_at_rest_is_well_conditioned(oracle):
             scale = max(np.abs(states[0][0][a]).max() for a in (1, 2, 3))
         assert np.abs(states[0][0][v] - states[1][0][v]).max() <= 1e-10 * scale, v
     assert np.abs(states[0][1] - states[1][1]).max() <= 1e-10 * np.abs(states[0][1]).max()
+
+
+def _rotate90(U, Bf, n):
+    """the 2D state on an n x n periodic unit square rotated by +90 degrees: point (x, y) -> (1 - y, x), vectors
+    (a_x, a_y) -> (-a_y, a_x); cell (i, j) -> (n - 1 - j, i), y-face (i, j - 1/2) -> x-face (n - j, i) with
+    b_x' = -b_y, x-face (i - 1/2, j) -> y-face (n - 1 - j, i) with b_y' = b_x"""
+    f = wl.split_faces(Bf, n, n, 1)
+    Ur = np.empty_like(U)
+    rot = lambda a: np.ascontiguousarray(a[0].T[:, ::-1])[None]           # q'[j' = i][i' = n-1-j] = q[j][i]
+    for v in (0, 3, 6, 7):
+        Ur[v] = rot(U[v])
+    Ur[1], Ur[2] = -rot(U[2]), rot(U[1])
+    Ur[4], Ur[5] = -rot(U[5]), rot(U[4])
+    bx, by = f["bx"][0], f["by"][0]                                      # [n][n+1], [n+1][n]
+    bxr = np.empty_like(bx)
+    byr = np.empty_like(by)
+    for j in range(n + 1):
+        bxr[:, n - j] = -by[j, :]                                         # bx'[j' = i][n - j] = -by[j][i]
+    for j in range(n):
+        byr[:, n - 1 - j] = bx[j, :]                                      # by'[j'_f = i][i' = n-1-j] = bx[j][i]
+    return Ur, wl.join_faces({"bx": bxr[None], "by": byr[None]}, n, n, 1)
+
+
+@pytest.mark.parametrize("emf", [0, 1])
+def test_quarter_turn_covariance(oracle, emf):
+    """the scheme commutes with a rotation of the square grid by 90 degrees: the orientation and the signs of the
+    two-dimensional edge composition (both rules) are consistent between the x and the y direction"""
+    n = 24
+    w = wl.random_smooth(n, n, 1, seed=31, limiter=1, amp=0.3, box=(1.0, 1.0, 1.0))
+    oracle.load(w)
+    oracle.set_emf(emf)
+    dts = []
+    for _ in range(6):
+        assert oracle.step(1) == 0
+        dts.append(oracle.get_dt())
+    Ua, Ba = oracle.get_state()
+    Ur0, Br0 = _rotate90(w.U, w.Bface, n)
+    assert oracle.init(n, n, 1, 2, w.gamma, w.cfl, 1) == 0
+    oracle.set_emf(emf)
+    oracle.set_box(1.0, 1.0, 1.0)
+    oracle.set_state(Ur0, Br0)
+    for dt in dts:
+        assert oracle.step_fixed_dt(1, dt) == 0
+    Ub, Bb = oracle.get_state()
+    oracle.set_emf(0)
+    Ue, Be = _rotate90(Ua, Ba, n)
+    assert np.abs(Ub - Ue).max() <= 1e-12 * np.abs(Ue).max()
+    assert np.abs(Bb - Be).max() <= 1e-12 * np.abs(Be).max()
+    assert np.abs(Ua - w.U).max() > 1e-3                                  # something happened
