@@ -296,3 +296,40 @@ def test_quarter_turn_covariance(oracle, emf):
     assert np.abs(Ub - Ue).max() <= 1e-12 * np.abs(Ue).max()
     assert np.abs(Bb - Be).max() <= 1e-12 * np.abs(Be).max()
     assert np.abs(Ua - w.U).max() > 1e-3                                  # something happened
+
+
+@pytest.mark.parametrize("emf", [0, 1])
+def test_cyclic_permutation_of_the_axes_3d(oracle, emf):
+    """a genuinely 3D state with the axes renamed cyclically (new x = old y, new y = old z, new z = old x) advances
+    to the renamed result: all three EMF components are one formula under the cyclic map (both rules)"""
+    w = wl.random_smooth(10, 8, 6, seed=41, limiter=1, amp=0.3, box=(1.0, 0.8, 0.6))
+    oracle.load(w)
+    oracle.set_emf(emf)
+    dts = []
+    for _ in range(4):
+        assert oracle.step(1) == 0
+        dts.append(oracle.get_dt())
+    Ua, Ba = oracle.get_state()
+
+    def rename(U, Bf):
+        f = wl.split_faces(Bf, w.nx, w.ny, w.nz)
+        tr = lambda a: np.ascontiguousarray(np.transpose(a, (2, 0, 1)))       # q'[i][k][j] = q[k][j][i]
+        Ur = np.empty((8, w.nx, w.nz, w.ny))
+        Ur[0], Ur[7] = tr(U[0]), tr(U[7])
+        for base in (1, 4):                                                    # a'_x = a_y, a'_y = a_z, a'_z = a_x
+            Ur[base + 0], Ur[base + 1], Ur[base + 2] = tr(U[base + 1]), tr(U[base + 2]), tr(U[base + 0])
+        faces = {"bx": tr(f["by"]), "by": tr(f["bz"]), "bz": tr(f["bx"])}
+        return Ur, wl.join_faces(faces, w.ny, w.nz, w.nx)
+    Ur0, Br0 = rename(w.U, w.Bface)
+    assert oracle.init(w.ny, w.nz, w.nx, 2, w.gamma, w.cfl, 1) == 0
+    oracle.set_emf(emf)
+    oracle.set_box(w.box[1], w.box[2], w.box[0])
+    oracle.set_state(Ur0, Br0)
+    for dt in dts:
+        assert oracle.step_fixed_dt(1, dt) == 0
+    Ub, Bb = oracle.get_state()
+    oracle.set_emf(0)
+    Ue, Be = rename(Ua, Ba)
+    assert np.abs(Ub - Ue).max() <= 1e-12 * np.abs(Ue).max()
+    assert np.abs(Bb - Be).max() <= 1e-12 * np.abs(Be).max()
+    assert np.abs(Ua - w.U).max() > 1e-3
