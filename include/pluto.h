@@ -203,6 +203,43 @@ int    pluto_set_psi(const double *psi);      /* [nz][ny][nx], host or device; G
 int    pluto_get_psi(double *psi);
 int    pluto_set_option(int opt, int value);
 
+/* pluto_cfl_dt_noalloc -- the CFL time step (reading R8; the same rule as pluto_get_dt) of a state the CALLER
+ * holds, computed without the library allocating anything: no context, no pluto_init, no cudaMalloc / cudaFree,
+ * no allocating library routine.
+ *
+ * Who needs it: a host code that gives all device memory to its own pool when it starts (an AMR framework's
+ * arena, a caching allocator run close to the full HBM) cannot rely on a library-side cudaMalloc succeeding;
+ * and a caller inside a latency-critical loop cannot pay for the device-wide synchronisation cudaMalloc and
+ * cudaFree bring.  pluto_init / pluto_get_dt allocate (or need a registered workspace of many arrays); this
+ * call needs only the caller's own input and output.
+ *
+ *   U_dev   : DEVICE pointer, 8*nz*ny*nx doubles in the layout of pluto_get_state's U (interior zones only,
+ *             cell-centred B in U[4..6]); only read
+ *   nx,ny,nz: zones (nx >= 2, ny >= 2, nz >= 1; 2D when nz == 1); Lx,Ly,Lz: box lengths, dx_d = L_d / n_d (R11)
+ *   out_dev : DEVICE pointer to 3 doubles the caller owns: out[0] = dt = cfl / max, out[1] = the maximum of
+ *             (|v_d| + c_f,d) / dx_d over zones and active d, out[2] = 1.0 if a zone with non-positive or
+ *             non-finite density / pressure was met (R13), else 0.0
+ *   cuda_stream : cudaStream_t to enqueue on (NULL: the default stream).  The call only enqueues (one memset
+ *             and two kernels) and does not wait: synchronise the stream before reading out_dev.
+ * For the same state, box, gamma and cfl, out[0] is bit-identical to pluto_get_dt() (R15).
+ *
+ * The scratch in between (one partial maximum per row of nx zones, plus a flag word) is a fixed array inside
+ * the library's device image: PLUTO_NOALLOC_SCRATCH_BYTES (1 MiB + 256 B) on every GPU that loads the library,
+ * held until the process exits.  Hence the limit ny * nz <= PLUTO_NOALLOC_MAX_ROWS (256^3 is 65 536 rows,
+ * 2048^2 is 2 048): larger boxes are refused with PLUTO_ENOMEM and a message in pluto_last_error; nothing is
+ * launched.  Every call on a device uses the same array and finds the previous call's contents in it: the call
+ * clears the flag word itself and overwrites every row maximum before reading it, so consecutive calls on one
+ * stream are independent -- but two calls that may run at the same time on one GPU (different streams, or
+ * different host threads) race on it and must be ordered by the caller.
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current) and keeps it; make that first call outside any stream capture.
+ * Errors: PLUTO_EINVAL (NULL pointer, sizes, lengths, gamma, cfl), PLUTO_ENOMEM (more rows than the scratch
+ * holds), PLUTO_ECUDA (no device -- there is no CPU fallback -- or a CUDA runtime error). */
+#define PLUTO_NOALLOC_MAX_ROWS      131072
+#define PLUTO_NOALLOC_SCRATCH_BYTES ((PLUTO_NOALLOC_MAX_ROWS + 32) * 8)
+int    pluto_cfl_dt_noalloc(const double *U_dev, int nx, int ny, int nz, double Lx, double Ly, double Lz,
+                            double gamma, double cfl, double *out_dev, void *cuda_stream);
+
 /* One Euler stage S -> S + L(S) from the CURRENT state with the given dt, for per-kernel parity
  * tests; the state is not advanced.  Any pointer may be NULL (host or device pointers).
  *   U1, Bf1 : layouts of U / Bface

@@ -35,7 +35,9 @@ SYMBOLS = [
     "pluto_probe_fp64_gflops",
     "pluto_init_slabs", "pluto_workspace_bytes_slabs", "pluto_local_planes", "pluto_export_slab",
     "pluto_attach_peer", "pluto_fill_ghosts", "pluto_slab_planes", "pluto_set_psi", "pluto_get_psi", "pluto_step_begin", "pluto_dt_max_bits", "pluto_step_stage",
+    "pluto_cfl_dt_noalloc",
 ]
+NOALLOC_MAX_ROWS = 131072          # PLUTO_NOALLOC_MAX_ROWS of include/pluto.h
 
 
 class PlutoError(RuntimeError):
@@ -87,6 +89,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pluto_step_stage.argtypes = [i32, i32]
     L.pluto_set_psi.argtypes = [vp]
     L.pluto_get_psi.argtypes = [vp]
+    L.pluto_cfl_dt_noalloc.argtypes = [vp, i32, i32, i32, dbl, dbl, dbl, dbl, dbl, vp, vp]
     return L
 
 
@@ -224,6 +227,19 @@ class Pluto:
 
     def finalize(self):
         return self.L.pluto_finalize()
+
+    def cfl_dt_noalloc(self, U, box, gamma, cfl, out, stream=None):
+        """pluto_cfl_dt_noalloc: the CFL dt of a state the caller holds, for callers whose memory is all in their
+        own pool (the library allocates nothing here; its scratch is a fixed array inside the library, which is why
+        ny * nz may not exceed NOALLOC_MAX_ROWS).  U: CUDA float64 tensor [8][nz][ny][nx] as get_state returns it;
+        out: CUDA float64 tensor of 3 (dt, max signal speed / dx, unphysical flag), written asynchronously on
+        `stream` (a torch.cuda.Stream; default: this object's stream) -- synchronise it before reading out.
+        Calls that could overlap on the GPU share the scratch and must be ordered by the caller."""
+        assert U.is_cuda and out.is_cuda and U.dim() == 4 and U.shape[0] == 8 and out.numel() >= 3
+        _, nz, ny, nx = U.shape
+        s = self.stream if stream is None else stream
+        return self._check(self.L.pluto_cfl_dt_noalloc(_addr(U), nx, ny, nz, box[0], box[1], box[2], gamma, cfl,
+                                                       _addr(out), s.cuda_stream))
 
     def set_emf(self, mode):
         """EMF average of the CT step: EMF_CONTACT (default, reading R6) or EMF_UCT_HLLD (reading R19)"""

@@ -6,7 +6,9 @@
 // block shared memory -> atomicMax on the bit pattern (all candidates are positive doubles, for
 // which the IEEE ordering equals the unsigned integer ordering of the bits).
 #include "grid.h"
+#include "../../include/pluto.h"
 #include <cuda_runtime.h>
+#include <mutex>
 
 namespace pluto {
 
@@ -264,3 +266,146 @@ double probe_fp64_gflops(cudaStream_t s)
 }
 
 } // namespace pluto
+
+// ---------------------------------------------------------------- pluto_cfl_dt_noalloc (include/pluto.h)
+// The CFL reduction above, for callers that must not let this library allocate: a host application that
+// hands every byte of device memory to its own pool at start-up (an AMR framework's arena, a caching
+// allocator run at a high memory fraction) cannot count on a cudaMalloc inside a library succeeding, and
+// one that calls from a latency-critical loop cannot afford the device-wide synchronisation that
+// cudaMalloc / cudaFree imply.  pluto_init needs a context (state arrays, scalars, bound grid); this entry
+// point needs none: the caller passes its own state and its own output, and the only memory in between --
+// one partial maximum per row of zones plus a flag word -- lives in the file-scope array below, which is
+// part of the loaded module on every device (PLUTO_NOALLOC_SCRATCH_BYTES, held until the process exits).
+//
+// The per-zone candidate is zone_sigma_exact() of this file, so for the same state the dt is bit-identical
+// to pluto_get_dt().  There are no filters here: every zone takes the IEEE evaluation.
+namespace pluto { int report_error(int code, const char *fmt, ...); }
+
+namespace {
+
+constexpr int kNoallocMaxRows = PLUTO_NOALLOC_MAX_ROWS;
+constexpr int kNoallocHeader = 32;                         // 256 bytes in front of the row maxima: [0] = unphysical-zone flag
+static_assert((kNoallocMaxRows + kNoallocHeader) * 8 == PLUTO_NOALLOC_SCRATCH_BYTES, "header and limit disagree");
+
+// Scratch of pluto_cfl_dt_noalloc.  In HOST code this name is only a handle for cudaGetSymbolAddress (passing
+// it to a kernel would hand the kernel a host address); noalloc_scratch() below resolves the device address.
+static __device__ __align__(256) unsigned long long g_noalloc_scratch[kNoallocMaxRows + kNoallocHeader];
+
+// One warp per row of nx zones of the caller's unpadded state U[8][nz][ny][nx] (cell-centred B in U[4..6]).
+// Writes the row's maximum candidate (bit pattern of a non-negative double) to scratch[header + row].
+__global__ void __launch_bounds__(256)
+k_rowmax_noalloc(pluto::Grid g, const double *__restrict__ U, unsigned long long *__restrict__ scratch)
+{
+    const int nx = g.n[0];
+    const long long nrows = (long long)g.n[1] * g.n[2];
+    const long long zones = nrows * nx;
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const long long nwarps = (long long)gridDim.x * (blockDim.x >> 5);
+    int bad = 0;
+    for (long long row = warp0; row < nrows; row += nwarps) {
+        const double *__restrict__ r = U + row * nx;
+        double smax = 0.0;
+        for (int i = lane; i < nx; i += 32) {
+            const double B[3] = { r[4 * zones + i], r[5 * zones + i], r[6 * zones + i] };
+            const double sig = pluto::zone_sigma_exact(g, r[i], r[zones + i], r[2 * zones + i], r[3 * zones + i],
+                                                       r[7 * zones + i], B, bad);
+            if (sig > smax) smax = sig;
+        }
+        for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+        if (lane == 0) scratch[kNoallocHeader + row] = (unsigned long long)__double_as_longlong(smax);
+    }
+    if (bad) scratch[0] = 1ull;
+}
+
+// One block: the maximum of the row maxima, then out[0] = dt = cfl / max, out[1] = max, out[2] = 1.0 if a zone
+// with non-positive or non-finite density / pressure was met (else 0.0).
+__global__ void __launch_bounds__(1024)
+k_finish_noalloc(double cfl, long long nrows, const unsigned long long *__restrict__ scratch, double *__restrict__ out)
+{
+    __shared__ unsigned long long sm[32];
+    unsigned long long m = 0ull;                            // candidates are non-negative: bit order = value order
+    for (long long r = threadIdx.x; r < nrows; r += blockDim.x) {
+        const unsigned long long v = scratch[kNoallocHeader + r];
+        if (v > m) m = v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long v = __shfl_xor_sync(0xffffffffu, m, o);
+        if (v > m) m = v;
+    }
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); w++) if (sm[w] > m) m = sm[w];
+        const double smax = __longlong_as_double((long long)m);
+        out[0] = cfl / smax;
+        out[1] = smax;
+        out[2] = scratch[0] ? 1.0 : 0.0;
+    }
+}
+
+// Device address of g_noalloc_scratch on the CURRENT device, resolved once per device ordinal.
+unsigned long long *noalloc_scratch(int dev, cudaError_t &err)
+{
+    constexpr int kMaxDevices = 64;
+    static std::mutex mu;
+    static unsigned long long *addr[kMaxDevices] = {};
+    err = cudaSuccess;
+    if (dev < 0 || dev >= kMaxDevices) { err = cudaErrorInvalidDevice; return nullptr; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void *p = nullptr;
+        err = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (err != cudaSuccess) return nullptr;
+        addr[dev] = (unsigned long long *)p;
+    }
+    return addr[dev];
+}
+
+} // namespace
+
+extern "C" int pluto_cfl_dt_noalloc(const double *U_dev, int nx, int ny, int nz, double Lx, double Ly, double Lz,
+                                    double gamma, double cfl, double *out_dev, void *cuda_stream)
+{
+    using pluto::report_error;
+    if (!U_dev || !out_dev) return report_error(PLUTO_EINVAL, "pluto_cfl_dt_noalloc: U_dev and out_dev must be device pointers, not NULL");
+    if (nx < 2 || ny < 2 || nz < 1) return report_error(PLUTO_EINVAL, "pluto_cfl_dt_noalloc: needs nx >= 2, ny >= 2, nz >= 1");
+    if (!(Lx > 0.0) || !(Ly > 0.0) || !(Lz > 0.0) || !(gamma > 1.0) || !(cfl > 0.0))
+        return report_error(PLUTO_EINVAL, "pluto_cfl_dt_noalloc: box lengths and cfl must be positive, gamma > 1");
+    const long long nrows = (long long)ny * nz;
+    if (nrows > kNoallocMaxRows)
+        return report_error(PLUTO_ENOMEM, "pluto_cfl_dt_noalloc: ny * nz = %lld rows exceed the built-in scratch of "
+                            "PLUTO_NOALLOC_MAX_ROWS = %d rows (this entry point never allocates; use pluto_init / "
+                            "pluto_get_dt for larger boxes)", nrows, kNoallocMaxRows);
+    int dev = -1, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return report_error(PLUTO_ECUDA, "pluto_cfl_dt_noalloc: no CUDA device (%s): there is no CPU fallback", cudaGetErrorString(e));
+    unsigned long long *scratch = noalloc_scratch(dev, e);
+    if (!scratch) return report_error(PLUTO_ECUDA, "pluto_cfl_dt_noalloc: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) sms = 148;
+
+    pluto::Grid g{};
+    const int n[3] = { nx, ny, nz };
+    const double L[3] = { Lx, Ly, Lz };
+    for (int a = 0; a < 3; a++) {
+        g.n[a] = n[a];
+        g.act[a] = n[a] > 1;
+        g.dx[a] = L[a] / n[a];                // the arithmetic of pluto_set_box, so that 1/dx agrees to the bit
+        g.idx[a] = 1.0 / g.dx[a];
+    }
+    g.gamma = gamma;
+    g.cfl = cfl;
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // the flag word keeps the previous call's value: it has to start at zero (the row maxima need no clearing,
+    // every row this call reads is written by this call first)
+    e = cudaMemsetAsync(scratch, 0, kNoallocHeader * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return report_error(PLUTO_ECUDA, "pluto_cfl_dt_noalloc: cudaMemsetAsync: %s", cudaGetErrorString(e));
+    const long long want = (nrows + 7) / 8;                                  // 8 warps per block, one row per warp
+    const int blocks = (int)(want < (long long)sms * 8 ? want : (long long)sms * 8);
+    k_rowmax_noalloc<<<blocks, 256, 0, s>>>(g, U_dev, scratch);
+    k_finish_noalloc<<<1, 1024, 0, s>>>(cfl, nrows, scratch, out_dev);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return report_error(PLUTO_ECUDA, "pluto_cfl_dt_noalloc: launch: %s", cudaGetErrorString(e));
+    return PLUTO_OK;
+}

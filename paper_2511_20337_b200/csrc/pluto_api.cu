@@ -877,6 +877,19 @@ int set_state_glm(const double *U)
 
 } // namespace
 
+// error reporting for the entry points that live in other translation units (dt_kernel.cu): same buffer as
+// fail(), read back with pluto_last_error
+namespace pluto {
+int report_error(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(C.err, sizeof C.err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+}
+
 // ================================================================== C ABI
 
 extern "C" {
