@@ -8,6 +8,10 @@ flux update, CT, RK2 combine, dt reduction) over the whole grid of the workload.
 N = 1 is BASELINE.json configs[3] (3D MHD blast 256^3, minmod, CFL 0.3): the configuration the
 north_star's target is quoted on.  Inputs are seeded and synthetic (paper_2511_20337_b200.workloads).
 
+`python bench.py --gpus N` with N > 1 re-executes itself under torch.distributed.run (one rank per GPU) when no
+launcher set WORLD_SIZE, and refuses when the box has fewer than N devices.  `--gpus 1 --slab-path` times the
+same decomposed code path as a one-rank NCCL group.
+
 Prints ONE JSON line (rank 0).  Timing: CUDA events on the library's stream, barrier +
 synchronize on both sides, max over ranks.  The state (>= 1 GB) is larger than L2 (126 MB), so no
 explicit flush is needed between steps.
@@ -286,6 +290,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--repeats", type=int, default=3, help="timed repeats of the K steps (median and best reported)")
     ap.add_argument("--no-sustained", action="store_true", help="skip the one-second sustained-stepping figure")
+    ap.add_argument("--slab-path", action="store_true",
+                    help="with --gpus 1: time the z-slab decomposed step (the N > 1 code path: SlabPluto, NCCL collectives on "
+                         "the library's stream) with the whole box as the single slab of a one-rank group")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -294,12 +301,20 @@ def main():
     from paper_2511_20337_b200 import workloads as wl
     from paper_2511_20337_b200.binding import Pluto
 
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        return respawn_under_torchrun(args)          # plain `python bench.py --gpus N`: start the N ranks ourselves
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
-    if world > 1:
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU")
+    if world > torch.cuda.device_count():
+        raise SystemExit(f"bench.py: --gpus {world} needs {world} CUDA devices, this box has {torch.cuda.device_count()}")
+    if world > 1 or args.slab_path:
+        if "WORLD_SIZE" not in os.environ:           # --gpus 1 --slab-path: a one-rank NCCL group in this process
+            os.environ.update({"MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(free_port()), "RANK": "0", "WORLD_SIZE": "1"})
         return main_slabs(args, rank, world, local)
 
     w = wl.config(args.config)
@@ -470,6 +485,27 @@ def main():
     print(json.dumps(line))
 
 
+def free_port():
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` with N > 1 and no launcher: re-execute under torch.distributed.run, one rank per
+    GPU of this node; refuse loudly when the box has fewer devices (never time one GPU and call it N)"""
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, this box has {have}")
+    os.environ.setdefault("NCCL_DEBUG", "INFO")      # the log names the ranks and the transport (NVLS / P2P)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__), *sys.argv[1:]]
+    sys.stdout.flush()
+    os.execv(sys.executable, cmd)
+
+
 def main_slabs(args, rank, world, local):
     """N > 1: one z slab per rank (paper_2511_20337_b200.distributed.SlabPluto), weak scaling"""
     import torch
@@ -477,6 +513,7 @@ def main_slabs(args, rank, world, local):
     from paper_2511_20337_b200 import workloads as wl
     from paper_2511_20337_b200.distributed import SlabPluto
 
+    torch.cuda.set_device(local)
     dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if args.config not in (3, 4):
         raise SystemExit("--gpus N > 1 times the weak-scaling blast: per-GPU mesh and scheme of configs[3] (default) or configs[4]")

@@ -60,6 +60,8 @@ enum { PLUTO_MINMOD = 0, PLUTO_MC = 1, PLUTO_WENOZ = 2 };
  * Lx = 1 (override with pluto_set_box).  nx >= 2 and ny >= 2 (2D when nz == 1, 3D when nz >= 2); every
  * active extent >= ghost.  ghost = layers kept around the padded device arrays: >= 2 for PLM, >= 3 for
  * WENO-Z (R9), at most 16.  gamma > 1, cfl > 0 (R8), limiter = PLUTO_MINMOD | PLUTO_MC | PLUTO_WENOZ (R4, R18).
+ * A call rejected with PLUTO_EINVAL (or PLUTO_ENOMEM for a registered workspace that is too small) leaves the
+ * previous context untouched; once the arguments are accepted the previous context is released first.
  * Memory: allocates pluto_workspace_bytes(...) of device memory itself unless a workspace of at least that
  * size was registered with pluto_set_workspace (then the caller keeps ownership and must keep it alive
  * until pluto_finalize).  Errors: PLUTO_ECUDA (no device: there is no CPU fallback), PLUTO_EINVAL
@@ -162,21 +164,6 @@ int    pluto_step_stage(int stage, int fixed);
 int    pluto_step_async(int nsteps);
 int    pluto_sync(void);
 
-/* Number of kernel launches enqueued by this library since pluto_init (for bench.py's gpu_launches). */
-long long pluto_launch_count(void);
-
-/* Per-kernel device timing with CUDA events on the launching stream (for bench.py's roofline).
- * pluto_profile(1) starts (plain launches, every launch bracketed by an event pair), pluto_profile(0)
- * stops.  pluto_profile_get returns the accumulated time and launch count of kernel class `kernel`
- * (0 <= kernel, pluto_kernel_name(kernel) != NULL). */
-int    pluto_profile(int on);
-int    pluto_profile_get(int kernel, double *total_ms, long long *launches);
-const char *pluto_kernel_name(int kernel);
-
-/* Measured fp64 FMA throughput of the device in GFLOP/s (2 flops per DFMA): a register-resident
- * DFMA loop on every SM, timed with CUDA events.  The denominator of the "alu" roofline. */
-double pluto_probe_fp64_gflops(void);
-
 /* Tuning switches: opt = PLUTO_OPT_*, returns the previous value or PLUTO_EINVAL. */
 enum {
     PLUTO_OPT_GRAPH = 1,   /* 1 (default): replay one captured CUDA graph per step; 0: plain launches */
@@ -240,15 +227,8 @@ int    pluto_set_option(int opt, int value);
 int    pluto_cfl_dt_noalloc(const double *U_dev, int nx, int ny, int nz, double Lx, double Ly, double Lz,
                             double gamma, double cfl, double *out_dev, void *cuda_stream);
 
-/* One Euler stage S -> S + L(S) from the CURRENT state with the given dt, for per-kernel parity
- * tests; the state is not advanced.  Any pointer may be NULL (host or device pointers).
- *   U1, Bf1 : layouts of U / Bface
- *   W       : [3][nz][ny][nx] upwind weight on the LOWER d-face of each cell (R6)
- *   Fem     : [3][2][nz][ny][nx] the two induction fluxes kept for CT on that face:
- *             d = x: (F_x[B_y], F_x[B_z]);  d = y: (F_y[B_z], F_y[B_x]);  d = z: (F_z[B_x], F_z[B_y])
- *   Eedge   : [3][nz][ny][nx] Ex at (i, j-1/2, k-1/2), Ey at (i-1/2, j, k-1/2), Ez at (i-1/2, j-1/2, k)
- * entries of inactive directions are zero. */
-int    pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem, double *Eedge);
+/* Test, timing and profiling entry points (pluto_debug_euler, pluto_profile*, pluto_launch_count,
+ * pluto_graph_captures, pluto_probe_fp64_gflops) are exported by the same library and declared in pluto_debug.h. */
 
 #ifdef __cplusplus
 }

@@ -25,7 +25,7 @@ DIVB_CT, DIVB_GLM = 0, 1
 OPT_EMF = 6
 EMF_CONTACT, EMF_UCT_HLLD = 0, 1
 
-# every symbol include/pluto.h declares
+# every symbol include/pluto.h and include/pluto_debug.h declare
 SYMBOLS = [
     "pluto_init", "pluto_set_state", "pluto_step", "pluto_get_dt", "pluto_get_state",
     "pluto_set_box", "pluto_step_fixed_dt", "pluto_get_time", "pluto_set_stream",
@@ -35,7 +35,7 @@ SYMBOLS = [
     "pluto_probe_fp64_gflops",
     "pluto_init_slabs", "pluto_workspace_bytes_slabs", "pluto_local_planes", "pluto_export_slab",
     "pluto_attach_peer", "pluto_fill_ghosts", "pluto_slab_planes", "pluto_set_psi", "pluto_get_psi", "pluto_step_begin", "pluto_dt_max_bits", "pluto_step_stage",
-    "pluto_cfl_dt_noalloc",
+    "pluto_cfl_dt_noalloc", "pluto_graph_captures",
 ]
 NOALLOC_MAX_ROWS = 131072          # PLUTO_NOALLOC_MAX_ROWS of include/pluto.h
 
@@ -70,6 +70,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.pluto_last_error.restype = C.c_char_p
     L.pluto_step_async.argtypes = [i32]
     L.pluto_launch_count.restype = C.c_longlong
+    L.pluto_graph_captures.restype = C.c_longlong
     L.pluto_set_option.argtypes = [i32, i32]
     L.pluto_debug_euler.argtypes = [dbl, vp, vp, vp, vp, vp]
     L.pluto_profile.argtypes = [i32]
@@ -195,6 +196,9 @@ class Pluto:
 
     def launch_count(self):
         return self.L.pluto_launch_count()
+
+    def graph_captures(self):
+        return self.L.pluto_graph_captures()
 
     def set_option(self, opt, value):
         return self.L.pluto_set_option(opt, value)

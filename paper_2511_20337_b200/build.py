@@ -36,7 +36,7 @@ def _sources():
     out = []
     for root, _, files in os.walk(_CSRC):
         out += [os.path.join(root, f) for f in files if f.endswith((".cu", ".cuh", ".h"))]
-    out.append(os.path.join(_INC, "pluto.h"))
+    out += [os.path.join(_INC, "pluto.h"), os.path.join(_INC, "pluto_debug.h")]
     return out
 
 

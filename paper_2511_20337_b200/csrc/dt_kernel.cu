@@ -204,7 +204,7 @@ __global__ void k_dtfinish(Grid g, StepParams *P, int mode)
     double h = 0.0;
     for (int d = 0; d < 3; d++) if (g.act[d] && (h == 0.0 || g.dx[d] < h)) h = g.dx[d];
     P->glm_ch = g.cfl * h / dt;
-    P->glm_damp = exp(-dt * P->glm_ch / 0.18);
+    P->glm_damp = exp(-dt * P->glm_ch / kGlmCr);
 }
 
 __global__ void k_advance_time(StepParams *P) { P->time += P->dt; }

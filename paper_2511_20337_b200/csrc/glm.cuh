@@ -20,7 +20,7 @@
 
 namespace pluto {
 
-constexpr double kGlmCr = 0.18;      // c_p^2 / c_h of [43]
+// kGlmCr (c_p^2 / c_h of [43]) lives in grid.h: k_dtfinish (dt_kernel.cu) forms the damping factor from it
 
 // the nine stored values of one zone: rho, m_x, m_y, m_z, E, B_x, B_y, B_z, psi
 __device__ __forceinline__ void glm_load(const Grid &g, const double *__restrict__ S, const double *__restrict__ psi,

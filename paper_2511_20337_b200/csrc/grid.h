@@ -11,6 +11,7 @@
 namespace pluto {
 
 constexpr int XOFF = 16;   // doubles in front of interior cell i = 0 (>= ghost)
+constexpr double kGlmCr = 0.18;   // GLM variant (glm.cuh, reading R20): c_r = c_p^2 / c_h, the recommendation of [43]
 
 struct Grid {
     int n[3];          // interior extents nx, ny, nz

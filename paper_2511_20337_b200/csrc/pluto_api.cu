@@ -6,6 +6,7 @@
 // only places where slabs meet are the ghost fill (z-ghost planes are pulled out of the neighbour slab's
 // interior, in this process or peer-mapped from another GPU) and the single max that fixes dt.
 #include "../../include/pluto.h"
+#include "../../include/pluto_debug.h"
 #include "kernels.cuh"
 #include "ct_tma.cuh"
 #include "glm.cuh"
@@ -71,6 +72,7 @@ struct Context {
     cudaStream_t own_stream = nullptr;
     int own_stream_dev = -1;
     long long launches = 0;
+    long long captures = 0;          // whole-step graph captures since load (pluto_graph_captures)
     long long per_step[2] = { 0, 0 };
     int use_graph = 1;
     int fuse_xy = 1;
@@ -595,6 +597,7 @@ int run_steps(int nsteps, bool fixed)
         e = cudaGraphInstantiate(&C.graph[gi], graph, 0);
         cudaGraphDestroy(graph);
         if (e != cudaSuccess) return fail(PLUTO_ECUDA, "graph instantiate: %s", cudaGetErrorString(e));
+        C.captures++;
         C.per_step[gi] = C.launches - before;
         C.launches = before;                      // capture enqueued nothing
     }
@@ -679,6 +682,7 @@ void free_domains()
 int ensure_rk3_storage()
 {
     if (C.rk_order != 3) return PLUTO_OK;
+    bool changed = false;            // captured graphs hold the S^2 pointers: they are stale only if one moved
     for (Domain &d : C.dom) {
         if (d.narrays >= A_COUNT || d.sc) continue;
         if (!C.whole()) return fail(PLUTO_ESTATE, "select SSP-RK3 before pluto_init_slabs (peers map one allocation per slab)");
@@ -686,17 +690,21 @@ int ensure_rk3_storage()
         cudaError_t e = cudaMalloc((void **)&d.sc, bytes);
         if (e != cudaSuccess) { cudaGetLastError(); d.sc = nullptr; return fail(PLUTO_ENOMEM, "cudaMalloc(%zu) for the RK3 stage state: %s", bytes, cudaGetErrorString(e)); }
         d.own_sc = true;
+        changed = true;
         CUDA_TRY(cudaMemsetAsync(d.sc, 0, bytes, C.stream));
     }
     // neighbours inside this process: their S^2 lives where arr() finds it
     for (size_t s = 0; s < C.dom.size(); s++) {
         Domain &d = C.dom[s];
         if (C.whole()) {
-            d.nb[0].sc = C.dom[(s + C.dom.size() - 1) % C.dom.size()].sc;
-            d.nb[1].sc = C.dom[(s + 1) % C.dom.size()].sc;
+            double *lo = C.dom[(s + C.dom.size() - 1) % C.dom.size()].sc;
+            double *hi = C.dom[(s + 1) % C.dom.size()].sc;
+            if (d.nb[0].sc != lo || d.nb[1].sc != hi) changed = true;
+            d.nb[0].sc = lo;
+            d.nb[1].sc = hi;
         }
     }
-    destroy_graphs();
+    if (changed) destroy_graphs();
     return PLUTO_OK;
 }
 
@@ -733,14 +741,9 @@ int init_common(int nslab, int first, int count, int nx, int ny, int nz, int gho
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); ndev = 0; }
     if (ndev < 1) return fail(PLUTO_ECUDA, "no CUDA device: this library has no CPU fallback");
-    release();
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (!C.stream || (C.stream == C.own_stream && C.own_stream_dev != dev)) {
-        C.stream = nullptr;
-        int rc = pluto_set_stream(nullptr);
-        if (rc) return rc;
-    }
+    // every argument is checked before the live context is touched: a call rejected with PLUTO_EINVAL (or with
+    // PLUTO_ENOMEM for a registered workspace that is too small) leaves the previous context, its state and its
+    // peer mappings as they were
     if (nslab < 1 || first < 0 || count < 1 || first + count > nslab) return fail(PLUTO_EINVAL, "bad slab range");
     Grid gg;
     if (!make_grid(gg, nx, ny, nz, ghost))
@@ -753,8 +756,28 @@ int init_common(int nslab, int first, int count, int nx, int ny, int nz, int gho
         return fail(PLUTO_EINVAL, "every z slab needs at least ghost + 1 = %d planes", ghost + 1);
     if (C.divb == 1 && (nslab != 1 || limiter == PLUTO_WENOZ))
         return fail(PLUTO_EINVAL, "the GLM variant runs PLM on a single domain");
-    C.glm = C.divb == 1;
     const int narrays = C.rk_order == 3 ? A_COUNT : A_COUNT_RK2;
+    {
+        size_t need = 0;
+        for (int s = 0; s < count; s++) {
+            Grid gs;
+            int k0 = 0, nzl = nz;
+            slab_range(nz, nslab, first + s, k0, nzl);
+            if (!make_grid(gs, nx, ny, nzl, ghost)) return fail(PLUTO_EINVAL, "bad slab");
+            if ((long long)gs.tot[2] * 8 > 65535 || gs.tot[1] > 65535) return fail(PLUTO_EINVAL, "extent too large for the launch grid");
+            need += layout_bytes(gs, narrays);
+        }
+        if (C.ws && C.ws_bytes < need) return fail(PLUTO_ENOMEM, "workspace has %zu bytes, need %zu", C.ws_bytes, need);
+    }
+    release();
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!C.stream || (C.stream == C.own_stream && C.own_stream_dev != dev)) {
+        C.stream = nullptr;
+        int rc = pluto_set_stream(nullptr);
+        if (rc) return rc;
+    }
+    C.glm = C.divb == 1;
     C.nslab = nslab; C.first = first; C.nzg = nz;
     C.dom.resize(count);
     int kbase = 0, dummy = 0;
@@ -1051,6 +1074,9 @@ int pluto_set_box(double Lx, double Ly, double Lz)
     for (Domain &d : C.dom)
         for (int a = 0; a < 3; a++) { d.g.dx[a] = L[a] / n[a]; d.g.idx[a] = 1.0 / d.g.dx[a]; }
     destroy_graphs();          // kernels take the grid by value: captured copies are stale
+    // the dt bound grid was built with the old 1/dx: after a change of the box the bounds left by the last step may
+    // lie below the true candidates, and filter 0 of k_dtmax would then skip the row that holds the maximum
+    if (C.have_state) reset_bounds();
     return PLUTO_OK;
 }
 
@@ -1285,6 +1311,11 @@ int pluto_step_stage(int stage, int fixed)
 {
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
     if (stage < 0 || stage >= C.rk_order) return fail(PLUTO_EINVAL, "stage out of range");
+    // a stage without its pluto_step_begin, or an option switched in between: the stage kernels would read a
+    // neighbour that is not there, or work arrays that were never allocated
+    if (!peers_attached()) return fail(PLUTO_ESTATE, "a neighbour slab is not attached (pluto_attach_peer)");
+    if (int rc = ensure_rk3_storage()) return rc;
+    if (int rc = ensure_uct_storage()) return rc;
     if (stage == 0) LAUNCH(K_SCALAR, launch_dtfinish(C.dom[0].g, C.P, fixed ? 1 : 0, C.stream));
     enqueue_rk_stage(stage);
     if (stage == C.rk_order - 1) {
@@ -1320,6 +1351,7 @@ double pluto_get_time(void)
 }
 
 long long pluto_launch_count(void) { return C.launches; }
+long long pluto_graph_captures(void) { return C.captures; }
 
 int pluto_profile(int on)
 {
@@ -1368,6 +1400,9 @@ int pluto_debug_euler(double dt, double *U1, double *Bf1, double *W, double *Fem
     if (!C.init || !C.have_state) return fail(PLUTO_ESTATE, "no state");
     if (C.dom.size() != 1 || !C.whole() || C.glm) return fail(PLUTO_ESTATE, "pluto_debug_euler works on a single domain of the CT scheme");
     if (!(dt > 0.0)) return fail(PLUTO_EINVAL, "dt must be positive");
+    // in UCT-HLLD mode the CT work arrays hold the a / d coefficients and transverse velocities of R19 instead of
+    // the upwind weight and the two induction fluxes: there is no W or Fem to hand out
+    if (C.emf == 1 && (W || Fem)) return fail(PLUTO_ESTATE, "pluto_debug_euler: W and Fem do not exist in UCT-HLLD mode (pass NULL)");
     if (int rc = ensure_uct_storage()) return rc;
     const Domain &d = C.dom[0];
     const Grid &g = d.g;

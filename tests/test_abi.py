@@ -11,10 +11,35 @@ from paper_2511_20337_b200 import binding
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared():
-    txt = open(os.path.join(ROOT, "include", "pluto.h")).read()
-    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(pluto_[a-z_0-9]+)\s*\(", txt)))
+HEADERS = ("pluto.h", "pluto_debug.h")          # the product ABI, and the test / bench entry points
+
+
+def _declared(headers=HEADERS):
+    names = set()
+    for h in headers:
+        txt = open(os.path.join(ROOT, "include", h)).read()
+        txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+        names |= set(re.findall(r"\b(pluto_[a-z_0-9]+)\s*\(", txt))
+    return sorted(names)
+
+
+def test_product_header_holds_no_test_plumbing():
+    """pluto.h is the five calls, their extensions, the slab calls and the options; counters, timers,
+    the peak probe and the per-kernel debug call live in pluto_debug.h (same library)"""
+    product, debug = _declared(("pluto.h",)), _declared(("pluto_debug.h",))
+    assert not set(product) & set(debug)
+    for name in ("pluto_init", "pluto_set_state", "pluto_step", "pluto_get_dt", "pluto_get_state", "pluto_init_slabs",
+                 "pluto_set_option", "pluto_cfl_dt_noalloc"):
+        assert name in product
+    for name in ("pluto_debug_euler", "pluto_profile", "pluto_profile_get", "pluto_kernel_name", "pluto_launch_count",
+                 "pluto_graph_captures", "pluto_probe_fp64_gflops"):
+        assert name in debug and name not in product
+    # both headers are plain C
+    import subprocess, tempfile
+    with tempfile.TemporaryDirectory() as td:
+        src = os.path.join(td, "t.c")
+        open(src, "w").write('#include "pluto.h"\n#include "pluto_debug.h"\nint main(void) { return PLUTO_NOALLOC_SCRATCH_BYTES > 0 ? 0 : 1; }\n')
+        subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", "-I", os.path.join(ROOT, "include"), src], check=True)
 
 
 def test_header_and_binding_list_the_same_symbols():

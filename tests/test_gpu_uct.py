@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from paper_2511_20337_b200 import workloads as wl
-from paper_2511_20337_b200.binding import EMF_CONTACT, EMF_UCT_HLLD
+from paper_2511_20337_b200.binding import EMF_CONTACT, EMF_UCT_HLLD, ESTATE
 from test_gpu_parity import (TOL_1STEP_MAXREL, TOL_100STEP_L1REL, compare_state, l1rel, l1rel_vector_scaled, maxrel,
                              maxrel_vector_scaled)
 
@@ -56,7 +56,10 @@ def test_uct_parity(uct, oracle, name, make, rk, ghost):
     dt = oracle.get_dt()
     assert uct.get_dt() == dt
     n1, nl = (maxrel_vector_scaled, l1rel_vector_scaled) if name.startswith("ot3d") else (maxrel, l1rel)
-    g = uct.debug_euler(dt)
+    # the UCT-HLLD scheme keeps no upwind weight and no pair of induction fluxes: asking for them is refused
+    assert uct.debug_euler(dt, want=("W",))["rc"] == ESTATE
+    assert uct.debug_euler(dt, want=("U1", "Fem"))["rc"] == ESTATE
+    g = uct.debug_euler(dt, want=("U1", "Bf1", "E"))
     o = oracle.debug_euler(dt)
     assert g["rc"] == 0 and o["rc"] == 0
     escale = max(np.abs(o["E"]).max(), 1e-300)

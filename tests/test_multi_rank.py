@@ -40,11 +40,15 @@ def _spawn(target, world, *args, timeout=300):
     return res
 
 
-def _init(rank, world, port):
+def _init(rank, world, port, backend="gloo"):
     sys.path.insert(0, ROOT)
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
-    dist.init_process_group("gloo", rank=rank, world_size=world)
+    if backend == "nccl":
+        torch.cuda.set_device(0)
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", 0))
+    else:
+        dist.init_process_group("gloo", rank=rank, world_size=world)
 
 
 # ---------------------------------------------------------------- CPU: host-side logic
@@ -127,8 +131,8 @@ def test_handle_exchange_and_array_plumbing_two_ranks():
 
 # ---------------------------------------------------------------- GPU: two slabs, two processes, one device
 
-def _worker_slab(rank, world, port, out, case):
-    _init(rank, world, port)
+def _worker_slab(rank, world, port, out, case, backend="gloo"):
+    _init(rank, world, port, backend)
     from paper_2511_20337_b200 import workloads as wl
     from paper_2511_20337_b200.distributed import SlabPluto
     name, rk, ghost, steps = case
@@ -181,3 +185,52 @@ def test_two_processes_one_slab_each_match_the_single_domain(case):
         assert dts == dt and ts == t
     U, Bf = join_parts([(k0, nzl, Ul, Bl) for _, k0, nzl, Ul, Bl, _, _ in res], w.nx, w.ny, w.nz)
     assert np.array_equal(U, Ur) and np.array_equal(Bf, Br)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", [("smooth_mc", 2, 2, 3), ("ot3d_wenoz", 3, 3, 2)], ids=lambda c: c[0])
+def test_nccl_branch_one_rank_matches_the_single_domain(case):
+    """the device-side collectives of SlabPluto (backend nccl: the MAX all-reduce on a tensor wrapped around the raw
+    pluto_dt_max_bits pointer, and the token all-reduce that serves as the barrier, both ordered on the library's
+    stream) in a group of ONE rank: one GPU is all this box has, and ranks whose kernels wait on one another must not
+    share a GPU.  The decomposed step with the whole box as its single slab equals the single-domain run bit for bit."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    sys.path.insert(0, ROOT)
+    from paper_2511_20337_b200.binding import Pluto
+    name, rk, ghost, steps = case
+    w = _case(name)
+    ref = Pluto()
+    ref.set_integrator(rk)
+    ref.load(w, ghost=ghost)
+    ref.step(steps)
+    dt, t = ref.get_dt(), ref.get_time()
+    ref.step_fixed_dt(1, 0.5 * dt)
+    Ur, Br = ref.get_state()
+    ref.set_integrator(2)
+    ref.finalize()
+    (_, k0, nzl, Ul, Bl, dts, ts), = _spawn(_worker_slab, 1, case, "nccl", timeout=600)
+    assert (k0, nzl) == (0, w.nz) and dts == dt and ts == t
+    assert np.array_equal(Ul.reshape(Ur.shape), Ur) and np.array_equal(Bl, Br)
+
+
+@pytest.mark.gpu
+def test_bench_refuses_more_gpus_than_the_box_has_and_runs_the_slab_path():
+    """`python bench.py --gpus N` without a launcher starts its own ranks; with fewer than N devices it must fail
+    loudly instead of timing one GPU.  `--gpus 1 --slab-path` runs the decomposed step (one-rank NCCL group)."""
+    import json
+    import subprocess
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    too_many = torch.cuda.device_count() + 1
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", str(too_many), "--steps", "1"],
+                       capture_output=True, text=True, env=env, timeout=600)
+    assert p.returncode != 0 and f"needs {too_many} CUDA devices" in p.stderr and not p.stdout.strip()
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "1", "--slab-path", "--steps", "3",
+                        "--warmup", "3", "--repeats", "1", "--e2e-steps", "1"],
+                       capture_output=True, text=True, env=env, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    line = json.loads(p.stdout.strip().splitlines()[-1])
+    assert line["n_gpus"] == 1 and line["value"] > 0 and line["gpu_launches"] > 0
+    assert "z slab" in line["config"]["parallelism"] and line["config"]["zones"] == 256 ** 3
