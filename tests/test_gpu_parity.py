@@ -826,8 +826,8 @@ def ctypes_int():
 
 
 # ---------------------------------------------------------------- memory-safety checks of our own
-# compute-sanitizer is closed on the GPU pool this repo is measured on (tests/sanitizer_cases.py is the
-# driver that was prepared for it), so the three properties its tools check are tested directly:
+# compute-sanitizer is closed on the GPU pool this repo is measured on, so the three properties its tools
+# check are tested directly:
 #   initcheck  -> a workspace poisoned with NaN bit patterns gives the same bits as a zeroed one
 #   memcheck   -> guard bands around the registered workspace stay untouched
 #   racecheck  -> repeated runs of every kernel variant give identical bits (a data race on shared or

@@ -233,4 +233,4 @@ def test_bench_refuses_more_gpus_than_the_box_has_and_runs_the_slab_path():
     assert p.returncode == 0, p.stderr[-2000:]
     line = json.loads(p.stdout.strip().splitlines()[-1])
     assert line["n_gpus"] == 1 and line["value"] > 0 and line["gpu_launches"] > 0
-    assert "z slab" in line["config"]["parallelism"] and line["config"]["zones"] == 256 ** 3
+    assert "z-slab" in line["config"]["parallelism"] and line["config"]["zones"] == 256 ** 3
